@@ -1,0 +1,155 @@
+/* best.h — C-ABI boundary of the B200-native hot path of BEST
+ * ("Posterior sampling in the Age of Emulators", arxiv/paper_2606_04895; PAPER.md = "P").
+ *
+ * What sits behind it (SURVEY.md §8(a), rows A1–A9): many MCMC chains advanced in lockstep on one
+ * GPU, every step evaluating a differentiable MLP log-likelihood emulator and its θ-gradient for
+ * the whole chain batch (P:L7, L38, L147-149).  The interface follows the paper's statement of the
+ * problem: target + bounds at construction, method / n_steps / n_chains at sampling,
+ * acceptance counters / evaluations / samples / covariance out.
+ *
+ * Conventions
+ *  - Every function returns BEST_OK (0) or a negative error code; nothing throws.  The text of
+ *    the last error on the calling thread is returned by best_last_error().
+ *  - "host" pointers are ordinary CPU memory, "dev" pointers are CUDA device memory on the
+ *    current device, "host|dev" means either (detected with cudaPointerGetAttributes).
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Kernels are
+ *    enqueued on it and the call returns without waiting, unless stated otherwise; calls that
+ *    take host output buffers synchronise the stream before returning.
+ *  - best_create / best_state_create deep-copy their inputs; the caller keeps its arrays.
+ *  - θ, log π and ∇θ log π at this boundary are in the ORIGINAL (unwhitened) space and log π is
+ *    unnormalised: the constant log|det L| of eq (2.12) is NOT added — it cancels in
+ *    every accept ratio.
+ *  - There is no CPU fallback and no other backend: without a CUDA device every compute entry
+ *    point returns BEST_ERR_CUDA.
+ */
+#ifndef BEST_H_
+#define BEST_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct best_ctx best_ctx;     /* opaque: device copies of weights, R, L, box, scratch */
+typedef struct best_state best_state; /* opaque: chain state on the device                    */
+
+enum {
+  BEST_OK = 0,
+  BEST_ERR_ARG = -1,         /* bad argument (NULL, size, eps <= 0, odd walker count, a <= 1 …) */
+  BEST_ERR_CUDA = -2,        /* CUDA runtime error / no device                                   */
+  BEST_ERR_NOT_SPD = -3,     /* Sigma_inv not SPD, or diag(L) not positive                       */
+  BEST_ERR_UNSUPPORTED = -4, /* shape not supported by the requested precision path              */
+  BEST_ERR_ALLOC = -5
+};
+enum { BEST_ACT_TANH = 0, BEST_ACT_SILU = 1 };
+enum {
+  BEST_PREC_FP32 = 0, /* FFMA emulator, fp64 chain state and Gaussian/whitening algebra          */
+  BEST_PREC_BF16 = 1  /* tcgen05 tensor-core emulator: bf16 operands, fp32 accumulate            */
+};
+
+/* Target  log π(θ) = −½(θ−μ)ᵀΣ⁻¹(θ−μ) + s·MLP(θ) − (θ_j − θ_i²)²/(2σ²) − pen(θ)
+ * (the synthetic stand-in for the paper's emulator log_prob_fn).
+ * MLP (A1b): h₀=θ; h_k = act(W_k h_{k−1} + b_k), k=1..n_affine−1; out = W_last h + b_last (scalar).
+ * pen (A1e, reading R6 of "smooth exponential penalty"):
+ *   t_i = γ·max(0, lo_i−θ_i, θ_i−hi_i)/(hi_i−lo_i); pen = κ Σ f(t_i);
+ *   f(t) = eᵗ−1−t (t ≤ 40), continued linearly with slope e⁴⁰−1 beyond.                         */
+typedef struct {
+  int32_t d;               /* parameter dimension, 1..32                                         */
+  int32_t n_affine;        /* number of affine maps (hidden layers + 1); 0 ⇒ no MLP term         */
+  const int32_t* widths;   /* host [n_affine+1] = {d, n1, …, nK, 1}                              */
+  const float* W_flat;     /* host: W_1 … W_{n_affine} concatenated, W_k row-major
+                              [widths[k]][widths[k−1]]                                           */
+  const float* b_flat;     /* host: b_1 … b_{n_affine} concatenated                              */
+  int32_t activation;      /* BEST_ACT_*                                                         */
+  float mlp_scale;         /* s                                                                  */
+  const double* mu;        /* host [d]; NULL ⇒ no Gaussian term                                  */
+  const double* Sigma_inv; /* host [d*d] SPD precision, row-major; factored Σ⁻¹=RᵀR in fp64      */
+  const double* lo;        /* host [d] box; NULL ⇒ unbounded                                     */
+  const double* hi;        /* host [d]                                                           */
+  float pen_kappa, pen_gamma;
+  int32_t banana_i, banana_j; /* −(θ_j − θ_i²)²/(2σ²) (A1d); banana_i < 0 ⇒ off                 */
+  float banana_sigma;
+  const double* L;         /* host [d*d] lower-triangular whitening factor, eq (2.4) P:L78;
+                              NULL ⇒ identity.  Only the lower triangle is read.                 */
+  int32_t precision;       /* BEST_PREC_*                                                        */
+} best_config;
+
+/* Build a context (host work: fp64 Cholesky of Sigma_inv, packing and upload of the weights).
+ * Errors: BEST_ERR_ARG, BEST_ERR_NOT_SPD, BEST_ERR_UNSUPPORTED (bf16 path: hidden widths must be
+ * equal and a multiple of 64, ≤ 512 … see DESIGN.md), BEST_ERR_CUDA, BEST_ERR_ALLOC.            */
+int best_create(const best_config* cfg, best_ctx** out);
+void best_destroy(best_ctx* ctx);
+
+/* log π(θ) and ∇θ log π(θ) for n points (A1a–A1e).  theta [n*d] row-major float, host|dev;
+ * logp [n] and grad [n*d] (nullable ⇒ forward only) float, host|dev.  With any host pointer the
+ * call copies through the device and synchronises `stream` before returning.                    */
+int best_logp_grad(best_ctx* ctx, const float* theta, int64_t n, float* logp, float* grad,
+                   void* stream);
+
+/* Chain state: n_chains chains at theta0 [n_chains*d] (float, host|dev); evaluates and caches
+ * log π and ∇θ log π at θ₀; step counter 0, accept counters 0.                                   */
+int best_state_create(best_ctx* ctx, int64_t n_chains, const float* theta0, void* stream,
+                      best_state** out);
+void best_state_destroy(best_state* st);
+
+/* Samplers.  The Philox4x32-10 stream is keyed by (seed; chain, global step, slot) (north_star;
+ * reading R1), and the state's global step counter keeps increasing across calls, so one call of
+ * N steps equals k calls of N/k steps bit for bit.  trace_dev (nullable, device) receives the
+ * post-accept θ every `thin` steps as float [n_steps/thin][n_chains][d]; thin ≤ 0 ⇒ no trace.
+ *
+ * MH   (A4; reading R5): θ' = θ + ε L ξ, ξ~N(0,1); log α = log π(θ') − log π(θ).
+ * MALA (A5; eq (2.3) P:L70 in whitened space; reading R4): z' = z + ε g_z + √(2ε) ξ,
+ *       g_z = Lᵀ∇θ log π; Hastings ratio with q(·|z) = N(z + ε g_z, 2ε·1).
+ * HMC  (A6; eq (2.1),(2.8) P:L56, L96): q~N(0,1); n_leapfrog kick-drift-kick steps of size ε in
+ *       whitened space (identity mass); log α = H(z,q) − H(z',q'); one "step" = one
+ *       trajectory.
+ * AIES (A7; eq (2.13)-(2.15) P:L159-168): two half-ensembles [0,B/2), [B/2,B); walker i moves
+ *       against a uniformly drawn partner j of the other half: θ' = θ_j + z(θ_i − θ_j),
+ *       z = (u(a−1)+1)²/a, log α = (d−1) ln z + log π(θ') − log π(θ_i); no whitening.
+ * All: accept iff log u < log α (NaN ⇒ reject; reading R7).
+ * Errors: BEST_ERR_ARG for eps <= 0, n_leapfrog < 1, a <= 1, odd or < 2 walker count (AIES).    */
+int best_step_mh(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, float eps,
+                 float* trace_dev, int32_t thin, void* stream);
+int best_step_mala(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, float eps,
+                   float* trace_dev, int32_t thin, void* stream);
+int best_step_hmc(best_ctx* ctx, best_state* st, int64_t n_traj, uint64_t seed, float eps,
+                  int32_t n_leapfrog, float* trace_dev, int32_t thin, void* stream);
+int best_step_aies(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, float a,
+                   float* trace_dev, int32_t thin, void* stream);
+
+/* Running covariance adaptation (A9; reading R14).  While adapt_every > 0 the
+ * MH/MALA/HMC steps of `st` accumulate n, Σθ, Σθθᵀ (fp64) of the post-accept states of all chains;
+ * every adapt_every steps  C = scatter/(n−1),  C_ii *= (1+jitter),  L = chol(C)  is computed ON
+ * DEVICE and replaces the whitening factor (jitter×10 retries up to 5 times, else L is kept).
+ * adapt_every = 0 switches it off.  Not used by AIES.                                  */
+int best_set_adaptation(best_ctx* ctx, best_state* st, int32_t adapt_every, double jitter);
+/* number of successful / failed whitening updates so far (synchronises) */
+int best_adapt_stats(best_ctx* ctx, int64_t* n_updates, int64_t* n_failures);
+
+/* Whitening factor L (host [d*d], row-major, lower triangle).  get synchronises the device.     */
+int best_get_whitening(best_ctx* ctx, double* L_host);
+int best_set_whitening(best_ctx* ctx, const double* L_host);
+
+/* Read the state back (all pointers host, each nullable): theta [B*d], logp [B], grad [B*d]
+ * (float, original space), global step counter, per-chain accept counters [B], total emulator
+ * evaluations.  Synchronises `stream`.                                                          */
+int best_state_get(best_state* st, float* theta, float* logp, float* grad, uint64_t* step,
+                   uint64_t* n_accept, uint64_t* n_evals, void* stream);
+/* Same state in the library's internal precision (fp64 on the fp32 path): exact checkpoints.    */
+int best_state_get_f64(best_state* st, double* theta, double* logp, double* grad, void* stream);
+/* log α of every chain's most recent proposal (host [B]); synchronises.  Diagnostics / tests.   */
+int best_state_last_log_alpha(best_state* st, double* log_alpha, void* stream);
+/* Overwrite θ (host|dev float [B*d]) and the step counter; recomputes log π and ∇θ log π;
+ * accept counters are kept.                                                                     */
+int best_state_set(best_state* st, const float* theta, uint64_t step, void* stream);
+
+/* Number of kernels this library has launched so far in this process (all contexts). */
+uint64_t best_launch_count(void);
+const char* best_last_error(void);
+const char* best_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BEST_H_ */

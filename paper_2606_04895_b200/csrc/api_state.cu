@@ -1,0 +1,300 @@
+// C-ABI entry points, part 2: best_logp_grad, chain state, sampler dispatch, whitening, adaptation.
+#include <cstring>
+
+#include "best_internal.h"
+#include "tc_fused.h"
+
+using namespace best;
+
+namespace {
+
+struct DevBuf {  // RAII scratch
+  void* p = nullptr;
+  ~DevBuf() { if (p) cudaFree(p); }
+  int alloc(size_t bytes) {
+    if (cudaMalloc(&p, bytes ? bytes : 1) != cudaSuccess) {
+      cudaGetLastError();
+      set_error("cudaMalloc failed");
+      return BEST_ERR_ALLOC;
+    }
+    return BEST_OK;
+  }
+};
+
+int refresh_cache(best_ctx* ctx, best_state* st, cudaStream_t s) {
+  if (ctx->precision == BEST_PREC_BF16) return tc_state_init(ctx, st, s);
+  BEST_TRY(eval_target_soa(ctx, st->theta, st->B, st->B, st->logp, st->grad, s));
+  st->grad_valid = true;
+  st->n_evals += (uint64_t)st->B;
+  return BEST_OK;
+}
+
+int check_step_args(best_ctx* ctx, best_state* st, int64_t n, const float* trace, int thin) {
+  if (!ctx || !st || st->ctx != ctx) { set_error("step: bad ctx/state"); return BEST_ERR_ARG; }
+  if (n < 0) { set_error("step: n_steps < 0"); return BEST_ERR_ARG; }
+  if (trace && thin > 0 && !is_device_ptr(trace)) { set_error("step: trace must be a device pointer"); return BEST_ERR_ARG; }
+  return BEST_OK;
+}
+
+enum { M_MH = 0, M_MALA = 1, M_HMC = 2, M_AIES = 3 };
+
+}  // namespace
+
+extern "C" {
+
+int best_logp_grad(best_ctx* ctx, const float* theta, int64_t n, float* logp, float* grad,
+                   void* stream) {
+  if (!ctx || n < 0) { set_error("best_logp_grad: bad argument"); return BEST_ERR_ARG; }
+  if (n == 0) return BEST_OK;
+  if (!theta || !logp) { set_error("best_logp_grad: NULL buffer"); return BEST_ERR_ARG; }
+  cudaStream_t s = (cudaStream_t)stream;
+  const int d = ctx->d;
+  const bool th_dev = is_device_ptr(theta), lp_dev = is_device_ptr(logp);
+  const bool g_dev = grad ? is_device_ptr(grad) : true;
+  DevBuf b_th, b_lp, b_g;
+  const float* th_d = theta;
+  float* lp_d = logp;
+  float* g_d = grad;
+  if (!th_dev) {
+    BEST_TRY(b_th.alloc(sizeof(float) * n * d));
+    BEST_CUDA(cudaMemcpyAsync(b_th.p, theta, sizeof(float) * n * d, cudaMemcpyHostToDevice, s));
+    th_d = (const float*)b_th.p;
+  }
+  if (!lp_dev) { BEST_TRY(b_lp.alloc(sizeof(float) * n)); lp_d = (float*)b_lp.p; }
+  if (grad && !g_dev) { BEST_TRY(b_g.alloc(sizeof(float) * n * d)); g_d = (float*)b_g.p; }
+
+  if (ctx->precision == BEST_PREC_BF16) {
+    BEST_TRY(tc_logp_grad(ctx, th_d, n, lp_d, g_d, s));
+  } else {
+    DevBuf soa_th, soa_g, lp64;
+    BEST_TRY(soa_th.alloc(sizeof(double) * n * d));
+    BEST_TRY(lp64.alloc(sizeof(double) * n));
+    if (grad) BEST_TRY(soa_g.alloc(sizeof(double) * n * d));
+    BEST_TRY(rows_f32_to_soa_f64(th_d, (double*)soa_th.p, n, d, n, s));
+    BEST_TRY(eval_target_soa(ctx, (double*)soa_th.p, n, n, (double*)lp64.p, (double*)soa_g.p, s));
+    BEST_TRY(soa_f64_to_rows_f32((double*)lp64.p, lp_d, n, 1, n, s));
+    if (grad) BEST_TRY(soa_f64_to_rows_f32((double*)soa_g.p, g_d, n, d, n, s));
+    BEST_CUDA(cudaStreamSynchronize(s));  // scratch above is freed on return
+  }
+  if (!lp_dev) BEST_CUDA(cudaMemcpyAsync(logp, lp_d, sizeof(float) * n, cudaMemcpyDeviceToHost, s));
+  if (grad && !g_dev) BEST_CUDA(cudaMemcpyAsync(grad, g_d, sizeof(float) * n * d, cudaMemcpyDeviceToHost, s));
+  if (!th_dev || !lp_dev || (grad && !g_dev)) BEST_CUDA(cudaStreamSynchronize(s));
+  return BEST_OK;
+}
+
+int best_state_create(best_ctx* ctx, int64_t n_chains, const float* theta0, void* stream,
+                      best_state** out) {
+  if (!ctx || !theta0 || !out || n_chains < 1 || n_chains > (int64_t)1 << 31) {
+    set_error("best_state_create: bad argument");
+    return BEST_ERR_ARG;
+  }
+  *out = nullptr;
+  best_state* st = new best_state();
+  st->ctx = ctx;
+  st->B = n_chains;
+  const size_t B = (size_t)n_chains, d = (size_t)ctx->d;
+  int rc = BEST_OK;
+  auto A = [&](double** p, size_t n) { if (!rc) rc = dev_alloc(p, n); };
+  A(&st->theta, B * d); A(&st->grad, B * d); A(&st->logp, B);
+  A(&st->p_theta, B * d); A(&st->p_grad, B * d); A(&st->p_logp, B);
+  A(&st->q, B * d); A(&st->h0, B); A(&st->last_la, B);
+  if (!rc) rc = dev_alloc(&st->n_accept, B);
+  if (rc) { best_state_destroy(st); return rc; }
+  cudaMemset(st->n_accept, 0, sizeof(unsigned long long) * B);
+  cudaMemset(st->last_la, 0, sizeof(double) * B);
+  rc = best_state_set(st, theta0, 0, stream);
+  if (rc) { best_state_destroy(st); return rc; }
+  *out = st;
+  return BEST_OK;
+}
+
+void best_state_destroy(best_state* st) {
+  if (!st) return;
+  cudaFree(st->theta); cudaFree(st->grad); cudaFree(st->logp);
+  cudaFree(st->p_theta); cudaFree(st->p_grad); cudaFree(st->p_logp);
+  cudaFree(st->q); cudaFree(st->h0); cudaFree(st->last_la); cudaFree(st->n_accept);
+  delete st;
+}
+
+int best_state_set(best_state* st, const float* theta, uint64_t step, void* stream) {
+  if (!st || !theta) { set_error("best_state_set: bad argument"); return BEST_ERR_ARG; }
+  cudaStream_t s = (cudaStream_t)stream;
+  best_ctx* ctx = st->ctx;
+  const size_t nb = sizeof(float) * st->B * ctx->d;
+  DevBuf tmp;
+  const float* src = theta;
+  if (!is_device_ptr(theta)) {
+    BEST_TRY(tmp.alloc(nb));
+    BEST_CUDA(cudaMemcpyAsync(tmp.p, theta, nb, cudaMemcpyHostToDevice, s));
+    src = (const float*)tmp.p;
+  }
+  BEST_TRY(rows_f32_to_soa_f64(src, st->theta, st->B, ctx->d, st->B, s));
+  st->step = step;
+  BEST_TRY(refresh_cache(ctx, st, s));
+  BEST_CUDA(cudaStreamSynchronize(s));
+  return BEST_OK;
+}
+
+int best_state_get(best_state* st, float* theta, float* logp, float* grad, uint64_t* step,
+                   uint64_t* n_accept, uint64_t* n_evals, void* stream) {
+  if (!st) { set_error("best_state_get: NULL state"); return BEST_ERR_ARG; }
+  cudaStream_t s = (cudaStream_t)stream;
+  best_ctx* ctx = st->ctx;
+  const int64_t B = st->B;
+  const int d = ctx->d;
+  if (grad && !st->grad_valid) {
+    BEST_TRY(eval_target_soa(ctx, st->theta, B, B, st->logp, st->grad, s));
+    st->grad_valid = true;
+  }
+  DevBuf tmp;
+  BEST_TRY(tmp.alloc(sizeof(float) * B * d));
+  if (theta) {
+    BEST_TRY(soa_f64_to_rows_f32(st->theta, (float*)tmp.p, B, d, B, s));
+    BEST_CUDA(cudaMemcpyAsync(theta, tmp.p, sizeof(float) * B * d, cudaMemcpyDeviceToHost, s));
+    BEST_CUDA(cudaStreamSynchronize(s));
+  }
+  if (grad) {
+    BEST_TRY(soa_f64_to_rows_f32(st->grad, (float*)tmp.p, B, d, B, s));
+    BEST_CUDA(cudaMemcpyAsync(grad, tmp.p, sizeof(float) * B * d, cudaMemcpyDeviceToHost, s));
+    BEST_CUDA(cudaStreamSynchronize(s));
+  }
+  if (logp) {
+    BEST_TRY(soa_f64_to_rows_f32(st->logp, (float*)tmp.p, B, 1, B, s));
+    BEST_CUDA(cudaMemcpyAsync(logp, tmp.p, sizeof(float) * B, cudaMemcpyDeviceToHost, s));
+  }
+  if (n_accept)
+    BEST_CUDA(cudaMemcpyAsync(n_accept, st->n_accept, sizeof(uint64_t) * B, cudaMemcpyDeviceToHost, s));
+  BEST_CUDA(cudaStreamSynchronize(s));
+  if (step) *step = st->step;
+  if (n_evals) *n_evals = st->n_evals;
+  return BEST_OK;
+}
+
+int best_state_get_f64(best_state* st, double* theta, double* logp, double* grad, void* stream) {
+  if (!st) { set_error("best_state_get_f64: NULL state"); return BEST_ERR_ARG; }
+  cudaStream_t s = (cudaStream_t)stream;
+  const int64_t B = st->B;
+  const int d = st->ctx->d;
+  BEST_CUDA(cudaStreamSynchronize(s));
+  std::vector<double> tmp((size_t)B * d);
+  auto fetch = [&](const double* src, double* dst) -> int {
+    BEST_CUDA(cudaMemcpy(tmp.data(), src, sizeof(double) * B * d, cudaMemcpyDeviceToHost));
+    for (int64_t c = 0; c < B; ++c)
+      for (int i = 0; i < d; ++i) dst[c * d + i] = tmp[(size_t)i * B + c];
+    return BEST_OK;
+  };
+  if (theta) BEST_TRY(fetch(st->theta, theta));
+  if (grad) {
+    if (!st->grad_valid) {
+      BEST_TRY(eval_target_soa(st->ctx, st->theta, B, B, st->logp, st->grad, s));
+      BEST_CUDA(cudaStreamSynchronize(s));
+      st->grad_valid = true;
+    }
+    BEST_TRY(fetch(st->grad, grad));
+  }
+  if (logp) BEST_CUDA(cudaMemcpy(logp, st->logp, sizeof(double) * B, cudaMemcpyDeviceToHost));
+  return BEST_OK;
+}
+
+int best_state_last_log_alpha(best_state* st, double* log_alpha, void* stream) {
+  if (!st || !log_alpha) { set_error("best_state_last_log_alpha: bad argument"); return BEST_ERR_ARG; }
+  BEST_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+  BEST_CUDA(cudaMemcpy(log_alpha, st->last_la, sizeof(double) * st->B, cudaMemcpyDeviceToHost));
+  return BEST_OK;
+}
+
+static int run_step(best_ctx* ctx, best_state* st, int method, int64_t n, uint64_t seed, float eps,
+                    int nl, float* trace, int thin, void* stream) {
+  BEST_TRY(check_step_args(ctx, st, n, trace, thin));
+  cudaStream_t s = (cudaStream_t)stream;
+  if (method != M_AIES && !(eps > 0.f)) { set_error("step: eps must be > 0"); return BEST_ERR_ARG; }
+  if (method == M_HMC && nl < 1) { set_error("hmc: n_leapfrog must be >= 1"); return BEST_ERR_ARG; }
+  if (method == M_AIES) {
+    if (!(eps > 1.f)) { set_error("aies: a must be > 1"); return BEST_ERR_ARG; }
+    if (st->B < 2 || (st->B & 1)) { set_error("aies: walker count must be even and >= 2"); return BEST_ERR_ARG; }
+  }
+  if (n == 0) return BEST_OK;
+  int rc;
+  if (ctx->precision == BEST_PREC_BF16) {
+    rc = tc_step(ctx, st, method, n, seed, eps, nl, trace, thin, s);
+  } else {
+    if ((method == M_MALA || method == M_HMC) && !st->grad_valid) {
+      BEST_TRY(eval_target_soa(ctx, st->theta, st->B, st->B, st->logp, st->grad, s));
+      st->grad_valid = true;
+    }
+    switch (method) {
+      case M_MH: rc = step_mh(ctx, st, n, seed, eps, trace, thin, s); st->grad_valid = false; break;
+      case M_MALA: rc = step_mala(ctx, st, n, seed, eps, trace, thin, s); break;
+      case M_HMC: rc = step_hmc(ctx, st, n, seed, eps, nl, trace, thin, s); break;
+      default: rc = step_aies(ctx, st, n, seed, eps, trace, thin, s); st->grad_valid = false; break;
+    }
+  }
+  if (rc) return rc;
+  st->step += (uint64_t)n;
+  st->n_evals += (uint64_t)st->B * (uint64_t)n * (uint64_t)(method == M_HMC ? nl : 1);
+  return BEST_OK;
+}
+
+int best_step_mh(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, float eps,
+                 float* trace_dev, int32_t thin, void* stream) {
+  return run_step(ctx, st, M_MH, n_steps, seed, eps, 0, trace_dev, thin, stream);
+}
+int best_step_mala(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, float eps,
+                   float* trace_dev, int32_t thin, void* stream) {
+  return run_step(ctx, st, M_MALA, n_steps, seed, eps, 0, trace_dev, thin, stream);
+}
+int best_step_hmc(best_ctx* ctx, best_state* st, int64_t n_traj, uint64_t seed, float eps,
+                  int32_t n_leapfrog, float* trace_dev, int32_t thin, void* stream) {
+  return run_step(ctx, st, M_HMC, n_traj, seed, eps, n_leapfrog, trace_dev, thin, stream);
+}
+int best_step_aies(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, float a,
+                   float* trace_dev, int32_t thin, void* stream) {
+  return run_step(ctx, st, M_AIES, n_steps, seed, a, 0, trace_dev, thin, stream);
+}
+
+int best_set_adaptation(best_ctx* ctx, best_state* st, int32_t adapt_every, double jitter) {
+  if (!ctx || !st || st->ctx != ctx || adapt_every < 0 || !(jitter >= 0.0)) {
+    set_error("best_set_adaptation: bad argument");
+    return BEST_ERR_ARG;
+  }
+  ctx->adapt_every = adapt_every;
+  ctx->jitter = jitter;
+  if (adapt_every > 0) BEST_TRY(adapt_reset(ctx, st, 0));
+  return BEST_OK;
+}
+
+int best_adapt_stats(best_ctx* ctx, int64_t* n_updates, int64_t* n_failures) {
+  if (!ctx) { set_error("best_adapt_stats: NULL ctx"); return BEST_ERR_ARG; }
+  int64_t h[2];
+  BEST_CUDA(cudaDeviceSynchronize());
+  BEST_CUDA(cudaMemcpy(h, ctx->adapt_counts, sizeof(h), cudaMemcpyDeviceToHost));
+  if (n_updates) *n_updates = h[0];
+  if (n_failures) *n_failures = h[1];
+  return BEST_OK;
+}
+
+int best_get_whitening(best_ctx* ctx, double* L_host) {
+  if (!ctx || !L_host) { set_error("best_get_whitening: bad argument"); return BEST_ERR_ARG; }
+  BEST_CUDA(cudaDeviceSynchronize());
+  BEST_CUDA(cudaMemcpy(L_host, ctx->L_dev, sizeof(double) * ctx->d * ctx->d, cudaMemcpyDeviceToHost));
+  return BEST_OK;
+}
+
+int best_set_whitening(best_ctx* ctx, const double* L_host) {
+  if (!ctx || !L_host) { set_error("best_set_whitening: bad argument"); return BEST_ERR_ARG; }
+  const int d = ctx->d;
+  std::vector<double> L((size_t)d * d, 0.0);
+  for (int i = 0; i < d; ++i)
+    for (int j = 0; j <= i; ++j) {
+      L[(size_t)i * d + j] = L_host[(size_t)i * d + j];
+      if (i == j && !(L_host[(size_t)i * d + j] > 0.0)) {
+        set_error("best_set_whitening: diag(L) must be positive");
+        return BEST_ERR_NOT_SPD;
+      }
+    }
+  BEST_CUDA(cudaDeviceSynchronize());
+  BEST_CUDA(cudaMemcpy(ctx->L_dev, L.data(), sizeof(double) * d * d, cudaMemcpyHostToDevice));
+  return BEST_OK;
+}
+
+}  // extern "C"

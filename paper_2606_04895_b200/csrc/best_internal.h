@@ -1,0 +1,139 @@
+// Internal declarations of libbest.so (host side).  Not part of the public boundary.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+#include <string>
+#include <vector>
+
+#include "../../include/best.h"
+
+namespace best {
+
+void set_error(const std::string& msg);
+extern std::atomic<uint64_t> g_launches;
+inline void count_launch(uint64_t n = 1) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+#define BEST_CUDA(expr)                                                                    \
+  do {                                                                                     \
+    cudaError_t _e = (expr);                                                               \
+    if (_e != cudaSuccess) {                                                               \
+      best::set_error(std::string(#expr) + ": " + cudaGetErrorString(_e));                 \
+      return BEST_ERR_CUDA;                                                                \
+    }                                                                                      \
+  } while (0)
+
+#define BEST_TRY(expr)           \
+  do {                           \
+    int _rc = (expr);            \
+    if (_rc != BEST_OK) return _rc; \
+  } while (0)
+
+inline bool is_device_ptr(const void* p) {
+  if (!p) return false;
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+template <typename T>
+int dev_alloc(T** p, size_t n) {
+  *p = nullptr;
+  if (n == 0) n = 1;
+  if (cudaMalloc((void**)p, sizeof(T) * n) != cudaSuccess) {
+    cudaGetLastError();
+    set_error("cudaMalloc failed");
+    return BEST_ERR_ALLOC;
+  }
+  return BEST_OK;
+}
+
+constexpr int kMaxD = 32;
+constexpr int64_t kEvalChunk = 16384;  // chains per emulator pass on the fp32 path (bounds scratch)
+
+// Target terms that every kernel needs by value (device pointers inside).
+struct TargetDev {
+  int d;
+  int has_gauss, has_box;
+  const double* mu;   // [d]
+  const double* R;    // [d*d] upper triangular, Sigma_inv = R^T R
+  const double* lo;   // [d]
+  const double* hi;   // [d]
+  double pen_kappa, pen_gamma;
+  int banana_i, banana_j;
+  double banana_sigma;
+  double mlp_scale;
+  int has_mlp;
+};
+
+struct TcPlan;  // bf16 tensor-core path (tc_fused.cu)
+
+}  // namespace best
+
+struct best_ctx {
+  int d = 0, dp = 0;  // dp = d rounded up to 4 (row pitch of MLP input / theta-gradient)
+  int n_affine = 0;
+  std::vector<int> widths, wp;  // wp: widths padded to multiples of 4 (wp[0] = dp, last = 1)
+  int activation = 0;
+  int precision = 0;
+  best::TargetDev tgt{};
+  // fp32 emulator weights, zero padded: W[k] [wp[k+1]][wp[k]], b[k] [wp[k+1]]
+  std::vector<float*> W, b;
+  double* dev_consts = nullptr;  // mu | R | lo | hi | L  (5 blocks)
+  double* L_dev = nullptr;       // [d*d] lower triangular, updated on device by adaptation
+  // fp32 emulator scratch (sized for scratch_n chains)
+  int64_t scratch_n = 0;
+  float* X0 = nullptr;            // [n][dp]
+  std::vector<float*> H, Dact;    // per hidden layer [n][wp[k+1]]
+  float* delta[2] = {nullptr, nullptr};
+  float* mlp_out = nullptr;       // [n]
+  float* mlp_grad = nullptr;      // [n][dp]
+  // adaptation (A9)
+  int adapt_every = 0;
+  double jitter = 1e-6;
+  int64_t win_steps = 0;
+  double* cov_acc = nullptr;      // [nblk_max][1 + d + d*d] per-block partial sums (fp64)
+  int cov_blocks = 0;
+  double* cov_ref = nullptr;      // [d] shift
+  int64_t* adapt_counts = nullptr;  // device [2]: updates, failures
+  best::TcPlan* tc = nullptr;
+};
+
+struct best_state {
+  best_ctx* ctx = nullptr;
+  int64_t B = 0;
+  uint64_t step = 0;
+  uint64_t n_evals = 0;
+  bool grad_valid = true;  // AIES does not maintain the cached gradient
+  // SoA [d][B] fp64
+  double *theta = nullptr, *grad = nullptr, *logp = nullptr;
+  double *p_theta = nullptr, *p_grad = nullptr, *p_logp = nullptr;
+  double *q = nullptr, *h0 = nullptr;
+  double* last_la = nullptr;
+  unsigned long long* n_accept = nullptr;
+};
+
+namespace best {
+
+// fp32 emulator (emulator_fp32.cu): MLP forward (+ input gradient) for n points.
+// X0 = ctx->X0 must already hold the inputs [n][dp]; results in ctx->mlp_out / ctx->mlp_grad.
+int mlp_fp32_reserve(best_ctx* ctx, int64_t n);
+int mlp_fp32_run(best_ctx* ctx, int64_t n, bool want_grad, cudaStream_t s);
+
+// Full target for SoA fp64 inputs (samplers.cu): theta [d][ld] (first n columns used).
+int eval_target_soa(best_ctx* ctx, const double* theta, int64_t ld, int64_t n, double* logp,
+                    double* grad /*nullable, [d][ld]*/, cudaStream_t s);
+
+int step_mh(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cudaStream_t);
+int step_mala(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cudaStream_t);
+int step_hmc(best_ctx*, best_state*, int64_t, uint64_t, double, int, float*, int, cudaStream_t);
+int step_aies(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cudaStream_t);
+int adapt_reset(best_ctx* ctx, best_state* st, cudaStream_t s);
+
+// layout helpers (samplers.cu)
+int rows_f32_to_soa_f64(const float* rows_dev, double* soa, int64_t n, int d, int64_t ld, cudaStream_t s);
+int soa_f64_to_rows_f32(const double* soa, float* rows_dev, int64_t n, int d, int64_t ld, cudaStream_t s);
+
+}  // namespace best

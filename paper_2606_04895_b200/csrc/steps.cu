@@ -1,0 +1,403 @@
+// Exact-path step kernels: MH (A4), MALA (A5), HMC (A6), AIES (A7), accept/trace/counters (A8).
+// One thread per chain, fp64, SoA state [d][B].  Each kernel is one half of a step (propose /
+// accept) with the emulator passes (emulator_fp32.cu) in between.
+#include "best_internal.h"
+#include "device_math.cuh"
+
+namespace best {
+namespace {
+
+constexpr int TPB = 128;
+inline int nblocks(int64_t n) { return (int)((n + TPB - 1) / TPB); }
+
+struct Chains {  // device pointers of one best_state
+  int64_t B;
+  int d;
+  double *theta, *grad, *logp, *p_theta, *p_grad, *p_logp, *q, *h0, *last_la;
+  unsigned long long* n_accept;
+};
+
+__device__ __forceinline__ void load_col(const double* a, int64_t ld, int64_t c, int d, double* v) {
+  for (int i = 0; i < d; ++i) v[i] = a[i * ld + c];
+}
+__device__ __forceinline__ void store_col(double* a, int64_t ld, int64_t c, int d, const double* v) {
+  for (int i = 0; i < d; ++i) a[i * ld + c] = v[i];
+}
+
+// ---- MH: theta' = theta + eps L xi -----------------------------------------------------------
+__global__ void k_mh_propose(Chains S, const double* __restrict__ L, uint64_t seed, uint64_t step,
+                             double eps) {
+  const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (c >= S.B) return;
+  const int d = S.d;
+  double xi[kMaxD], dx[kMaxD];
+  draw_normals<double>(seed, (uint32_t)c, step, d, xi);
+  for (int i = 0; i < d; ++i) xi[i] *= eps;
+  tri_L_apply<double>(L, d, xi, dx);
+  for (int i = 0; i < d; ++i) S.p_theta[i * S.B + c] = S.theta[i * S.B + c] + dx[i];
+}
+
+__global__ void k_mh_accept(Chains S, uint64_t seed, uint64_t step) {
+  const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (c >= S.B) return;
+  const uint4 w = philox4x32_10((uint32_t)c, step, 0u, seed);
+  const double la = S.p_logp[c] - S.logp[c];
+  S.last_la[c] = la;
+  if (accept_rule<double>(u01<double>(w.x), la)) {
+    for (int i = 0; i < S.d; ++i) S.theta[i * S.B + c] = S.p_theta[i * S.B + c];
+    S.logp[c] = S.p_logp[c];
+    S.n_accept[c] += 1ull;
+  }
+}
+
+// ---- MALA: z' = z + eps g_z + sqrt(2 eps) xi  (eq 2.3) -----------------------------------------
+__global__ void k_mala_propose(Chains S, const double* __restrict__ L, uint64_t seed, uint64_t step,
+                               double eps) {
+  const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (c >= S.B) return;
+  const int d = S.d;
+  double xi[kMaxD], g[kMaxD], gz[kMaxD], dx[kMaxD];
+  draw_normals<double>(seed, (uint32_t)c, step, d, xi);
+  load_col(S.grad, S.B, c, d, g);
+  tri_Lt_apply<double>(L, d, g, gz);
+  const double sq = sqrt(2.0 * eps);
+  for (int i = 0; i < d; ++i) gz[i] = eps * gz[i] + sq * xi[i];
+  tri_L_apply<double>(L, d, gz, dx);
+  for (int i = 0; i < d; ++i) S.p_theta[i * S.B + c] = S.theta[i * S.B + c] + dx[i];
+}
+
+__global__ void k_mala_accept(Chains S, const double* __restrict__ L, uint64_t seed, uint64_t step,
+                              double eps) {
+  const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (c >= S.B) return;
+  const int d = S.d;
+  double xi[kMaxD], g[kMaxD], gz[kMaxD], gzp[kMaxD];
+  draw_normals<double>(seed, (uint32_t)c, step, d, xi);
+  load_col(S.grad, S.B, c, d, g);
+  tri_Lt_apply<double>(L, d, g, gz);
+  load_col(S.p_grad, S.B, c, d, g);
+  tri_Lt_apply<double>(L, d, g, gzp);
+  const double sq = sqrt(2.0 * eps);
+  double fwd = 0.0, bwd = 0.0;
+  for (int i = 0; i < d; ++i) {
+    const double f = sq * xi[i];
+    const double r = -(eps * (gz[i] + gzp[i]) + sq * xi[i]);
+    fwd += f * f;
+    bwd += r * r;
+  }
+  const double la = S.p_logp[c] - S.logp[c] + (-bwd / (4.0 * eps)) - (-fwd / (4.0 * eps));
+  S.last_la[c] = la;
+  const uint4 w = philox4x32_10((uint32_t)c, step, 0u, seed);
+  if (accept_rule<double>(u01<double>(w.x), la)) {
+    for (int i = 0; i < d; ++i) {
+      S.theta[i * S.B + c] = S.p_theta[i * S.B + c];
+      S.grad[i * S.B + c] = g[i];
+    }
+    S.logp[c] = S.p_logp[c];
+    S.n_accept[c] += 1ull;
+  }
+}
+
+// ---- HMC: kick-drift-kick leapfrog in whitened space (eq 2.1 / 2.8) ----------------------------
+__global__ void k_hmc_begin(Chains S, const double* __restrict__ L, uint64_t seed, uint64_t step,
+                            double eps) {
+  const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (c >= S.B) return;
+  const int d = S.d;
+  double q[kMaxD], g[kMaxD], gz[kMaxD], dx[kMaxD];
+  draw_normals<double>(seed, (uint32_t)c, step, d, q);
+  double kin = 0.0;
+  for (int i = 0; i < d; ++i) kin += q[i] * q[i];
+  S.h0[c] = -S.logp[c] + 0.5 * kin;
+  load_col(S.grad, S.B, c, d, g);
+  tri_Lt_apply<double>(L, d, g, gz);
+  for (int i = 0; i < d; ++i) q[i] += 0.5 * eps * gz[i];
+  store_col(S.q, S.B, c, d, q);
+  for (int i = 0; i < d; ++i) gz[i] = eps * q[i];
+  tri_L_apply<double>(L, d, gz, dx);
+  for (int i = 0; i < d; ++i) S.p_theta[i * S.B + c] = S.theta[i * S.B + c] + dx[i];
+}
+
+// after the gradient at the l-th drift position: kick, then either drift again or accept
+__global__ void k_hmc_kick(Chains S, const double* __restrict__ L, uint64_t seed, uint64_t step,
+                           double eps, int last) {
+  const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (c >= S.B) return;
+  const int d = S.d;
+  double q[kMaxD], g[kMaxD], gz[kMaxD], dx[kMaxD];
+  load_col(S.q, S.B, c, d, q);
+  load_col(S.p_grad, S.B, c, d, g);
+  tri_Lt_apply<double>(L, d, g, gz);
+  const double cc = last ? 0.5 * eps : eps;
+  for (int i = 0; i < d; ++i) q[i] += cc * gz[i];
+  if (!last) {
+    store_col(S.q, S.B, c, d, q);
+    for (int i = 0; i < d; ++i) gz[i] = eps * q[i];
+    tri_L_apply<double>(L, d, gz, dx);
+    for (int i = 0; i < d; ++i) S.p_theta[i * S.B + c] += dx[i];
+    return;
+  }
+  double kin = 0.0;
+  for (int i = 0; i < d; ++i) kin += q[i] * q[i];
+  const double H1 = -S.p_logp[c] + 0.5 * kin;
+  const double la = S.h0[c] - H1;
+  S.last_la[c] = la;
+  const uint4 w = philox4x32_10((uint32_t)c, step, 0u, seed);
+  if (accept_rule<double>(u01<double>(w.x), la)) {
+    for (int i = 0; i < d; ++i) {
+      S.theta[i * S.B + c] = S.p_theta[i * S.B + c];
+      S.grad[i * S.B + c] = g[i];
+    }
+    S.logp[c] = S.p_logp[c];
+    S.n_accept[c] += 1ull;
+  }
+}
+
+// ---- AIES stretch move, one half-ensemble (eq 2.13-2.15) ---------------------------------------
+__global__ void k_aies_propose(Chains S, uint64_t seed, uint64_t step, double a, int64_t own0,
+                               int64_t oth0, int64_t half) {
+  const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (r >= half) return;
+  const int64_t i = own0 + r;
+  const uint4 w = philox4x32_10((uint32_t)i, step, 0u, seed);
+  const int64_t j = oth0 + (int64_t)__umulhi(w.z, (uint32_t)half);
+  const double t = u01<double>(w.y) * (a - 1.0) + 1.0;
+  const double z = t * t / a;
+  for (int k = 0; k < S.d; ++k) {
+    const double xi = S.theta[k * S.B + i], xj = S.theta[k * S.B + j];
+    S.p_theta[k * S.B + r] = xj + z * (xi - xj);
+  }
+}
+
+__global__ void k_aies_accept(Chains S, uint64_t seed, uint64_t step, double a, int64_t own0,
+                              int64_t half) {
+  const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (r >= half) return;
+  const int64_t i = own0 + r;
+  const uint4 w = philox4x32_10((uint32_t)i, step, 0u, seed);
+  const double t = u01<double>(w.y) * (a - 1.0) + 1.0;
+  const double z = t * t / a;
+  const double la = (double)(S.d - 1) * log(z) + S.p_logp[r] - S.logp[i];
+  S.last_la[i] = la;
+  if (accept_rule<double>(u01<double>(w.x), la)) {
+    for (int k = 0; k < S.d; ++k) S.theta[k * S.B + i] = S.p_theta[k * S.B + r];
+    S.logp[i] = S.p_logp[r];
+    S.n_accept[i] += 1ull;
+  }
+}
+
+__global__ void k_trace(const double* __restrict__ theta, int64_t B, int d, float* __restrict__ out) {
+  const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (c >= B) return;
+  for (int i = 0; i < d; ++i) out[c * d + i] = (float)theta[i * B + c];
+}
+
+// ---- A9: running covariance, deterministic per-block partial sums ------------------------------
+constexpr int COV_TPB = 256;
+// acc[blk][e]: e = 0 count, 1..d sums of (theta - ref), then d*d sums of products
+__global__ void __launch_bounds__(COV_TPB)
+k_cov_accumulate(const double* __restrict__ theta, int64_t B, int d, const double* __restrict__ ref,
+                 double* __restrict__ acc) {
+  extern __shared__ double xs[];  // [d][COV_TPB]
+  const int64_t c0 = blockIdx.x * (int64_t)COV_TPB;
+  const int64_t c = c0 + threadIdx.x;
+  const int nvalid = (int)((B - c0 < COV_TPB) ? (B - c0) : COV_TPB);
+  for (int i = 0; i < d; ++i)
+    xs[i * COV_TPB + threadIdx.x] = (c < B) ? theta[i * B + c] - ref[i] : 0.0;
+  __syncthreads();
+  const int ne = 1 + d + d * d;
+  double* mine = acc + (size_t)blockIdx.x * ne;
+  for (int e = threadIdx.x; e < ne; e += COV_TPB) {
+    double s = 0.0;
+    if (e == 0) {
+      s = (double)nvalid;
+    } else if (e <= d) {
+      const double* x = xs + (e - 1) * COV_TPB;
+      for (int t = 0; t < nvalid; ++t) s += x[t];
+    } else {
+      const int i = (e - 1 - d) / d, j = (e - 1 - d) % d;
+      const double *x = xs + i * COV_TPB, *y = xs + j * COV_TPB;
+      for (int t = 0; t < nvalid; ++t) s += x[t] * y[t];
+    }
+    mine[e] += s;
+  }
+}
+
+// C = scatter/(n-1), C_ii *= (1+jitter), L = chol(C) with jitter x10 retries; swap L on success.
+__global__ void k_cov_finalize(double* __restrict__ acc, int nblk, int d, double jitter,
+                               double* __restrict__ L, long long* __restrict__ counts) {
+  __shared__ double S[1 + kMaxD + kMaxD * kMaxD];
+  __shared__ double Cm[kMaxD * kMaxD], Lt[kMaxD * kMaxD];
+  const int ne = 1 + d + d * d;
+  for (int e = threadIdx.x; e < ne; e += blockDim.x) {
+    double s = 0.0;
+    for (int b = 0; b < nblk; ++b) { s += acc[(size_t)b * ne + e]; acc[(size_t)b * ne + e] = 0.0; }
+    S[e] = s;
+  }
+  __syncthreads();
+  if (threadIdx.x != 0) return;
+  const double n = S[0];
+  bool ok = false;
+  if (n >= 2.0) {
+    double jit = jitter;
+    for (int attempt = 0; attempt < 6 && !ok; ++attempt) {
+      for (int i = 0; i < d; ++i)
+        for (int j = 0; j < d; ++j) {
+          const double sij = 0.5 * (S[1 + d + i * d + j] + S[1 + d + j * d + i]);
+          Cm[i * d + j] = (sij - S[1 + i] * S[1 + j] / n) / (n - 1.0);
+        }
+      for (int i = 0; i < d; ++i) Cm[i * d + i] *= (1.0 + jit);
+      ok = true;
+      for (int j = 0; j < d && ok; ++j) {
+        double s = Cm[j * d + j];
+        for (int k = 0; k < j; ++k) s -= Lt[j * d + k] * Lt[j * d + k];
+        if (!(s > 0.0)) { ok = false; break; }
+        const double ljj = sqrt(s);
+        Lt[j * d + j] = ljj;
+        for (int i = j + 1; i < d; ++i) {
+          double t = Cm[i * d + j];
+          for (int k = 0; k < j; ++k) t -= Lt[i * d + k] * Lt[j * d + k];
+          Lt[i * d + j] = t / ljj;
+        }
+      }
+      jit *= 10.0;
+    }
+  }
+  if (ok) {
+    for (int i = 0; i < d; ++i)
+      for (int j = 0; j < d; ++j) L[i * d + j] = (j <= i) ? Lt[i * d + j] : 0.0;
+    counts[0] += 1;
+  } else {
+    counts[1] += 1;
+  }
+}
+
+Chains chains_of(best_state* st) {
+  Chains S;
+  S.B = st->B; S.d = st->ctx->d;
+  S.theta = st->theta; S.grad = st->grad; S.logp = st->logp;
+  S.p_theta = st->p_theta; S.p_grad = st->p_grad; S.p_logp = st->p_logp;
+  S.q = st->q; S.h0 = st->h0; S.last_la = st->last_la; S.n_accept = st->n_accept;
+  return S;
+}
+
+int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin, bool adapt,
+               cudaStream_t s) {
+  if (trace && thin > 0 && (t + 1) % thin == 0) {
+    const int64_t slot = (t + 1) / thin - 1;
+    k_trace<<<nblocks(st->B), TPB, 0, s>>>(st->theta, st->B, ctx->d,
+                                           trace + (size_t)slot * st->B * ctx->d);
+    count_launch();
+  }
+  if (adapt && ctx->adapt_every > 0) {
+    const int nblk = (int)((st->B + COV_TPB - 1) / COV_TPB);
+    k_cov_accumulate<<<nblk, COV_TPB, sizeof(double) * ctx->d * COV_TPB, s>>>(
+        st->theta, st->B, ctx->d, ctx->cov_ref, ctx->cov_acc);
+    count_launch();
+    if (++ctx->win_steps >= ctx->adapt_every) {
+      k_cov_finalize<<<1, 256, 0, s>>>(ctx->cov_acc, nblk, ctx->d, ctx->jitter, ctx->L_dev,
+                                       (long long*)ctx->adapt_counts);
+      count_launch();
+      ctx->win_steps = 0;
+    }
+  }
+  return BEST_OK;
+}
+
+}  // namespace
+
+int adapt_reset(best_ctx* ctx, best_state* st, cudaStream_t s) {
+  const int nblk = (int)((st->B + COV_TPB - 1) / COV_TPB);
+  const size_t ne = 1 + ctx->d + (size_t)ctx->d * ctx->d;
+  if (nblk > ctx->cov_blocks) {
+    if (ctx->cov_acc) cudaFree(ctx->cov_acc);
+    ctx->cov_acc = nullptr;
+    BEST_CUDA(cudaMalloc(&ctx->cov_acc, sizeof(double) * ne * nblk));
+    ctx->cov_blocks = nblk;
+  }
+  BEST_CUDA(cudaMemsetAsync(ctx->cov_acc, 0, sizeof(double) * ne * ctx->cov_blocks, s));
+  // shift = chain 0's current position (any fixed reference removes the large mean^2 term)
+  std::vector<double> ref(ctx->d);
+  BEST_CUDA(cudaStreamSynchronize(s));
+  for (int i = 0; i < ctx->d; ++i)
+    BEST_CUDA(cudaMemcpy(&ref[i], st->theta + (size_t)i * st->B, sizeof(double), cudaMemcpyDeviceToHost));
+  BEST_CUDA(cudaMemcpy(ctx->cov_ref, ref.data(), sizeof(double) * ctx->d, cudaMemcpyHostToDevice));
+  ctx->win_steps = 0;
+  return BEST_OK;
+}
+
+int step_mh(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, double eps, float* trace,
+            int thin, cudaStream_t s) {
+  Chains S = chains_of(st);
+  const int nb = nblocks(st->B);
+  for (int64_t t = 0; t < n_steps; ++t) {
+    const uint64_t step = st->step + (uint64_t)t;
+    k_mh_propose<<<nb, TPB, 0, s>>>(S, ctx->L_dev, seed, step, eps);
+    count_launch();
+    BEST_TRY(eval_target_soa(ctx, st->p_theta, st->B, st->B, st->p_logp, nullptr, s));
+    k_mh_accept<<<nb, TPB, 0, s>>>(S, seed, step);
+    count_launch();
+    BEST_TRY(after_step(ctx, st, t, trace, thin, true, s));
+  }
+  BEST_CUDA(cudaGetLastError());
+  return BEST_OK;
+}
+
+int step_mala(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, double eps,
+              float* trace, int thin, cudaStream_t s) {
+  Chains S = chains_of(st);
+  const int nb = nblocks(st->B);
+  for (int64_t t = 0; t < n_steps; ++t) {
+    const uint64_t step = st->step + (uint64_t)t;
+    k_mala_propose<<<nb, TPB, 0, s>>>(S, ctx->L_dev, seed, step, eps);
+    count_launch();
+    BEST_TRY(eval_target_soa(ctx, st->p_theta, st->B, st->B, st->p_logp, st->p_grad, s));
+    k_mala_accept<<<nb, TPB, 0, s>>>(S, ctx->L_dev, seed, step, eps);
+    count_launch();
+    BEST_TRY(after_step(ctx, st, t, trace, thin, true, s));
+  }
+  BEST_CUDA(cudaGetLastError());
+  return BEST_OK;
+}
+
+int step_hmc(best_ctx* ctx, best_state* st, int64_t n_traj, uint64_t seed, double eps, int n_leapfrog,
+             float* trace, int thin, cudaStream_t s) {
+  Chains S = chains_of(st);
+  const int nb = nblocks(st->B);
+  for (int64_t t = 0; t < n_traj; ++t) {
+    const uint64_t step = st->step + (uint64_t)t;
+    k_hmc_begin<<<nb, TPB, 0, s>>>(S, ctx->L_dev, seed, step, eps);
+    count_launch();
+    for (int l = 1; l <= n_leapfrog; ++l) {
+      BEST_TRY(eval_target_soa(ctx, st->p_theta, st->B, st->B, st->p_logp, st->p_grad, s));
+      k_hmc_kick<<<nb, TPB, 0, s>>>(S, ctx->L_dev, seed, step, eps, l == n_leapfrog ? 1 : 0);
+      count_launch();
+    }
+    BEST_TRY(after_step(ctx, st, t, trace, thin, true, s));
+  }
+  BEST_CUDA(cudaGetLastError());
+  return BEST_OK;
+}
+
+int step_aies(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, double a, float* trace,
+              int thin, cudaStream_t s) {
+  Chains S = chains_of(st);
+  const int64_t half = st->B / 2;
+  const int nb = nblocks(half);
+  for (int64_t t = 0; t < n_steps; ++t) {
+    const uint64_t step = st->step + (uint64_t)t;
+    for (int hh = 0; hh < 2; ++hh) {
+      const int64_t own0 = hh == 0 ? 0 : half, oth0 = hh == 0 ? half : 0;
+      k_aies_propose<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, oth0, half);
+      count_launch();
+      BEST_TRY(eval_target_soa(ctx, st->p_theta, st->B, half, st->p_logp, nullptr, s));
+      k_aies_accept<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, half);
+      count_launch();
+    }
+    BEST_TRY(after_step(ctx, st, t, trace, thin, false, s));
+  }
+  BEST_CUDA(cudaGetLastError());
+  return BEST_OK;
+}
+
+}  // namespace best

@@ -1,0 +1,297 @@
+"""GPU parity tests of the exact path (BEST_PREC_FP32) against the oracle, through the C-ABI.
+T1 logp/grad, T2 single-step maps, T3 HMC trajectories, T4 split invariance, T5 moments,
+T6 adaptation, T7 non-finite handling."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2606_04895_b200 import workloads as WL
+from parity_util import TOL, accept_margins, check_logp_grad
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_04895_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import oracle
+    oracle.lib()
+    return oracle
+
+
+def _targets(name):
+    if name == "tiny":
+        return WL.tiny(), 4096
+    if name == "tiny_silu":
+        return WL.tiny(activation=WL.ACT_SILU, hidden=(50, 37)), 1111   # ragged widths and count
+    if name == "lcdm":
+        return WL.lcdm(n_chains=8), 4096
+    if name == "lcdm_s3":
+        return WL.lcdm(n_chains=8, mlp_scale=3.0), 1024
+    if name == "sterile":
+        return WL.sterile(n_chains=8), 1024
+    raise KeyError(name)
+
+
+@pytest.mark.parametrize("name", ["tiny", "tiny_silu", "lcdm", "lcdm_s3", "sterile"])
+@pytest.mark.parametrize("variant", ["full", "mlp_only", "gauss_only"])
+def test_T1_logp_grad(B, O, name, variant):
+    w, n = _targets(name)
+    pts = WL.probe_points(w, n, seed=17)
+    if variant == "mlp_only":
+        w = WL.mlp_only(w)
+    elif variant == "gauss_only":
+        w = WL.gaussian_only(w)
+    ctx = B.Context(w, B.PREC_FP32)
+    lp = np.zeros(n, np.float32)
+    g = np.zeros((n, w.d), np.float32)
+    ctx.logp_grad(pts, n, lp, g)
+    lp_ref, g_ref = O.Oracle(w).logp_grad(pts)
+    check_logp_grad(lp, g, lp_ref, g_ref, TOL[0], f"{name}/{variant}")
+    # forward-only call and device-pointer call agree with the host-pointer call
+    import torch
+    lp2 = np.zeros(n, np.float32)
+    ctx.logp_grad(pts, n, lp2, None)
+    assert np.array_equal(lp, lp2)
+    t_pts = torch.from_numpy(pts).cuda()
+    t_lp = torch.empty(n, device="cuda")
+    t_g = torch.empty(n, w.d, device="cuda")
+    ctx.logp_grad(t_pts, n, t_lp, t_g, stream=torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(t_lp.cpu().numpy(), lp) and np.array_equal(t_g.cpu().numpy(), g)
+    ctx.close()
+
+
+def _single_step(B, O, w, method, seed, **kw):
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(w.theta0)
+    ost = O.Oracle(w).new_state(w.theta0)
+    th0 = ost.theta.copy()
+    getattr(st, "step_" + method)(1, seed, **kw)
+    getattr(ost, "step_" + method)(1, seed, **kw)
+    la = st.last_log_alpha()
+    th, lp, gr = st.get_f64(want_grad=(method in ("mala", "hmc")))
+    acc = st.get(want_grad=False)["n_accept"].astype(np.int64)
+    acc_ref = ost.n_accept.astype(np.int64)
+    m = accept_margins(O, seed, 0, w.n_chains, ost.last_log_alpha)
+    mism = acc != acc_ref
+    info = dict(n=w.n_chains, mismatches=int(mism.sum()),
+                max_margin_of_mismatch=float(m[mism].max()) if mism.any() else 0.0,
+                max_dla=float(np.nanmax(np.abs(la - ost.last_log_alpha))),
+                accept_rate=float(acc_ref.mean()))
+    print(f"[T2] {w.name}/{method}: {info}")
+    # accept bits identical outside the logged margin set |log u − log α| < 1e-6 (north_star)
+    assert not (mism & (m >= 1e-6)).any(), info
+    same = ~mism
+    # post-state: accepted chains carry the proposal (rel 1e-6 of the step scale), others unchanged
+    scale = np.abs(ost.theta).max(axis=0)
+    assert (np.abs(th[same] - ost.theta[same]) <= 1e-6 * scale + 1e-9).all()
+    rej = same & (acc_ref == 0)
+    assert np.array_equal(th[rej], th0[rej])
+    assert np.abs(lp[same] - ost.logp[same]).max() <= TOL[0] * np.abs(ost.logp).max()
+    if gr is not None:
+        num = np.linalg.norm(gr[same] - ost.grad[same], axis=1)
+        assert (num <= TOL[0] * np.linalg.norm(ost.grad[same], axis=1)).all()
+    st.close()
+    ctx.close()
+    return info
+
+
+@pytest.mark.parametrize("method,kw", [("mh", dict(eps=0.3)), ("mala", dict(eps=0.3)), ("aies", dict(a=2.0))])
+def test_T2_single_step_tiny_64k(B, O, method, kw):
+    w = WL.tiny().with_chains(65536, seed=5)
+    _single_step(B, O, w, method, seed=1234, **kw)
+
+
+@pytest.mark.parametrize("method,kw", [("mh", dict(eps=0.3)), ("mala", dict(eps=0.3))])
+def test_T2_single_step_lcdm(B, O, method, kw):
+    w = WL.lcdm(n_chains=2048)
+    _single_step(B, O, w, method, seed=77, **kw)
+
+
+def test_T2_single_step_sterile_aies_and_mala(B, O):
+    w = WL.sterile(n_chains=1024)
+    _single_step(B, O, w, "aies", seed=9, a=2.0)
+    _single_step(B, O, w, "mala", seed=9, eps=0.01)
+
+
+@pytest.mark.parametrize("nl", [1, 8, 16])
+def test_T3_hmc_trajectory(B, O, nl):
+    w = WL.tiny().with_chains(4096, seed=6)
+    _single_step(B, O, w, "hmc", seed=31, eps=0.2, n_leapfrog=nl)
+    if nl == 16:
+        w = WL.lcdm(n_chains=512, mlp_scale=3.0)
+        _single_step(B, O, w, "hmc", seed=32, eps=0.1, n_leapfrog=16)
+
+
+def test_T4_split_invariance(B):
+    import torch
+    w = WL.tiny().with_chains(300, seed=8)
+    ctx = B.Context(w, B.PREC_FP32)
+    a, b = ctx.new_state(w.theta0), ctx.new_state(w.theta0)
+    tr = torch.zeros(3, 300, w.d, device="cuda")
+    a.step_mala(60, 3, 0.3, trace=tr, thin=20)
+    for _ in range(6):
+        b.step_mala(10, 3, 0.3)
+    ga, gb = a.get(), b.get()
+    for k in ("theta", "logp", "grad", "n_accept"):
+        assert np.array_equal(ga[k], gb[k]), k
+    assert ga["step"] == gb["step"] == 60 and ga["n_evals"] == gb["n_evals"] == 300 * 61
+    torch.cuda.synchronize()
+    assert np.array_equal(tr[-1].cpu().numpy(), ga["theta"])
+    for meth, kw in (("mh", dict(eps=0.3)), ("hmc", dict(eps=0.2, n_leapfrog=5)), ("aies", dict(a=2.0))):
+        a, b = ctx.new_state(w.theta0), ctx.new_state(w.theta0)
+        getattr(a, "step_" + meth)(12, 3, **kw)
+        getattr(b, "step_" + meth)(5, 3, **kw)
+        getattr(b, "step_" + meth)(7, 3, **kw)
+        assert np.array_equal(a.get()["theta"], b.get()["theta"]), meth
+    ctx.close()
+
+
+def _moments_vs_exact(trace, mu, Sigma, nsig=4.0):
+    T, Bn, d = trace.shape
+    m_c = trace.mean(axis=0)
+    se = m_c.std(axis=0, ddof=1) / math.sqrt(Bn)
+    assert np.all(np.abs(m_c.mean(axis=0) - mu) < nsig * se)
+    xc = trace - mu
+    for i in range(d):
+        for j in range(i, d):
+            p = (xc[:, :, i] * xc[:, :, j]).mean(axis=0)
+            assert abs(p.mean() - Sigma[i, j]) < nsig * p.std(ddof=1) / math.sqrt(Bn), (i, j)
+
+
+@pytest.mark.parametrize("method", ["mh", "mala", "hmc", "aies"])
+@pytest.mark.parametrize("d", [6, 27])
+def test_T5_gaussian_closed_form_moments(B, method, d):
+    import torch
+    if method == "aies" and d == 27:
+        pytest.skip("AIES moment parity is tested at small d (slow mixing at d=27, SURVEY §8(c))")
+    w = WL.gaussian(d, 512, seed=40 + d, cond=100.0 if d == 6 else 1e4)
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(w.theta0)
+    plan = {"mh": (dict(eps=2.4 / math.sqrt(d)), 400, 2400, 4), "mala": (dict(eps=0.5 if d == 6 else 0.3), 100, 800, 2),
+            "hmc": (dict(eps=0.4 if d == 6 else 0.25, n_leapfrog=4), 30, 300, 1), "aies": (dict(a=2.0), 400, 3000, 5)}
+    kw, burn, n, thin = plan[method]
+    getattr(st, "step_" + method)(burn, 11, **kw)
+    tr = torch.zeros(n // thin, 512, d, device="cuda")
+    getattr(st, "step_" + method)(n, 11, trace=tr, thin=thin, **kw)
+    torch.cuda.synchronize()
+    trace = tr.cpu().numpy().astype(np.float64)
+    if method == "aies":       # walkers are coupled: batch means over time
+        xc = (trace - w.mu) / np.sqrt(np.diag(w.Sigma))
+        v = (xc ** 2).mean(axis=1).reshape(30, -1, d).mean(axis=1)
+        se = v.std(axis=0, ddof=1) / math.sqrt(30)
+        assert np.all(np.abs(v.mean(axis=0) - 1.0) < 4 * se + 0.01)
+    else:
+        _moments_vs_exact(trace, w.mu, w.Sigma)
+    rate = st.get(want_grad=False)["n_accept"].mean() / (burn + n)
+    print(f"[T5] {method} d={d}: acceptance {rate:.3f}")
+    assert 0.1 < rate <= 1.0
+    ctx.close()
+
+
+def test_T5_tiny_moments_gpu_vs_oracle(B, O):
+    """tiny config, MALA: GPU long-run moments vs the oracle's (4 MC standard errors of the difference)."""
+    import torch
+    w = WL.tiny().with_chains(256, seed=12)
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(w.theta0)
+    ost = O.Oracle(w).new_state(w.theta0)
+    st.step_mala(100, 5, 0.3)
+    ost.step_mala(100, 6, 0.3)          # different seed: independent runs
+    tr = torch.zeros(500, 256, w.d, device="cuda")
+    st.step_mala(500, 5, 0.3, trace=tr, thin=1)
+    otr = ost.step_mala(500, 6, 0.3, thin=1)
+    torch.cuda.synchronize()
+    a, b = tr.cpu().numpy().astype(np.float64).mean(axis=0), otr.mean(axis=0)
+    se = np.sqrt(a.var(axis=0, ddof=1) / 256 + b.var(axis=0, ddof=1) / 256)
+    assert np.all(np.abs(a.mean(axis=0) - b.mean(axis=0)) < 4 * se)
+    ra = st.get(want_grad=False)["n_accept"].mean() / 600
+    assert abs(ra - ost.n_accept.mean() / 600) < 0.02
+    ctx.close()
+
+
+def test_T6_adaptation(B, O):
+    """L after each window vs the oracle's covariance/Cholesky of the GPU's own trace (rel 1e-6)."""
+    import torch
+    w = WL.sterile(n_chains=1024, hidden=64, n_hidden=2)
+    w.L = np.diag(np.sqrt(np.diag(w.Sigma)))
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(w.theta0)
+    st.set_adaptation(100, 1e-6)
+    o = O.Oracle(w)
+    for win in range(3):
+        tr = torch.zeros(100, 1024, w.d, device="cuda")
+        st.step_mh(100, 21, 0.3, trace=tr, thin=1)
+        torch.cuda.synchronize()
+        Lg = ctx.get_whitening()
+        # the trace is fp32-rounded θ; the GPU accumulates fp64 θ ⇒ compare at fp32-trace accuracy
+        rc, _, Lo = o.cov_chol(tr.cpu().numpy().astype(np.float64).reshape(-1, w.d), 1e-6)
+        assert rc == 0
+        scale = np.sqrt(np.outer(np.diag(Lo @ Lo.T), np.ones(w.d)))
+        assert np.abs(Lg - Lo).max() / scale.max() < 1e-6, win
+        assert np.allclose(np.triu(Lg, 1), 0.0)
+    assert ctx.adapt_stats() == (3, 0)
+    st.set_adaptation(0)
+    ctx.close()
+
+
+def test_T6_adaptation_matches_oracle_driver(B, O):
+    """Same seeds, same windows: GPU whitening after 2 windows tracks the oracle's own adaptive run."""
+    w = WL.gaussian(5, 256, seed=81)
+    w.L = np.diag(np.sqrt(np.diag(w.Sigma)))
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(w.theta0)
+    st.set_adaptation(50, 1e-6)
+    o = O.Oracle(w)
+    o.set_adaptation(50, 1e-6)
+    ost = o.new_state(w.theta0)
+    st.step_mala(100, 4, 0.4)
+    ost.step_mala(100, 4, 0.4)
+    np.testing.assert_allclose(ctx.get_whitening(), o.get_whitening(), rtol=1e-9, atol=1e-11)
+    th, _, _ = st.get_f64(want_grad=False)
+    np.testing.assert_allclose(th, ost.theta, rtol=1e-9, atol=1e-9)
+    ctx.close()
+
+
+def test_T7_nonfinite_and_far_outside(B):
+    w = WL.lcdm(n_chains=256, hidden=64, n_hidden=2, mlp_scale=3.0)
+    th0 = w.theta0.copy()
+    th0[:128] += 1e6 * (w.hi - w.lo).astype(np.float32)        # far outside the box: huge penalty slope
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(th0)
+    before = st.get()
+    st.step_hmc(2, 5, 50.0, 8)                                  # absurd ε ⇒ divergent trajectories
+    after = st.get()
+    assert np.isfinite(after["theta"]).all() and np.isfinite(after["logp"]).all()
+    rejected = after["n_accept"] == 0
+    assert rejected.sum() >= 200
+    assert np.array_equal(after["theta"][rejected], before["theta"][rejected])
+    ctx.close()
+
+
+def test_argument_errors(B):
+    w = WL.tiny().with_chains(7, seed=1)
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(w.theta0)
+    for call in (lambda: st.step_aies(1, 1, 2.0), lambda: st.step_mh(1, 1, 0.0), lambda: st.step_mala(1, 1, -1.0),
+                 lambda: st.step_hmc(1, 1, 0.1, 0)):
+        with pytest.raises(B.BestError) as e:
+            call()
+        assert e.value.code == B.BEST_ERR_ARG
+    st2 = ctx.new_state(w.theta0[:6])
+    with pytest.raises(B.BestError):
+        st2.step_aies(1, 1, 1.0)
+    st2.step_aies(2, 1, 2.0)
+    st.step_mh(0, 1, 0.3)                                        # empty call is a no-op
+    assert st.get()["step"] == 0
+    lp = np.zeros(0, np.float32)
+    ctx.logp_grad(np.zeros((0, w.d), np.float32), 0, lp, None)   # empty batch
+    ctx.close()
