@@ -193,7 +193,7 @@ __global__ void k_trace(const double* __restrict__ theta, int64_t B, int d, floa
 }
 
 // ---- A9: running covariance, deterministic per-block partial sums ------------------------------
-constexpr int COV_TPB = 256;
+constexpr int COV_TPB = 128;  // d*COV_TPB doubles of dynamic smem: 32 KB at d = 32
 // acc[blk][e]: e = 0 count, 1..d sums of (theta - ref), then d*d sums of products
 __global__ void __launch_bounds__(COV_TPB)
 k_cov_accumulate(const double* __restrict__ theta, int64_t B, int d, const double* __restrict__ ref,

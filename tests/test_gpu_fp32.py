@@ -69,7 +69,13 @@ def test_T1_logp_grad(B, O, name, variant):
     ctx.close()
 
 
+def f32(x):
+    """The C-ABI takes ε and a as float: hand the oracle the very same value."""
+    return float(np.float32(x))
+
+
 def _single_step(B, O, w, method, seed, **kw):
+    kw = {k: (f32(v) if isinstance(v, float) else v) for k, v in kw.items()}
     ctx = B.Context(w, B.PREC_FP32)
     st = ctx.new_state(w.theta0)
     ost = O.Oracle(w).new_state(w.theta0)
@@ -205,10 +211,10 @@ def test_T5_tiny_moments_gpu_vs_oracle(B, O):
     st = ctx.new_state(w.theta0)
     ost = O.Oracle(w).new_state(w.theta0)
     st.step_mala(100, 5, 0.3)
-    ost.step_mala(100, 6, 0.3)          # different seed: independent runs
+    ost.step_mala(100, 6, f32(0.3))     # different seed: independent runs
     tr = torch.zeros(500, 256, w.d, device="cuda")
     st.step_mala(500, 5, 0.3, trace=tr, thin=1)
-    otr = ost.step_mala(500, 6, 0.3, thin=1)
+    otr = ost.step_mala(500, 6, f32(0.3), thin=1)
     torch.cuda.synchronize()
     a, b = tr.cpu().numpy().astype(np.float64).mean(axis=0), otr.mean(axis=0)
     se = np.sqrt(a.var(axis=0, ddof=1) / 256 + b.var(axis=0, ddof=1) / 256)
@@ -254,7 +260,7 @@ def test_T6_adaptation_matches_oracle_driver(B, O):
     o.set_adaptation(50, 1e-6)
     ost = o.new_state(w.theta0)
     st.step_mala(100, 4, 0.4)
-    ost.step_mala(100, 4, 0.4)
+    ost.step_mala(100, 4, f32(0.4))
     np.testing.assert_allclose(ctx.get_whitening(), o.get_whitening(), rtol=1e-9, atol=1e-11)
     th, _, _ = st.get_f64(want_grad=False)
     np.testing.assert_allclose(th, ost.theta, rtol=1e-9, atol=1e-9)
