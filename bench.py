@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the B200 hot path on BASELINE.json's workloads.
+
+One "step" = one best_step_* call advancing ALL chains by `inner` sampler steps (one persistent
+kernel launch on the bf16 path).  `value` = whole-job chain-steps/s with the state resident in
+HBM; `e2e` = the same metric through the C-ABI with HOST buffers (best_state_set from host memory,
+best_step_*, best_state_get to host memory inside the timed region).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload lcdm_mala|hmc|aies|sweep_*]
+                  [--precision bf16|fp32] [--impl ours|reference]
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+WORKLOADS = {
+    # name: (maker kwargs, method, sampler kwargs, inner steps per bench step, config index)
+    "lcdm_mala": dict(cfg=1, make="lcdm", n_chains=4096, mlp_scale=1.0, method="mala", eps=0.3, inner=100),
+    "hmc": dict(cfg=2, make="lcdm", n_chains=16384, mlp_scale=3.0, method="hmc", eps=0.1, n_leapfrog=16, inner=8),
+    "lcdm_mala_16k": dict(cfg=1, make="lcdm", n_chains=16384, mlp_scale=1.0, method="mala", eps=0.3, inner=100),
+    "lcdm_mh_16k": dict(cfg=1, make="lcdm", n_chains=16384, mlp_scale=1.0, method="mh", eps=0.3, inner=100),
+    "tiny_mala": dict(cfg=0, make="tiny", n_chains=64, mlp_scale=0.1, method="mala", eps=0.3, inner=100),
+}
+
+
+def make_workload(spec, n_chains=None):
+    from paper_2606_04895_b200 import workloads as WL
+    n = n_chains or spec["n_chains"]
+    if spec["make"] == "lcdm":
+        return WL.lcdm(n_chains=n, mlp_scale=spec["mlp_scale"])
+    if spec["make"] == "tiny":
+        return WL.tiny(n_chains=n)
+    if spec["make"] == "sterile":
+        return WL.sterile(n_chains=n)
+    raise KeyError(spec["make"])
+
+
+def evals_per_chain_step(spec):
+    return spec.get("n_leapfrog", 1) if spec["method"] == "hmc" else 1
+
+
+def flops_per_chain_step(w, spec):
+    per_eval = (4 if spec["method"] in ("mala", "hmc") else 2) * w.macs   # fwd 2·MACs, +bwd 2·MACs
+    return per_eval * evals_per_chain_step(spec)
+
+
+def run_steps(st, spec, n, seed, stream=0):
+    m = spec["method"]
+    if m == "mala":
+        st.step_mala(n, seed, spec["eps"], stream=stream)
+    elif m == "mh":
+        st.step_mh(n, seed, spec["eps"], stream=stream)
+    elif m == "hmc":
+        st.step_hmc(n, seed, spec["eps"], spec["n_leapfrog"], stream=stream)
+    else:
+        st.step_aies(n, seed, spec.get("a", 2.0), stream=stream)
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons while the timed region runs (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_evt = index, [], threading.Event()
+
+    def run(self):
+        while not self._stop_evt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([x.strip() for x in out.strip().split(",")])
+            except Exception:
+                pass
+            self._stop_evt.wait(0.1)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=6)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 6 for i in range(4) if r[2 + i] == "Active"})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def cpu_baseline(spec, budget_s=12.0):
+    """The oracle as it stands, timed on the host cores on a bounded sample of the same workload."""
+    from oracle import oracle as O
+    n_sample = 256 if spec["make"] != "tiny" else 64
+    w = make_workload(spec, n_sample)
+    o = O.Oracle(w)
+    ost = o.new_state(w.theta0)
+    steps_done, t0 = 0, time.perf_counter()
+    chunk = 1 if spec["method"] == "hmc" else 2
+    while True:
+        m = spec["method"]
+        if m == "mala":
+            ost.step_mala(chunk, 1, float(np.float32(spec["eps"])))
+        elif m == "mh":
+            ost.step_mh(chunk, 1, float(np.float32(spec["eps"])))
+        elif m == "hmc":
+            ost.step_hmc(chunk, 1, float(np.float32(spec["eps"])), spec["n_leapfrog"])
+        else:
+            ost.step_aies(chunk, 1, spec.get("a", 2.0))
+        steps_done += chunk
+        el = time.perf_counter() - t0
+        if el > budget_s:
+            break
+    return {"value": n_sample * steps_done / el, "unit": "chain-steps/s", "cores": O.num_threads(),
+            "kind": "oracle", "sample": f"{n_sample} chains x {steps_done} {spec['method']} steps "
+                                        f"({el:.1f} s, OpenMP over chains, fp64 scalar loops)"}
+
+
+def reference_arm(args, spec):
+    """--impl reference: the oracle on the host cores; each step = a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    n_sample = 64
+    inner = 1
+    w = make_workload(spec, n_sample)
+    o = O.Oracle(w)
+    ost = o.new_state(w.theta0)
+
+    def one():
+        m = spec["method"]
+        eps = float(np.float32(spec.get("eps", 0.0)))
+        if m == "mala":
+            ost.step_mala(inner, 1, eps)
+        elif m == "mh":
+            ost.step_mh(inner, 1, eps)
+        elif m == "hmc":
+            ost.step_hmc(inner, 1, eps, spec["n_leapfrog"])
+        else:
+            ost.step_aies(inner, 1, spec.get("a", 2.0))
+
+    for _ in range(args.warmup):
+        one()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        one()
+    el = time.perf_counter() - t0
+    val = n_sample * inner * args.steps / el
+    sample = f"{n_sample} chains x {inner} {spec['method']} step per bench step (oracle, fp64, {O.num_threads()} threads)"
+    line = {"impl": "reference", "metric": "chain-steps/s", "value": val, "unit": "chain-steps/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": "chain-steps/s", "cores": O.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": val, "unit": "chain-steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="lcdm_mala", choices=sorted(WORKLOADS))
+    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp32"])
+    ap.add_argument("--inner", type=int, default=0, help="sampler steps per bench step (0 = workload default)")
+    ap.add_argument("--chains", type=int, default=0, help="override the number of chains per GPU")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true")
+    args = ap.parse_args()
+    spec = dict(WORKLOADS[args.workload])
+    if args.inner:
+        spec["inner"] = args.inner
+    if args.chains:
+        spec["n_chains"] = args.chains
+    if args.impl == "reference":
+        reference_arm(args, spec)
+        return
+
+    import torch
+    import __graft_entry__ as entry
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if rank == 0:
+        entry.build()
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist.barrier()
+    from paper_2606_04895_b200 import binding as B
+    B.lib()
+    prec = B.PREC_BF16 if args.precision == "bf16" else B.PREC_FP32
+
+    def barrier():
+        if world > 1:
+            torch.distributed.barrier()
+        torch.cuda.synchronize()
+
+    def measure(spec, steps, warmup, with_e2e):
+        """returns dict(ms_per_step(max over ranks), launches, clocks, e2e…) for this rank's shard."""
+        w = make_workload(spec)
+        if world > 1:   # weak scaling: every rank advances its own n_chains chains (seeded by rank)
+            w = w.with_chains(spec["n_chains"], seed=1000 + rank)
+        ctx = B.Context(w, prec)
+        st = ctx.new_state(w.theta0)
+        stream = torch.cuda.current_stream().cuda_stream
+        flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+        inner = spec["inner"]
+        for i in range(warmup):
+            run_steps(st, spec, inner, 7, stream)
+        barrier()
+        clocks = ClockSampler(local_rank)
+        clocks.start()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        l0 = B.launch_count()
+        t_wall = time.perf_counter()
+        for i in range(steps):
+            flush.fill_(i & 0xFF)                      # L2 flush between timed iterations (untimed)
+            ev[i][0].record()
+            run_steps(st, spec, inner, 7, stream)
+            ev[i][1].record()
+        barrier()
+        t_wall = time.perf_counter() - t_wall
+        launches = B.launch_count() - l0
+        ck = clocks.stop()
+        dev_ms = sum(a.elapsed_time(b) for a, b in ev)
+        t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
+        if world > 1:
+            torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+        dev_ms = float(t.item())
+        acc = st.get(want_grad=False)
+        res = dict(w=w, ms_total=dev_ms, launches=int(launches), clocks=ck, wall_s=t_wall,
+                   accept_rate=float(acc["n_accept"].mean() / max(acc["step"], 1)))
+        if with_e2e:
+            host_theta = torch.from_numpy(w.theta0).pin_memory()
+            out_theta = np.zeros_like(w.theta0)
+            out_logp = np.zeros(w.n_chains, np.float32)
+            import ctypes as C
+            lib = B.lib()
+            n_e2e = max(3, steps // 4)
+
+            def e2e_once():
+                st.set(host_theta, step=0)                       # H2D of θ (+ logp/grad refresh on device)
+                run_steps(st, spec, inner, 7, stream)
+                rc = lib.best_state_get(st._h, out_theta.ctypes.data, out_logp.ctypes.data, None, None, None,
+                                        None, None)              # D2H of θ, logp (synchronises)
+                assert rc == 0
+            e2e_once()
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(n_e2e):
+                e2e_once()
+            barrier()
+            el = time.perf_counter() - t0
+            t = torch.tensor([el], dtype=torch.float64, device="cuda")
+            if world > 1:
+                torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
+            res["e2e_s_per_step"] = float(t.item()) / n_e2e
+            res["h2d"] = int(w.theta0.nbytes)
+            res["d2h"] = int(out_theta.nbytes + out_logp.nbytes)
+        st.close()
+        ctx.close()
+        del flush
+        return res
+
+    r = measure(spec, args.steps, args.warmup, with_e2e=True)
+    w = r["w"]
+    Btot = spec["n_chains"] * world
+    inner = spec["inner"]
+    ms_per_step = r["ms_total"] / args.steps
+    value = Btot * inner / (ms_per_step * 1e-3)
+    peaks = {}
+    pk_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(pk_path):
+        peaks = json.load(open(pk_path))
+    peak_tf = peaks.get("bf16_tflops", 1590.0)
+    peak_src = "MEASURED_PEAKS.json bf16_tflops (burst), of measured" if peaks else "1590 TF fallback, of fallback"
+    flops_per_launch = flops_per_chain_step(w, spec) * spec["n_chains"] * inner
+    achieved_tf = flops_per_launch / (ms_per_step * 1e-3) / 1e12
+    if args.precision == "fp32":
+        peak_tf, peak_src = 148 * 128 * 2 * 1.965e9 / 1e12, "FP32 FFMA peak 148 SM x 128 lanes x 2 x 1.965 GHz (derived)"
+    line = {
+        "metric": "chain-steps/s", "value": value, "unit": "chain-steps/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": args.precision, "data": "synthetic",
+        "config": {"workload": f"{args.workload} (BASELINE configs[{spec['cfg']}]): d={w.d}, MLP "
+                               + "x".join(map(str, w.widths)) + f", {spec['n_chains']} chains/GPU, {spec['method']}",
+                   "sampler_steps_per_step": inner, "method": spec["method"],
+                   "n_leapfrog": spec.get("n_leapfrog"), "eps": spec.get("eps"),
+                   "l2": "flushed (256 MB write) between timed iterations", "precision": args.precision},
+        "grad_evals_per_s": value * evals_per_chain_step(spec),
+        "accept_rate": r["accept_rate"],
+        "clocks": r["clocks"],
+        "gpu_launches": r["launches"],
+        "e2e": {"value": Btot * inner / r["e2e_s_per_step"], "unit": "chain-steps/s",
+                "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"]},
+        "roofline": {"bound": "tensor" if args.precision == "bf16" else "alu", "achieved": achieved_tf,
+                     "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": None,
+                     "peak_source": peak_src,
+                     "frac_of_sustained": (achieved_tf / peaks["bf16_tflops_sustained"]) if peaks and args.precision == "bf16" else None,
+                     "kernel": "best_tc_kernel<%s>" % spec["method"], "flops_per_launch": flops_per_launch},
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(spec)
+    if world == 1 and not args.no_extra and args.workload == "lcdm_mala":
+        extra = {}
+        for name in ("hmc", "lcdm_mala_16k", "lcdm_mh_16k"):
+            sp = dict(WORKLOADS[name])
+            rr = measure(sp, max(3, args.steps // 4), 3, with_e2e=False)
+            ms = rr["ms_total"] / max(3, args.steps // 4)
+            v = sp["n_chains"] * sp["inner"] / (ms * 1e-3)
+            tf = flops_per_chain_step(rr["w"], sp) * v / 1e12
+            extra[name] = {"chain_steps_per_s": v, "grad_evals_per_s": v * evals_per_chain_step(sp),
+                           "tflops": tf, "frac_of_peak": tf / peak_tf, "ms_per_step": ms,
+                           "accept_rate": rr["accept_rate"], "inner": sp["inner"]}
+        line["extra"] = extra
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        torch.distributed.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -131,6 +131,8 @@ int step_mala(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cu
 int step_hmc(best_ctx*, best_state*, int64_t, uint64_t, double, int, float*, int, cudaStream_t);
 int step_aies(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cudaStream_t);
 int adapt_reset(best_ctx* ctx, best_state* st, cudaStream_t s);
+// after step index t of a call: trace slot (every `thin` steps) and covariance accumulation / update
+int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin, bool adapt, cudaStream_t s);
 
 // layout helpers (samplers.cu)
 int rows_f32_to_soa_f64(const float* rows_dev, double* soa, int64_t n, int d, int64_t ld, cudaStream_t s);

@@ -281,6 +281,8 @@ Chains chains_of(best_state* st) {
   return S;
 }
 
+}  // namespace
+
 int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin, bool adapt,
                cudaStream_t s) {
   if (trace && thin > 0 && (t + 1) % thin == 0) {
@@ -303,8 +305,6 @@ int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin,
   }
   return BEST_OK;
 }
-
-}  // namespace
 
 int adapt_reset(best_ctx* ctx, best_state* st, cudaStream_t s) {
   const int nblk = (int)((st->B + COV_TPB - 1) / COV_TPB);

@@ -1,15 +1,184 @@
-// bf16 tensor-core path — placeholder until the tcgen05 kernel lands (next commit).
+// bf16 tensor-core path (BEST_PREC_BF16): ONE persistent kernel per best_step_* call.
+//
+// A CTA owns a tile of 128 chains for all n_steps.  TMEM lane r == chain r == epilogue thread r:
+//   warp 0 (1 lane)  weight producer: streams pre-swizzled bf16 weight tiles L2 -> SMEM ring with
+//                    cp.async.bulk + mbarrier complete_tx (weights are packed once at best_create)
+//   warp 1 (1 lane)  MMA issuer: tcgen05.mma.cta_group::1.kind::f16, M=128, N<=256, K=16;
+//                    A = activations resident in SMEM (128B swizzle, written in place by the
+//                    epilogue), B = weight stage (64B swizzle), D = fp32 in TMEM (2 x 256 columns)
+//   warp 2           TMEM allocation
+//   warps 4-7        one thread per chain: Philox, whitened proposal, tcgen05.ld epilogues
+//                    (bias + activation + act' / delta), Gaussian / banana / box terms, accept.
+// The MLP forward and its input-gradient backprop (A1b, A1c) are a chain of GEMMs whose
+// activations never leave the SM; only act' (bf16) is parked in an L2-resident scratch between
+// the forward and backward sweeps.  See DESIGN.md §"tensor-core kernel".
+#include <cstring>
+
+#include "device_math.cuh"
 #include "tc_fused.h"
+#include "tc_ptx.cuh"
 
 namespace best {
-int tc_plan_create(best_ctx*, const best_config*) {
-  set_error("BEST_PREC_BF16: tensor-core path not built yet");
-  return BEST_ERR_UNSUPPORTED;
+
+namespace tc {
+
+constexpr int kRows = 128;           // chains per CTA == TMEM lanes
+constexpr int kAChunkBytes = 16384;  // A k-chunk: 128 rows x 64 bf16 (128 B rows, SW128)
+constexpr int kMaxKch = 8;           // hidden width <= 512
+constexpr int kStageBytes = 16384;   // weight stage: <=256 rows x 32 bf16 (64 B rows, SW64)
+constexpr int kStages = 4;
+constexpr int kMaxOps = 12;
+constexpr int kThreads = 256;
+constexpr int kDP = 32;              // parameter vectors are padded to 32 inside the kernel
+
+enum { EPI_FWD_HID = 0, EPI_FWD_LAST = 1, EPI_BWD_HID = 2, EPI_BWD_FINAL = 3 };
+enum { M_MH = 0, M_MALA = 1, M_HMC = 2, M_AIES = 3, M_EVAL = 4 };
+enum { IO_ROWS_F32 = 0, IO_SOA_F64 = 1 };
+
+struct OpDesc {
+  int kch;    // 64-wide k-chunks of the A operand
+  int nch;    // n-chunks (each one TMEM buffer)
+  int ncols;  // columns per n-chunk (MMA N)
+  int epi;
+  int layer;  // FWD: hidden layer index (0-based) whose bias/act is applied; BWD_HID: layer whose act' multiplies
+};
+
+struct Params {
+  int d, H, n_hidden, act;
+  float mlp_scale, b_out;
+  int n_ops_fwd, n_ops_all;
+  OpDesc ops[kMaxOps];
+  const uint8_t* wpack;   // packed tiles: forward ops then backward ops, consumption order
+  const float* bias;      // [n_hidden][H]
+  const float* w_out;     // [H]
+  uint16_t* dact;         // scratch: per tile [n_hidden-1][H/64][8 pieces][128 rows][8] bf16
+  size_t dact_tile_elems;
+  // target terms (fp64 masters on device, converted to fp32 in SMEM at kernel start)
+  int has_gauss, has_box, banana_i, banana_j;
+  float banana_sigma, pen_kappa, pen_gamma;
+  const double *mu, *R, *lo, *hi, *L;
+};
+
+struct Run {
+  int method, want_grad, io_mode;
+  int64_t B;            // chains (or points) covered by this launch
+  int64_t ld;           // leading dimension of the SoA state arrays
+  int64_t n_steps;
+  uint64_t step0, seed;
+  float eps;            // MH/MALA/HMC step size; AIES: a
+  int n_leapfrog;
+  // state (fp64 SoA [d][ld])
+  double *theta, *grad, *logp, *last_la;
+  unsigned long long* n_accept;
+  // EVAL i/o
+  const float* in_rows; float* out_logp; float* out_grad;
+  // AIES
+  int64_t own0, oth0;
+};
+
+// shared-memory carve-up (dynamic, 1024-byte aligned base)
+struct SmemLayout {
+  static constexpr int A = 0;
+  static constexpr int STAGES = A + kMaxKch * kAChunkBytes;          // 131072
+  static constexpr int BIAS = STAGES + kStages * kStageBytes;        // 196608, 2048 floats
+  static constexpr int WOUT = BIAS + 2048 * 4;                       // 512 floats
+  static constexpr int WOUTS = WOUT + 512 * 4;                       // 512 floats (s * w_out)
+  static constexpr int LMAT = WOUTS + 512 * 4;                       // 32x32 floats
+  static constexpr int RMAT = LMAT + 1024 * 4;
+  static constexpr int VECS = RMAT + 1024 * 4;                       // mu, lo, hi, 1/width: 4x32 floats
+  static constexpr int BARS = VECS + 4 * 32 * 4;
+  // barriers: full[4] empty[4] a_ready[8] a_free[8] d_full[2] d_free[2]
+  static constexpr int NBARS = 2 * kStages + 2 * kMaxKch + 4;
+  static constexpr int TMEMPTR = BARS + NBARS * 8;
+  static constexpr int TOTAL = TMEMPTR + 16;
+};
+static_assert(SmemLayout::TOTAL + 1024 <= 227 * 1024, "shared memory budget");
+
+struct Bars {
+  uint32_t full[kStages], empty[kStages], a_ready[kMaxKch], a_free[kMaxKch], d_full[2], d_free[2];
+};
+
+__device__ __forceinline__ Bars make_bars(uint32_t base) {
+  Bars b;
+  uint32_t p = base;
+  for (int i = 0; i < kStages; ++i) { b.full[i] = p; p += 8; }
+  for (int i = 0; i < kStages; ++i) { b.empty[i] = p; p += 8; }
+  for (int i = 0; i < kMaxKch; ++i) { b.a_ready[i] = p; p += 8; }
+  for (int i = 0; i < kMaxKch; ++i) { b.a_free[i] = p; p += 8; }
+  for (int i = 0; i < 2; ++i) { b.d_full[i] = p; p += 8; }
+  for (int i = 0; i < 2; ++i) { b.d_free[i] = p; p += 8; }
+  return b;
 }
-void tc_plan_destroy(best_ctx*) {}
-int tc_logp_grad(best_ctx*, const float*, int64_t, float*, float*, cudaStream_t) { return BEST_ERR_UNSUPPORTED; }
-int tc_state_init(best_ctx*, best_state*, cudaStream_t) { return BEST_ERR_UNSUPPORTED; }
-int tc_step(best_ctx*, best_state*, int, int64_t, uint64_t, float, int, float*, int, cudaStream_t) {
-  return BEST_ERR_UNSUPPORTED;
+
+// ------------------------------------------------------------------------------------------------
+// weight producer (one thread)
+// ------------------------------------------------------------------------------------------------
+__device__ void producer_loop(const Params& P, const Bars& bars, uint32_t stage_base, int64_t n_evals,
+                              int n_ops) {
+  uint32_t t = 0;  // running tile counter: stage = t % kStages, use = t / kStages
+  for (int64_t e = 0; e < n_evals; ++e) {
+    const uint8_t* src = P.wpack;
+    for (int oi = 0; oi < n_ops; ++oi) {
+      const OpDesc op = P.ops[oi];
+      const uint32_t bytes = (uint32_t)op.ncols * 64u;
+      const int ntiles = op.nch * op.kch * 2;
+      for (int i = 0; i < ntiles; ++i, ++t) {
+        const uint32_t s = t % kStages, use = t / kStages;
+        ptx::mbar_wait(bars.empty[s], (use & 1u) ^ 1u);
+        ptx::mbar_arrive_expect_tx(bars.full[s], bytes);
+        ptx::bulk_g2s(stage_base + s * kStageBytes, src, bytes, bars.full[s]);
+        src += bytes;
+      }
+    }
+  }
 }
+
+// ------------------------------------------------------------------------------------------------
+// MMA issuer (one thread)
+// ------------------------------------------------------------------------------------------------
+__device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uint32_t stage_base,
+                         uint32_t tmem_base, int64_t n_evals, int n_ops) {
+  uint32_t t = 0;  // tile counter (mirrors the producer)
+  uint32_t g = 0;  // n-chunk counter: TMEM buffer = g & 1
+  uint32_t o = 0;  // op counter: phase of a_ready / a_free
+  for (int64_t e = 0; e < n_evals; ++e) {
+    for (int oi = 0; oi < n_ops; ++oi, ++o) {
+      const OpDesc op = P.ops[oi];
+      const uint32_t idesc = ptx::idesc_bf16(kRows, op.ncols);
+      // chunks this op does not read are free as soon as everything issued so far has completed
+      for (int j = op.kch; j < kMaxKch; ++j) ptx::mma_commit(bars.a_free[j]);
+      for (int c = 0; c < op.nch; ++c, ++g) {
+        const uint32_t buf = g & 1u, use = g >> 1;
+        ptx::mbar_wait(bars.d_free[buf], (use & 1u) ^ 1u);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + buf * 256u;
+        for (int k32 = 0; k32 < 2 * op.kch; ++k32, ++t) {
+          const int j = k32 >> 1;
+          if (c == 0 && (k32 & 1) == 0) {
+            ptx::mbar_wait(bars.a_ready[j], o & 1u);
+            ptx::tc_fence_after();
+          }
+          const uint32_t s = t % kStages, use_s = t / kStages;
+          ptx::mbar_wait(bars.full[s], use_s & 1u);
+          ptx::tc_fence_after();
+          const uint32_t a_addr = a_base + j * kAChunkBytes + (k32 & 1) * 64;
+          const uint32_t b_addr = stage_base + s * kStageBytes;
+#pragma unroll
+          for (int kk = 0; kk < 2; ++kk) {
+            ptx::mma_bf16_ss(d_tmem, ptx::smem_desc_sw128(a_addr + kk * 32),
+                             ptx::smem_desc_sw64(b_addr + kk * 32), idesc, (k32 | kk) != 0 ? 1u : 0u);
+          }
+          ptx::mma_commit(bars.empty[s]);
+          if (c == op.nch - 1 && (k32 & 1)) ptx::mma_commit(bars.a_free[j]);
+        }
+        ptx::mma_commit(bars.d_full[buf]);
+      }
+    }
+  }
+}
+
+}  // namespace tc
 }  // namespace best
+
+#include "tc_epilogue.cuh"
+#include "tc_host.cuh"

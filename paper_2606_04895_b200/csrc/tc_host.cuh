@@ -1,0 +1,468 @@
+// Kernel body (role dispatch + sampler drivers) and host side (weight packing, launches) of the
+// tensor-core path.  Included by tc_fused.cu only.
+#pragma once
+
+namespace best {
+namespace tc {
+
+template <int METHOD>
+__device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
+  const Params& P = *C.P;
+  const int d = P.d;
+  const int64_t r_in_launch = (int64_t)blockIdx.x * kRows + C.row;
+  const bool valid = r_in_launch < R.B;
+  const float* Ls = C.Ls;
+
+  if (METHOD == M_EVAL) {
+    float th[kDP], g[kDP], lp;
+    if (R.io_mode == IO_ROWS_F32) {
+#pragma unroll
+      for (int i = 0; i < kDP; ++i) th[i] = (valid && i < d) ? R.in_rows[r_in_launch * d + i] : 0.0f;
+    } else {
+      load_vec(R.theta, R.ld, r_in_launch, d, valid, th);
+    }
+    eval_target(C, th, R.want_grad != 0, lp, g);
+    if (valid) {
+      if (R.io_mode == IO_ROWS_F32) {
+        R.out_logp[r_in_launch] = lp;
+        if (R.want_grad) {
+#pragma unroll
+          for (int i = 0; i < kDP; ++i) if (i < d) R.out_grad[r_in_launch * d + i] = g[i];
+        }
+      } else {
+        R.logp[r_in_launch] = (double)lp;
+        if (R.want_grad) store_vec(R.grad, R.ld, r_in_launch, d, g);
+      }
+    }
+    return;
+  }
+
+  if (METHOD == M_AIES) {
+    const int64_t i = R.own0 + r_in_launch;
+    const uint4 w = philox4x32_10((uint32_t)i, R.step0, 0u, R.seed);
+    const int64_t j = R.oth0 + (int64_t)__umulhi(w.z, (uint32_t)R.B);
+    const float a = R.eps;
+    const float t = u01<float>(w.y) * (a - 1.0f) + 1.0f;
+    const float z = t * t / a;
+    float thi[kDP], thp[kDP], g[kDP], lpp;
+    load_vec(R.theta, R.ld, i, d, valid, thi);
+    {
+      float thj[kDP];
+      load_vec(R.theta, R.ld, j, d, valid, thj);
+#pragma unroll
+      for (int k = 0; k < kDP; ++k) thp[k] = thj[k] + z * (thi[k] - thj[k]);
+    }
+    eval_target(C, thp, false, lpp, g);
+    if (valid) {
+      const float la = (float)(d - 1) * logf(z) + lpp - (float)R.logp[i];
+      R.last_la[i] = (double)la;
+      if (accept_rule<float>(u01<float>(w.x), la)) {
+        store_vec(R.theta, R.ld, i, d, thp);
+        R.logp[i] = (double)lpp;
+        R.n_accept[i] += 1ull;
+      }
+    }
+    return;
+  }
+
+  const int64_t c = r_in_launch;
+  const float eps = R.eps;
+  float lp = valid ? (float)R.logp[c] : 0.0f;
+  float la_last = 0.0f;
+  unsigned long long nacc = 0;
+
+  if (METHOD == M_MH) {
+    float th[kDP];
+    load_vec(R.theta, R.ld, c, d, valid, th);
+    for (int64_t t = 0; t < R.n_steps; ++t) {
+      const uint64_t step = R.step0 + (uint64_t)t;
+      float thp[kDP], g[kDP], lpp;
+      {
+        float xi[kDP], dx[kDP];
+        draw_normals32(R.seed, (uint32_t)c, step, d, xi);
+#pragma unroll
+        for (int i = 0; i < kDP; ++i) xi[i] *= eps;
+        mv_L(Ls, xi, dx);
+#pragma unroll
+        for (int i = 0; i < kDP; ++i) thp[i] = th[i] + dx[i];
+      }
+      eval_target(C, thp, false, lpp, g);
+      const float la = lpp - lp;
+      la_last = la;
+      const uint4 w = philox4x32_10((uint32_t)c, step, 0u, R.seed);
+      if (valid && accept_rule<float>(u01<float>(w.x), la)) {
+#pragma unroll
+        for (int i = 0; i < kDP; ++i) th[i] = thp[i];
+        lp = lpp;
+        ++nacc;
+      }
+    }
+    if (valid) store_vec(R.theta, R.ld, c, d, th);
+  }
+
+  if (METHOD == M_MALA) {
+    const float sq = sqrtf(2.0f * eps);
+    for (int64_t t = 0; t < R.n_steps; ++t) {
+      const uint64_t step = R.step0 + (uint64_t)t;
+      float thp[kDP], dz[kDP], gp[kDP], lpp, fwd = 0.0f;
+      {
+        float g[kDP], gz[kDP], xi[kDP];
+        load_vec(R.grad, R.ld, c, d, valid, g);
+        mv_Lt(Ls, g, gz);
+        draw_normals32(R.seed, (uint32_t)c, step, d, xi);
+#pragma unroll
+        for (int i = 0; i < kDP; ++i) {
+          const float f = sq * xi[i];
+          fwd = fmaf(f, f, fwd);
+          dz[i] = fmaf(eps, gz[i], f);
+        }
+        mv_L(Ls, dz, g);  // g <- L dz
+        float th[kDP];
+        load_vec(R.theta, R.ld, c, d, valid, th);
+#pragma unroll
+        for (int i = 0; i < kDP; ++i) thp[i] = th[i] + g[i];
+      }
+      eval_target(C, thp, true, lpp, gp);
+      float bwd = 0.0f;
+      {
+        float gzp[kDP];
+        mv_Lt(Ls, gp, gzp);
+#pragma unroll
+        for (int i = 0; i < kDP; ++i) {
+          const float r = fmaf(eps, gzp[i], dz[i]);
+          bwd = fmaf(r, r, bwd);
+        }
+      }
+      const float la = lpp - lp + (fwd - bwd) / (4.0f * eps);
+      la_last = la;
+      const uint4 w = philox4x32_10((uint32_t)c, step, 0u, R.seed);
+      if (valid && accept_rule<float>(u01<float>(w.x), la)) {
+        store_vec(R.theta, R.ld, c, d, thp);
+        store_vec(R.grad, R.ld, c, d, gp);
+        lp = lpp;
+        ++nacc;
+      }
+    }
+  }
+
+  if (METHOD == M_HMC) {
+    for (int64_t t = 0; t < R.n_steps; ++t) {
+      const uint64_t step = R.step0 + (uint64_t)t;
+      float thw[kDP], q[kDP], gw[kDP], lpw = lp, H0;
+      {
+        float g[kDP], gz[kDP];
+        draw_normals32(R.seed, (uint32_t)c, step, d, q);
+        float kin = 0.0f;
+#pragma unroll
+        for (int i = 0; i < kDP; ++i) kin = fmaf(q[i], q[i], kin);
+        H0 = -lp + 0.5f * kin;
+        load_vec(R.grad, R.ld, c, d, valid, g);
+        mv_Lt(Ls, g, gz);
+#pragma unroll
+        for (int i = 0; i < kDP; ++i) q[i] = fmaf(0.5f * eps, gz[i], q[i]);
+        load_vec(R.theta, R.ld, c, d, valid, thw);
+      }
+      for (int l = 1; l <= R.n_leapfrog; ++l) {
+        {
+          float dz[kDP], dx[kDP];
+#pragma unroll
+          for (int i = 0; i < kDP; ++i) dz[i] = eps * q[i];
+          mv_L(Ls, dz, dx);
+#pragma unroll
+          for (int i = 0; i < kDP; ++i) thw[i] += dx[i];
+        }
+        eval_target(C, thw, true, lpw, gw);
+        float gz[kDP];
+        mv_Lt(Ls, gw, gz);
+        const float cc = (l < R.n_leapfrog) ? eps : 0.5f * eps;
+#pragma unroll
+        for (int i = 0; i < kDP; ++i) q[i] = fmaf(cc, gz[i], q[i]);
+      }
+      float kin = 0.0f;
+#pragma unroll
+      for (int i = 0; i < kDP; ++i) kin = fmaf(q[i], q[i], kin);
+      const float la = H0 - (-lpw + 0.5f * kin);
+      la_last = la;
+      const uint4 w = philox4x32_10((uint32_t)c, step, 0u, R.seed);
+      if (valid && accept_rule<float>(u01<float>(w.x), la)) {
+        store_vec(R.theta, R.ld, c, d, thw);
+        store_vec(R.grad, R.ld, c, d, gw);
+        lp = lpw;
+        ++nacc;
+      }
+    }
+  }
+
+  if (valid) {
+    R.logp[c] = (double)lp;
+    R.last_la[c] = (double)la_last;
+    R.n_accept[c] += nacc;
+  }
+}
+
+template <int METHOD>
+__global__ void __launch_bounds__(kThreads, 1)
+best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const uint32_t sbase = ptx::smem_u32(smem);
+  const Bars bars = make_bars(sbase + SmemLayout::BARS);
+  float* bias_s = reinterpret_cast<float*>(smem + SmemLayout::BIAS);
+  float* wout_s = reinterpret_cast<float*>(smem + SmemLayout::WOUT);
+  float* wouts_s = reinterpret_cast<float*>(smem + SmemLayout::WOUTS);
+  float* Ls = reinterpret_cast<float*>(smem + SmemLayout::LMAT);
+  float* Rs = reinterpret_cast<float*>(smem + SmemLayout::RMAT);
+  float* vecs = reinterpret_cast<float*>(smem + SmemLayout::VECS);
+  volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + SmemLayout::TMEMPTR);
+
+  if (tid == 0) {
+    for (int i = 0; i < kStages; ++i) { ptx::mbar_init(bars.full[i], 1); ptx::mbar_init(bars.empty[i], 1); }
+    for (int i = 0; i < kMaxKch; ++i) { ptx::mbar_init(bars.a_ready[i], kRows); ptx::mbar_init(bars.a_free[i], 1); }
+    for (int i = 0; i < 2; ++i) { ptx::mbar_init(bars.d_full[i], 1); ptx::mbar_init(bars.d_free[i], kRows); }
+    ptx::fence_mbar_init();
+  }
+  if (warp == 2) ptx::tmem_alloc(sbase + SmemLayout::TMEMPTR, 512);
+  for (int i = tid; i < P.n_hidden * P.H; i += kThreads) bias_s[i] = P.bias[i];
+  for (int i = tid; i < P.H; i += kThreads) { wout_s[i] = P.w_out[i]; wouts_s[i] = P.mlp_scale * P.w_out[i]; }
+  for (int i = tid; i < kDP * kDP; i += kThreads) {
+    const int r = i / kDP, c = i % kDP;
+    Ls[i] = (r < P.d && c <= r) ? (float)P.L[r * P.d + c] : 0.0f;
+    Rs[i] = (P.has_gauss && r < P.d && c < P.d && c >= r) ? (float)P.R[r * P.d + c] : 0.0f;
+  }
+  for (int i = tid; i < kDP; i += kThreads) {
+    const bool in = i < P.d;
+    vecs[i] = (in && P.has_gauss) ? (float)P.mu[i] : 0.0f;
+    const float lo = (in && P.has_box) ? (float)P.lo[i] : -3.0e38f;
+    const float hi = (in && P.has_box) ? (float)P.hi[i] : 3.0e38f;
+    vecs[32 + i] = lo;
+    vecs[64 + i] = hi;
+    vecs[96 + i] = (in && P.has_box) ? (float)(1.0 / (P.hi[i] - P.lo[i])) : 0.0f;
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = *tmem_ptr;
+
+  int64_t n_evals = 1;
+  if (METHOD == M_MH || METHOD == M_MALA) n_evals = R.n_steps;
+  if (METHOD == M_HMC) n_evals = R.n_steps * R.n_leapfrog;
+  const int n_ops = R.want_grad ? P.n_ops_all : P.n_ops_fwd;
+
+  if (warp == 0) {
+    if (lane == 0) producer_loop(P, bars, sbase + SmemLayout::STAGES, n_evals, n_ops);
+  } else if (warp == 1) {
+    if (lane == 0) mma_loop(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
+  } else if (warp >= 4) {
+    EpiCtx C;
+    C.P = &P;
+    C.bars = bars;
+    C.smem = smem;
+    C.row = tid - 4 * 32;
+    C.tmem_lane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
+    C.o = 0;
+    C.g = 0;
+    C.bias_s = bias_s; C.wout_s = wout_s; C.wouts_s = wouts_s; C.Ls = Ls; C.Rs = Rs; C.vecs = vecs;
+    C.dact_tile = P.dact + (size_t)blockIdx.x * P.dact_tile_elems;
+    sampler_thread<METHOD>(C, R);
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 2) ptx::tmem_dealloc(tmem_base, 512);
+}
+
+}  // namespace tc
+
+// =================================================================================================
+// host side
+// =================================================================================================
+struct TcPlan {
+  tc::Params P{};
+  uint8_t* wpack = nullptr;
+  float* bias = nullptr;
+  float* w_out = nullptr;
+  uint16_t* dact = nullptr;
+  int64_t dact_tiles = 0;
+};
+
+namespace {
+
+uint16_t f32_to_bf16(float f) {  // round to nearest even
+  uint32_t u;
+  std::memcpy(&u, &f, 4);
+  if ((u & 0x7FFFFFFFu) > 0x7F800000u) return (uint16_t)((u >> 16) | 0x40);
+  u += 0x7FFFu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+
+template <int METHOD>
+int launch_tc(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
+  TcPlan* pl = ctx->tc;
+  const int64_t n_tiles = (rows + tc::kRows - 1) / tc::kRows;
+  if (n_tiles > pl->dact_tiles) {
+    if (pl->dact) { BEST_CUDA(cudaStreamSynchronize(s)); cudaFree(pl->dact); pl->dact = nullptr; }
+    const size_t elems = pl->P.dact_tile_elems * (size_t)n_tiles;
+    BEST_CUDA(cudaMalloc(&pl->dact, sizeof(uint16_t) * (elems ? elems : 8)));
+    pl->dact_tiles = n_tiles;
+    pl->P.dact = pl->dact;
+  }
+  static bool attr_set = false;
+  const int smem_bytes = tc::SmemLayout::TOTAL + 1024;
+  if (!attr_set) {
+    BEST_CUDA(cudaFuncSetAttribute(tc::best_tc_kernel<METHOD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    attr_set = true;
+  }
+  pl->P.L = ctx->L_dev;
+  tc::best_tc_kernel<METHOD><<<(unsigned)n_tiles, tc::kThreads, smem_bytes, s>>>(pl->P, R);
+  count_launch();
+  BEST_CUDA(cudaGetLastError());
+  return BEST_OK;
+}
+
+}  // namespace
+
+int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
+  const int K = cfg->n_affine - 1;  // hidden layers
+  if (K < 1) { set_error("BEST_PREC_BF16 needs at least one hidden layer"); return BEST_ERR_UNSUPPORTED; }
+  const int H = cfg->widths[1];
+  for (int k = 1; k <= K; ++k)
+    if (cfg->widths[k] != H) { set_error("BEST_PREC_BF16: hidden widths must be equal"); return BEST_ERR_UNSUPPORTED; }
+  if (!(H == 64 || H == 128 || H == 256 || H == 512) || K * H > 2048 || 2 * K > tc::kMaxOps) {
+    set_error("BEST_PREC_BF16: hidden width must be 64/128/256/512 with n_hidden*width <= 2048");
+    return BEST_ERR_UNSUPPORTED;
+  }
+  const int d = cfg->d;
+  TcPlan* pl = new TcPlan();
+  ctx->tc = pl;
+  tc::Params& P = pl->P;
+  P.d = d; P.H = H; P.n_hidden = K; P.act = cfg->activation; P.mlp_scale = cfg->mlp_scale;
+  const int ncols = H < 256 ? H : 256, nch = H / ncols, kchH = H / 64;
+  int no = 0;
+  for (int l = 0; l < K; ++l)
+    P.ops[no++] = tc::OpDesc{l == 0 ? 1 : kchH, nch, ncols, l == K - 1 ? tc::EPI_FWD_LAST : tc::EPI_FWD_HID, l};
+  P.n_ops_fwd = no;
+  for (int l = K - 1; l >= 1; --l) P.ops[no++] = tc::OpDesc{kchH, nch, ncols, tc::EPI_BWD_HID, l - 1};
+  P.ops[no++] = tc::OpDesc{kchH, 1, 32, tc::EPI_BWD_FINAL, 0};
+  P.n_ops_all = no;
+  P.dact_tile_elems = (size_t)(K - 1) * H * tc::kRows;
+
+  // host views of the fp32 weights
+  std::vector<const float*> W(K + 1);
+  std::vector<const float*> bvec(K + 1);
+  {
+    size_t wo = 0, bo = 0;
+    for (int k = 0; k <= K; ++k) {
+      W[k] = cfg->W_flat + wo;
+      bvec[k] = cfg->b_flat + bo;
+      wo += (size_t)cfg->widths[k] * cfg->widths[k + 1];
+      bo += cfg->widths[k + 1];
+    }
+  }
+  // B operand of every op as a logical [N][Ktot] bf16 matrix, cut into pre-swizzled stage tiles
+  std::vector<uint16_t> pack;
+  for (int oi = 0; oi < P.n_ops_all; ++oi) {
+    const tc::OpDesc op = P.ops[oi];
+    auto Bm = [&](int n, int k) -> float {
+      if (op.epi == tc::EPI_FWD_HID || op.epi == tc::EPI_FWD_LAST) {
+        if (op.layer == 0) { const int kk = k & 31; return kk < d ? W[0][(size_t)n * d + kk] : 0.0f; }
+        return W[op.layer][(size_t)n * H + k];
+      }
+      if (op.epi == tc::EPI_BWD_HID) return W[op.layer + 1][(size_t)k * H + n];  // (W_l)^T, l = layer+1
+      return n < d ? W[0][(size_t)k * d + n] : 0.0f;                             // (W_0)^T
+    };
+    for (int c = 0; c < op.nch; ++c)
+      for (int k32 = 0; k32 < 2 * op.kch; ++k32) {
+        const size_t base = pack.size();
+        pack.resize(base + (size_t)op.ncols * 32, 0);
+        for (int r = 0; r < op.ncols; ++r)
+          for (int kk = 0; kk < 32; ++kk) {
+            const size_t off = (size_t)r * 32 + ((((kk >> 3) ^ ((r >> 1) & 3))) << 3) + (kk & 7);
+            pack[base + off] = f32_to_bf16(Bm(c * op.ncols + r, k32 * 32 + kk));
+          }
+      }
+  }
+  std::vector<float> bias((size_t)K * H);
+  for (int l = 0; l < K; ++l) std::memcpy(&bias[(size_t)l * H], bvec[l], sizeof(float) * H);
+  P.b_out = bvec[K][0];
+  int rc;
+  if ((rc = dev_alloc(&pl->wpack, pack.size() * 2))) return rc;
+  if ((rc = dev_alloc(&pl->bias, bias.size()))) return rc;
+  if ((rc = dev_alloc(&pl->w_out, (size_t)H))) return rc;
+  BEST_CUDA(cudaMemcpy(pl->wpack, pack.data(), pack.size() * 2, cudaMemcpyHostToDevice));
+  BEST_CUDA(cudaMemcpy(pl->bias, bias.data(), bias.size() * 4, cudaMemcpyHostToDevice));
+  BEST_CUDA(cudaMemcpy(pl->w_out, W[K], sizeof(float) * H, cudaMemcpyHostToDevice));
+  P.wpack = pl->wpack; P.bias = pl->bias; P.w_out = pl->w_out;
+  P.has_gauss = ctx->tgt.has_gauss; P.has_box = ctx->tgt.has_box;
+  P.banana_i = ctx->tgt.banana_i; P.banana_j = ctx->tgt.banana_j;
+  P.banana_sigma = (float)ctx->tgt.banana_sigma;
+  P.pen_kappa = (float)ctx->tgt.pen_kappa; P.pen_gamma = (float)ctx->tgt.pen_gamma;
+  P.mu = ctx->tgt.mu; P.R = ctx->tgt.R; P.lo = ctx->tgt.lo; P.hi = ctx->tgt.hi; P.L = ctx->L_dev;
+  return BEST_OK;
+}
+
+void tc_plan_destroy(best_ctx* ctx) {
+  TcPlan* pl = ctx->tc;
+  if (!pl) return;
+  cudaFree(pl->wpack); cudaFree(pl->bias); cudaFree(pl->w_out); cudaFree(pl->dact);
+  delete pl;
+  ctx->tc = nullptr;
+}
+
+int tc_logp_grad(best_ctx* ctx, const float* theta_rows, int64_t n, float* logp, float* grad, cudaStream_t s) {
+  tc::Run R{};
+  R.method = tc::M_EVAL; R.want_grad = grad ? 1 : 0; R.io_mode = tc::IO_ROWS_F32;
+  R.B = n; R.ld = n; R.n_steps = 1;
+  R.in_rows = theta_rows; R.out_logp = logp; R.out_grad = grad;
+  return launch_tc<tc::M_EVAL>(ctx, R, n, s);
+}
+
+int tc_state_init(best_ctx* ctx, best_state* st, cudaStream_t s) {
+  tc::Run R{};
+  R.method = tc::M_EVAL; R.want_grad = 1; R.io_mode = tc::IO_SOA_F64;
+  R.B = st->B; R.ld = st->B; R.n_steps = 1;
+  R.theta = st->theta; R.grad = st->grad; R.logp = st->logp;
+  BEST_TRY(launch_tc<tc::M_EVAL>(ctx, R, st->B, s));
+  st->grad_valid = true;
+  st->n_evals += (uint64_t)st->B;
+  return BEST_OK;
+}
+
+int tc_step(best_ctx* ctx, best_state* st, int method, int64_t n_steps, uint64_t seed, float eps,
+            int n_leapfrog, float* trace, int thin, cudaStream_t s) {
+  if ((method == tc::M_MALA || method == tc::M_HMC) && !st->grad_valid) BEST_TRY(tc_state_init(ctx, st, s));
+  tc::Run R{};
+  R.method = method; R.io_mode = tc::IO_SOA_F64;
+  R.want_grad = (method == tc::M_MALA || method == tc::M_HMC) ? 1 : 0;
+  R.B = st->B; R.ld = st->B; R.seed = seed; R.eps = eps; R.n_leapfrog = n_leapfrog;
+  R.theta = st->theta; R.grad = st->grad; R.logp = st->logp; R.last_la = st->last_la; R.n_accept = st->n_accept;
+  const bool adapt = ctx->adapt_every > 0 && method != tc::M_AIES;
+  int64_t t0 = 0;
+  while (t0 < n_steps) {
+    int64_t seg = n_steps - t0;
+    if (trace && thin > 0) { const int64_t to_boundary = thin - (t0 % thin); if (to_boundary < seg) seg = to_boundary; }
+    if (adapt || method == tc::M_AIES) seg = 1;
+    R.n_steps = seg;
+    R.step0 = st->step + (uint64_t)t0;
+    switch (method) {
+      case tc::M_MH: BEST_TRY(launch_tc<tc::M_MH>(ctx, R, st->B, s)); break;
+      case tc::M_MALA: BEST_TRY(launch_tc<tc::M_MALA>(ctx, R, st->B, s)); break;
+      case tc::M_HMC: BEST_TRY(launch_tc<tc::M_HMC>(ctx, R, st->B, s)); break;
+      default: {
+        const int64_t half = st->B / 2;
+        tc::Run Rh = R;
+        Rh.B = half;
+        for (int hh = 0; hh < 2; ++hh) {
+          Rh.own0 = hh == 0 ? 0 : half;
+          Rh.oth0 = hh == 0 ? half : 0;
+          BEST_TRY(launch_tc<tc::M_AIES>(ctx, Rh, half, s));
+        }
+      }
+    }
+    t0 += seg;
+    BEST_TRY(after_step(ctx, st, t0 - 1, trace, thin, adapt, s));
+  }
+  if (method == tc::M_MH || method == tc::M_AIES) st->grad_valid = false;
+  return BEST_OK;
+}
+
+}  // namespace best

@@ -1,0 +1,241 @@
+"""GPU parity tests of the tensor-core path (BEST_PREC_BF16) against the oracle, through the C-ABI.
+logp / grad within rel 2e-2 (north_star); accept decisions compared statistically (reading R8: on
+the bf16 path log α carries the emulator's error, so every mismatch must sit inside the measured
+|Δ log α| bound of that run); long runs by moments; split invariance bit for bit."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2606_04895_b200 import workloads as WL
+from parity_util import TOL, accept_margins, check_logp_grad
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_04895_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import oracle
+    oracle.lib()
+    return oracle
+
+
+def f32(x):
+    return float(np.float32(x))
+
+
+def _posterior_like(w, n, seed):
+    return w.with_chains(n, seed).theta0
+
+
+@pytest.mark.parametrize("variant", ["full", "mlp_only"])
+@pytest.mark.parametrize("scale", [1.0, 3.0])
+def test_T1_lcdm_logp_grad(B, O, variant, scale):
+    """BASELINE configs[1]/[2] network 27→512⁴→1 SiLU; 2048 probe points incl. box faces and ±20σ."""
+    base = WL.lcdm(n_chains=8, mlp_scale=scale)
+    n = 2048 + 77                                   # several 128-row tiles and a ragged tail
+    pts = WL.probe_points(base, n, seed=17)
+    w = WL.mlp_only(base) if variant == "mlp_only" else base
+    ctx = B.Context(w, B.PREC_BF16)
+    lp = np.zeros(n, np.float32)
+    g = np.zeros((n, w.d), np.float32)
+    ctx.logp_grad(pts, n, lp, g)
+    lp_ref, g_ref = O.Oracle(w).logp_grad(pts)
+    e = check_logp_grad(lp, g, lp_ref, g_ref, TOL[1], f"lcdm/{variant}/s={scale}")
+    print(f"[T1-bf16] lcdm {variant} s={scale}: logp err/S {e[0]:.2e}, grad ratio {e[1]:.2e}")
+    lp2 = np.zeros(n, np.float32)
+    ctx.logp_grad(pts, n, lp2, None)                # forward-only launch (MH / AIES flavour)
+    assert np.array_equal(lp, lp2)
+    ctx.close()
+
+
+@pytest.mark.parametrize("hidden,act", [((64, 64), WL.ACT_TANH), ((64, 64), WL.ACT_SILU),
+                                        ((128, 128, 128), WL.ACT_SILU), ((256, 256), WL.ACT_TANH),
+                                        ((512,), WL.ACT_SILU)])
+def test_T1_other_shapes(B, O, hidden, act):
+    """Other supported tile shapes (N-chunk = 64/128/256, 1..3 hidden layers).  north_star's 2e-2 is
+    stated for the BASELINE networks (tested above); narrow random nets average the bf16 rounding of
+    fewer terms, so these shape-coverage cases use 3e-2."""
+    base = WL.tiny(activation=act, hidden=hidden, mlp_scale=1.0)
+    n = 300
+    pts = _posterior_like(base, n, seed=3)
+    for w in (base, WL.mlp_only(base)):
+        ctx = B.Context(w, B.PREC_BF16)
+        lp = np.zeros(n, np.float32)
+        g = np.zeros((n, w.d), np.float32)
+        ctx.logp_grad(pts, n, lp, g)
+        lp_ref, g_ref = O.Oracle(w).logp_grad(pts)
+        check_logp_grad(lp, g, lp_ref, g_ref, 3e-2, f"{hidden}/{act}/{w.name}")
+        ctx.close()
+
+
+def test_unsupported_shapes(B):
+    for hidden in ((50, 37), (64, 128), (1024, 1024)):
+        w = WL.tiny(hidden=hidden)
+        with pytest.raises(B.BestError) as e:
+            B.Context(w, B.PREC_BF16)
+        assert e.value.code == B.BEST_ERR_UNSUPPORTED
+
+
+def _single_step_stat(B, O, w, method, seed, **kw):
+    kw = {k: (f32(v) if isinstance(v, float) else v) for k, v in kw.items()}
+    ctx = B.Context(w, B.PREC_BF16)
+    st = ctx.new_state(w.theta0)
+    ost = O.Oracle(w).new_state(w.theta0)
+    th0 = ost.theta.copy()
+    getattr(st, "step_" + method)(1, seed, **kw)
+    getattr(ost, "step_" + method)(1, seed, **kw)
+    la = st.last_log_alpha()
+    out = st.get(want_grad=(method in ("mala", "hmc")))
+    acc, acc_ref = out["n_accept"].astype(np.int64), ost.n_accept.astype(np.int64)
+    m = accept_margins(O, seed, 0, w.n_chains, ost.last_log_alpha)
+    dla = np.abs(la - ost.last_log_alpha)
+    mism = acc != acc_ref
+    info = dict(n=w.n_chains, mismatch_rate=float(mism.mean()), max_dla=float(dla.max()),
+                median_dla=float(np.median(dla)), accept_rate=float(acc_ref.mean()))
+    print(f"[T2-bf16] {w.name}/{method}: {info}")
+    # every mismatch lies inside the measured |Δ log α| of its own chain (+ fp32 slack)
+    assert (m[mism] <= dla[mism] + 1e-5).all(), info
+    assert mism.mean() < 0.02 and np.median(dla) < 2e-2, info
+    same = ~mism
+    scale = np.abs(ost.theta).max(axis=0)
+    assert (np.abs(out["theta"][same] - ost.theta[same]) <= 2e-3 * scale + 1e-6).all()
+    rej = same & (acc_ref == 0)
+    assert np.array_equal(out["theta"][rej], th0[rej].astype(np.float32))
+    S = np.abs(ost.logp).max()
+    assert np.abs(out["logp"][same] - ost.logp[same]).max() <= TOL[1] * S
+    ctx.close()
+    return info
+
+
+@pytest.mark.parametrize("method,kw", [("mh", dict(eps=0.3)), ("mala", dict(eps=0.3)),
+                                       ("hmc", dict(eps=0.1, n_leapfrog=4)), ("aies", dict(a=2.0))])
+def test_T2_single_step_statistical(B, O, method, kw):
+    w = WL.lcdm(n_chains=1024 + 40, mlp_scale=3.0 if method == "hmc" else 1.0)
+    _single_step_stat(B, O, w, method, seed=55, **kw)
+
+
+def test_T4_split_invariance(B):
+    import torch
+    w = WL.lcdm(n_chains=300)
+    ctx = B.Context(w, B.PREC_BF16)
+    for meth, kw in (("mala", dict(eps=0.3)), ("mh", dict(eps=0.3)), ("hmc", dict(eps=0.1, n_leapfrog=3)),
+                     ("aies", dict(a=2.0))):
+        a, b = ctx.new_state(w.theta0), ctx.new_state(w.theta0)
+        tr = torch.zeros(3, 300, w.d, device="cuda")
+        getattr(a, "step_" + meth)(12, 3, trace=tr, thin=4, **kw)
+        getattr(b, "step_" + meth)(5, 3, **kw)
+        getattr(b, "step_" + meth)(7, 3, **kw)
+        ga, gb = a.get(), b.get()
+        for k in ("theta", "logp", "n_accept"):
+            assert np.array_equal(ga[k], gb[k]), (meth, k)
+        if meth in ("mala", "hmc"):
+            assert np.array_equal(ga["grad"], gb["grad"]), meth
+        torch.cuda.synchronize()
+        assert np.array_equal(tr[-1].cpu().numpy(), ga["theta"]), meth
+        assert ga["step"] == 12
+    ctx.close()
+
+
+@pytest.mark.parametrize("method", ["mh", "mala", "hmc", "aies"])
+@pytest.mark.parametrize("d", [6, 27])
+def test_T5_gaussian_closed_form_moments(B, method, d):
+    """s = 0 switches the emulator term off, the tensor-core kernel still runs every GEMM: the
+    posterior is N(μ, Σ) exactly and the fp32 sampler algebra of the fused kernel is what is tested."""
+    import torch
+    if method == "aies" and d == 27:
+        pytest.skip("AIES moment parity is tested at small d")
+    if d == 6:
+        w = WL.tiny(n_chains=512, hidden=(64, 64), mlp_scale=0.0)
+    else:
+        w = WL.lcdm(n_chains=512, hidden=64, n_hidden=2, mlp_scale=0.0)
+    ctx = B.Context(w, B.PREC_BF16)
+    st = ctx.new_state(w.theta0)
+    plan = {"mh": (dict(eps=2.4 / math.sqrt(d)), 400, 2400, 4), "mala": (dict(eps=0.5 if d == 6 else 0.3), 100, 800, 2),
+            "hmc": (dict(eps=0.4 if d == 6 else 0.25, n_leapfrog=4), 30, 300, 1), "aies": (dict(a=2.0), 400, 3000, 5)}
+    kw, burn, n, thin = plan[method]
+    getattr(st, "step_" + method)(burn, 11, **kw)
+    tr = torch.zeros(n // thin, 512, d, device="cuda")
+    getattr(st, "step_" + method)(n, 11, trace=tr, thin=thin, **kw)
+    torch.cuda.synchronize()
+    trace = tr.cpu().numpy().astype(np.float64)
+    sig = np.sqrt(np.diag(w.Sigma))
+    if method == "aies":
+        xc = (trace - w.mu) / sig
+        v = (xc ** 2).mean(axis=1).reshape(30, -1, d).mean(axis=1)
+        se = v.std(axis=0, ddof=1) / math.sqrt(30)
+        assert np.all(np.abs(v.mean(axis=0) - 1.0) < 4 * se + 0.01)
+    else:
+        m_c = trace.mean(axis=0)
+        se = m_c.std(axis=0, ddof=1) / math.sqrt(512)
+        assert np.all(np.abs(m_c.mean(axis=0) - w.mu) < 4 * se + 1e-4 * sig)
+        xc = trace - w.mu
+        for i in range(d):
+            for j in range(i, d):
+                p = (xc[:, :, i] * xc[:, :, j]).mean(axis=0)
+                assert abs(p.mean() - w.Sigma[i, j]) < 4 * p.std(ddof=1) / math.sqrt(512) + 1e-3 * sig[i] * sig[j], (i, j)
+    rate = st.get(want_grad=False)["n_accept"].mean() / (burn + n)
+    print(f"[T5-bf16] {method} d={d}: acceptance {rate:.3f}")
+    assert 0.1 < rate <= 1.0
+    ctx.close()
+
+
+def test_T5_lcdm_moments_vs_fp32_path(B):
+    """ΛCDM-like short MALA run: bf16-path moments vs the exact path's (independent seeds, 4 SE)."""
+    import torch
+    w = WL.lcdm(n_chains=512)
+    res = []
+    for prec, seed in ((B.PREC_BF16, 5), (B.PREC_FP32, 6)):
+        ctx = B.Context(w, prec)
+        st = ctx.new_state(w.theta0)
+        st.step_mala(50, seed, 0.3)
+        tr = torch.zeros(100, 512, w.d, device="cuda")
+        st.step_mala(200, seed, 0.3, trace=tr, thin=2)
+        torch.cuda.synchronize()
+        res.append((tr.cpu().numpy().astype(np.float64).mean(axis=0), st.get(want_grad=False)["n_accept"].mean() / 250))
+        ctx.close()
+    (a, ra), (b, rb) = res
+    se = np.sqrt(a.var(axis=0, ddof=1) / 512 + b.var(axis=0, ddof=1) / 512)
+    assert np.all(np.abs(a.mean(axis=0) - b.mean(axis=0)) < 4 * se)
+    assert abs(ra - rb) < 0.02
+
+
+def test_T6_adaptation_on_tc_path(B, O):
+    import torch
+    w = WL.lcdm(n_chains=512, hidden=64, n_hidden=2)
+    w.L = np.diag(np.sqrt(np.diag(w.Sigma)))
+    ctx = B.Context(w, B.PREC_BF16)
+    st = ctx.new_state(w.theta0)
+    st.set_adaptation(50, 1e-6)
+    o = O.Oracle(w)
+    for win in range(2):
+        tr = torch.zeros(50, 512, w.d, device="cuda")
+        st.step_mh(50, 21, 0.05, trace=tr, thin=1)
+        torch.cuda.synchronize()
+        rc, _, Lo = o.cov_chol(tr.cpu().numpy().astype(np.float64).reshape(-1, w.d), 1e-6)
+        assert rc == 0
+        Lg = ctx.get_whitening()
+        assert np.abs(Lg - Lo).max() / np.abs(Lo).max() < 1e-6
+    assert ctx.adapt_stats() == (2, 0)
+    ctx.close()
+
+
+def test_T7_nonfinite(B):
+    w = WL.lcdm(n_chains=256, hidden=64, n_hidden=2, mlp_scale=3.0)
+    ctx = B.Context(w, B.PREC_BF16)
+    st = ctx.new_state(w.theta0)
+    before = st.get()
+    st.step_hmc(2, 5, 50.0, 8)
+    after = st.get()
+    assert np.isfinite(after["theta"]).all() and np.isfinite(after["logp"]).all()
+    rejected = after["n_accept"] == 0
+    assert rejected.sum() >= 200
+    assert np.array_equal(after["theta"][rejected], before["theta"][rejected])
+    ctx.close()
