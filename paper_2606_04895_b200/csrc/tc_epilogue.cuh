@@ -1,5 +1,12 @@
-// Epilogue / sampler side of the fused tensor-core kernel: one thread per chain (TMEM lane).
-// Included by tc_fused.cu only.
+// Epilogue / sampler side of the fused tensor-core kernel.  Included by tc_fused.cu only.
+//
+// 16 epilogue warps = 512 threads.  Thread (row, k): row = TMEM lane = chain, k = 0..3.
+//   * MLP epilogues: of every 64-column group the thread handles columns [16k, 16k+16).
+//   * sampler algebra: the thread owns parameter dimensions [8k, 8k+8) of its chain; the four
+//     threads of a chain (same lane, four different warps of one TMEM lane quarter) exchange
+//     matvec inputs and partial sums through SMEM with a 128-thread named barrier.
+// Four resident warps per SM sub-partition hide the ALU / MUFU / LDS latencies that a single
+// warp per sub-partition cannot.
 #pragma once
 
 namespace best {
@@ -8,300 +15,365 @@ namespace tc {
 struct EpiCtx {
   const Params* P;
   Bars bars;
-  uint8_t* smem;        // generic pointer to the dynamic smem base
+  uint8_t* smem;
   uint32_t tmem_lane;   // tmem base + (lane quarter << 16)
   int row;              // 0..127
+  int k;                // 0..3
   uint32_t o, g;        // op / n-chunk counters (mirror the MMA issuer)
-  const float *bias_s, *wout_s, *wouts_s, *Ls, *Rs, *vecs;
-  uint16_t* dact_tile;  // this CTA's act' scratch
+  uint32_t vslot, pslot;  // rotating scratch slots
+  const float *bias_s, *wout_s, *wouts_s, *Ls, *LTs, *Rs, *RTs, *vecs;
+  float* part;          // [2][4][128]
+  uint16_t* dact_tile;
 };
 
-// h = act(a), dact = act'(a).  One MUFU.EX2 + one MUFU.RCP per element, ~fp32 accurate.
-__device__ __forceinline__ void act_eval(int kind, float a, float& h, float& dact) {
-  if (kind == BEST_ACT_SILU) {
-    const float e = ptx::ex2_approx(-1.4426950408889634f * fabsf(a));
-    const float r = ptx::rcp_approx(1.0f + e);
-    const float sg = (a >= 0.0f) ? r : e * r;
-    h = a * sg;
-    dact = fmaf(h, 1.0f - sg, sg);
-  } else {
-    const float e = ptx::ex2_approx(-2.8853900817779268f * fabsf(a));
-    const float t = (1.0f - e) * ptx::rcp_approx(1.0f + e);
-    h = copysignf(t, a);
-    dact = fmaf(-h, h, 1.0f);
-  }
-}
-
-__device__ __forceinline__ void st_shared_v4(uint8_t* p, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
-  *reinterpret_cast<uint4*>(p) = make_uint4(a, b, c, d);
-}
+using ptx::f32x2;
 
 // address of 16-byte piece `p` of row `row` in A k-chunk `j` (128B swizzle)
 __device__ __forceinline__ uint8_t* a_piece(const EpiCtx& C, int j, int p) {
   return C.smem + SmemLayout::A + j * kAChunkBytes + C.row * 128 + ((p ^ (C.row & 7)) << 4);
 }
-
 __device__ __forceinline__ size_t dact_off(const Params& P, int layer, int j, int p, int row) {
   return ((((size_t)layer * (P.H / 64) + j) * 8 + p) * kRows + row) * 8;
 }
+__device__ __forceinline__ void qbar(const EpiCtx& C) { ptx::named_bar_sync(1 + (C.row >> 5), 128); }
 
-// The first A operand of an evaluation: theta split into bf16 hi | lo halves (K = 64), so the
-// input layer sees ~16 mantissa bits of theta although the MMA operands are bf16.
-__device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[kDP]) {
-  ptx::mbar_wait(C.bars.a_free[0], (C.o & 1u) ^ 1u);  // previous op has finished reading chunk 0
-  uint32_t hi[16], lo[16];
+// ---- activations on fp32 pairs ---------------------------------------------------------------
+// SiLU: h = a*sg, dact = sg + h*(1 - sg), sg = 1/(1 + 2^(-a log2 e)).
+// kFastAct: sg = 0.5 + 0.5 tanh.approx(a/2)             (1 MUFU / element)
+// else    : ex2.approx + bit-trick reciprocal + 2 Newton steps on the FMA pipe (1 MUFU / element,
+//           relative error of sg ~2e-4, no cancellation for a << 0)
+template <bool kFast>
+__device__ __forceinline__ void silu2(f32x2 a, f32x2& h, f32x2& dact) {
+  f32x2 sg;
+  if (kFast) {
+    float x0, x1;
+    ptx::unpack2(ptx::mul2(a, ptx::pack2(0.5f, 0.5f)), x0, x1);
+    const f32x2 t = ptx::pack2(ptx::tanh_approx(x0), ptx::tanh_approx(x1));
+    sg = ptx::fma2(t, ptx::pack2(0.5f, 0.5f), ptx::pack2(0.5f, 0.5f));
+  } else {
+    float x0, x1;
+    ptx::unpack2(ptx::mul2(a, ptx::pack2(-1.4426950408889634f, -1.4426950408889634f)), x0, x1);
+    const f32x2 e = ptx::pack2(ptx::ex2_approx(fminf(x0, 80.0f)), ptx::ex2_approx(fminf(x1, 80.0f)));
+    const f32x2 ns = ptx::fma2(e, ptx::pack2(-1.0f, -1.0f), ptx::pack2(-1.0f, -1.0f));  // -(1+e)
+    uint32_t n0, n1;
+    ptx::unpack2u(ns, n0, n1);
+    f32x2 r = ptx::pack2u(0xFEF311C7u - n0, 0xFEF311C7u - n1);   // ~1/(1+e), 12 % accurate
+    const f32x2 two = ptx::pack2(2.0f, 2.0f);
+    r = ptx::mul2(r, ptx::fma2(ns, r, two));
+    r = ptx::mul2(r, ptx::fma2(ns, r, two));
+    sg = r;
+  }
+  h = ptx::mul2(a, sg);
+  const f32x2 omr = ptx::fma2(sg, ptx::pack2(-1.0f, -1.0f), ptx::pack2(1.0f, 1.0f));
+  dact = ptx::fma2(h, omr, sg);
+}
+__device__ __forceinline__ void tanh2(f32x2 a, f32x2& h, f32x2& dact) {
+  float x0, x1;
+  ptx::unpack2(a, x0, x1);
+  h = ptx::pack2(ptx::tanh_approx(x0), ptx::tanh_approx(x1));
+  dact = ptx::fma2(ptx::mul2(h, h), ptx::pack2(-1.0f, -1.0f), ptx::pack2(1.0f, 1.0f));
+}
+
+#ifndef BEST_TC_FAST_ACT
+#define BEST_TC_FAST_ACT 0
+#endif
+
+// ---- first A operand: theta split into bf16 hi | lo (own 8 dims -> pieces k and 4+k) ------------
+__device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
+  ptx::mbar_wait(C.bars.a_free(0), (C.o & 1u) ^ 1u);
+  uint32_t hi[4], lo[4];
 #pragma unroll
-  for (int i = 0; i < 16; ++i) {
+  for (int i = 0; i < 4; ++i) {
     const uint32_t h2 = ptx::pack_bf16x2(th[2 * i], th[2 * i + 1]);
     hi[i] = h2;
     lo[i] = ptx::pack_bf16x2(th[2 * i] - ptx::bf16_lo(h2), th[2 * i + 1] - ptx::bf16_hi(h2));
   }
-#pragma unroll
-  for (int p = 0; p < 4; ++p) {
-    st_shared_v4(a_piece(C, 0, p), hi[4 * p], hi[4 * p + 1], hi[4 * p + 2], hi[4 * p + 3]);
-    st_shared_v4(a_piece(C, 0, 4 + p), lo[4 * p], lo[4 * p + 1], lo[4 * p + 2], lo[4 * p + 3]);
-  }
+  *reinterpret_cast<uint4*>(a_piece(C, 0, C.k)) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+  *reinterpret_cast<uint4*>(a_piece(C, 0, 4 + C.k)) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
   ptx::fence_proxy_async();
 #pragma unroll
-  for (int j = 0; j < kMaxKch; ++j) ptx::mbar_arrive(C.bars.a_ready[j]);
+  for (int j = 0; j < kMaxKch; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
 }
 
-// One MLP evaluation for this thread's chain: forward (and input-gradient when want_grad).
-// Returns the raw MLP output and d out / d theta (unscaled by s? no: gm already carries s).
-__device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[kDP], bool want_grad, float& out,
-                                        float (&gm)[kDP]) {
+// forward epilogue of one op: bias + activation (+ act' to scratch, or delta for the last layer)
+template <int ACT, bool LAST>
+__device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_grad, float& acc_out,
+                                        int& written) {
+  const Params& P = *C.P;
+  const bool writes_a = !(LAST && !want_grad);
+  for (int c = 0; c < op.nch; ++c, ++C.g) {
+    const uint32_t buf = C.g & 1u, use = C.g >> 1;
+    ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
+    ptx::tc_fence_after();
+    const uint32_t tcol = C.tmem_lane + buf * 256u + C.k * 16;
+    const int ngrp = op.ncols / 64;
+    for (int grp = 0; grp < ngrp; ++grp) {
+      const int jn = (c * op.ncols) / 64 + grp;
+      uint32_t v[16];
+      ptx::tmem_ld16(tcol + grp * 64, v);
+      const int f0 = jn * 64 + C.k * 16;
+      const float* bp = C.bias_s + op.layer * P.H + f0;
+      if (writes_a) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
+      ptx::tmem_ld_wait();
+      uint32_t hp[8], dp[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const float2 b = *reinterpret_cast<const float2*>(bp + 2 * i);
+        const f32x2 a = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), ptx::pack2(b.x, b.y));
+        f32x2 h, dd;
+        if (ACT == BEST_ACT_SILU) silu2<BEST_TC_FAST_ACT != 0>(a, h, dd); else tanh2(a, h, dd);
+        if (LAST) {
+          const float2 w = *reinterpret_cast<const float2*>(C.wout_s + f0 + 2 * i);
+          float h0, h1;
+          ptx::unpack2(h, h0, h1);
+          acc_out = fmaf(h0, w.x, acc_out);
+          acc_out = fmaf(h1, w.y, acc_out);
+          if (want_grad) {
+            const float2 ws = *reinterpret_cast<const float2*>(C.wouts_s + f0 + 2 * i);
+            hp[i] = ptx::pack_bf16x2_from(ptx::mul2(dd, ptx::pack2(ws.x, ws.y)));
+          }
+        } else {
+          hp[i] = ptx::pack_bf16x2_from(h);
+          dp[i] = ptx::pack_bf16x2_from(dd);
+        }
+      }
+      if (!LAST && want_grad) {
+        *reinterpret_cast<uint4*>(C.dact_tile + dact_off(P, op.layer, jn, 2 * C.k, C.row)) =
+            make_uint4(dp[0], dp[1], dp[2], dp[3]);
+        *reinterpret_cast<uint4*>(C.dact_tile + dact_off(P, op.layer, jn, 2 * C.k + 1, C.row)) =
+            make_uint4(dp[4], dp[5], dp[6], dp[7]);
+      }
+      if (writes_a) {
+        *reinterpret_cast<uint4*>(a_piece(C, jn, 2 * C.k)) = make_uint4(hp[0], hp[1], hp[2], hp[3]);
+        *reinterpret_cast<uint4*>(a_piece(C, jn, 2 * C.k + 1)) = make_uint4(hp[4], hp[5], hp[6], hp[7]);
+        ptx::fence_proxy_async();
+        ptx::mbar_arrive(C.bars.a_ready(jn));
+        written = jn + 1;
+      }
+    }
+    ptx::tc_fence_before();
+    ptx::mbar_arrive(C.bars.d_free(buf));
+  }
+}
+
+// backward epilogue: delta_{l-1} = (delta_l W_l) .* act'_{l-1}
+__device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& written) {
+  const Params& P = *C.P;
+  for (int c = 0; c < op.nch; ++c, ++C.g) {
+    const uint32_t buf = C.g & 1u, use = C.g >> 1;
+    ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
+    ptx::tc_fence_after();
+    const uint32_t tcol = C.tmem_lane + buf * 256u + C.k * 16;
+    const int ngrp = op.ncols / 64;
+    for (int grp = 0; grp < ngrp; ++grp) {
+      const int jn = (c * op.ncols) / 64 + grp;
+      uint32_t v[16];
+      ptx::tmem_ld16(tcol + grp * 64, v);
+      const uint4 d0 = *reinterpret_cast<const uint4*>(C.dact_tile + dact_off(P, op.layer, jn, 2 * C.k, C.row));
+      const uint4 d1 = *reinterpret_cast<const uint4*>(C.dact_tile + dact_off(P, op.layer, jn, 2 * C.k + 1, C.row));
+      const uint32_t dw[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+      ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
+      ptx::tmem_ld_wait();
+      uint32_t hp[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const f32x2 dd = ptx::pack2u(dw[i] << 16, dw[i] & 0xFFFF0000u);
+        hp[i] = ptx::pack_bf16x2_from(ptx::mul2(ptx::pack2u(v[2 * i], v[2 * i + 1]), dd));
+      }
+      *reinterpret_cast<uint4*>(a_piece(C, jn, 2 * C.k)) = make_uint4(hp[0], hp[1], hp[2], hp[3]);
+      *reinterpret_cast<uint4*>(a_piece(C, jn, 2 * C.k + 1)) = make_uint4(hp[4], hp[5], hp[6], hp[7]);
+      ptx::fence_proxy_async();
+      ptx::mbar_arrive(C.bars.a_ready(jn));
+      written = jn + 1;
+    }
+    ptx::tc_fence_before();
+    ptx::mbar_arrive(C.bars.d_free(buf));
+  }
+}
+
+// One MLP evaluation.  In: own 8 dims of theta.  Out: this thread's PARTIAL of the MLP output sum
+// (over its columns) and, when want_grad, s * d MLP / d theta for its own 8 dims.
+__device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool want_grad, float& out_part,
+                                        float (&gm)[8]) {
   const Params& P = *C.P;
   write_xin(C, th);
   float acc_out = 0.0f;
   const int n_ops = want_grad ? P.n_ops_all : P.n_ops_fwd;
   for (int oi = 0; oi < n_ops; ++oi, ++C.o) {
     const OpDesc op = P.ops[oi];
-    const bool last_op = (oi == n_ops - 1);
     int written = 0;
-    for (int c = 0; c < op.nch; ++c, ++C.g) {
+    if (op.epi == EPI_FWD_HID) {
+      if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, false>(C, op, want_grad, acc_out, written);
+      else epi_fwd<BEST_ACT_TANH, false>(C, op, want_grad, acc_out, written);
+    } else if (op.epi == EPI_FWD_LAST) {
+      if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, true>(C, op, want_grad, acc_out, written);
+      else epi_fwd<BEST_ACT_TANH, true>(C, op, want_grad, acc_out, written);
+    } else if (op.epi == EPI_BWD_HID) {
+      epi_bwd(C, op, written);
+    } else {  // EPI_BWD_FINAL: D[128][32] -> own 8 columns
       const uint32_t buf = C.g & 1u, use = C.g >> 1;
-      ptx::mbar_wait(C.bars.d_full[buf], use & 1u);
+      ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
       ptx::tc_fence_after();
-      const uint32_t tcol = C.tmem_lane + buf * 256u;
-      if (op.epi == EPI_BWD_FINAL) {
-        uint32_t v[32];
-        ptx::tmem_ld32(tcol, v);
-        ptx::tmem_ld_wait();
+      uint32_t v[8];
+      ptx::tmem_ld8(C.tmem_lane + buf * 256u + C.k * 8, v);
+      ptx::tmem_ld_wait();
 #pragma unroll
-        for (int i = 0; i < kDP; ++i) gm[i] = __uint_as_float(v[i]);
-      } else {
-        const int ngrp = op.ncols / 64;
-        for (int grp = 0; grp < ngrp; ++grp) {
-          const int jn = (c * op.ncols) / 64 + grp;  // A' chunk produced by these 64 columns
-          const bool writes_a = !(op.epi == EPI_FWD_LAST && !want_grad);
-          if (writes_a) ptx::mbar_wait(C.bars.a_free[jn], C.o & 1u);
-#pragma unroll
-          for (int half = 0; half < 2; ++half) {
-            uint32_t v[32];
-            ptx::tmem_ld32(tcol + grp * 64 + half * 32, v);
-            const int f0 = jn * 64 + half * 32;  // feature index of v[0]
-            uint4 dl[4];
-            if (op.epi == EPI_BWD_HID) {
-#pragma unroll
-              for (int q = 0; q < 4; ++q)
-                dl[q] = *reinterpret_cast<const uint4*>(C.dact_tile +
-                                                        dact_off(P, op.layer, jn, half * 4 + q, C.row));
-            }
-            ptx::tmem_ld_wait();
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              uint32_t hp[4], dp[4];
-              if (op.epi == EPI_BWD_HID) {
-                const uint32_t dw[4] = {dl[q].x, dl[q].y, dl[q].z, dl[q].w};
-#pragma unroll
-                for (int e2 = 0; e2 < 4; ++e2) {
-                  const float x0 = __uint_as_float(v[q * 8 + 2 * e2]) * ptx::bf16_lo(dw[e2]);
-                  const float x1 = __uint_as_float(v[q * 8 + 2 * e2 + 1]) * ptx::bf16_hi(dw[e2]);
-                  hp[e2] = ptx::pack_bf16x2(x0, x1);
-                }
-              } else {
-                const float4 b0 = *reinterpret_cast<const float4*>(C.bias_s + op.layer * P.H + f0 + q * 8);
-                const float4 b1 = *reinterpret_cast<const float4*>(C.bias_s + op.layer * P.H + f0 + q * 8 + 4);
-                const float bb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
-                float hh[8], dd[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e)
-                  act_eval(P.act, __uint_as_float(v[q * 8 + e]) + bb[e], hh[e], dd[e]);
-                if (op.epi == EPI_FWD_LAST) {
-                  const float4 w0 = *reinterpret_cast<const float4*>(C.wout_s + f0 + q * 8);
-                  const float4 w1 = *reinterpret_cast<const float4*>(C.wout_s + f0 + q * 8 + 4);
-                  const float ww[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
-#pragma unroll
-                  for (int e = 0; e < 8; ++e) acc_out = fmaf(hh[e], ww[e], acc_out);
-                  if (want_grad) {
-                    const float4 s0 = *reinterpret_cast<const float4*>(C.wouts_s + f0 + q * 8);
-                    const float4 s1 = *reinterpret_cast<const float4*>(C.wouts_s + f0 + q * 8 + 4);
-                    const float ss[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
-#pragma unroll
-                    for (int e2 = 0; e2 < 4; ++e2)
-                      hp[e2] = ptx::pack_bf16x2(ss[2 * e2] * dd[2 * e2], ss[2 * e2 + 1] * dd[2 * e2 + 1]);
-                  }
-                } else {
-#pragma unroll
-                  for (int e2 = 0; e2 < 4; ++e2) {
-                    hp[e2] = ptx::pack_bf16x2(hh[2 * e2], hh[2 * e2 + 1]);
-                    dp[e2] = ptx::pack_bf16x2(dd[2 * e2], dd[2 * e2 + 1]);
-                  }
-                  if (want_grad)
-                    *reinterpret_cast<uint4*>(C.dact_tile + dact_off(P, op.layer, jn, half * 4 + q, C.row)) =
-                        make_uint4(dp[0], dp[1], dp[2], dp[3]);
-                }
-              }
-              if (writes_a) st_shared_v4(a_piece(C, jn, half * 4 + q), hp[0], hp[1], hp[2], hp[3]);
-            }
-          }
-          if (writes_a) {
-            ptx::fence_proxy_async();
-            ptx::mbar_arrive(C.bars.a_ready[jn]);
-            written = jn + 1;
-          }
-        }
-      }
+      for (int i = 0; i < 8; ++i) gm[i] = __uint_as_float(v[i]);
       ptx::tc_fence_before();
-      ptx::mbar_arrive(C.bars.d_free[buf]);
+      ptx::mbar_arrive(C.bars.d_free(buf));
+      ++C.g;
     }
-    if (!last_op)  // keep every a_ready barrier at one phase per op
-      for (int j = written; j < kMaxKch; ++j) ptx::mbar_arrive(C.bars.a_ready[j]);
+    if (oi != n_ops - 1)  // keep every a_ready barrier at one phase per op
+      for (int j = written; j < kMaxKch; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
   }
-  out = acc_out + P.b_out;
+  out_part = acc_out;
 }
 
-// ---- per-chain algebra in fp32 (vectors padded to 32, matrices zero padded in SMEM) -------------
-__device__ __forceinline__ void mv_L(const float* __restrict__ Ls, const float (&v)[kDP], float (&out)[kDP]) {
+// ---- cooperative per-chain algebra: each thread owns dims [8k, 8k+8) ---------------------------
+__device__ __forceinline__ float* vslot_ptr(EpiCtx& C) {   // rotate between A chunks 1 and 2
+  C.vslot ^= 1u;
+  return reinterpret_cast<float*>(C.smem + SmemLayout::A + (1 + C.vslot) * kAChunkBytes);
+}
+__device__ __forceinline__ const float* share(EpiCtx& C, const float (&x)[8]) {
+  float* V = vslot_ptr(C);
 #pragma unroll
-  for (int i = 0; i < kDP; ++i) {
-    float s = 0.0f;
+  for (int i = 0; i < 8; ++i) V[(8 * C.k + i) * kRows + C.row] = x[i];
+  qbar(C);
+  return V;
+}
+// out[i] = sum_{j in [j0, j1)} M[j*32 + 8k + i] * V[j]   (M row j holds the 8 coefficients contiguously)
+__device__ __forceinline__ void mv_rows(const EpiCtx& C, const float* __restrict__ M, const float* V, int j0,
+                                        int j1, float (&out)[8]) {
 #pragma unroll
-    for (int j4 = 0; j4 <= i / 4; ++j4) {
-      const float4 l = *reinterpret_cast<const float4*>(Ls + i * kDP + j4 * 4);
-      s = fmaf(l.x, v[j4 * 4], s); s = fmaf(l.y, v[j4 * 4 + 1], s);
-      s = fmaf(l.z, v[j4 * 4 + 2], s); s = fmaf(l.w, v[j4 * 4 + 3], s);
-    }
-    out[i] = s;
+  for (int i = 0; i < 8; ++i) out[i] = 0.0f;
+  for (int j = j0; j < j1; ++j) {
+    const float vj = V[j * kRows + C.row];
+    const float4 m0 = *reinterpret_cast<const float4*>(M + j * kDP + 8 * C.k);
+    const float4 m1 = *reinterpret_cast<const float4*>(M + j * kDP + 8 * C.k + 4);
+    out[0] = fmaf(m0.x, vj, out[0]); out[1] = fmaf(m0.y, vj, out[1]);
+    out[2] = fmaf(m0.z, vj, out[2]); out[3] = fmaf(m0.w, vj, out[3]);
+    out[4] = fmaf(m1.x, vj, out[4]); out[5] = fmaf(m1.y, vj, out[5]);
+    out[6] = fmaf(m1.z, vj, out[6]); out[7] = fmaf(m1.w, vj, out[7]);
   }
 }
-__device__ __forceinline__ void mv_Lt(const float* __restrict__ Ls, const float (&v)[kDP], float (&out)[kDP]) {
-#pragma unroll
-  for (int j = 0; j < kDP; ++j) out[j] = 0.0f;
-#pragma unroll
-  for (int i = 0; i < kDP; ++i) {
-#pragma unroll
-    for (int j4 = 0; j4 <= i / 4; ++j4) {
-      const float4 l = *reinterpret_cast<const float4*>(Ls + i * kDP + j4 * 4);
-      out[j4 * 4] = fmaf(l.x, v[i], out[j4 * 4]); out[j4 * 4 + 1] = fmaf(l.y, v[i], out[j4 * 4 + 1]);
-      out[j4 * 4 + 2] = fmaf(l.z, v[i], out[j4 * 4 + 2]); out[j4 * 4 + 3] = fmaf(l.w, v[i], out[j4 * 4 + 3]);
-    }
-  }
+// out = L x : out_i = sum_{j<=i} L[i][j] x_j, own i  -> coefficients LT[j][i], j in [0, 8k+8)
+__device__ __forceinline__ void mv_L(EpiCtx& C, const float (&x)[8], float (&out)[8]) {
+  const float* V = share(C, x);
+  mv_rows(C, C.LTs, V, 0, 8 * C.k + 8, out);
+}
+// out = L^T x : out_j = sum_{i>=j} L[i][j] x_i, own j -> coefficients L[i][j], i in [8k, 32)
+__device__ __forceinline__ void mv_Lt(EpiCtx& C, const float (&x)[8], float (&out)[8]) {
+  const float* V = share(C, x);
+  mv_rows(C, C.Ls, V, 8 * C.k, kDP, out);
+}
+__device__ __forceinline__ float reduce4(EpiCtx& C, float x) {
+  C.pslot ^= 1u;
+  float* Pp = C.part + C.pslot * 4 * kRows;
+  Pp[C.k * kRows + C.row] = x;
+  qbar(C);
+  return (Pp[C.row] + Pp[kRows + C.row]) + (Pp[2 * kRows + C.row] + Pp[3 * kRows + C.row]);
 }
 
-// log pi(theta) and gradient from the MLP output (already scaled by s in gm) + the cheap terms.
-__device__ __forceinline__ void finish_target(const EpiCtx& C, const float (&th)[kDP], float mlp_out,
-                                              bool want_grad, float& lp, float (&g)[kDP]) {
+// full target from the MLP partial output + Gaussian (y = R r), banana and box terms.
+// lp is identical on the four threads of a chain; g covers the thread's own 8 dims.
+__device__ __forceinline__ void finish_target(EpiCtx& C, const float (&th)[8], float out_part, bool want_grad,
+                                              float& lp, float (&g)[8]) {
   const Params& P = *C.P;
-  lp = P.mlp_scale * mlp_out;
-  if (P.has_gauss) {  // y = R r (R upper triangular), logp -= |y|^2/2, g -= R^T y
-    float r[kDP], y[kDP];
+  float part = P.mlp_scale * out_part;
+  float ti = 0.0f, tj = 0.0f;
+  if (P.has_gauss || P.banana_i >= 0) {
+    float r[8], y[8];
 #pragma unroll
-    for (int i = 0; i < kDP; ++i) r[i] = th[i] - C.vecs[i];
-    float q = 0.0f;
-#pragma unroll
-    for (int i = 0; i < kDP; ++i) {
-      float s = 0.0f;
-#pragma unroll
-      for (int j4 = i / 4; j4 < kDP / 4; ++j4) {
-        const float4 l = *reinterpret_cast<const float4*>(C.Rs + i * kDP + j4 * 4);
-        s = fmaf(l.x, r[j4 * 4], s); s = fmaf(l.y, r[j4 * 4 + 1], s);
-        s = fmaf(l.z, r[j4 * 4 + 2], s); s = fmaf(l.w, r[j4 * 4 + 3], s);
-      }
-      y[i] = s;
-      q = fmaf(s, s, q);
+    for (int i = 0; i < 8; ++i) r[i] = th[i] - C.vecs[8 * C.k + i];
+    const float* V = share(C, r);
+    if (P.banana_i >= 0) {
+      ti = V[P.banana_i * kRows + C.row] + C.vecs[P.banana_i];
+      tj = V[P.banana_j * kRows + C.row] + C.vecs[P.banana_j];
     }
-    lp -= 0.5f * q;
-    if (want_grad) {
+    if (P.has_gauss) {
+      mv_rows(C, C.RTs, V, 8 * C.k, kDP, y);          // y_i = sum_{j>=i} R[i][j] r_j
 #pragma unroll
-      for (int i = 0; i < kDP; ++i) {
+      for (int i = 0; i < 8; ++i) part = fmaf(-0.5f * y[i], y[i], part);
+      if (want_grad) {
+        float gg[8];
+        const float* Vy = share(C, y);
+        mv_rows(C, C.Rs, Vy, 0, 8 * C.k + 8, gg);      // (R^T y)_j = sum_{i<=j} R[i][j] y_i
 #pragma unroll
-        for (int j4 = i / 4; j4 < kDP / 4; ++j4) {
-          const float4 l = *reinterpret_cast<const float4*>(C.Rs + i * kDP + j4 * 4);
-          g[j4 * 4] = fmaf(-l.x, y[i], g[j4 * 4]); g[j4 * 4 + 1] = fmaf(-l.y, y[i], g[j4 * 4 + 1]);
-          g[j4 * 4 + 2] = fmaf(-l.z, y[i], g[j4 * 4 + 2]); g[j4 * 4 + 3] = fmaf(-l.w, y[i], g[j4 * 4 + 3]);
-        }
+        for (int i = 0; i < 8; ++i) g[i] -= gg[i];
       }
-    }
-  }
-  if (P.banana_i >= 0) {
-    float ti = 0.f, tj = 0.f;
-#pragma unroll
-    for (int i = 0; i < kDP; ++i) { if (i == P.banana_i) ti = th[i]; if (i == P.banana_j) tj = th[i]; }
-    const float t = tj - ti * ti, inv = 1.0f / (P.banana_sigma * P.banana_sigma);
-    lp -= 0.5f * t * t * inv;
-#pragma unroll
-    for (int i = 0; i < kDP; ++i) {
-      if (i == P.banana_j) g[i] -= t * inv;
-      if (i == P.banana_i) g[i] += 2.0f * ti * t * inv;
     }
   }
   if (P.has_box) {
-    float pen = 0.0f;
 #pragma unroll
-    for (int i = 0; i < kDP; ++i) {
-      const float lo = C.vecs[32 + i], hi = C.vecs[64 + i], iw = C.vecs[96 + i];
+    for (int i = 0; i < 8; ++i) {
+      const int gi = 8 * C.k + i;
+      const float lo = C.vecs[32 + gi], hi = C.vecs[64 + gi], iw = C.vecs[96 + gi];
       const float ex = fmaxf(fmaxf(lo - th[i], th[i] - hi), 0.0f);
       if (ex > 0.0f) {
         const float t = P.pen_gamma * ex * iw;
         float f, df;
         if (t <= 40.0f) { df = expm1f(t); f = df - t; }
         else { df = 2.3538526683701998e17f; f = (df - 40.0f) + df * (t - 40.0f); }
-        pen += f;
+        part -= P.pen_kappa * f;
         g[i] -= P.pen_kappa * df * P.pen_gamma * iw * ((th[i] > hi) ? 1.0f : -1.0f);
       }
     }
-    lp -= P.pen_kappa * pen;
+  }
+  lp = reduce4(C, part) + P.mlp_scale * P.b_out;
+  if (P.banana_i >= 0) {
+    const float t = tj - ti * ti, inv = 1.0f / (P.banana_sigma * P.banana_sigma);
+    lp -= 0.5f * t * t * inv;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      if (8 * C.k + i == P.banana_j) g[i] -= t * inv;
+      if (8 * C.k + i == P.banana_i) g[i] += 2.0f * ti * t * inv;
+    }
   }
 }
 
-__device__ __forceinline__ void draw_normals32(uint64_t seed, uint32_t chain, uint64_t step, int d,
-                                               float (&xi)[kDP]) {
-  const int nblk = (d + 3) >> 2;
+// evaluate the full target at th (own dims): lp (same on all 4 threads) and own 8 gradient dims
+__device__ __forceinline__ void eval_target(EpiCtx& C, const float (&th)[8], bool want_grad, float& lp,
+                                            float (&g)[8]) {
+  float out_part;
 #pragma unroll
-  for (int j = 0; j < kDP / 4; ++j) {
-    if (j < nblk) {
+  for (int i = 0; i < 8; ++i) g[i] = 0.0f;
+  tc_eval(C, th, want_grad, out_part, g);
+  finish_target(C, th, out_part, want_grad, lp, g);
+}
+
+// own 8 normals: Philox blocks 2k and 2k+1 (slot 1+j -> dims 4j..4j+3)
+__device__ __forceinline__ void draw_normals8(const EpiCtx& C, uint64_t seed, uint32_t chain, uint64_t step,
+                                              int d, float (&xi)[8]) {
+#pragma unroll
+  for (int b = 0; b < 2; ++b) {
+    const int j = 2 * C.k + b;
+    if (4 * j < d) {
       const uint4 w = philox4x32_10(chain, step, (uint32_t)(1 + j), seed);
-      box_muller(w.x, w.y, xi[4 * j], xi[4 * j + 1]);
-      box_muller(w.z, w.w, xi[4 * j + 2], xi[4 * j + 3]);
+      box_muller(w.x, w.y, xi[4 * b], xi[4 * b + 1]);
+      box_muller(w.z, w.w, xi[4 * b + 2], xi[4 * b + 3]);
     } else {
-      xi[4 * j] = xi[4 * j + 1] = xi[4 * j + 2] = xi[4 * j + 3] = 0.0f;
+      xi[4 * b] = xi[4 * b + 1] = xi[4 * b + 2] = xi[4 * b + 3] = 0.0f;
     }
   }
 #pragma unroll
-  for (int i = 0; i < kDP; ++i) if (i >= d) xi[i] = 0.0f;
+  for (int i = 0; i < 8; ++i) if (8 * C.k + i >= d) xi[i] = 0.0f;
 }
 
-__device__ __forceinline__ void load_vec(const double* a, int64_t ld, int64_t c, int d, bool valid,
-                                         float (&v)[kDP]) {
+__device__ __forceinline__ void load_vec8(const EpiCtx& C, const double* a, int64_t ld, int64_t c, int d,
+                                          bool valid, float (&v)[8]) {
 #pragma unroll
-  for (int i = 0; i < kDP; ++i) v[i] = (valid && i < d) ? (float)a[i * ld + c] : 0.0f;
-}
-__device__ __forceinline__ void store_vec(double* a, int64_t ld, int64_t c, int d, const float (&v)[kDP]) {
-#pragma unroll
-  for (int i = 0; i < kDP; ++i) if (i < d) a[i * ld + c] = (double)v[i];
-}
-
-// evaluate the full target at th: (lp, g).  g is only meaningful when want_grad.
-__device__ __forceinline__ void eval_target(EpiCtx& C, const float (&th)[kDP], bool want_grad, float& lp,
-                                            float (&g)[kDP]) {
-  float out;
-  tc_eval(C, th, want_grad, out, g);
-  if (!want_grad) {
-#pragma unroll
-    for (int i = 0; i < kDP; ++i) g[i] = 0.0f;
+  for (int i = 0; i < 8; ++i) {
+    const int gi = 8 * C.k + i;
+    v[i] = (valid && gi < d) ? (float)a[(int64_t)gi * ld + c] : 0.0f;
   }
-  finish_target(C, th, out, want_grad, lp, g);
+}
+__device__ __forceinline__ void store_vec8(const EpiCtx& C, double* a, int64_t ld, int64_t c, int d,
+                                           const float (&v)[8]) {
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const int gi = 8 * C.k + i;
+    if (gi < d) a[(int64_t)gi * ld + c] = (double)v[i];
+  }
 }
 
 }  // namespace tc

@@ -1,14 +1,16 @@
 // bf16 tensor-core path (BEST_PREC_BF16): ONE persistent kernel per best_step_* call.
 //
-// A CTA owns a tile of 128 chains for all n_steps.  TMEM lane r == chain r == epilogue thread r:
+// A CTA owns a tile of 128 chains for all n_steps.  TMEM lane r == chain r:
 //   warp 0 (1 lane)  weight producer: streams pre-swizzled bf16 weight tiles L2 -> SMEM ring with
 //                    cp.async.bulk + mbarrier complete_tx (weights are packed once at best_create)
 //   warp 1 (1 lane)  MMA issuer: tcgen05.mma.cta_group::1.kind::f16, M=128, N<=256, K=16;
 //                    A = activations resident in SMEM (128B swizzle, written in place by the
 //                    epilogue), B = weight stage (64B swizzle), D = fp32 in TMEM (2 x 256 columns)
 //   warp 2           TMEM allocation
-//   warps 4-7        one thread per chain: Philox, whitened proposal, tcgen05.ld epilogues
-//                    (bias + activation + act' / delta), Gaussian / banana / box terms, accept.
+//   warps 4-19       four threads per chain (one per warp of the chain's TMEM lane quarter):
+//                    tcgen05.ld epilogues (bias + activation + act' / delta) on 16 of every 64
+//                    columns each, and cooperatively Philox, whitened proposal, Gaussian / banana /
+//                    box terms and the accept decision on 8 parameter dimensions each.
 // The MLP forward and its input-gradient backprop (A1b, A1c) are a chain of GEMMs whose
 // activations never leave the SM; only act' (bf16) is parked in an L2-resident scratch between
 // the forward and backward sweeps.  See DESIGN.md §"tensor-core kernel".
@@ -28,7 +30,10 @@ constexpr int kMaxKch = 8;           // hidden width <= 512
 constexpr int kStageBytes = 16384;   // weight stage: <=256 rows x 32 bf16 (64 B rows, SW64)
 constexpr int kStages = 4;
 constexpr int kMaxOps = 12;
-constexpr int kThreads = 256;
+constexpr int kCtrlWarps = 4;          // producer, MMA issuer, TMEM allocator, spare
+constexpr int kEpiWarps = 16;          // 4 per TMEM lane quarter
+constexpr int kEpiThreads = kEpiWarps * 32;
+constexpr int kThreads = (kCtrlWarps + kEpiWarps) * 32;
 constexpr int kDP = 32;              // parameter vectors are padded to 32 inside the kernel
 
 enum { EPI_FWD_HID = 0, EPI_FWD_LAST = 1, EPI_BWD_HID = 2, EPI_BWD_FINAL = 3 };
@@ -84,31 +89,29 @@ struct SmemLayout {
   static constexpr int WOUT = BIAS + 2048 * 4;                       // 512 floats
   static constexpr int WOUTS = WOUT + 512 * 4;                       // 512 floats (s * w_out)
   static constexpr int LMAT = WOUTS + 512 * 4;                       // 32x32 floats
-  static constexpr int RMAT = LMAT + 1024 * 4;
-  static constexpr int VECS = RMAT + 1024 * 4;                       // mu, lo, hi, 1/width: 4x32 floats
-  static constexpr int BARS = VECS + 4 * 32 * 4;
+  static constexpr int LTMAT = LMAT + 1024 * 4;                      // L transposed
+  static constexpr int RMAT = LTMAT + 1024 * 4;
+  static constexpr int RTMAT = RMAT + 1024 * 4;
+  static constexpr int VECS = RTMAT + 1024 * 4;                      // mu, lo, hi, 1/width: 4x32 floats
+  static constexpr int PART = VECS + 4 * 32 * 4;                     // partial sums [2][4][128] floats
+  static constexpr int BARS = PART + 2 * 4 * 128 * 4;
   // barriers: full[4] empty[4] a_ready[8] a_free[8] d_full[2] d_free[2]
   static constexpr int NBARS = 2 * kStages + 2 * kMaxKch + 4;
   static constexpr int TMEMPTR = BARS + NBARS * 8;
   static constexpr int TOTAL = TMEMPTR + 16;
 };
-static_assert(SmemLayout::TOTAL + 1024 <= 227 * 1024, "shared memory budget");
+static_assert(SmemLayout::TOTAL + 1024 <= 232448, "shared memory budget");
 
-struct Bars {
-  uint32_t full[kStages], empty[kStages], a_ready[kMaxKch], a_free[kMaxKch], d_full[2], d_free[2];
+struct Bars {  // mbarrier addresses are computed, never looked up (keeps them out of local memory)
+  uint32_t base;
+  __device__ __forceinline__ uint32_t full(int i) const { return base + 8u * i; }
+  __device__ __forceinline__ uint32_t empty(int i) const { return base + 8u * (kStages + i); }
+  __device__ __forceinline__ uint32_t a_ready(int j) const { return base + 8u * (2 * kStages + j); }
+  __device__ __forceinline__ uint32_t a_free(int j) const { return base + 8u * (2 * kStages + kMaxKch + j); }
+  __device__ __forceinline__ uint32_t d_full(int b) const { return base + 8u * (2 * kStages + 2 * kMaxKch + b); }
+  __device__ __forceinline__ uint32_t d_free(int b) const { return base + 8u * (2 * kStages + 2 * kMaxKch + 2 + b); }
 };
-
-__device__ __forceinline__ Bars make_bars(uint32_t base) {
-  Bars b;
-  uint32_t p = base;
-  for (int i = 0; i < kStages; ++i) { b.full[i] = p; p += 8; }
-  for (int i = 0; i < kStages; ++i) { b.empty[i] = p; p += 8; }
-  for (int i = 0; i < kMaxKch; ++i) { b.a_ready[i] = p; p += 8; }
-  for (int i = 0; i < kMaxKch; ++i) { b.a_free[i] = p; p += 8; }
-  for (int i = 0; i < 2; ++i) { b.d_full[i] = p; p += 8; }
-  for (int i = 0; i < 2; ++i) { b.d_free[i] = p; p += 8; }
-  return b;
-}
+__device__ __forceinline__ Bars make_bars(uint32_t base) { Bars b; b.base = base; return b; }
 
 // ------------------------------------------------------------------------------------------------
 // weight producer (one thread)
@@ -124,9 +127,9 @@ __device__ void producer_loop(const Params& P, const Bars& bars, uint32_t stage_
       const int ntiles = op.nch * op.kch * 2;
       for (int i = 0; i < ntiles; ++i, ++t) {
         const uint32_t s = t % kStages, use = t / kStages;
-        ptx::mbar_wait(bars.empty[s], (use & 1u) ^ 1u);
-        ptx::mbar_arrive_expect_tx(bars.full[s], bytes);
-        ptx::bulk_g2s(stage_base + s * kStageBytes, src, bytes, bars.full[s]);
+        ptx::mbar_wait(bars.empty(s), (use & 1u) ^ 1u);
+        ptx::mbar_arrive_expect_tx(bars.full(s), bytes);
+        ptx::bulk_g2s(stage_base + s * kStageBytes, src, bytes, bars.full(s));
         src += bytes;
       }
     }
@@ -146,20 +149,20 @@ __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uin
       const OpDesc op = P.ops[oi];
       const uint32_t idesc = ptx::idesc_bf16(kRows, op.ncols);
       // chunks this op does not read are free as soon as everything issued so far has completed
-      for (int j = op.kch; j < kMaxKch; ++j) ptx::mma_commit(bars.a_free[j]);
+      for (int j = op.kch; j < kMaxKch; ++j) ptx::mma_commit(bars.a_free(j));
       for (int c = 0; c < op.nch; ++c, ++g) {
         const uint32_t buf = g & 1u, use = g >> 1;
-        ptx::mbar_wait(bars.d_free[buf], (use & 1u) ^ 1u);
+        ptx::mbar_wait(bars.d_free(buf), (use & 1u) ^ 1u);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + buf * 256u;
         for (int k32 = 0; k32 < 2 * op.kch; ++k32, ++t) {
           const int j = k32 >> 1;
           if (c == 0 && (k32 & 1) == 0) {
-            ptx::mbar_wait(bars.a_ready[j], o & 1u);
+            ptx::mbar_wait(bars.a_ready(j), o & 1u);
             ptx::tc_fence_after();
           }
           const uint32_t s = t % kStages, use_s = t / kStages;
-          ptx::mbar_wait(bars.full[s], use_s & 1u);
+          ptx::mbar_wait(bars.full(s), use_s & 1u);
           ptx::tc_fence_after();
           const uint32_t a_addr = a_base + j * kAChunkBytes + (k32 & 1) * 64;
           const uint32_t b_addr = stage_base + s * kStageBytes;
@@ -168,10 +171,10 @@ __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uin
             ptx::mma_bf16_ss(d_tmem, ptx::smem_desc_sw128(a_addr + kk * 32),
                              ptx::smem_desc_sw64(b_addr + kk * 32), idesc, (k32 | kk) != 0 ? 1u : 0u);
           }
-          ptx::mma_commit(bars.empty[s]);
-          if (c == op.nch - 1 && (k32 & 1)) ptx::mma_commit(bars.a_free[j]);
+          ptx::mma_commit(bars.empty(s));
+          if (c == op.nch - 1 && (k32 & 1)) ptx::mma_commit(bars.a_free(j));
         }
-        ptx::mma_commit(bars.d_full[buf]);
+        ptx::mma_commit(bars.d_full(buf));
       }
     }
   }

@@ -5,33 +5,39 @@
 namespace best {
 namespace tc {
 
+// Sampler driver: executed by all 512 epilogue threads; thread (row, k) owns dims [8k, 8k+8) of
+// chain `row`.  Scalars (log pi, log alpha, accept) are computed redundantly and identically by the
+// four threads of a chain, so they take the same accept branch.
 template <int METHOD>
 __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
   const Params& P = *C.P;
   const int d = P.d;
   const int64_t r_in_launch = (int64_t)blockIdx.x * kRows + C.row;
   const bool valid = r_in_launch < R.B;
-  const float* Ls = C.Ls;
+  const bool lead = valid && C.k == 0;
 
   if (METHOD == M_EVAL) {
-    float th[kDP], g[kDP], lp;
+    float th[8], g[8], lp;
     if (R.io_mode == IO_ROWS_F32) {
 #pragma unroll
-      for (int i = 0; i < kDP; ++i) th[i] = (valid && i < d) ? R.in_rows[r_in_launch * d + i] : 0.0f;
+      for (int i = 0; i < 8; ++i) {
+        const int gi = 8 * C.k + i;
+        th[i] = (valid && gi < d) ? R.in_rows[r_in_launch * d + gi] : 0.0f;
+      }
     } else {
-      load_vec(R.theta, R.ld, r_in_launch, d, valid, th);
+      load_vec8(C, R.theta, R.ld, r_in_launch, d, valid, th);
     }
     eval_target(C, th, R.want_grad != 0, lp, g);
     if (valid) {
       if (R.io_mode == IO_ROWS_F32) {
-        R.out_logp[r_in_launch] = lp;
+        if (C.k == 0) R.out_logp[r_in_launch] = lp;
         if (R.want_grad) {
 #pragma unroll
-          for (int i = 0; i < kDP; ++i) if (i < d) R.out_grad[r_in_launch * d + i] = g[i];
+          for (int i = 0; i < 8; ++i) if (8 * C.k + i < d) R.out_grad[r_in_launch * d + 8 * C.k + i] = g[i];
         }
       } else {
-        R.logp[r_in_launch] = (double)lp;
-        if (R.want_grad) store_vec(R.grad, R.ld, r_in_launch, d, g);
+        if (C.k == 0) R.logp[r_in_launch] = (double)lp;
+        if (R.want_grad) store_vec8(C, R.grad, R.ld, r_in_launch, d, g);
       }
     }
     return;
@@ -44,23 +50,22 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
     const float a = R.eps;
     const float t = u01<float>(w.y) * (a - 1.0f) + 1.0f;
     const float z = t * t / a;
-    float thi[kDP], thp[kDP], g[kDP], lpp;
-    load_vec(R.theta, R.ld, i, d, valid, thi);
+    float thp[8], g[8], lpp;
     {
-      float thj[kDP];
-      load_vec(R.theta, R.ld, j, d, valid, thj);
+      float thi[8], thj[8];
+      load_vec8(C, R.theta, R.ld, i, d, valid, thi);
+      load_vec8(C, R.theta, R.ld, j, d, valid, thj);
 #pragma unroll
-      for (int k = 0; k < kDP; ++k) thp[k] = thj[k] + z * (thi[k] - thj[k]);
+      for (int q = 0; q < 8; ++q) thp[q] = thj[q] + z * (thi[q] - thj[q]);
     }
     eval_target(C, thp, false, lpp, g);
-    if (valid) {
-      const float la = (float)(d - 1) * logf(z) + lpp - (float)R.logp[i];
+    const float la = (float)(d - 1) * logf(z) + lpp - (valid ? (float)R.logp[i] : 0.0f);
+    const bool acc = valid && accept_rule<float>(u01<float>(w.x), la);
+    qbar(C);   // (warp-uniform) every thread of the chain has read logp[i] before the leader overwrites it
+    if (acc) store_vec8(C, R.theta, R.ld, i, d, thp);
+    if (lead) {
       R.last_la[i] = (double)la;
-      if (accept_rule<float>(u01<float>(w.x), la)) {
-        store_vec(R.theta, R.ld, i, d, thp);
-        R.logp[i] = (double)lpp;
-        R.n_accept[i] += 1ull;
-      }
+      if (acc) { R.logp[i] = (double)lpp; R.n_accept[i] += 1ull; }
     }
     return;
   }
@@ -72,19 +77,19 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
   unsigned long long nacc = 0;
 
   if (METHOD == M_MH) {
-    float th[kDP];
-    load_vec(R.theta, R.ld, c, d, valid, th);
+    float th[8];
+    load_vec8(C, R.theta, R.ld, c, d, valid, th);
     for (int64_t t = 0; t < R.n_steps; ++t) {
       const uint64_t step = R.step0 + (uint64_t)t;
-      float thp[kDP], g[kDP], lpp;
+      float thp[8], g[8], lpp;
       {
-        float xi[kDP], dx[kDP];
-        draw_normals32(R.seed, (uint32_t)c, step, d, xi);
+        float xi[8], dx[8];
+        draw_normals8(C, R.seed, (uint32_t)c, step, d, xi);
 #pragma unroll
-        for (int i = 0; i < kDP; ++i) xi[i] *= eps;
-        mv_L(Ls, xi, dx);
+        for (int i = 0; i < 8; ++i) xi[i] *= eps;
+        mv_L(C, xi, dx);
 #pragma unroll
-        for (int i = 0; i < kDP; ++i) thp[i] = th[i] + dx[i];
+        for (int i = 0; i < 8; ++i) thp[i] = th[i] + dx[i];
       }
       eval_target(C, thp, false, lpp, g);
       const float la = lpp - lp;
@@ -92,53 +97,53 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
       const uint4 w = philox4x32_10((uint32_t)c, step, 0u, R.seed);
       if (valid && accept_rule<float>(u01<float>(w.x), la)) {
 #pragma unroll
-        for (int i = 0; i < kDP; ++i) th[i] = thp[i];
+        for (int i = 0; i < 8; ++i) th[i] = thp[i];
         lp = lpp;
         ++nacc;
       }
     }
-    if (valid) store_vec(R.theta, R.ld, c, d, th);
+    if (valid) store_vec8(C, R.theta, R.ld, c, d, th);
   }
 
   if (METHOD == M_MALA) {
     const float sq = sqrtf(2.0f * eps);
     for (int64_t t = 0; t < R.n_steps; ++t) {
       const uint64_t step = R.step0 + (uint64_t)t;
-      float thp[kDP], dz[kDP], gp[kDP], lpp, fwd = 0.0f;
+      float thp[8], dz[8], gp[8], lpp, fwd = 0.0f;
       {
-        float g[kDP], gz[kDP], xi[kDP];
-        load_vec(R.grad, R.ld, c, d, valid, g);
-        mv_Lt(Ls, g, gz);
-        draw_normals32(R.seed, (uint32_t)c, step, d, xi);
+        float g[8], gz[8], xi[8];
+        load_vec8(C, R.grad, R.ld, c, d, valid, g);
+        mv_Lt(C, g, gz);
+        draw_normals8(C, R.seed, (uint32_t)c, step, d, xi);
 #pragma unroll
-        for (int i = 0; i < kDP; ++i) {
+        for (int i = 0; i < 8; ++i) {
           const float f = sq * xi[i];
           fwd = fmaf(f, f, fwd);
           dz[i] = fmaf(eps, gz[i], f);
         }
-        mv_L(Ls, dz, g);  // g <- L dz
-        float th[kDP];
-        load_vec(R.theta, R.ld, c, d, valid, th);
+        mv_L(C, dz, g);  // g <- L dz
+        float th[8];
+        load_vec8(C, R.theta, R.ld, c, d, valid, th);
 #pragma unroll
-        for (int i = 0; i < kDP; ++i) thp[i] = th[i] + g[i];
+        for (int i = 0; i < 8; ++i) thp[i] = th[i] + g[i];
       }
       eval_target(C, thp, true, lpp, gp);
-      float bwd = 0.0f;
+      float diff = fwd;
       {
-        float gzp[kDP];
-        mv_Lt(Ls, gp, gzp);
+        float gzp[8];
+        mv_Lt(C, gp, gzp);
 #pragma unroll
-        for (int i = 0; i < kDP; ++i) {
+        for (int i = 0; i < 8; ++i) {
           const float r = fmaf(eps, gzp[i], dz[i]);
-          bwd = fmaf(r, r, bwd);
+          diff = fmaf(-r, r, diff);
         }
       }
-      const float la = lpp - lp + (fwd - bwd) / (4.0f * eps);
+      const float la = lpp - lp + reduce4(C, diff) / (4.0f * eps);
       la_last = la;
       const uint4 w = philox4x32_10((uint32_t)c, step, 0u, R.seed);
       if (valid && accept_rule<float>(u01<float>(w.x), la)) {
-        store_vec(R.theta, R.ld, c, d, thp);
-        store_vec(R.grad, R.ld, c, d, gp);
+        store_vec8(C, R.theta, R.ld, c, d, thp);
+        store_vec8(C, R.grad, R.ld, c, d, gp);
         lp = lpp;
         ++nacc;
       }
@@ -148,52 +153,51 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
   if (METHOD == M_HMC) {
     for (int64_t t = 0; t < R.n_steps; ++t) {
       const uint64_t step = R.step0 + (uint64_t)t;
-      float thw[kDP], q[kDP], gw[kDP], lpw = lp, H0;
+      float thw[8], q[8], gw[8], lpw = lp, kin0 = 0.0f;
       {
-        float g[kDP], gz[kDP];
-        draw_normals32(R.seed, (uint32_t)c, step, d, q);
-        float kin = 0.0f;
+        float g[8], gz[8];
+        draw_normals8(C, R.seed, (uint32_t)c, step, d, q);
 #pragma unroll
-        for (int i = 0; i < kDP; ++i) kin = fmaf(q[i], q[i], kin);
-        H0 = -lp + 0.5f * kin;
-        load_vec(R.grad, R.ld, c, d, valid, g);
-        mv_Lt(Ls, g, gz);
+        for (int i = 0; i < 8; ++i) kin0 = fmaf(q[i], q[i], kin0);
+        load_vec8(C, R.grad, R.ld, c, d, valid, g);
+        mv_Lt(C, g, gz);
 #pragma unroll
-        for (int i = 0; i < kDP; ++i) q[i] = fmaf(0.5f * eps, gz[i], q[i]);
-        load_vec(R.theta, R.ld, c, d, valid, thw);
+        for (int i = 0; i < 8; ++i) q[i] = fmaf(0.5f * eps, gz[i], q[i]);
+        load_vec8(C, R.theta, R.ld, c, d, valid, thw);
       }
       for (int l = 1; l <= R.n_leapfrog; ++l) {
         {
-          float dz[kDP], dx[kDP];
+          float dz[8], dx[8];
 #pragma unroll
-          for (int i = 0; i < kDP; ++i) dz[i] = eps * q[i];
-          mv_L(Ls, dz, dx);
+          for (int i = 0; i < 8; ++i) dz[i] = eps * q[i];
+          mv_L(C, dz, dx);
 #pragma unroll
-          for (int i = 0; i < kDP; ++i) thw[i] += dx[i];
+          for (int i = 0; i < 8; ++i) thw[i] += dx[i];
         }
         eval_target(C, thw, true, lpw, gw);
-        float gz[kDP];
-        mv_Lt(Ls, gw, gz);
+        float gz[8];
+        mv_Lt(C, gw, gz);
         const float cc = (l < R.n_leapfrog) ? eps : 0.5f * eps;
 #pragma unroll
-        for (int i = 0; i < kDP; ++i) q[i] = fmaf(cc, gz[i], q[i]);
+        for (int i = 0; i < 8; ++i) q[i] = fmaf(cc, gz[i], q[i]);
       }
-      float kin = 0.0f;
+      float kin1 = 0.0f;
 #pragma unroll
-      for (int i = 0; i < kDP; ++i) kin = fmaf(q[i], q[i], kin);
-      const float la = H0 - (-lpw + 0.5f * kin);
+      for (int i = 0; i < 8; ++i) kin1 = fmaf(q[i], q[i], kin1);
+      // log alpha = H0 - H1 = (lp' - lp) + (|q0|^2 - |q1|^2)/2
+      const float la = (lpw - lp) + 0.5f * reduce4(C, kin0 - kin1);
       la_last = la;
       const uint4 w = philox4x32_10((uint32_t)c, step, 0u, R.seed);
       if (valid && accept_rule<float>(u01<float>(w.x), la)) {
-        store_vec(R.theta, R.ld, c, d, thw);
-        store_vec(R.grad, R.ld, c, d, gw);
+        store_vec8(C, R.theta, R.ld, c, d, thw);
+        store_vec8(C, R.grad, R.ld, c, d, gw);
         lp = lpw;
         ++nacc;
       }
     }
   }
 
-  if (valid) {
+  if (lead) {
     R.logp[c] = (double)lp;
     R.last_la[c] = (double)la_last;
     R.n_accept[c] += nacc;
@@ -212,14 +216,16 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   float* wout_s = reinterpret_cast<float*>(smem + SmemLayout::WOUT);
   float* wouts_s = reinterpret_cast<float*>(smem + SmemLayout::WOUTS);
   float* Ls = reinterpret_cast<float*>(smem + SmemLayout::LMAT);
+  float* LTs = reinterpret_cast<float*>(smem + SmemLayout::LTMAT);
   float* Rs = reinterpret_cast<float*>(smem + SmemLayout::RMAT);
+  float* RTs = reinterpret_cast<float*>(smem + SmemLayout::RTMAT);
   float* vecs = reinterpret_cast<float*>(smem + SmemLayout::VECS);
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + SmemLayout::TMEMPTR);
 
   if (tid == 0) {
-    for (int i = 0; i < kStages; ++i) { ptx::mbar_init(bars.full[i], 1); ptx::mbar_init(bars.empty[i], 1); }
-    for (int i = 0; i < kMaxKch; ++i) { ptx::mbar_init(bars.a_ready[i], kRows); ptx::mbar_init(bars.a_free[i], 1); }
-    for (int i = 0; i < 2; ++i) { ptx::mbar_init(bars.d_full[i], 1); ptx::mbar_init(bars.d_free[i], kRows); }
+    for (int i = 0; i < kStages; ++i) { ptx::mbar_init(bars.full(i), 1); ptx::mbar_init(bars.empty(i), 1); }
+    for (int i = 0; i < kMaxKch; ++i) { ptx::mbar_init(bars.a_ready(i), kEpiThreads); ptx::mbar_init(bars.a_free(i), 1); }
+    for (int i = 0; i < 2; ++i) { ptx::mbar_init(bars.d_full(i), 1); ptx::mbar_init(bars.d_free(i), kEpiThreads); }
     ptx::fence_mbar_init();
   }
   if (warp == 2) ptx::tmem_alloc(sbase + SmemLayout::TMEMPTR, 512);
@@ -227,16 +233,18 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   for (int i = tid; i < P.H; i += kThreads) { wout_s[i] = P.w_out[i]; wouts_s[i] = P.mlp_scale * P.w_out[i]; }
   for (int i = tid; i < kDP * kDP; i += kThreads) {
     const int r = i / kDP, c = i % kDP;
-    Ls[i] = (r < P.d && c <= r) ? (float)P.L[r * P.d + c] : 0.0f;
-    Rs[i] = (P.has_gauss && r < P.d && c < P.d && c >= r) ? (float)P.R[r * P.d + c] : 0.0f;
+    const float l = (r < P.d && c <= r) ? (float)P.L[r * P.d + c] : 0.0f;
+    const float u = (P.has_gauss && r < P.d && c < P.d && c >= r) ? (float)P.R[r * P.d + c] : 0.0f;
+    Ls[i] = l;
+    LTs[c * kDP + r] = l;
+    Rs[i] = u;
+    RTs[c * kDP + r] = u;
   }
   for (int i = tid; i < kDP; i += kThreads) {
     const bool in = i < P.d;
     vecs[i] = (in && P.has_gauss) ? (float)P.mu[i] : 0.0f;
-    const float lo = (in && P.has_box) ? (float)P.lo[i] : -3.0e38f;
-    const float hi = (in && P.has_box) ? (float)P.hi[i] : 3.0e38f;
-    vecs[32 + i] = lo;
-    vecs[64 + i] = hi;
+    vecs[32 + i] = (in && P.has_box) ? (float)P.lo[i] : -3.0e38f;
+    vecs[64 + i] = (in && P.has_box) ? (float)P.hi[i] : 3.0e38f;
     vecs[96 + i] = (in && P.has_box) ? (float)(1.0 / (P.hi[i] - P.lo[i])) : 0.0f;
   }
   ptx::tc_fence_before();
@@ -253,16 +261,18 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     if (lane == 0) producer_loop(P, bars, sbase + SmemLayout::STAGES, n_evals, n_ops);
   } else if (warp == 1) {
     if (lane == 0) mma_loop(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
-  } else if (warp >= 4) {
+  } else if (warp >= kCtrlWarps) {
     EpiCtx C;
     C.P = &P;
     C.bars = bars;
     C.smem = smem;
-    C.row = tid - 4 * 32;
+    C.row = (warp & 3) * 32 + lane;
+    C.k = (warp - kCtrlWarps) >> 2;
     C.tmem_lane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
-    C.o = 0;
-    C.g = 0;
-    C.bias_s = bias_s; C.wout_s = wout_s; C.wouts_s = wouts_s; C.Ls = Ls; C.Rs = Rs; C.vecs = vecs;
+    C.o = 0; C.g = 0; C.vslot = 0; C.pslot = 0;
+    C.bias_s = bias_s; C.wout_s = wout_s; C.wouts_s = wouts_s;
+    C.Ls = Ls; C.LTs = LTs; C.Rs = Rs; C.RTs = RTs; C.vecs = vecs;
+    C.part = reinterpret_cast<float*>(smem + SmemLayout::PART);
     C.dact_tile = P.dact + (size_t)blockIdx.x * P.dact_tile_elems;
     sampler_thread<METHOD>(C, R);
   }
