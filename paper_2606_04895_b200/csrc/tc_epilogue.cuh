@@ -24,6 +24,9 @@ struct EpiCtx {
   const float *bias_s, *wout_s, *wouts_s, *Ls, *LTs, *Rs, *RTs, *vecs;
   float* part;          // [2][4][128]
   uint16_t* dact_tile;
+  // per-thread constants: byte offsets of this thread's two 16-B pieces inside an A k-chunk
+  // (128B swizzle) and its element offset inside a [8 pieces][128 rows][8] act' block
+  uint32_t a_off0, a_off1, dact_row_off;
 };
 
 using ptx::f32x2;
@@ -32,8 +35,12 @@ using ptx::f32x2;
 __device__ __forceinline__ uint8_t* a_piece(const EpiCtx& C, int j, int p) {
   return C.smem + SmemLayout::A + j * kAChunkBytes + C.row * 128 + ((p ^ (C.row & 7)) << 4);
 }
-__device__ __forceinline__ size_t dact_off(const Params& P, int layer, int j, int p, int row) {
-  return ((((size_t)layer * (P.H / 64) + j) * 8 + p) * kRows + row) * 8;
+// act' scratch: [layer][chunk j][8 pieces][128 rows][8 bf16]; one (layer, j) block = 8192 elements
+__device__ __forceinline__ uint16_t* dact_ptr(const EpiCtx& C, int layer, int j) {
+  return C.dact_tile + (uint32_t)(layer * (C.P->H >> 6) + j) * 8192u + C.dact_row_off;
+}
+__device__ __forceinline__ uint8_t* a_chunk(const EpiCtx& C, int j) {
+  return C.smem + SmemLayout::A + j * kAChunkBytes;
 }
 __device__ __forceinline__ void qbar(const EpiCtx& C) { ptx::named_bar_sync(1 + (C.row >> 5), 128); }
 
@@ -138,14 +145,14 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
         }
       }
       if (!LAST && want_grad) {
-        *reinterpret_cast<uint4*>(C.dact_tile + dact_off(P, op.layer, jn, 2 * C.k, C.row)) =
-            make_uint4(dp[0], dp[1], dp[2], dp[3]);
-        *reinterpret_cast<uint4*>(C.dact_tile + dact_off(P, op.layer, jn, 2 * C.k + 1, C.row)) =
-            make_uint4(dp[4], dp[5], dp[6], dp[7]);
+        uint16_t* dptr = dact_ptr(C, op.layer, jn);
+        *reinterpret_cast<uint4*>(dptr) = make_uint4(dp[0], dp[1], dp[2], dp[3]);
+        *reinterpret_cast<uint4*>(dptr + 1024) = make_uint4(dp[4], dp[5], dp[6], dp[7]);
       }
       if (writes_a) {
-        *reinterpret_cast<uint4*>(a_piece(C, jn, 2 * C.k)) = make_uint4(hp[0], hp[1], hp[2], hp[3]);
-        *reinterpret_cast<uint4*>(a_piece(C, jn, 2 * C.k + 1)) = make_uint4(hp[4], hp[5], hp[6], hp[7]);
+        uint8_t* ach = a_chunk(C, jn);
+        *reinterpret_cast<uint4*>(ach + C.a_off0) = make_uint4(hp[0], hp[1], hp[2], hp[3]);
+        *reinterpret_cast<uint4*>(ach + C.a_off1) = make_uint4(hp[4], hp[5], hp[6], hp[7]);
         ptx::fence_proxy_async();
         ptx::mbar_arrive(C.bars.a_ready(jn));
         written = jn + 1;
@@ -169,8 +176,9 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
       const int jn = (c * op.ncols) / 64 + grp;
       uint32_t v[16];
       ptx::tmem_ld16(tcol + grp * 64, v);
-      const uint4 d0 = *reinterpret_cast<const uint4*>(C.dact_tile + dact_off(P, op.layer, jn, 2 * C.k, C.row));
-      const uint4 d1 = *reinterpret_cast<const uint4*>(C.dact_tile + dact_off(P, op.layer, jn, 2 * C.k + 1, C.row));
+      const uint16_t* dptr = dact_ptr(C, op.layer, jn);
+      const uint4 d0 = *reinterpret_cast<const uint4*>(dptr);
+      const uint4 d1 = *reinterpret_cast<const uint4*>(dptr + 1024);
       const uint32_t dw[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
       ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
       ptx::tmem_ld_wait();
@@ -180,8 +188,9 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
         const f32x2 dd = ptx::pack2u(dw[i] << 16, dw[i] & 0xFFFF0000u);
         hp[i] = ptx::pack_bf16x2_from(ptx::mul2(ptx::pack2u(v[2 * i], v[2 * i + 1]), dd));
       }
-      *reinterpret_cast<uint4*>(a_piece(C, jn, 2 * C.k)) = make_uint4(hp[0], hp[1], hp[2], hp[3]);
-      *reinterpret_cast<uint4*>(a_piece(C, jn, 2 * C.k + 1)) = make_uint4(hp[4], hp[5], hp[6], hp[7]);
+      uint8_t* ach = a_chunk(C, jn);
+      *reinterpret_cast<uint4*>(ach + C.a_off0) = make_uint4(hp[0], hp[1], hp[2], hp[3]);
+      *reinterpret_cast<uint4*>(ach + C.a_off1) = make_uint4(hp[4], hp[5], hp[6], hp[7]);
       ptx::fence_proxy_async();
       ptx::mbar_arrive(C.bars.a_ready(jn));
       written = jn + 1;

@@ -114,8 +114,20 @@ struct Bars {  // mbarrier addresses are computed, never looked up (keeps them o
 __device__ __forceinline__ Bars make_bars(uint32_t base) { Bars b; b.base = base; return b; }
 
 // ------------------------------------------------------------------------------------------------
-// weight producer (one thread)
+// weight producer (warp 0, warp-converged; one elected lane issues the copies)
 // ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "elect.sync _|p, 0xffffffff;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(pred));
+  return pred != 0;
+}
+
 __device__ void producer_loop(const Params& P, const Bars& bars, uint32_t stage_base, int64_t n_evals,
                               int n_ops) {
   uint32_t t = 0;  // running tile counter: stage = t % kStages, use = t / kStages
@@ -128,8 +140,11 @@ __device__ void producer_loop(const Params& P, const Bars& bars, uint32_t stage_
       for (int i = 0; i < ntiles; ++i, ++t) {
         const uint32_t s = t % kStages, use = t / kStages;
         ptx::mbar_wait(bars.empty(s), (use & 1u) ^ 1u);
-        ptx::mbar_arrive_expect_tx(bars.full(s), bytes);
-        ptx::bulk_g2s(stage_base + s * kStageBytes, src, bytes, bars.full(s));
+        if (elect_one()) {
+          ptx::mbar_arrive_expect_tx(bars.full(s), bytes);
+          ptx::bulk_g2s(stage_base + s * kStageBytes, src, bytes, bars.full(s));
+        }
+        __syncwarp();
         src += bytes;
       }
     }
@@ -137,44 +152,54 @@ __device__ void producer_loop(const Params& P, const Bars& bars, uint32_t stage_
 }
 
 // ------------------------------------------------------------------------------------------------
-// MMA issuer (one thread)
+// MMA issuer (warp 1, warp-converged so that descriptors live in uniform registers; one elected
+// lane issues tcgen05.mma / tcgen05.commit)
 // ------------------------------------------------------------------------------------------------
 __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uint32_t stage_base,
                          uint32_t tmem_base, int64_t n_evals, int n_ops) {
   uint32_t t = 0;  // tile counter (mirrors the producer)
   uint32_t g = 0;  // n-chunk counter: TMEM buffer = g & 1
   uint32_t o = 0;  // op counter: phase of a_ready / a_free
+  const uint64_t adesc0 = ptx::smem_desc_sw128(a_base);
+  const uint64_t bdesc0 = ptx::smem_desc_sw64(stage_base);
   for (int64_t e = 0; e < n_evals; ++e) {
     for (int oi = 0; oi < n_ops; ++oi, ++o) {
       const OpDesc op = P.ops[oi];
       const uint32_t idesc = ptx::idesc_bf16(kRows, op.ncols);
       // chunks this op does not read are free as soon as everything issued so far has completed
-      for (int j = op.kch; j < kMaxKch; ++j) ptx::mma_commit(bars.a_free(j));
+      if (elect_one())
+        for (int j = op.kch; j < kMaxKch; ++j) ptx::mma_commit(bars.a_free(j));
+      __syncwarp();
       for (int c = 0; c < op.nch; ++c, ++g) {
         const uint32_t buf = g & 1u, use = g >> 1;
         ptx::mbar_wait(bars.d_free(buf), (use & 1u) ^ 1u);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + buf * 256u;
-        for (int k32 = 0; k32 < 2 * op.kch; ++k32, ++t) {
-          const int j = k32 >> 1;
-          if (c == 0 && (k32 & 1) == 0) {
+        const bool last_c = (c == op.nch - 1);
+        for (int j = 0; j < op.kch; ++j) {
+          if (c == 0) {
             ptx::mbar_wait(bars.a_ready(j), o & 1u);
             ptx::tc_fence_after();
           }
-          const uint32_t s = t % kStages, use_s = t / kStages;
-          ptx::mbar_wait(bars.full(s), use_s & 1u);
-          ptx::tc_fence_after();
-          const uint32_t a_addr = a_base + j * kAChunkBytes + (k32 & 1) * 64;
-          const uint32_t b_addr = stage_base + s * kStageBytes;
 #pragma unroll
-          for (int kk = 0; kk < 2; ++kk) {
-            ptx::mma_bf16_ss(d_tmem, ptx::smem_desc_sw128(a_addr + kk * 32),
-                             ptx::smem_desc_sw64(b_addr + kk * 32), idesc, (k32 | kk) != 0 ? 1u : 0u);
+          for (int h = 0; h < 2; ++h, ++t) {
+            const uint32_t s = t % kStages, use_s = t / kStages;
+            ptx::mbar_wait(bars.full(s), use_s & 1u);
+            ptx::tc_fence_after();
+            // descriptor start-address fields are in 16-byte units
+            const uint64_t ad = adesc0 + (uint64_t)((j * kAChunkBytes + h * 64) >> 4);
+            const uint64_t bd = bdesc0 + (uint64_t)((s * kStageBytes) >> 4);
+            if (elect_one()) {
+              ptx::mma_bf16_ss(d_tmem, ad, bd, idesc, (j | h) != 0 ? 1u : 0u);
+              ptx::mma_bf16_ss(d_tmem, ad + 2, bd + 2, idesc, 1u);
+              ptx::mma_commit(bars.empty(s));
+              if (last_c && h == 1) ptx::mma_commit(bars.a_free(j));
+            }
+            __syncwarp();
           }
-          ptx::mma_commit(bars.empty(s));
-          if (c == op.nch - 1 && (k32 & 1)) ptx::mma_commit(bars.a_free(j));
         }
-        ptx::mma_commit(bars.d_full(buf));
+        if (elect_one()) ptx::mma_commit(bars.d_full(buf));
+        __syncwarp();
       }
     }
   }

@@ -258,9 +258,9 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   const int n_ops = R.want_grad ? P.n_ops_all : P.n_ops_fwd;
 
   if (warp == 0) {
-    if (lane == 0) producer_loop(P, bars, sbase + SmemLayout::STAGES, n_evals, n_ops);
+    producer_loop(P, bars, sbase + SmemLayout::STAGES, n_evals, n_ops);
   } else if (warp == 1) {
-    if (lane == 0) mma_loop(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
+    mma_loop(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
   } else if (warp >= kCtrlWarps) {
     EpiCtx C;
     C.P = &P;
@@ -274,6 +274,9 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     C.Ls = Ls; C.LTs = LTs; C.Rs = Rs; C.RTs = RTs; C.vecs = vecs;
     C.part = reinterpret_cast<float*>(smem + SmemLayout::PART);
     C.dact_tile = P.dact + (size_t)blockIdx.x * P.dact_tile_elems;
+    C.a_off0 = C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4);
+    C.a_off1 = C.row * 128 + (((2 * C.k + 1) ^ (C.row & 7)) << 4);
+    C.dact_row_off = (uint32_t)(2 * C.k * kRows + C.row) * 8u;
     sampler_thread<METHOD>(C, R);
   }
   ptx::tc_fence_before();
