@@ -5,85 +5,78 @@
 //   * sampler algebra: the thread owns parameter dimensions [8k, 8k+8) of its chain; the four
 //     threads of a chain (same lane, four different warps of one TMEM lane quarter) exchange
 //     matvec inputs and partial sums through SMEM with a 128-thread named barrier.
-// Four resident warps per SM sub-partition hide the ALU / MUFU / LDS latencies that a single
-// warp per sub-partition cannot.
+// The r1a profile (profiles/r1a_hmc_ncu_full.md) showed these warps to be ISSUE-bound (62.6 k
+// issue cycles per evaluation against 50.7 k MMA cycles), so everything here is written for
+// instruction count: 32-bit shared-space addresses, packed f32x2 math, one MUFU per element,
+// per-thread addresses hoisted into EpiCtx.
 #pragma once
 
 namespace best {
 namespace tc {
 
+using ptx::f32x2;
+
 struct EpiCtx {
   const Params* P;
   Bars bars;
-  uint8_t* smem;
+  uint32_t sbase;       // shared-space address of the carve-up base
   uint32_t tmem_lane;   // tmem base + (lane quarter << 16)
   int row;              // 0..127
   int k;                // 0..3
   uint32_t o, g;        // op / n-chunk counters (mirror the MMA issuer)
   uint32_t vslot, pslot;  // rotating scratch slots
-  const float *bias_s, *wout_s, *wouts_s, *Ls, *LTs, *Rs, *RTs, *vecs;
-  float* part;          // [2][4][128]
-  uint16_t* dact_tile;
-  // per-thread constants: byte offsets of this thread's two 16-B pieces inside an A k-chunk
-  // (128B swizzle) and its element offset inside a [8 pieces][128 rows][8] act' block
-  uint32_t a_off0, a_off1, dact_row_off;
+  // per-thread constants
+  uint32_t a_thr0, a_thr1;  // shared addresses of this thread's two 16-B pieces in A k-chunk 0 (SW128)
+  uint32_t bias_thr;        // shared address of bias[0][16k]
+  uint32_t wouts_thr;       // shared address of (s * w_out)[16k]
+  uint32_t v_thr;           // byte offset of this row inside an exchange slot: row * 8
+  uint8_t* dact_thr;        // global: this thread's 16 bytes inside act' block (layer 0, chunk 0)
 };
 
-using ptx::f32x2;
-
-// address of 16-byte piece `p` of row `row` in A k-chunk `j` (128B swizzle)
-__device__ __forceinline__ uint8_t* a_piece(const EpiCtx& C, int j, int p) {
-  return C.smem + SmemLayout::A + j * kAChunkBytes + C.row * 128 + ((p ^ (C.row & 7)) << 4);
-}
-// act' scratch: [layer][chunk j][8 pieces][128 rows][8 bf16]; one (layer, j) block = 8192 elements
-__device__ __forceinline__ uint16_t* dact_ptr(const EpiCtx& C, int layer, int j) {
-  return C.dact_tile + (uint32_t)(layer * (C.P->H >> 6) + j) * 8192u + C.dact_row_off;
-}
-__device__ __forceinline__ uint8_t* a_chunk(const EpiCtx& C, int j) {
-  return C.smem + SmemLayout::A + j * kAChunkBytes;
-}
 __device__ __forceinline__ void qbar(const EpiCtx& C) { ptx::named_bar_sync(1 + (C.row >> 5), 128); }
 
-// ---- activations on fp32 pairs ---------------------------------------------------------------
-// SiLU: h = a*sg, dact = sg + h*(1 - sg), sg = 1/(1 + 2^(-a log2 e)).
-// kFastAct: sg = 0.5 + 0.5 tanh.approx(a/2)             (1 MUFU / element)
-// else    : ex2.approx + bit-trick reciprocal + 2 Newton steps on the FMA pipe (1 MUFU / element,
-//           relative error of sg ~2e-4, no cancellation for a << 0)
-template <bool kFast>
-__device__ __forceinline__ void silu2(f32x2 a, f32x2& h, f32x2& dact) {
-  f32x2 sg;
-  if (kFast) {
-    float x0, x1;
-    ptx::unpack2(ptx::mul2(a, ptx::pack2(0.5f, 0.5f)), x0, x1);
-    const f32x2 t = ptx::pack2(ptx::tanh_approx(x0), ptx::tanh_approx(x1));
-    sg = ptx::fma2(t, ptx::pack2(0.5f, 0.5f), ptx::pack2(0.5f, 0.5f));
-  } else {
-    float x0, x1;
-    ptx::unpack2(ptx::mul2(a, ptx::pack2(-1.4426950408889634f, -1.4426950408889634f)), x0, x1);
-    const f32x2 e = ptx::pack2(ptx::ex2_approx(fminf(x0, 80.0f)), ptx::ex2_approx(fminf(x1, 80.0f)));
-    const f32x2 ns = ptx::fma2(e, ptx::pack2(-1.0f, -1.0f), ptx::pack2(-1.0f, -1.0f));  // -(1+e)
-    uint32_t n0, n1;
-    ptx::unpack2u(ns, n0, n1);
-    f32x2 r = ptx::pack2u(0xFEF311C7u - n0, 0xFEF311C7u - n1);   // ~1/(1+e), 12 % accurate
-    const f32x2 two = ptx::pack2(2.0f, 2.0f);
-    r = ptx::mul2(r, ptx::fma2(ns, r, two));
-    r = ptx::mul2(r, ptx::fma2(ns, r, two));
-    sg = r;
-  }
-  h = ptx::mul2(a, sg);
-  const f32x2 omr = ptx::fma2(sg, ptx::pack2(-1.0f, -1.0f), ptx::pack2(1.0f, 1.0f));
-  dact = ptx::fma2(h, omr, sg);
+#ifndef BEST_TC_FAST_ACT
+#define BEST_TC_FAST_ACT 1
+#endif
+// With the fast SiLU the forward weights and biases of every hidden layer are packed pre-scaled by
+// 1/2 (exact in bf16), so the accumulator holds a/2 and
+//   t = tanh(a/2):  sigma(a) = (1+t)/2,  h = a sigma = (a/2)(1+t),  h' = sigma + h (1 - sigma)
+// costs one MUFU and four FFMA2 per element pair.  tanh.approx has ~2^-11 relative error, below
+// the 2^-9 of the bf16 rounding that follows.
+constexpr bool kSiluHalfPrescale = (BEST_TC_FAST_ACT != 0);
+
+__device__ __forceinline__ void silu_pair(f32x2 a, f32x2& h, f32x2& dact) {
+#if BEST_TC_FAST_ACT
+  float x0, x1;
+  ptx::unpack2(a, x0, x1);   // a holds (pre-activation)/2
+  const f32x2 t = ptx::pack2(ptx::tanh_approx(x0), ptx::tanh_approx(x1));
+  h = ptx::fma2(a, t, a);
+  const f32x2 sg = ptx::fma2(t, ptx::pack2(0.5f, 0.5f), ptx::pack2(0.5f, 0.5f));
+  const f32x2 om = ptx::fma2(t, ptx::pack2(-0.5f, -0.5f), ptx::pack2(0.5f, 0.5f));
+  dact = ptx::fma2(h, om, sg);
+#else
+  // ex2.approx + bit-trick reciprocal + 2 Newton steps on the FMA pipe (sigma to ~2e-4 relative)
+  float x0, x1;
+  ptx::unpack2(ptx::mul2(a, ptx::pack2(-1.4426950408889634f, -1.4426950408889634f)), x0, x1);
+  const f32x2 e = ptx::pack2(ptx::ex2_approx(fminf(x0, 80.0f)), ptx::ex2_approx(fminf(x1, 80.0f)));
+  const f32x2 ns = ptx::fma2(e, ptx::pack2(-1.0f, -1.0f), ptx::pack2(-1.0f, -1.0f));  // -(1+e)
+  uint32_t n0, n1;
+  ptx::unpack2u(ns, n0, n1);
+  f32x2 r = ptx::pack2u(0xFEF311C7u - n0, 0xFEF311C7u - n1);
+  const f32x2 two = ptx::pack2(2.0f, 2.0f);
+  r = ptx::mul2(r, ptx::fma2(ns, r, two));
+  r = ptx::mul2(r, ptx::fma2(ns, r, two));
+  h = ptx::mul2(a, r);
+  const f32x2 omr = ptx::fma2(r, ptx::pack2(-1.0f, -1.0f), ptx::pack2(1.0f, 1.0f));
+  dact = ptx::fma2(h, omr, r);
+#endif
 }
-__device__ __forceinline__ void tanh2(f32x2 a, f32x2& h, f32x2& dact) {
+__device__ __forceinline__ void tanh_pair(f32x2 a, f32x2& h, f32x2& dact) {
   float x0, x1;
   ptx::unpack2(a, x0, x1);
   h = ptx::pack2(ptx::tanh_approx(x0), ptx::tanh_approx(x1));
   dact = ptx::fma2(ptx::mul2(h, h), ptx::pack2(-1.0f, -1.0f), ptx::pack2(1.0f, 1.0f));
 }
-
-#ifndef BEST_TC_FAST_ACT
-#define BEST_TC_FAST_ACT 0
-#endif
 
 // ---- first A operand: theta split into bf16 hi | lo (own 8 dims -> pieces k and 4+k) ------------
 __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
@@ -95,8 +88,9 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
     hi[i] = h2;
     lo[i] = ptx::pack_bf16x2(th[2 * i] - ptx::bf16_lo(h2), th[2 * i + 1] - ptx::bf16_hi(h2));
   }
-  *reinterpret_cast<uint4*>(a_piece(C, 0, C.k)) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-  *reinterpret_cast<uint4*>(a_piece(C, 0, 4 + C.k)) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+  const uint32_t rowa = C.sbase + SmemLayout::A + C.row * 128;
+  ptx::sts_128(rowa + (((uint32_t)C.k ^ (C.row & 7)) << 4), hi[0], hi[1], hi[2], hi[3]);
+  ptx::sts_128(rowa + (((uint32_t)(4 + C.k) ^ (C.row & 7)) << 4), lo[0], lo[1], lo[2], lo[3]);
   ptx::fence_proxy_async();
 #pragma unroll
   for (int j = 0; j < kMaxKch; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
@@ -104,55 +98,53 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
 
 // forward epilogue of one op: bias + activation (+ act' to scratch, or delta for the last layer)
 template <int ACT, bool LAST>
-__device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_grad, float& acc_out,
+__device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_grad, f32x2& acc2,
                                         int& written) {
-  const Params& P = *C.P;
   const bool writes_a = !(LAST && !want_grad);
+  const int ngrp = op.ncols >> 6;
+  const uint32_t bias_l = C.bias_thr + (uint32_t)(op.layer * C.P->H) * 4u;
+  uint8_t* dact_l = C.dact_thr + (size_t)(op.layer * (C.P->H >> 6)) * 16384u;
   for (int c = 0; c < op.nch; ++c, ++C.g) {
     const uint32_t buf = C.g & 1u, use = C.g >> 1;
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * 256u + C.k * 16;
-    const int ngrp = op.ncols / 64;
     for (int grp = 0; grp < ngrp; ++grp) {
-      const int jn = (c * op.ncols) / 64 + grp;
+      const int jn = c * ngrp + grp;
       uint32_t v[16];
       ptx::tmem_ld16(tcol + grp * 64, v);
-      const int f0 = jn * 64 + C.k * 16;
-      const float* bp = C.bias_s + op.layer * P.H + f0;
+      f32x2 b[8];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) ptx::lds_c2x64(bias_l + jn * 256 + i * 16, b[2 * i], b[2 * i + 1]);
+      f32x2 ws[8];
+      if (LAST) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i) ptx::lds_c2x64(C.wouts_thr + jn * 256 + i * 16, ws[2 * i], ws[2 * i + 1]);
+      }
       if (writes_a) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
       ptx::tmem_ld_wait();
       uint32_t hp[8], dp[8];
 #pragma unroll
       for (int i = 0; i < 8; ++i) {
-        const float2 b = *reinterpret_cast<const float2*>(bp + 2 * i);
-        const f32x2 a = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), ptx::pack2(b.x, b.y));
+        const f32x2 a = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), b[i]);
         f32x2 h, dd;
-        if (ACT == BEST_ACT_SILU) silu2<BEST_TC_FAST_ACT != 0>(a, h, dd); else tanh2(a, h, dd);
+        if (ACT == BEST_ACT_SILU) silu_pair(a, h, dd); else tanh_pair(a, h, dd);
         if (LAST) {
-          const float2 w = *reinterpret_cast<const float2*>(C.wout_s + f0 + 2 * i);
-          float h0, h1;
-          ptx::unpack2(h, h0, h1);
-          acc_out = fmaf(h0, w.x, acc_out);
-          acc_out = fmaf(h1, w.y, acc_out);
-          if (want_grad) {
-            const float2 ws = *reinterpret_cast<const float2*>(C.wouts_s + f0 + 2 * i);
-            hp[i] = ptx::pack_bf16x2_from(ptx::mul2(dd, ptx::pack2(ws.x, ws.y)));
-          }
+          acc2 = ptx::fma2(h, ws[i], acc2);
+          if (want_grad) hp[i] = ptx::pack_bf16x2_from(ptx::mul2(dd, ws[i]));
         } else {
           hp[i] = ptx::pack_bf16x2_from(h);
           dp[i] = ptx::pack_bf16x2_from(dd);
         }
       }
       if (!LAST && want_grad) {
-        uint16_t* dptr = dact_ptr(C, op.layer, jn);
-        *reinterpret_cast<uint4*>(dptr) = make_uint4(dp[0], dp[1], dp[2], dp[3]);
-        *reinterpret_cast<uint4*>(dptr + 1024) = make_uint4(dp[4], dp[5], dp[6], dp[7]);
+        uint8_t* dptr = dact_l + (size_t)jn * 16384u;
+        ptx::stg_128(dptr, dp[0], dp[1], dp[2], dp[3]);
+        ptx::stg_128(dptr + 2048, dp[4], dp[5], dp[6], dp[7]);
       }
       if (writes_a) {
-        uint8_t* ach = a_chunk(C, jn);
-        *reinterpret_cast<uint4*>(ach + C.a_off0) = make_uint4(hp[0], hp[1], hp[2], hp[3]);
-        *reinterpret_cast<uint4*>(ach + C.a_off1) = make_uint4(hp[4], hp[5], hp[6], hp[7]);
+        ptx::sts_128(C.a_thr0 + jn * kAChunkBytes, hp[0], hp[1], hp[2], hp[3]);
+        ptx::sts_128(C.a_thr1 + jn * kAChunkBytes, hp[4], hp[5], hp[6], hp[7]);
         ptx::fence_proxy_async();
         ptx::mbar_arrive(C.bars.a_ready(jn));
         written = jn + 1;
@@ -165,21 +157,25 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
 
 // backward epilogue: delta_{l-1} = (delta_l W_l) .* act'_{l-1}
 __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& written) {
-  const Params& P = *C.P;
+  const int ngrp = op.ncols >> 6;
+  const uint8_t* dact_l = C.dact_thr + (size_t)(op.layer * (C.P->H >> 6)) * 16384u;
   for (int c = 0; c < op.nch; ++c, ++C.g) {
     const uint32_t buf = C.g & 1u, use = C.g >> 1;
+    // act' of the first group can be fetched before the accumulator is complete
+    uint4 d0 = ptx::ldg_128(dact_l + (size_t)(c * ngrp) * 16384u);
+    uint4 d1 = ptx::ldg_128(dact_l + (size_t)(c * ngrp) * 16384u + 2048);
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * 256u + C.k * 16;
-    const int ngrp = op.ncols / 64;
     for (int grp = 0; grp < ngrp; ++grp) {
-      const int jn = (c * op.ncols) / 64 + grp;
+      const int jn = c * ngrp + grp;
       uint32_t v[16];
       ptx::tmem_ld16(tcol + grp * 64, v);
-      const uint16_t* dptr = dact_ptr(C, op.layer, jn);
-      const uint4 d0 = *reinterpret_cast<const uint4*>(dptr);
-      const uint4 d1 = *reinterpret_cast<const uint4*>(dptr + 1024);
       const uint32_t dw[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+      if (grp + 1 < ngrp) {   // prefetch the next group's act'
+        d0 = ptx::ldg_128(dact_l + (size_t)(jn + 1) * 16384u);
+        d1 = ptx::ldg_128(dact_l + (size_t)(jn + 1) * 16384u + 2048);
+      }
       ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
       ptx::tmem_ld_wait();
       uint32_t hp[8];
@@ -188,9 +184,8 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
         const f32x2 dd = ptx::pack2u(dw[i] << 16, dw[i] & 0xFFFF0000u);
         hp[i] = ptx::pack_bf16x2_from(ptx::mul2(ptx::pack2u(v[2 * i], v[2 * i + 1]), dd));
       }
-      uint8_t* ach = a_chunk(C, jn);
-      *reinterpret_cast<uint4*>(ach + C.a_off0) = make_uint4(hp[0], hp[1], hp[2], hp[3]);
-      *reinterpret_cast<uint4*>(ach + C.a_off1) = make_uint4(hp[4], hp[5], hp[6], hp[7]);
+      ptx::sts_128(C.a_thr0 + jn * kAChunkBytes, hp[0], hp[1], hp[2], hp[3]);
+      ptx::sts_128(C.a_thr1 + jn * kAChunkBytes, hp[4], hp[5], hp[6], hp[7]);
       ptx::fence_proxy_async();
       ptx::mbar_arrive(C.bars.a_ready(jn));
       written = jn + 1;
@@ -200,23 +195,24 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
   }
 }
 
-// One MLP evaluation.  In: own 8 dims of theta.  Out: this thread's PARTIAL of the MLP output sum
-// (over its columns) and, when want_grad, s * d MLP / d theta for its own 8 dims.
+// One MLP evaluation.  In: own 8 dims of theta.  Out: this thread's PARTIAL of s * MLP output
+// (over its columns, without the output bias) and, when want_grad, s * d MLP / d theta for its
+// own 8 dims.
 __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool want_grad, float& out_part,
                                         float (&gm)[8]) {
   const Params& P = *C.P;
   write_xin(C, th);
-  float acc_out = 0.0f;
+  f32x2 acc2 = ptx::pack2(0.0f, 0.0f);
   const int n_ops = want_grad ? P.n_ops_all : P.n_ops_fwd;
   for (int oi = 0; oi < n_ops; ++oi, ++C.o) {
     const OpDesc op = P.ops[oi];
     int written = 0;
     if (op.epi == EPI_FWD_HID) {
-      if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, false>(C, op, want_grad, acc_out, written);
-      else epi_fwd<BEST_ACT_TANH, false>(C, op, want_grad, acc_out, written);
+      if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, false>(C, op, want_grad, acc2, written);
+      else epi_fwd<BEST_ACT_TANH, false>(C, op, want_grad, acc2, written);
     } else if (op.epi == EPI_FWD_LAST) {
-      if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, true>(C, op, want_grad, acc_out, written);
-      else epi_fwd<BEST_ACT_TANH, true>(C, op, want_grad, acc_out, written);
+      if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, true>(C, op, want_grad, acc2, written);
+      else epi_fwd<BEST_ACT_TANH, true>(C, op, want_grad, acc2, written);
     } else if (op.epi == EPI_BWD_HID) {
       epi_bwd(C, op, written);
     } else {  // EPI_BWD_FINAL: D[128][32] -> own 8 columns
@@ -235,52 +231,66 @@ __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool wa
     if (oi != n_ops - 1)  // keep every a_ready barrier at one phase per op
       for (int j = written; j < kMaxKch; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
   }
-  out_part = acc_out;
+  float a0, a1;
+  ptx::unpack2(acc2, a0, a1);
+  out_part = a0 + a1;
 }
 
 // ---- cooperative per-chain algebra: each thread owns dims [8k, 8k+8) ---------------------------
-__device__ __forceinline__ float* vslot_ptr(EpiCtx& C) {   // rotate between A chunks 1 and 2
+// Exchange slot layout: [16 dim pairs][128 rows][2] floats (16 KB, rotating between A chunks 1 and
+// 2, which are idle between evaluations): a thread publishes its 8 values with four STS.64 and
+// reads any pair of dims of its own chain with one LDS.64.
+__device__ __forceinline__ uint32_t share(EpiCtx& C, const float (&x)[8]) {
   C.vslot ^= 1u;
-  return reinterpret_cast<float*>(C.smem + SmemLayout::A + (1 + C.vslot) * kAChunkBytes);
-}
-__device__ __forceinline__ const float* share(EpiCtx& C, const float (&x)[8]) {
-  float* V = vslot_ptr(C);
+  const uint32_t V = C.sbase + SmemLayout::A + (1 + C.vslot) * kAChunkBytes + C.v_thr;
 #pragma unroll
-  for (int i = 0; i < 8; ++i) V[(8 * C.k + i) * kRows + C.row] = x[i];
+  for (int m = 0; m < 4; ++m) ptx::sts_64(V + (uint32_t)(4 * C.k + m) * 1024u, ptx::pack2(x[2 * m], x[2 * m + 1]));
   qbar(C);
   return V;
 }
-// out[i] = sum_{j in [j0, j1)} M[j*32 + 8k + i] * V[j]   (M row j holds the 8 coefficients contiguously)
-__device__ __forceinline__ void mv_rows(const EpiCtx& C, const float* __restrict__ M, const float* V, int j0,
-                                        int j1, float (&out)[8]) {
+// out[i] = sum_{j in [j0, j1)} M[j][8k + i] * x_j   (j0, j1 even; M is a [32][32] float table)
+__device__ __forceinline__ void mv_rows(const EpiCtx& C, uint32_t M, uint32_t V, int j0, int j1,
+                                        float (&out)[8]) {
+  f32x2 o[4];
 #pragma unroll
-  for (int i = 0; i < 8; ++i) out[i] = 0.0f;
-  for (int j = j0; j < j1; ++j) {
-    const float vj = V[j * kRows + C.row];
-    const float4 m0 = *reinterpret_cast<const float4*>(M + j * kDP + 8 * C.k);
-    const float4 m1 = *reinterpret_cast<const float4*>(M + j * kDP + 8 * C.k + 4);
-    out[0] = fmaf(m0.x, vj, out[0]); out[1] = fmaf(m0.y, vj, out[1]);
-    out[2] = fmaf(m0.z, vj, out[2]); out[3] = fmaf(m0.w, vj, out[3]);
-    out[4] = fmaf(m1.x, vj, out[4]); out[5] = fmaf(m1.y, vj, out[5]);
-    out[6] = fmaf(m1.z, vj, out[6]); out[7] = fmaf(m1.w, vj, out[7]);
+  for (int i = 0; i < 4; ++i) o[i] = ptx::pack2(0.0f, 0.0f);
+  const uint32_t Mk = M + (uint32_t)C.k * 32u;
+  for (int jp = j0 >> 1; jp < (j1 >> 1); ++jp) {
+    float v0, v1;
+    ptx::unpack2(ptx::lds_64(V + (uint32_t)jp * 1024u), v0, v1);
+    f32x2 m0, m1, m2, m3;
+    ptx::lds_c2x64(Mk + (uint32_t)jp * 256u, m0, m1);
+    ptx::lds_c2x64(Mk + (uint32_t)jp * 256u + 16u, m2, m3);
+    const f32x2 vv0 = ptx::pack2(v0, v0);
+    o[0] = ptx::fma2(m0, vv0, o[0]); o[1] = ptx::fma2(m1, vv0, o[1]);
+    o[2] = ptx::fma2(m2, vv0, o[2]); o[3] = ptx::fma2(m3, vv0, o[3]);
+    ptx::lds_c2x64(Mk + (uint32_t)jp * 256u + 128u, m0, m1);
+    ptx::lds_c2x64(Mk + (uint32_t)jp * 256u + 144u, m2, m3);
+    const f32x2 vv1 = ptx::pack2(v1, v1);
+    o[0] = ptx::fma2(m0, vv1, o[0]); o[1] = ptx::fma2(m1, vv1, o[1]);
+    o[2] = ptx::fma2(m2, vv1, o[2]); o[3] = ptx::fma2(m3, vv1, o[3]);
   }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) ptx::unpack2(o[i], out[2 * i], out[2 * i + 1]);
 }
 // out = L x : out_i = sum_{j<=i} L[i][j] x_j, own i  -> coefficients LT[j][i], j in [0, 8k+8)
 __device__ __forceinline__ void mv_L(EpiCtx& C, const float (&x)[8], float (&out)[8]) {
-  const float* V = share(C, x);
-  mv_rows(C, C.LTs, V, 0, 8 * C.k + 8, out);
+  const uint32_t V = share(C, x);
+  mv_rows(C, C.sbase + SmemLayout::LTMAT, V, 0, 8 * C.k + 8, out);
 }
 // out = L^T x : out_j = sum_{i>=j} L[i][j] x_i, own j -> coefficients L[i][j], i in [8k, 32)
 __device__ __forceinline__ void mv_Lt(EpiCtx& C, const float (&x)[8], float (&out)[8]) {
-  const float* V = share(C, x);
-  mv_rows(C, C.Ls, V, 8 * C.k, kDP, out);
+  const uint32_t V = share(C, x);
+  mv_rows(C, C.sbase + SmemLayout::LMAT, V, 8 * C.k, kDP, out);
 }
+// sum of one value per thread over the four threads of a chain (same result on all four)
 __device__ __forceinline__ float reduce4(EpiCtx& C, float x) {
   C.pslot ^= 1u;
-  float* Pp = C.part + C.pslot * 4 * kRows;
-  Pp[C.k * kRows + C.row] = x;
+  const uint32_t Pp = C.sbase + SmemLayout::PART + C.pslot * 2048u + (uint32_t)C.row * 16u;
+  ptx::sts_32(Pp + (uint32_t)C.k * 4u, x);
   qbar(C);
-  return (Pp[C.row] + Pp[kRows + C.row]) + (Pp[2 * kRows + C.row] + Pp[3 * kRows + C.row]);
+  const float4 p = ptx::lds_128f(Pp);
+  return (p.x + p.y) + (p.z + p.w);
 }
 
 // full target from the MLP partial output + Gaussian (y = R r), banana and box terms.
@@ -288,25 +298,28 @@ __device__ __forceinline__ float reduce4(EpiCtx& C, float x) {
 __device__ __forceinline__ void finish_target(EpiCtx& C, const float (&th)[8], float out_part, bool want_grad,
                                               float& lp, float (&g)[8]) {
   const Params& P = *C.P;
-  float part = P.mlp_scale * out_part;
+  const uint32_t vecs = C.sbase + SmemLayout::VECS;
+  float part = out_part;
   float ti = 0.0f, tj = 0.0f;
   if (P.has_gauss || P.banana_i >= 0) {
     float r[8], y[8];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) r[i] = th[i] - C.vecs[8 * C.k + i];
-    const float* V = share(C, r);
+    for (int i = 0; i < 8; ++i) r[i] = th[i] - ptx::lds_c32(vecs + (uint32_t)(8 * C.k + i) * 4u);
+    const uint32_t V = share(C, r);
     if (P.banana_i >= 0) {
-      ti = V[P.banana_i * kRows + C.row] + C.vecs[P.banana_i];
-      tj = V[P.banana_j * kRows + C.row] + C.vecs[P.banana_j];
+      ti = ptx::lds_32(V + (uint32_t)(P.banana_i >> 1) * 1024u + (uint32_t)(P.banana_i & 1) * 4u) +
+           ptx::lds_c32(vecs + (uint32_t)P.banana_i * 4u);
+      tj = ptx::lds_32(V + (uint32_t)(P.banana_j >> 1) * 1024u + (uint32_t)(P.banana_j & 1) * 4u) +
+           ptx::lds_c32(vecs + (uint32_t)P.banana_j * 4u);
     }
     if (P.has_gauss) {
-      mv_rows(C, C.RTs, V, 8 * C.k, kDP, y);          // y_i = sum_{j>=i} R[i][j] r_j
+      mv_rows(C, C.sbase + SmemLayout::RTMAT, V, 8 * C.k, kDP, y);   // y_i = sum_{j>=i} R[i][j] r_j
 #pragma unroll
       for (int i = 0; i < 8; ++i) part = fmaf(-0.5f * y[i], y[i], part);
       if (want_grad) {
         float gg[8];
-        const float* Vy = share(C, y);
-        mv_rows(C, C.Rs, Vy, 0, 8 * C.k + 8, gg);      // (R^T y)_j = sum_{i<=j} R[i][j] y_i
+        const uint32_t Vy = share(C, y);
+        mv_rows(C, C.sbase + SmemLayout::RMAT, Vy, 0, 8 * C.k + 8, gg);  // (R^T y)_j = sum_{i<=j} R[i][j] y_i
 #pragma unroll
         for (int i = 0; i < 8; ++i) g[i] -= gg[i];
       }
@@ -315,10 +328,11 @@ __device__ __forceinline__ void finish_target(EpiCtx& C, const float (&th)[8], f
   if (P.has_box) {
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
-      const int gi = 8 * C.k + i;
-      const float lo = C.vecs[32 + gi], hi = C.vecs[64 + gi], iw = C.vecs[96 + gi];
+      const uint32_t gi = (uint32_t)(8 * C.k + i) * 4u;
+      const float lo = ptx::lds_c32(vecs + 128u + gi), hi = ptx::lds_c32(vecs + 256u + gi);
       const float ex = fmaxf(fmaxf(lo - th[i], th[i] - hi), 0.0f);
       if (ex > 0.0f) {
+        const float iw = ptx::lds_c32(vecs + 384u + gi);
         const float t = P.pen_gamma * ex * iw;
         float f, df;
         if (t <= 40.0f) { df = expm1f(t); f = df - t; }

@@ -213,7 +213,6 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   const uint32_t sbase = ptx::smem_u32(smem);
   const Bars bars = make_bars(sbase + SmemLayout::BARS);
   float* bias_s = reinterpret_cast<float*>(smem + SmemLayout::BIAS);
-  float* wout_s = reinterpret_cast<float*>(smem + SmemLayout::WOUT);
   float* wouts_s = reinterpret_cast<float*>(smem + SmemLayout::WOUTS);
   float* Ls = reinterpret_cast<float*>(smem + SmemLayout::LMAT);
   float* LTs = reinterpret_cast<float*>(smem + SmemLayout::LTMAT);
@@ -230,7 +229,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   }
   if (warp == 2) ptx::tmem_alloc(sbase + SmemLayout::TMEMPTR, 512);
   for (int i = tid; i < P.n_hidden * P.H; i += kThreads) bias_s[i] = P.bias[i];
-  for (int i = tid; i < P.H; i += kThreads) { wout_s[i] = P.w_out[i]; wouts_s[i] = P.mlp_scale * P.w_out[i]; }
+  for (int i = tid; i < P.H; i += kThreads) wouts_s[i] = P.mlp_scale * P.w_out[i];
   for (int i = tid; i < kDP * kDP; i += kThreads) {
     const int r = i / kDP, c = i % kDP;
     const float l = (r < P.d && c <= r) ? (float)P.L[r * P.d + c] : 0.0f;
@@ -265,18 +264,18 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     EpiCtx C;
     C.P = &P;
     C.bars = bars;
-    C.smem = smem;
+    C.sbase = sbase;
     C.row = (warp & 3) * 32 + lane;
     C.k = (warp - kCtrlWarps) >> 2;
     C.tmem_lane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
     C.o = 0; C.g = 0; C.vslot = 0; C.pslot = 0;
-    C.bias_s = bias_s; C.wout_s = wout_s; C.wouts_s = wouts_s;
-    C.Ls = Ls; C.LTs = LTs; C.Rs = Rs; C.RTs = RTs; C.vecs = vecs;
-    C.part = reinterpret_cast<float*>(smem + SmemLayout::PART);
-    C.dact_tile = P.dact + (size_t)blockIdx.x * P.dact_tile_elems;
-    C.a_off0 = C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4);
-    C.a_off1 = C.row * 128 + (((2 * C.k + 1) ^ (C.row & 7)) << 4);
-    C.dact_row_off = (uint32_t)(2 * C.k * kRows + C.row) * 8u;
+    C.a_thr0 = sbase + SmemLayout::A + C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4);
+    C.a_thr1 = sbase + SmemLayout::A + C.row * 128 + (((2 * C.k + 1) ^ (C.row & 7)) << 4);
+    C.bias_thr = sbase + SmemLayout::BIAS + C.k * 64;
+    C.wouts_thr = sbase + SmemLayout::WOUTS + C.k * 64;
+    C.v_thr = (uint32_t)C.row * 8u;
+    C.dact_thr = reinterpret_cast<uint8_t*>(P.dact + (size_t)blockIdx.x * P.dact_tile_elems) +
+                 (size_t)(2 * C.k * kRows + C.row) * 16u;
     sampler_thread<METHOD>(C, R);
   }
   ptx::tc_fence_before();
@@ -375,10 +374,12 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   std::vector<uint16_t> pack;
   for (int oi = 0; oi < P.n_ops_all; ++oi) {
     const tc::OpDesc op = P.ops[oi];
+    // forward SiLU layers are packed pre-scaled by 1/2 (exact), see silu_pair()
+    const float fs = (tc::kSiluHalfPrescale && cfg->activation == BEST_ACT_SILU) ? 0.5f : 1.0f;
     auto Bm = [&](int n, int k) -> float {
       if (op.epi == tc::EPI_FWD_HID || op.epi == tc::EPI_FWD_LAST) {
-        if (op.layer == 0) { const int kk = k & 31; return kk < d ? W[0][(size_t)n * d + kk] : 0.0f; }
-        return W[op.layer][(size_t)n * H + k];
+        if (op.layer == 0) { const int kk = k & 31; return kk < d ? fs * W[0][(size_t)n * d + kk] : 0.0f; }
+        return fs * W[op.layer][(size_t)n * H + k];
       }
       if (op.epi == tc::EPI_BWD_HID) return W[op.layer + 1][(size_t)k * H + n];  // (W_l)^T, l = layer+1
       return n < d ? W[0][(size_t)k * d + n] : 0.0f;                             // (W_0)^T
@@ -395,7 +396,11 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
       }
   }
   std::vector<float> bias((size_t)K * H);
-  for (int l = 0; l < K; ++l) std::memcpy(&bias[(size_t)l * H], bvec[l], sizeof(float) * H);
+  {
+    const float fs = (tc::kSiluHalfPrescale && cfg->activation == BEST_ACT_SILU) ? 0.5f : 1.0f;
+    for (int l = 0; l < K; ++l)
+      for (int i = 0; i < H; ++i) bias[(size_t)l * H + i] = fs * bvec[l][i];
+  }
   P.b_out = bvec[K][0];
   int rc;
   if ((rc = dev_alloc(&pl->wpack, pack.size() * 2))) return rc;
