@@ -34,6 +34,18 @@ constexpr int kCtrlWarps = 4;          // producer, MMA issuer, TMEM allocator, 
 constexpr int kEpiWarps = 16;          // 4 per TMEM lane quarter
 constexpr int kEpiThreads = kEpiWarps * 32;
 constexpr int kThreads = (kCtrlWarps + kEpiWarps) * 32;
+// Two register-allocation experiments, both measured SLOWER on B200 (HMC 16k chains: 1006 TFLOP/s
+// with neither, 938 with pinned per-thread constants, 881 with setmaxnreg 40/104) and so off:
+#ifndef BEST_TC_SETMAXNREG
+#define BEST_TC_SETMAXNREG 0
+#endif
+#ifndef BEST_TC_OPAQUE
+#define BEST_TC_OPAQUE 0
+#endif
+// setmaxnreg moves registers inside the CTA's own allocation (640 threads x 96 at launch): what the
+// control warpgroup gives up is all the epilogue warps can take, or setmaxnreg.inc never returns.
+constexpr int kLaunchRegs = 96, kCtrlRegs = 40, kEpiRegs = 104;
+static_assert(kCtrlWarps * 32 * kCtrlRegs + kEpiThreads * kEpiRegs <= kThreads * kLaunchRegs, "register pool");
 constexpr int kDP = 32;              // parameter vectors are padded to 32 inside the kernel
 
 enum { EPI_FWD_HID = 0, EPI_FWD_LAST = 1, EPI_BWD_HID = 2, EPI_BWD_FINAL = 3 };

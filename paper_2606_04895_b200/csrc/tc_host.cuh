@@ -256,11 +256,20 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   if (METHOD == M_HMC) n_evals = R.n_steps * R.n_leapfrog;
   const int n_ops = R.want_grad ? P.n_ops_all : P.n_ops_fwd;
 
-  if (warp == 0) {
-    producer_loop(P, bars, sbase + SmemLayout::STAGES, n_evals, n_ops);
-  } else if (warp == 1) {
-    mma_loop(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
-  } else if (warp >= kCtrlWarps) {
+  if (warp < kCtrlWarps) {
+    // the control warpgroup hands most of its registers to the 16 epilogue warps
+#if BEST_TC_SETMAXNREG
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kCtrlRegs));
+#endif
+    if (warp == 0) {
+      producer_loop(P, bars, sbase + SmemLayout::STAGES, n_evals, n_ops);
+    } else if (warp == 1) {
+      mma_loop(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
+    }
+  } else {
+#if BEST_TC_SETMAXNREG
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kEpiRegs));
+#endif
     EpiCtx C;
     C.P = &P;
     C.bars = bars;
@@ -276,6 +285,12 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     C.v_thr = (uint32_t)C.row * 8u;
     C.dact_thr = reinterpret_cast<uint8_t*>(P.dact + (size_t)blockIdx.x * P.dact_tile_elems) +
                  (size_t)(2 * C.k * kRows + C.row) * 16u;
+    // per-thread constants must stay in registers: without this the compiler rematerialises them
+    // from tid / blockIdx / kernel parameters inside every epilogue group (r1b profile)
+#if BEST_TC_OPAQUE
+    asm volatile("" : "+r"(C.a_thr0), "+r"(C.a_thr1), "+r"(C.bias_thr), "+r"(C.wouts_thr), "+r"(C.v_thr),
+                      "+r"(C.tmem_lane), "+r"(C.sbase), "+l"(C.dact_thr));
+#endif
     sampler_thread<METHOD>(C, R);
   }
   ptx::tc_fence_before();
