@@ -24,9 +24,24 @@ namespace best {
 
 namespace tc {
 
-constexpr int kRows = 128;           // chains per CTA == TMEM lanes
-constexpr int kAChunkBytes = 16384;  // A k-chunk: 128 rows x 64 bf16 (128 B rows, SW128)
-constexpr int kMaxKch = 8;           // hidden width <= 512
+constexpr int kRows = 128;           // TMEM lanes == MMA M
+// Two tile geometries (template parameter R64 of the kernel):
+//   R64 = false: 128 chains per CTA, hidden width <= 512.  A k-chunk = 128 rows x 64 bf16 = 16 KB;
+//                the epilogue rewrites the activation operand IN PLACE (a full layer of fp32
+//                accumulators, 128 x 512, is exactly the 512 TMEM columns).
+//   R64 = true : 64 chains per CTA, hidden width 1024.  A k-chunk = 64 rows x 64 bf16 = 8 KB at
+//                an 8 KB pitch, so that the MMA (still M = 128) reads the NEXT chunk as rows
+//                64..127: phantom rows whose accumulator lanes 64..127 nobody reads.  A layer of
+//                accumulators (1024 columns) no longer fits TMEM, so the epilogue writes the
+//                next operand to an L2-resident image and warp 3 copies it back chunk by chunk
+//                (cp.async.bulk) as soon as the last N-chunk's MMAs have released the chunk.
+template <bool R64> struct Geo {
+  static constexpr int kTileRows = R64 ? 64 : 128;
+  static constexpr int kAChunk = R64 ? 8192 : 16384;
+  static constexpr int kEpiActive = R64 ? 256 : 512;   // epilogue threads that own a real chain
+};
+constexpr int kAChunkBytes = 16384;  // R64 = false chunk pitch (also the exchange-slot size)
+constexpr int kMaxKch = 16;          // hidden width <= 1024
 constexpr int kStageBytes = 16384;   // weight stage: <=256 rows x 32 bf16 (64 B rows, SW64)
 constexpr int kStages = 4;
 constexpr int kMaxOps = 12;
@@ -66,10 +81,11 @@ struct Params {
   int n_ops_fwd, n_ops_all;
   OpDesc ops[kMaxOps];
   const uint8_t* wpack;   // packed tiles: forward ops then backward ops, consumption order
-  const float* bias;      // [n_hidden][H]
+  const float* bias;      // [n_hidden][H] fp32 (R64: the same values as bf16, 2 per word)
   const float* w_out;     // [H]
-  uint16_t* dact;         // scratch: per tile [n_hidden-1][H/64][8 pieces][128 rows][8] bf16
+  uint16_t* dact;         // scratch: per tile [n_hidden-1][H/64][8 pieces][tile rows][8] bf16
   size_t dact_tile_elems;
+  uint8_t* aimg;          // R64: per tile, SMEM image of the next A operand [16 chunks][64 rows][128 B]
   // target terms (fp64 masters on device, converted to fp32 in SMEM at kernel start)
   int has_gauss, has_box, banana_i, banana_j;
   float banana_sigma, pen_kappa, pen_gamma;
@@ -96,19 +112,18 @@ struct Run {
 // shared-memory carve-up (dynamic, 1024-byte aligned base)
 struct SmemLayout {
   static constexpr int A = 0;
-  static constexpr int STAGES = A + kMaxKch * kAChunkBytes;          // 131072
-  static constexpr int BIAS = STAGES + kStages * kStageBytes;        // 196608, 2048 floats
-  static constexpr int WOUT = BIAS + 2048 * 4;                       // 512 floats
-  static constexpr int WOUTS = WOUT + 512 * 4;                       // 512 floats (s * w_out)
-  static constexpr int LMAT = WOUTS + 512 * 4;                       // 32x32 floats
+  static constexpr int STAGES = A + 131072;                          // 8 x 16 KB or 16 x 8 KB chunks
+  static constexpr int BIAS = STAGES + kStages * kStageBytes;        // 196608: 2048 floats / 4096 bf16
+  static constexpr int WOUTS = BIAS + 2048 * 4;                      // 1024 floats (s * w_out)
+  static constexpr int LMAT = WOUTS + 1024 * 4;                      // 32x32 floats
   static constexpr int LTMAT = LMAT + 1024 * 4;                      // L transposed
   static constexpr int RMAT = LTMAT + 1024 * 4;
   static constexpr int RTMAT = RMAT + 1024 * 4;
   static constexpr int VECS = RTMAT + 1024 * 4;                      // mu, lo, hi, 1/width: 4x32 floats
   static constexpr int PART = VECS + 4 * 32 * 4;                     // partial sums [2][4][128] floats
   static constexpr int BARS = PART + 2 * 4 * 128 * 4;
-  // barriers: full[4] empty[4] a_ready[8] a_free[8] d_full[2] d_free[2]
-  static constexpr int NBARS = 2 * kStages + 2 * kMaxKch + 4;
+  // barriers: full[4] empty[4] a_ready[16] a_free[16] d_full[2] d_free[2] epi_done[4] xin_done
+  static constexpr int NBARS = 2 * kStages + 2 * kMaxKch + 4 + 5;
   static constexpr int TMEMPTR = BARS + NBARS * 8;
   static constexpr int TOTAL = TMEMPTR + 16;
 };
@@ -122,6 +137,8 @@ struct Bars {  // mbarrier addresses are computed, never looked up (keeps them o
   __device__ __forceinline__ uint32_t a_free(int j) const { return base + 8u * (2 * kStages + kMaxKch + j); }
   __device__ __forceinline__ uint32_t d_full(int b) const { return base + 8u * (2 * kStages + 2 * kMaxKch + b); }
   __device__ __forceinline__ uint32_t d_free(int b) const { return base + 8u * (2 * kStages + 2 * kMaxKch + 2 + b); }
+  __device__ __forceinline__ uint32_t epi_done(int c) const { return base + 8u * (2 * kStages + 2 * kMaxKch + 4 + c); }
+  __device__ __forceinline__ uint32_t xin_done() const { return base + 8u * (2 * kStages + 2 * kMaxKch + 8); }
 };
 __device__ __forceinline__ Bars make_bars(uint32_t base) { Bars b; b.base = base; return b; }
 
@@ -167,6 +184,7 @@ __device__ void producer_loop(const Params& P, const Bars& bars, uint32_t stage_
 // MMA issuer (warp 1, warp-converged so that descriptors live in uniform registers; one elected
 // lane issues tcgen05.mma / tcgen05.commit)
 // ------------------------------------------------------------------------------------------------
+template <bool R64>
 __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uint32_t stage_base,
                          uint32_t tmem_base, int64_t n_evals, int n_ops) {
   uint32_t t = 0;  // tile counter (mirrors the producer)
@@ -199,7 +217,7 @@ __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uin
             ptx::mbar_wait(bars.full(s), use_s & 1u);
             ptx::tc_fence_after();
             // descriptor start-address fields are in 16-byte units
-            const uint64_t ad = adesc0 + (uint64_t)((j * kAChunkBytes + h * 64) >> 4);
+            const uint64_t ad = adesc0 + (uint64_t)((j * Geo<R64>::kAChunk + h * 64) >> 4);
             const uint64_t bd = bdesc0 + (uint64_t)((s * kStageBytes) >> 4);
             if (elect_one()) {
               ptx::mma_bf16_ss(d_tmem, ad, bd, idesc, (j | h) != 0 ? 1u : 0u);
@@ -214,6 +232,41 @@ __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uin
         __syncwarp();
       }
     }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// A-operand loader (warp 3, R64 only): the only thread that arrives on a_ready.  Per evaluation:
+// the input chunk written by the sampler threads (xin_done), then after every op but the last the
+// 16 chunks of the next operand, copied L2 image -> SMEM as soon as (a) the epilogue has written
+// the N-chunk they come from (epi_done) and (b) the current op's MMAs have released them (a_free).
+// ------------------------------------------------------------------------------------------------
+__device__ void loader_loop(const Params& P, const Bars& bars, uint32_t a_base, const uint8_t* aimg_tile,
+                            int64_t n_evals, int n_ops) {
+  uint32_t o = 0;   // op counter (phase of a_ready / a_free / epi_done)
+  for (int64_t e = 0; e < n_evals; ++e) {
+    ptx::mbar_wait(bars.xin_done(), (uint32_t)(e & 1));
+    if (elect_one())
+      for (int j = 0; j < kMaxKch; ++j) ptx::mbar_arrive(bars.a_ready(j));
+    __syncwarp();
+    for (int oi = 0; oi + 1 < n_ops; ++oi, ++o) {
+      const OpDesc op = P.ops[oi];
+      const int out_kch = (op.nch * op.ncols) >> 6;   // k-chunks of the operand this op produces
+      for (int j = 0; j < kMaxKch; ++j) {
+        if (j < out_kch) {
+          ptx::mbar_wait(bars.epi_done((j * 64) / op.ncols), o & 1u);
+          ptx::mbar_wait(bars.a_free(j), o & 1u);
+          if (elect_one()) {
+            ptx::mbar_arrive_expect_tx(bars.a_ready(j), 8192);
+            ptx::bulk_g2s(a_base + j * 8192, aimg_tile + (size_t)j * 8192, 8192, bars.a_ready(j));
+          }
+        } else if (elect_one()) {
+          ptx::mbar_arrive(bars.a_ready(j));
+        }
+        __syncwarp();
+      }
+    }
+    ++o;   // the last op of the evaluation produces no operand
   }
 }
 

@@ -76,8 +76,43 @@ def test_T1_other_shapes(B, O, hidden, act):
         ctx.close()
 
 
+@pytest.mark.parametrize("variant", ["full", "mlp_only"])
+def test_T1_sterile_1024_logp_grad(B, O, variant):
+    """BASELINE configs[3]/[4] network 29→1024⁴→1 SiLU (64-chain tiles, operand round trip through
+    L2): probe points on/off the banana ridge, box faces, outliers; several tiles + ragged tail."""
+    base = WL.sterile(n_chains=8)
+    n = 64 * 5 + 37
+    pts = WL.probe_points(base, n, seed=23)
+    w = WL.mlp_only(base) if variant == "mlp_only" else base
+    ctx = B.Context(w, B.PREC_BF16)
+    lp = np.zeros(n, np.float32)
+    g = np.zeros((n, w.d), np.float32)
+    ctx.logp_grad(pts, n, lp, g)
+    lp_ref, g_ref = O.Oracle(w).logp_grad(pts)
+    e = check_logp_grad(lp, g, lp_ref, g_ref, TOL[1], f"sterile/{variant}")
+    print(f"[T1-bf16] sterile-1024 {variant}: logp err/S {e[0]:.2e}, grad ratio {e[1]:.2e}")
+    lp2 = np.zeros(n, np.float32)
+    ctx.logp_grad(pts, n, lp2, None)
+    assert np.array_equal(lp, lp2)
+    ctx.close()
+
+
+def test_T1_1024_two_hidden_tanh(B, O):
+    base = WL.tiny(activation=WL.ACT_TANH, hidden=(1024, 1024), mlp_scale=1.0)
+    n = 150
+    pts = _posterior_like(base, n, seed=5)
+    for w in (base, WL.mlp_only(base)):
+        ctx = B.Context(w, B.PREC_BF16)
+        lp = np.zeros(n, np.float32)
+        g = np.zeros((n, w.d), np.float32)
+        ctx.logp_grad(pts, n, lp, g)
+        lp_ref, g_ref = O.Oracle(w).logp_grad(pts)
+        check_logp_grad(lp, g, lp_ref, g_ref, 3e-2, f"1024x2/tanh/{w.name}")
+        ctx.close()
+
+
 def test_unsupported_shapes(B):
-    for hidden in ((50, 37), (64, 128), (1024, 1024)):
+    for hidden in ((50, 37), (64, 128), (2048,), (1024,) * 5):
         w = WL.tiny(hidden=hidden)
         with pytest.raises(B.BestError) as e:
             B.Context(w, B.PREC_BF16)
@@ -120,6 +155,26 @@ def _single_step_stat(B, O, w, method, seed, **kw):
 def test_T2_single_step_statistical(B, O, method, kw):
     w = WL.lcdm(n_chains=1024 + 40, mlp_scale=3.0 if method == "hmc" else 1.0)
     _single_step_stat(B, O, w, method, seed=55, **kw)
+
+
+@pytest.mark.parametrize("method,kw", [("aies", dict(a=2.0)), ("mala", dict(eps=0.01)), ("hmc", dict(eps=0.03, n_leapfrog=4))])
+def test_T2_sterile_1024_single_step(B, O, method, kw):
+    """single-step maps on the 29→1024⁴→1 banana target (64-chain tiles), 1024 + 38 chains"""
+    _single_step_stat(B, O, WL.sterile(n_chains=1062), method, seed=31, **kw)
+
+
+def test_T4_split_invariance_1024(B):
+    w = WL.sterile(n_chains=200)
+    ctx = B.Context(w, B.PREC_BF16)
+    a, b = ctx.new_state(w.theta0), ctx.new_state(w.theta0)
+    a.step_mala(6, 11, f32(0.01)); a.step_aies(4, 12, 2.0)
+    for _ in range(3):
+        b.step_mala(2, 11, f32(0.01))
+    for _ in range(2):
+        b.step_aies(2, 12, 2.0)
+    ga, gb = a.get(want_grad=False), b.get(want_grad=False)
+    assert np.array_equal(ga["theta"], gb["theta"]) and np.array_equal(ga["n_accept"], gb["n_accept"])
+    ctx.close()
 
 
 def test_T4_split_invariance(B):
