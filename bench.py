@@ -28,6 +28,10 @@ WORKLOADS = {
     "hmc": dict(cfg=2, make="lcdm", n_chains=16384, mlp_scale=3.0, method="hmc", eps=0.1, n_leapfrog=16, inner=8),
     "lcdm_mala_16k": dict(cfg=1, make="lcdm", n_chains=16384, mlp_scale=1.0, method="mala", eps=0.3, inner=100),
     "lcdm_mh_16k": dict(cfg=1, make="lcdm", n_chains=16384, mlp_scale=1.0, method="mh", eps=0.3, inner=100),
+    "aies": dict(cfg=3, make="sterile", n_chains=32768, mlp_scale=1.0, method="aies", a=2.0, inner=10),
+    "sterile_mala_16k": dict(cfg=4, make="sterile", n_chains=16384, mlp_scale=1.0, method="mala", eps=0.01, inner=20),
+    "sterile_mh_16k": dict(cfg=4, make="sterile", n_chains=16384, mlp_scale=1.0, method="mh", eps=0.3, inner=20),
+    "sterile_hmc_16k": dict(cfg=4, make="sterile", n_chains=16384, mlp_scale=1.0, method="hmc", eps=0.03, n_leapfrog=8, inner=4),
     "tiny_mala": dict(cfg=0, make="tiny", n_chains=64, mlp_scale=0.1, method="mala", eps=0.3, inner=100),
 }
 
