@@ -31,13 +31,13 @@ struct EpiCtx {
   uint32_t wouts_thr;       // shared address of (s * w_out)[16k]
   uint32_t v_thr;           // byte offset of this row inside an exchange slot: row * 8
   uint8_t* dact_thr;        // global: this thread's 16 bytes inside act' block (layer 0, chunk 0)
-  uint8_t* aimg_thr;        // R64: global image of the next A operand, this thread's first 16-B piece
+  uint8_t* aimg_thr;        // L2-image tiles: global image of the next A operand, this thread's first 16-B piece
 };
 
 // bias of the thread's 16 columns of group jn as 8 fp32 pairs
-template <bool R64>
+template <int ROWS>
 __device__ __forceinline__ void load_bias(const EpiCtx& C, int layer, int jn, f32x2 (&b)[8]) {
-  if (!R64) {
+  if (!C.P->bias16) {
     const uint32_t a = C.bias_thr + (uint32_t)(layer * C.P->H + jn * 64) * 4u;
 #pragma unroll
     for (int i = 0; i < 4; ++i) ptx::lds_c2x64(a + i * 16, b[2 * i], b[2 * i + 1]);
@@ -55,21 +55,20 @@ __device__ __forceinline__ void load_bias(const EpiCtx& C, int layer, int jn, f3
     }
   }
 }
-// store the thread's 16 bf16 results of group jn as the next A operand
-template <bool R64>
+// store the thread's 16 bf16 results of group jn as the next A operand (no fence / signal here)
+template <int ROWS>
 __device__ __forceinline__ void store_a(const EpiCtx& C, int jn, const uint32_t (&hp)[8]) {
-  if (!R64) {
+  if (Geo<ROWS>::kInPlace) {
     ptx::sts_128(C.a_thr0 + jn * kAChunkBytes, hp[0], hp[1], hp[2], hp[3]);
     ptx::sts_128(C.a_thr1 + jn * kAChunkBytes, hp[4], hp[5], hp[6], hp[7]);
-    ptx::fence_proxy_async();
-    ptx::mbar_arrive(C.bars.a_ready(jn));
   } else {
-    uint8_t* p0 = C.aimg_thr + (size_t)jn * 8192u;
+    uint8_t* p0 = C.aimg_thr + (size_t)jn * Geo<ROWS>::kAChunk;
     uint8_t* p1 = reinterpret_cast<uint8_t*>(reinterpret_cast<uintptr_t>(p0) ^ (uintptr_t)16);
     ptx::stg_128(p0, hp[0], hp[1], hp[2], hp[3]);
     ptx::stg_128(p1, hp[4], hp[5], hp[6], hp[7]);
   }
 }
+
 
 __device__ __forceinline__ void qbar(const EpiCtx& C) { ptx::named_bar_sync(1 + (C.row >> 5), 128); }
 
@@ -117,7 +116,7 @@ __device__ __forceinline__ void tanh_pair(f32x2 a, f32x2& h, f32x2& dact) {
 }
 
 // ---- first A operand: theta split into bf16 hi | lo (own 8 dims -> pieces k and 4+k) ------------
-template <bool R64>
+template <int ROWS>
 __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   ptx::mbar_wait(C.bars.a_free(0), (C.o & 1u) ^ 1u);
   uint32_t hi[4], lo[4];
@@ -131,7 +130,7 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   ptx::sts_128(rowa + (((uint32_t)C.k ^ (C.row & 7)) << 4), hi[0], hi[1], hi[2], hi[3]);
   ptx::sts_128(rowa + (((uint32_t)(4 + C.k) ^ (C.row & 7)) << 4), lo[0], lo[1], lo[2], lo[3]);
   ptx::fence_proxy_async();
-  if (R64) {
+  if ((!Geo<ROWS>::kInPlace)) {
     ptx::mbar_arrive(C.bars.xin_done());   // warp 3 publishes a_ready
   } else {
 #pragma unroll
@@ -139,57 +138,84 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   }
 }
 
-// forward epilogue of one op: bias + activation (+ act' to scratch, or delta for the last layer)
-template <int ACT, bool LAST, bool R64>
+// ---- MLP epilogues --------------------------------------------------------------------------
+// The epilogue warps are latency-bound (r1 timing decomposition): per 64-column
+// group a warp pays a TMEM load, an mbarrier wait, a proxy fence (MEMBAR + FENCE) and an arrive,
+// each a serialised 50-200 cycle stall.  The next op's MMAs wait on exactly these signals, so the
+// operand is published per 64-column group (publishing 128 columns at a time with one fence was
+// measured 10 % SLOWER); the a_free wait is skipped in the last N-chunk (its d_full commit is
+// ordered after every a_free commit of the op).
+
+// bias + activation (+ act' to scratch, or delta for the last layer) of one group, in registers
+template <int ACT, bool LAST, int ROWS>
+__device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, const uint32_t (&v)[16],
+                                          bool want_grad, uint8_t* dact_l, f32x2& acc2, uint32_t (&hp)[8]) {
+  constexpr uint32_t kDBlk = Geo<ROWS>::kTileRows * 128, kDPiece = Geo<ROWS>::kTileRows * 16;
+  f32x2 b[8];
+  load_bias<ROWS>(C, layer, jn, b);
+  f32x2 ws[8];
+  if (LAST) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) ptx::lds_c2x64(C.wouts_thr + jn * 256 + i * 16, ws[2 * i], ws[2 * i + 1]);
+  }
+  uint32_t dp[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const f32x2 a = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), b[i]);
+    f32x2 h, dd;
+    if (ACT == BEST_ACT_SILU) silu_pair(a, h, dd); else tanh_pair(a, h, dd);
+    if (LAST) {
+      acc2 = ptx::fma2(h, ws[i], acc2);
+      if (want_grad) hp[i] = ptx::pack_bf16x2_from(ptx::mul2(dd, ws[i]));
+    } else {
+      hp[i] = ptx::pack_bf16x2_from(h);
+      dp[i] = ptx::pack_bf16x2_from(dd);
+    }
+  }
+  if (!LAST && want_grad) {
+    uint8_t* dptr = dact_l + (size_t)jn * kDBlk;
+    ptx::stg_128(dptr, dp[0], dp[1], dp[2], dp[3]);
+    ptx::stg_128(dptr + kDPiece, dp[4], dp[5], dp[6], dp[7]);
+  }
+}
+
+// publish groups jn0 .. jn0+n-1 of the next operand (stores already issued)
+template <int ROWS>
+__device__ __forceinline__ void publish_a(EpiCtx& C, int jn0, int n) {
+  if (Geo<ROWS>::kInPlace) {
+    ptx::fence_proxy_async();
+    for (int i = 0; i < n; ++i) ptx::mbar_arrive(C.bars.a_ready(jn0 + i));
+  }
+}
+
+// forward epilogue of one op
+template <int ACT, bool LAST, int ROWS>
 __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_grad, f32x2& acc2,
                                         int& written) {
   const bool writes_a = !(LAST && !want_grad);
   const int ngrp = op.ncols >> 6;
-  constexpr uint32_t kDBlk = Geo<R64>::kTileRows * 128, kDPiece = Geo<R64>::kTileRows * 16;
+  constexpr uint32_t kDBlk = Geo<ROWS>::kTileRows * 128;
   uint8_t* dact_l = C.dact_thr + (size_t)(op.layer * (C.P->H >> 6)) * kDBlk;
   for (int c = 0; c < op.nch; ++c, ++C.g) {
     const uint32_t buf = C.g & 1u, use = C.g >> 1;
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * 256u + C.k * 16;
+    const bool gate = Geo<ROWS>::kInPlace && writes_a && (c != op.nch - 1);
     for (int grp = 0; grp < ngrp; ++grp) {
       const int jn = c * ngrp + grp;
-      uint32_t v[16];
+      uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
-      f32x2 b[8];
-      load_bias<R64>(C, op.layer, jn, b);
-      f32x2 ws[8];
-      if (LAST) {
-#pragma unroll
-        for (int i = 0; i < 4; ++i) ptx::lds_c2x64(C.wouts_thr + jn * 256 + i * 16, ws[2 * i], ws[2 * i + 1]);
-      }
-      if (writes_a && !R64) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
       ptx::tmem_ld_wait();
-      uint32_t hp[8], dp[8];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const f32x2 a = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), b[i]);
-        f32x2 h, dd;
-        if (ACT == BEST_ACT_SILU) silu_pair(a, h, dd); else tanh_pair(a, h, dd);
-        if (LAST) {
-          acc2 = ptx::fma2(h, ws[i], acc2);
-          if (want_grad) hp[i] = ptx::pack_bf16x2_from(ptx::mul2(dd, ws[i]));
-        } else {
-          hp[i] = ptx::pack_bf16x2_from(h);
-          dp[i] = ptx::pack_bf16x2_from(dd);
-        }
-      }
-      if (!LAST && want_grad) {
-        uint8_t* dptr = dact_l + (size_t)jn * kDBlk;
-        ptx::stg_128(dptr, dp[0], dp[1], dp[2], dp[3]);
-        ptx::stg_128(dptr + kDPiece, dp[4], dp[5], dp[6], dp[7]);
-      }
+      fwd_group<ACT, LAST, ROWS>(C, op.layer, jn, v, want_grad, dact_l, acc2, hp);
       if (writes_a) {
-        store_a<R64>(C, jn, hp);
+        if (gate) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
+        store_a<ROWS>(C, jn, hp);
+        publish_a<ROWS>(C, jn, 1);
         written = jn + 1;
       }
     }
-    if (R64 && writes_a) {   // this N-chunk of the next operand is in the L2 image
+    if ((!Geo<ROWS>::kInPlace) && writes_a) {   // this N-chunk of the next operand is in the L2 image
       ptx::fence_proxy_async_all();
       ptx::mbar_arrive(C.bars.epi_done(c));
     }
@@ -199,40 +225,47 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
 }
 
 // backward epilogue: delta_{l-1} = (delta_l W_l) .* act'_{l-1}
-template <bool R64>
+template <int ROWS>
+__device__ __forceinline__ void bwd_group(const uint32_t (&v)[16], const uint4& d0, const uint4& d1,
+                                          uint32_t (&hp)[8]) {
+  const uint32_t dw[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const f32x2 dd = ptx::pack2u(dw[i] << 16, dw[i] & 0xFFFF0000u);
+    hp[i] = ptx::pack_bf16x2_from(ptx::mul2(ptx::pack2u(v[2 * i], v[2 * i + 1]), dd));
+  }
+}
+template <int ROWS>
 __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& written) {
   const int ngrp = op.ncols >> 6;
-  constexpr uint32_t kDBlk = Geo<R64>::kTileRows * 128, kDPiece = Geo<R64>::kTileRows * 16;
+  constexpr uint32_t kDBlk = Geo<ROWS>::kTileRows * 128, kDPiece = Geo<ROWS>::kTileRows * 16;
   const uint8_t* dact_l = C.dact_thr + (size_t)(op.layer * (C.P->H >> 6)) * kDBlk;
   for (int c = 0; c < op.nch; ++c, ++C.g) {
     const uint32_t buf = C.g & 1u, use = C.g >> 1;
+    const bool gate = Geo<ROWS>::kInPlace && (c != op.nch - 1);
     // act' of the first group can be fetched before the accumulator is complete
-    uint4 d0 = ptx::ldg_128(dact_l + (size_t)(c * ngrp) * kDBlk);
-    uint4 d1 = ptx::ldg_128(dact_l + (size_t)(c * ngrp) * kDBlk + kDPiece);
+    const uint8_t* dp = dact_l + (size_t)(c * ngrp) * kDBlk;
+    uint4 a0 = ptx::ldg_128(dp), a1 = ptx::ldg_128(dp + kDPiece);
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * 256u + C.k * 16;
     for (int grp = 0; grp < ngrp; ++grp) {
       const int jn = c * ngrp + grp;
-      uint32_t v[16];
+      uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
-      const uint32_t dw[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+      const uint4 d0 = a0, d1 = a1;
       if (grp + 1 < ngrp) {   // prefetch the next group's act'
-        d0 = ptx::ldg_128(dact_l + (size_t)(jn + 1) * kDBlk);
-        d1 = ptx::ldg_128(dact_l + (size_t)(jn + 1) * kDBlk + kDPiece);
+        const uint8_t* dn = dact_l + (size_t)(jn + 1) * kDBlk;
+        a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
       }
-      if (!R64) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
       ptx::tmem_ld_wait();
-      uint32_t hp[8];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const f32x2 dd = ptx::pack2u(dw[i] << 16, dw[i] & 0xFFFF0000u);
-        hp[i] = ptx::pack_bf16x2_from(ptx::mul2(ptx::pack2u(v[2 * i], v[2 * i + 1]), dd));
-      }
-      store_a<R64>(C, jn, hp);
+      bwd_group<ROWS>(v, d0, d1, hp);
+      if (gate) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
+      store_a<ROWS>(C, jn, hp);
+      publish_a<ROWS>(C, jn, 1);
       written = jn + 1;
     }
-    if (R64) {
+    if (!Geo<ROWS>::kInPlace) {
       ptx::fence_proxy_async_all();
       ptx::mbar_arrive(C.bars.epi_done(c));
     }
@@ -241,27 +274,29 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
   }
 }
 
+
+
 // One MLP evaluation.  In: own 8 dims of theta.  Out: this thread's PARTIAL of s * MLP output
 // (over its columns, without the output bias) and, when want_grad, s * d MLP / d theta for its
 // own 8 dims.
-template <bool R64>
+template <int ROWS>
 __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool want_grad, float& out_part,
                                         float (&gm)[8]) {
   const Params& P = *C.P;
-  write_xin<R64>(C, th);
+  write_xin<ROWS>(C, th);
   f32x2 acc2 = ptx::pack2(0.0f, 0.0f);
   const int n_ops = want_grad ? P.n_ops_all : P.n_ops_fwd;
   for (int oi = 0; oi < n_ops; ++oi, ++C.o) {
     const OpDesc op = P.ops[oi];
     int written = 0;
     if (op.epi == EPI_FWD_HID) {
-      if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, false, R64>(C, op, want_grad, acc2, written);
-      else epi_fwd<BEST_ACT_TANH, false, R64>(C, op, want_grad, acc2, written);
+      if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, false, ROWS>(C, op, want_grad, acc2, written);
+      else epi_fwd<BEST_ACT_TANH, false, ROWS>(C, op, want_grad, acc2, written);
     } else if (op.epi == EPI_FWD_LAST) {
-      if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, true, R64>(C, op, want_grad, acc2, written);
-      else epi_fwd<BEST_ACT_TANH, true, R64>(C, op, want_grad, acc2, written);
+      if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, true, ROWS>(C, op, want_grad, acc2, written);
+      else epi_fwd<BEST_ACT_TANH, true, ROWS>(C, op, want_grad, acc2, written);
     } else if (op.epi == EPI_BWD_HID) {
-      epi_bwd<R64>(C, op, written);
+      epi_bwd<ROWS>(C, op, written);
     } else {  // EPI_BWD_FINAL: D[128][32] -> own 8 columns
       const uint32_t buf = C.g & 1u, use = C.g >> 1;
       ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
@@ -275,7 +310,7 @@ __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool wa
       ptx::mbar_arrive(C.bars.d_free(buf));
       ++C.g;
     }
-    if (R64) {   // keep every epi_done barrier at one phase per op (written = 64-column groups)
+    if ((!Geo<ROWS>::kInPlace)) {   // keep every epi_done barrier at one phase per op (written = 64-column groups)
       for (int c = (written * 64 + op.ncols - 1) / op.ncols; c < 4; ++c) ptx::mbar_arrive(C.bars.epi_done(c));
     } else if (oi != n_ops - 1) {  // keep every a_ready barrier at one phase per op
       for (int j = written; j < kMaxKch; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
@@ -405,13 +440,13 @@ __device__ __forceinline__ void finish_target(EpiCtx& C, const float (&th)[8], f
 }
 
 // evaluate the full target at th (own dims): lp (same on all 4 threads) and own 8 gradient dims
-template <bool R64>
+template <int ROWS>
 __device__ __forceinline__ void eval_target(EpiCtx& C, const float (&th)[8], bool want_grad, float& lp,
                                             float (&g)[8]) {
   float out_part;
 #pragma unroll
   for (int i = 0; i < 8; ++i) g[i] = 0.0f;
-  tc_eval<R64>(C, th, want_grad, out_part, g);
+  tc_eval<ROWS>(C, th, want_grad, out_part, g);
   finish_target(C, th, out_part, want_grad, lp, g);
 }
 

@@ -14,6 +14,7 @@
 // The MLP forward and its input-gradient backprop (A1b, A1c) are a chain of GEMMs whose
 // activations never leave the SM; only act' (bf16) is parked in an L2-resident scratch between
 // the forward and backward sweeps.  See DESIGN.md §"tensor-core kernel".
+#include <cstdlib>
 #include <cstring>
 
 #include "device_math.cuh"
@@ -25,20 +26,23 @@ namespace best {
 namespace tc {
 
 constexpr int kRows = 128;           // TMEM lanes == MMA M
-// Two tile geometries (template parameter R64 of the kernel):
-//   R64 = false: 128 chains per CTA, hidden width <= 512.  A k-chunk = 128 rows x 64 bf16 = 16 KB;
+// Tile geometries (template parameter ROWS of the kernel = chains per CTA):
+//   ROWS = 128 : 128 chains per CTA, hidden width <= 512.  A k-chunk = 128 rows x 64 bf16 = 16 KB;
 //                the epilogue rewrites the activation operand IN PLACE (a full layer of fp32
 //                accumulators, 128 x 512, is exactly the 512 TMEM columns).
-//   R64 = true : 64 chains per CTA, hidden width 1024.  A k-chunk = 64 rows x 64 bf16 = 8 KB at
-//                an 8 KB pitch, so that the MMA (still M = 128) reads the NEXT chunk as rows
-//                64..127: phantom rows whose accumulator lanes 64..127 nobody reads.  A layer of
+//   ROWS = 64 / 32: fewer chains per CTA (1024-wide layers, or batches too small to fill 148 SMs
+//                with 128-chain tiles).  A k-chunk = ROWS x 64 bf16 at a ROWS x 128 B pitch, so
+//                that the MMA (still M = 128) reads the FOLLOWING chunks as rows ROWS..127:
+//                phantom rows whose accumulator lanes nobody reads.  A layer of
 //                accumulators (1024 columns) no longer fits TMEM, so the epilogue writes the
 //                next operand to an L2-resident image and warp 3 copies it back chunk by chunk
 //                (cp.async.bulk) as soon as the last N-chunk's MMAs have released the chunk.
-template <bool R64> struct Geo {
-  static constexpr int kTileRows = R64 ? 64 : 128;
-  static constexpr int kAChunk = R64 ? 8192 : 16384;
-  static constexpr int kEpiActive = R64 ? 256 : 512;   // epilogue threads that own a real chain
+template <int ROWS> struct Geo {
+  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32, "tile rows");
+  static constexpr bool kInPlace = (ROWS == 128);
+  static constexpr int kTileRows = ROWS;
+  static constexpr int kAChunk = ROWS * 128;           // bytes of one 64-column k-chunk
+  static constexpr int kEpiActive = ROWS * 4;          // epilogue threads that own a real chain
 };
 constexpr int kAChunkBytes = 16384;  // R64 = false chunk pitch (also the exchange-slot size)
 constexpr int kMaxKch = 16;          // hidden width <= 1024
@@ -81,11 +85,12 @@ struct Params {
   int n_ops_fwd, n_ops_all;
   OpDesc ops[kMaxOps];
   const uint8_t* wpack;   // packed tiles: forward ops then backward ops, consumption order
-  const float* bias;      // [n_hidden][H] fp32 (R64: the same values as bf16, 2 per word)
+  const float* bias;      // [n_hidden][H] fp32 (bias16: staged in SMEM as bf16, 2 per word)
   const float* w_out;     // [H]
   uint16_t* dact;         // scratch: per tile [n_hidden-1][H/64][8 pieces][tile rows][8] bf16
   size_t dact_tile_elems;
-  uint8_t* aimg;          // R64: per tile, SMEM image of the next A operand [16 chunks][64 rows][128 B]
+  uint8_t* aimg;          // ROWS < 128: per tile, SMEM image of the next A operand [16 chunks][ROWS][128 B]
+  int bias16;             // bias table kept as bf16 in SMEM (1024-wide layers)
   // target terms (fp64 masters on device, converted to fp32 in SMEM at kernel start)
   int has_gauss, has_box, banana_i, banana_j;
   float banana_sigma, pen_kappa, pen_gamma;
@@ -184,7 +189,7 @@ __device__ void producer_loop(const Params& P, const Bars& bars, uint32_t stage_
 // MMA issuer (warp 1, warp-converged so that descriptors live in uniform registers; one elected
 // lane issues tcgen05.mma / tcgen05.commit)
 // ------------------------------------------------------------------------------------------------
-template <bool R64>
+template <int ROWS>
 __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uint32_t stage_base,
                          uint32_t tmem_base, int64_t n_evals, int n_ops) {
   uint32_t t = 0;  // tile counter (mirrors the producer)
@@ -217,7 +222,7 @@ __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uin
             ptx::mbar_wait(bars.full(s), use_s & 1u);
             ptx::tc_fence_after();
             // descriptor start-address fields are in 16-byte units
-            const uint64_t ad = adesc0 + (uint64_t)((j * Geo<R64>::kAChunk + h * 64) >> 4);
+            const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk + h * 64) >> 4);
             const uint64_t bd = bdesc0 + (uint64_t)((s * kStageBytes) >> 4);
             if (elect_one()) {
               ptx::mma_bf16_ss(d_tmem, ad, bd, idesc, (j | h) != 0 ? 1u : 0u);
@@ -236,13 +241,13 @@ __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uin
 }
 
 // ------------------------------------------------------------------------------------------------
-// A-operand loader (warp 3, R64 only): the only thread that arrives on a_ready.  Per evaluation:
+// A-operand loader (warp 3, ROWS < 128 only): the only thread that arrives on a_ready.  Per evaluation:
 // the input chunk written by the sampler threads (xin_done), then after every op but the last the
 // 16 chunks of the next operand, copied L2 image -> SMEM as soon as (a) the epilogue has written
 // the N-chunk they come from (epi_done) and (b) the current op's MMAs have released them (a_free).
 // ------------------------------------------------------------------------------------------------
 __device__ void loader_loop(const Params& P, const Bars& bars, uint32_t a_base, const uint8_t* aimg_tile,
-                            int64_t n_evals, int n_ops) {
+                            uint32_t chunk_bytes, int64_t n_evals, int n_ops) {
   uint32_t o = 0;   // op counter (phase of a_ready / a_free / epi_done)
   for (int64_t e = 0; e < n_evals; ++e) {
     ptx::mbar_wait(bars.xin_done(), (uint32_t)(e & 1));
@@ -257,8 +262,8 @@ __device__ void loader_loop(const Params& P, const Bars& bars, uint32_t a_base, 
           ptx::mbar_wait(bars.epi_done((j * 64) / op.ncols), o & 1u);
           ptx::mbar_wait(bars.a_free(j), o & 1u);
           if (elect_one()) {
-            ptx::mbar_arrive_expect_tx(bars.a_ready(j), 8192);
-            ptx::bulk_g2s(a_base + j * 8192, aimg_tile + (size_t)j * 8192, 8192, bars.a_ready(j));
+            ptx::mbar_arrive_expect_tx(bars.a_ready(j), chunk_bytes);
+            ptx::bulk_g2s(a_base + j * chunk_bytes, aimg_tile + (size_t)j * chunk_bytes, chunk_bytes, bars.a_ready(j));
           }
         } else if (elect_one()) {
           ptx::mbar_arrive(bars.a_ready(j));

@@ -8,11 +8,11 @@ namespace tc {
 // Sampler driver: executed by all 512 epilogue threads; thread (row, k) owns dims [8k, 8k+8) of
 // chain `row`.  Scalars (log pi, log alpha, accept) are computed redundantly and identically by the
 // four threads of a chain, so they take the same accept branch.
-template <int METHOD, bool R64>
+template <int METHOD, int ROWS>
 __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
   const Params& P = *C.P;
   const int d = P.d;
-  const int64_t r_in_launch = (int64_t)blockIdx.x * Geo<R64>::kTileRows + C.row;
+  const int64_t r_in_launch = (int64_t)blockIdx.x * Geo<ROWS>::kTileRows + C.row;
   const bool valid = r_in_launch < R.B;
   const bool lead = valid && C.k == 0;
 
@@ -27,7 +27,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
     } else {
       load_vec8(C, R.theta, R.ld, r_in_launch, d, valid, th);
     }
-    eval_target<R64>(C, th, R.want_grad != 0, lp, g);
+    eval_target<ROWS>(C, th, R.want_grad != 0, lp, g);
     if (valid) {
       if (R.io_mode == IO_ROWS_F32) {
         if (C.k == 0) R.out_logp[r_in_launch] = lp;
@@ -58,7 +58,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
 #pragma unroll
       for (int q = 0; q < 8; ++q) thp[q] = thj[q] + z * (thi[q] - thj[q]);
     }
-    eval_target<R64>(C, thp, false, lpp, g);
+    eval_target<ROWS>(C, thp, false, lpp, g);
     const float la = (float)(d - 1) * logf(z) + lpp - (valid ? (float)R.logp[i] : 0.0f);
     const bool acc = valid && accept_rule<float>(u01<float>(w.x), la);
     qbar(C);   // (warp-uniform) every thread of the chain has read logp[i] before the leader overwrites it
@@ -91,7 +91,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) thp[i] = th[i] + dx[i];
       }
-      eval_target<R64>(C, thp, false, lpp, g);
+      eval_target<ROWS>(C, thp, false, lpp, g);
       const float la = lpp - lp;
       la_last = la;
       const uint4 w = philox4x32_10((uint32_t)c, step, 0u, R.seed);
@@ -127,7 +127,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) thp[i] = th[i] + g[i];
       }
-      eval_target<R64>(C, thp, true, lpp, gp);
+      eval_target<ROWS>(C, thp, true, lpp, gp);
       float diff = fwd;
       {
         float gzp[8];
@@ -174,7 +174,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
 #pragma unroll
           for (int i = 0; i < 8; ++i) thw[i] += dx[i];
         }
-        eval_target<R64>(C, thw, true, lpw, gw);
+        eval_target<ROWS>(C, thw, true, lpw, gw);
         float gz[8];
         mv_Lt(C, gw, gz);
         const float cc = (l < R.n_leapfrog) ? eps : 0.5f * eps;
@@ -204,7 +204,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
   }
 }
 
-template <int METHOD, bool R64>
+template <int METHOD, int ROWS>
 __global__ void __launch_bounds__(kThreads, 1)
 best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) {
   extern __shared__ uint8_t smem_raw[];
@@ -224,16 +224,16 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   if (tid == 0) {
     for (int i = 0; i < kStages; ++i) { ptx::mbar_init(bars.full(i), 1); ptx::mbar_init(bars.empty(i), 1); }
     for (int i = 0; i < kMaxKch; ++i) {
-      ptx::mbar_init(bars.a_ready(i), R64 ? 1 : kEpiThreads);   // R64: warp 3 (+ bulk-copy bytes)
+      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : kEpiThreads);   // ROWS < 128: warp 3 (+ bulk-copy bytes)
       ptx::mbar_init(bars.a_free(i), 1);
     }
-    for (int i = 0; i < 2; ++i) { ptx::mbar_init(bars.d_full(i), 1); ptx::mbar_init(bars.d_free(i), Geo<R64>::kEpiActive); }
-    for (int i = 0; i < 4; ++i) ptx::mbar_init(bars.epi_done(i), Geo<R64>::kEpiActive);
-    ptx::mbar_init(bars.xin_done(), Geo<R64>::kEpiActive);
+    for (int i = 0; i < 2; ++i) { ptx::mbar_init(bars.d_full(i), 1); ptx::mbar_init(bars.d_free(i), Geo<ROWS>::kEpiActive); }
+    for (int i = 0; i < 4; ++i) ptx::mbar_init(bars.epi_done(i), Geo<ROWS>::kEpiActive);
+    ptx::mbar_init(bars.xin_done(), Geo<ROWS>::kEpiActive);
     ptx::fence_mbar_init();
   }
   if (warp == 2) ptx::tmem_alloc(sbase + SmemLayout::TMEMPTR, 512);
-  if (R64) {   // bf16 bias table, two per word
+  if (P.bias16) {   // bf16 bias table, two per word
     uint32_t* b16 = reinterpret_cast<uint32_t*>(bias_s);
     for (int i = tid; i < (P.n_hidden * P.H) >> 1; i += kThreads) b16[i] = ptx::pack_bf16x2(P.bias[2 * i], P.bias[2 * i + 1]);
   } else {
@@ -274,9 +274,10 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     if (warp == 0) {
       producer_loop(P, bars, sbase + SmemLayout::STAGES, n_evals, n_ops);
     } else if (warp == 1) {
-      mma_loop<R64>(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
-    } else if (R64 && warp == 3) {
-      loader_loop(P, bars, sbase + SmemLayout::A, P.aimg + (size_t)blockIdx.x * 131072u, n_evals, n_ops);
+      mma_loop<ROWS>(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
+    } else if ((!Geo<ROWS>::kInPlace) && warp == 3) {
+      loader_loop(P, bars, sbase + SmemLayout::A, P.aimg + (size_t)blockIdx.x * (16u * Geo<ROWS>::kAChunk),
+                  Geo<ROWS>::kAChunk, n_evals, n_ops);
     }
   } else {
 #if BEST_TC_SETMAXNREG
@@ -292,12 +293,12 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     C.o = 0; C.g = 0; C.vslot = 0; C.pslot = 0;
     C.a_thr0 = sbase + SmemLayout::A + C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4);
     C.a_thr1 = sbase + SmemLayout::A + C.row * 128 + (((2 * C.k + 1) ^ (C.row & 7)) << 4);
-    C.bias_thr = sbase + SmemLayout::BIAS + C.k * (R64 ? 32 : 64);
+    C.bias_thr = sbase + SmemLayout::BIAS + C.k * (P.bias16 ? 32 : 64);
     C.wouts_thr = sbase + SmemLayout::WOUTS + C.k * 64;
     C.v_thr = (uint32_t)C.row * 8u;
     C.dact_thr = reinterpret_cast<uint8_t*>(P.dact + (size_t)blockIdx.x * P.dact_tile_elems) +
-                 (size_t)(2 * C.k * Geo<R64>::kTileRows + C.row) * 16u;
-    C.aimg_thr = R64 ? P.aimg + (size_t)blockIdx.x * 131072u + C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4)
+                 (size_t)(2 * C.k * Geo<ROWS>::kTileRows + C.row) * 16u;
+    C.aimg_thr = (!Geo<ROWS>::kInPlace) ? P.aimg + (size_t)blockIdx.x * (16u * Geo<ROWS>::kAChunk) + C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4)
                      : nullptr;
     // per-thread constants must stay in registers: without this the compiler rematerialises them
     // from tid / blockIdx / kernel parameters inside every epilogue group (r1b profile)
@@ -305,7 +306,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     asm volatile("" : "+r"(C.a_thr0), "+r"(C.a_thr1), "+r"(C.bias_thr), "+r"(C.wouts_thr), "+r"(C.v_thr),
                       "+r"(C.tmem_lane), "+r"(C.sbase), "+l"(C.dact_thr));
 #endif
-    if (!R64 || C.row < 64) sampler_thread<METHOD, R64>(C, R);   // R64: lanes 64..127 are phantom rows
+    if (C.row < ROWS) sampler_thread<METHOD, ROWS>(C, R);   // lanes ROWS..127 are phantom rows
   }
   ptx::tc_fence_before();
   __syncthreads();
@@ -324,8 +325,9 @@ struct TcPlan {
   float* w_out = nullptr;
   uint16_t* dact = nullptr;
   uint8_t* aimg = nullptr;
-  int64_t dact_tiles = 0;
-  bool r64 = false;
+  size_t dact_cap = 0, aimg_cap = 0;
+  int n_sm = 0;
+  int force_rows = 0;   // BEST_TC_ROWS=128|64|32 (environment, read at best_create): measurements only
 };
 
 namespace {
@@ -338,37 +340,67 @@ uint16_t f32_to_bf16(float f) {  // round to nearest even
   return (uint16_t)(u >> 16);
 }
 
-template <int METHOD, bool R64>
+template <int METHOD, int ROWS>
 int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
   TcPlan* pl = ctx->tc;
-  constexpr int kTileRows = tc::Geo<R64>::kTileRows;
-  const int64_t n_tiles = (rows + kTileRows - 1) / kTileRows;
-  if (n_tiles > pl->dact_tiles) {
-    if (pl->dact || pl->aimg) BEST_CUDA(cudaStreamSynchronize(s));
-    if (pl->dact) { cudaFree(pl->dact); pl->dact = nullptr; }
-    if (pl->aimg) { cudaFree(pl->aimg); pl->aimg = nullptr; }
-    const size_t elems = pl->P.dact_tile_elems * (size_t)n_tiles;
-    BEST_CUDA(cudaMalloc(&pl->dact, sizeof(uint16_t) * (elems ? elems : 8)));
-    if (R64) BEST_CUDA(cudaMalloc(&pl->aimg, (size_t)131072 * (size_t)n_tiles));
-    pl->dact_tiles = n_tiles;
-    pl->P.dact = pl->dact;
-    pl->P.aimg = pl->aimg;
+  const int64_t n_tiles = (rows + ROWS - 1) / ROWS;
+  // scratch: act' blocks (forward -> backward) and, for ROWS < 128, the next-operand image
+  pl->P.dact_tile_elems = (size_t)(pl->P.n_hidden - 1) * pl->P.H * ROWS;
+  const size_t dact_bytes = sizeof(uint16_t) * pl->P.dact_tile_elems * (size_t)n_tiles + 16;
+  const size_t aimg_bytes = tc::Geo<ROWS>::kInPlace ? 16 : (size_t)16 * tc::Geo<ROWS>::kAChunk * (size_t)n_tiles;
+  if (dact_bytes > pl->dact_cap || aimg_bytes > pl->aimg_cap) {
+    BEST_CUDA(cudaStreamSynchronize(s));
+    if (dact_bytes > pl->dact_cap) {
+      if (pl->dact) cudaFree(pl->dact);
+      pl->dact = nullptr; pl->dact_cap = 0;
+      BEST_CUDA(cudaMalloc(&pl->dact, dact_bytes));
+      pl->dact_cap = dact_bytes;
+    }
+    if (aimg_bytes > pl->aimg_cap) {
+      if (pl->aimg) cudaFree(pl->aimg);
+      pl->aimg = nullptr; pl->aimg_cap = 0;
+      BEST_CUDA(cudaMalloc(&pl->aimg, aimg_bytes));
+      pl->aimg_cap = aimg_bytes;
+    }
   }
+  pl->P.dact = pl->dact;
+  pl->P.aimg = pl->aimg;
   static bool attr_set = false;
   const int smem_bytes = tc::SmemLayout::TOTAL + 1024;
   if (!attr_set) {
-    BEST_CUDA(cudaFuncSetAttribute(tc::best_tc_kernel<METHOD, R64>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    BEST_CUDA(cudaFuncSetAttribute(tc::best_tc_kernel<METHOD, ROWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
     attr_set = true;
   }
   pl->P.L = ctx->L_dev;
-  tc::best_tc_kernel<METHOD, R64><<<(unsigned)n_tiles, tc::kThreads, smem_bytes, s>>>(pl->P, R);
+  tc::best_tc_kernel<METHOD, ROWS><<<(unsigned)n_tiles, tc::kThreads, smem_bytes, s>>>(pl->P, R);
   count_launch();
   BEST_CUDA(cudaGetLastError());
   return BEST_OK;
 }
+
+// Chains per CTA.  Measured on B200 (27->512^4->1, one CTA alone, HMC ms per 128 evaluations):
+// 128-chain in-place tiles 6.69, 64-chain 9.33, 32-chain 7.82 -- the L2 round trip of the operand
+// costs more than the smaller epilogue saves, so widths <= 512 always use 128-chain tiles; only
+// 1024-wide layers (whose operand does not fit in place) use 64, or 32 when that fills more SMs.
+int pick_rows(const TcPlan* pl, int64_t rows, int n_sm) {
+  if (pl->force_rows) return pl->force_rows;
+  if (pl->P.H != 1024) return 128;
+  return (rows + 63) / 64 >= n_sm ? 64 : ((rows + 31) / 32 > (rows + 63) / 64 && rows <= 32 * (int64_t)n_sm ? 32 : 64);
+}
+
 template <int METHOD>
 int launch_tc(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
-  return ctx->tc->r64 ? launch_tc_geo<METHOD, true>(ctx, R, rows, s) : launch_tc_geo<METHOD, false>(ctx, R, rows, s);
+  TcPlan* pl = ctx->tc;
+  if (pl->n_sm == 0) {
+    int dev = 0;
+    BEST_CUDA(cudaGetDevice(&dev));
+    BEST_CUDA(cudaDeviceGetAttribute(&pl->n_sm, cudaDevAttrMultiProcessorCount, dev));
+  }
+  switch (pick_rows(pl, rows, pl->n_sm)) {
+    case 128: return launch_tc_geo<METHOD, 128>(ctx, R, rows, s);
+    case 64: return launch_tc_geo<METHOD, 64>(ctx, R, rows, s);
+    default: return launch_tc_geo<METHOD, 32>(ctx, R, rows, s);
+  }
 }
 
 }  // namespace
@@ -388,8 +420,12 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   const int d = cfg->d;
   TcPlan* pl = new TcPlan();
   ctx->tc = pl;
-  pl->r64 = r64;
+  if (const char* e = std::getenv("BEST_TC_ROWS")) {
+    const int v = std::atoi(e);
+    if ((v == 64 || v == 32 || (v == 128 && !r64))) pl->force_rows = v;
+  }
   tc::Params& P = pl->P;
+  P.bias16 = r64 ? 1 : 0;
   P.d = d; P.H = H; P.n_hidden = K; P.act = cfg->activation; P.mlp_scale = cfg->mlp_scale;
   const int ncols = H < 256 ? H : 256, nch = H / ncols, kchH = H / 64;
   int no = 0;
@@ -399,7 +435,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   for (int l = K - 1; l >= 1; --l) P.ops[no++] = tc::OpDesc{kchH, nch, ncols, tc::EPI_BWD_HID, l - 1};
   P.ops[no++] = tc::OpDesc{kchH, 1, 32, tc::EPI_BWD_FINAL, 0};
   P.n_ops_all = no;
-  P.dact_tile_elems = (size_t)(K - 1) * H * (r64 ? 64 : 128);
+  P.dact_tile_elems = 0;   // set per launch (depends on the tile geometry)
 
   // host views of the fp32 weights
   std::vector<const float*> W(K + 1);
