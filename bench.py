@@ -32,6 +32,7 @@ WORKLOADS = {
     "sterile_mala_16k": dict(cfg=4, make="sterile", n_chains=16384, mlp_scale=1.0, method="mala", eps=0.01, inner=20),
     "sterile_mh_16k": dict(cfg=4, make="sterile", n_chains=16384, mlp_scale=1.0, method="mh", eps=0.3, inner=20),
     "sterile_hmc_16k": dict(cfg=4, make="sterile", n_chains=16384, mlp_scale=1.0, method="hmc", eps=0.03, n_leapfrog=8, inner=4),
+    "lcdm256_hmc": dict(cfg=2, make="lcdm", hidden=256, n_chains=16384, mlp_scale=3.0, method="hmc", eps=0.1, n_leapfrog=16, inner=8),
     "tiny_mala": dict(cfg=0, make="tiny", n_chains=64, mlp_scale=0.1, method="mala", eps=0.3, inner=100),
 }
 
@@ -40,7 +41,7 @@ def make_workload(spec, n_chains=None):
     from paper_2606_04895_b200 import workloads as WL
     n = n_chains or spec["n_chains"]
     if spec["make"] == "lcdm":
-        return WL.lcdm(n_chains=n, mlp_scale=spec["mlp_scale"])
+        return WL.lcdm(n_chains=n, mlp_scale=spec["mlp_scale"], hidden=spec.get("hidden", 512))
     if spec["make"] == "tiny":
         return WL.tiny(n_chains=n)
     if spec["make"] == "sterile":
@@ -212,13 +213,15 @@ def main():
             torch.distributed.barrier()
         torch.cuda.synchronize()
 
-    def measure(spec, steps, warmup, with_e2e):
+    def measure(spec, steps, warmup, with_e2e, prec=prec, adapt_every=0):
         """returns dict(ms_per_step(max over ranks), launches, clocks, e2e…) for this rank's shard."""
         w = make_workload(spec)
         if world > 1:   # weak scaling: every rank advances its own n_chains chains (seeded by rank)
             w = w.with_chains(spec["n_chains"], seed=1000 + rank)
         ctx = B.Context(w, prec)
         st = ctx.new_state(w.theta0)
+        if adapt_every:
+            st.set_adaptation(adapt_every, 1e-6)
         stream = torch.cuda.current_stream().cuda_stream
         flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
         inner = spec["inner"]
@@ -320,15 +323,33 @@ def main():
         line["cpu_baseline"] = cpu_baseline(spec)
     if world == 1 and not args.no_extra and args.workload == "lcdm_mala":
         extra = {}
-        for name in ("hmc", "lcdm_mala_16k", "lcdm_mh_16k"):
-            sp = dict(WORKLOADS[name])
-            rr = measure(sp, max(3, args.steps // 4), 3, with_e2e=False)
-            ms = rr["ms_total"] / max(3, args.steps // 4)
+        n_x = max(3, args.steps // 4)
+        for name in ("hmc", "lcdm_mala_16k", "lcdm_mh_16k", "aies", "sterile_mala_16k", "hmc_fp32"):
+            sp = dict(WORKLOADS[name.replace("_fp32", "")])
+            if name.endswith("_fp32"):      # exact path: one launch per layer, much slower -> 1 trajectory
+                sp["inner"] = 1
+                rr = measure(sp, n_x, 3, with_e2e=False, prec=B.PREC_FP32)
+            else:
+                rr = measure(sp, n_x, 3, with_e2e=False)
+            ms = rr["ms_total"] / n_x
             v = sp["n_chains"] * sp["inner"] / (ms * 1e-3)
             tf = flops_per_chain_step(rr["w"], sp) * v / 1e12
             extra[name] = {"chain_steps_per_s": v, "grad_evals_per_s": v * evals_per_chain_step(sp),
                            "tflops": tf, "frac_of_peak": tf / peak_tf, "ms_per_step": ms,
                            "accept_rate": rr["accept_rate"], "inner": sp["inner"]}
+        # BASELINE configs[4]: chain-steps/s vs batch size on the 29->1024^4->1 banana target, with the
+        # running covariance -> Cholesky update every 500 steps on device (one window per point here)
+        sweep = {}
+        for meth, kw in (("mh", dict(eps=0.3)), ("mala", dict(eps=0.01)), ("hmc", dict(eps=0.03, n_leapfrog=8))):
+            for nb in (1, 64, 1024, 16384, 65536):
+                n_steps = 500 if nb <= 16384 and meth != "hmc" else (100 if nb <= 16384 else 50)
+                sp = dict(cfg=4, make="sterile", n_chains=nb, mlp_scale=1.0, method=meth, inner=n_steps, **kw)
+                rr = measure(sp, 1, 1, with_e2e=False, adapt_every=500)
+                v = nb * n_steps / (rr["ms_total"] * 1e-3)
+                sweep[f"{meth}_{nb}"] = {"chain_steps_per_s": v, "ms_per_sampler_step": rr["ms_total"] / n_steps,
+                                         "tflops": flops_per_chain_step(rr["w"], sp) * v / 1e12,
+                                         "accept_rate": rr["accept_rate"], "sampler_steps": n_steps}
+        extra["sweep_adapt500"] = sweep
         line["extra"] = extra
     if rank == 0:
         print(json.dumps(line))
