@@ -22,6 +22,11 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/r1c_ncu_full.md); None where no capture exists.
+NCU_TRAFFIC_BYTES = {("lcdm_mala", 100, "bf16"): 5.208064e6 + 0.152064e6,
+                     ("hmc", 1, "bf16"): 10.798848e6 + 9.035520e6}
+
 WORKLOADS = {
     # name: (maker kwargs, method, sampler kwargs, inner steps per bench step, config index)
     "lcdm_mala": dict(cfg=1, make="lcdm", n_chains=4096, mlp_scale=1.0, method="mala", eps=0.3, inner=100),
@@ -314,7 +319,9 @@ def main():
         "e2e": {"value": Btot * inner / r["e2e_s_per_step"], "unit": "chain-steps/s",
                 "h2d_bytes_per_step": r["h2d"], "d2h_bytes_per_step": r["d2h"]},
         "roofline": {"bound": "tensor" if args.precision == "bf16" else "alu", "achieved": achieved_tf,
-                     "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": None,
+                     "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
+                     "traffic": NCU_TRAFFIC_BYTES.get((args.workload, inner, args.precision)) if spec["n_chains"] == WORKLOADS[args.workload]["n_chains"] else None,
+                     "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1c_ncu_full.md)",
                      "peak_source": peak_src,
                      "frac_of_sustained": (achieved_tf / peaks["bf16_tflops_sustained"]) if peaks and args.precision == "bf16" else None,
                      "kernel": "best_tc_kernel<%s>" % spec["method"], "flops_per_launch": flops_per_launch},
