@@ -111,6 +111,37 @@ def test_T1_1024_two_hidden_tanh(B, O):
         ctx.close()
 
 
+@pytest.mark.parametrize("rows", [64, 32])
+def test_T1_small_tile_geometries(B, O, rows, monkeypatch):
+    """The 64-/32-chain tile geometries (operand through the L2 image) on the 27→512⁴→1 net: same
+    parity bar as the 128-chain tiles, plus one MALA and one AIES step against the 128-chain result."""
+    base = WL.lcdm(n_chains=8, mlp_scale=1.0)
+    n = 5 * rows + 19
+    pts = WL.probe_points(base, n, seed=29)
+    w = WL.mlp_only(base)
+    monkeypatch.setenv("BEST_TC_ROWS", str(rows))
+    ctx = B.Context(w, B.PREC_BF16)
+    lp = np.zeros(n, np.float32)
+    g = np.zeros((n, w.d), np.float32)
+    ctx.logp_grad(pts, n, lp, g)
+    lp_ref, g_ref = O.Oracle(w).logp_grad(pts)
+    check_logp_grad(lp, g, lp_ref, g_ref, TOL[1], f"lcdm/rows={rows}")
+    ctx.close()
+    # the geometry changes no arithmetic: a sampler step is bit-identical to the 128-chain tiles
+    wf = WL.lcdm(n_chains=300)
+    outs = []
+    for r in (rows, 128):
+        monkeypatch.setenv("BEST_TC_ROWS", str(r))
+        c2 = B.Context(wf, B.PREC_BF16)
+        st = c2.new_state(wf.theta0)
+        st.step_mala(3, 5, f32(0.3))
+        st.step_aies(2, 6, 2.0)
+        outs.append(st.get(want_grad=False))
+        c2.close()
+    assert np.array_equal(outs[0]["theta"], outs[1]["theta"])
+    assert np.array_equal(outs[0]["n_accept"], outs[1]["n_accept"])
+
+
 def test_unsupported_shapes(B):
     for hidden in ((50, 37), (64, 128), (2048,), (1024,) * 5):
         w = WL.tiny(hidden=hidden)
