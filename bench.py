@@ -54,6 +54,27 @@ def make_workload(spec, n_chains=None):
     raise KeyError(spec["make"])
 
 
+def shard_workload(spec, rank, world):
+    """Weak scaling: chains are independent, so every rank advances its OWN
+    spec['n_chains'] chains of the same target; rank r's chains start from θ₀ drawn with seed 1000+r.
+    No data-path collective exists."""
+    w = make_workload(spec)
+    if world > 1:
+        w = w.with_chains(spec["n_chains"], seed=1000 + rank)
+    return w
+
+
+def max_over_ranks(value, world, device="cuda"):
+    """device-timed milliseconds -> max over ranks (the slowest rank defines the step)"""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def evals_per_chain_step(spec):
     return spec.get("n_leapfrog", 1) if spec["method"] == "hmc" else 1
 
@@ -220,9 +241,7 @@ def main():
 
     def measure(spec, steps, warmup, with_e2e, prec=prec, adapt_every=0):
         """returns dict(ms_per_step(max over ranks), launches, clocks, e2e…) for this rank's shard."""
-        w = make_workload(spec)
-        if world > 1:   # weak scaling: every rank advances its own n_chains chains (seeded by rank)
-            w = w.with_chains(spec["n_chains"], seed=1000 + rank)
+        w = shard_workload(spec, rank, world)
         ctx = B.Context(w, prec)
         st = ctx.new_state(w.theta0)
         if adapt_every:
@@ -248,10 +267,7 @@ def main():
         launches = B.launch_count() - l0
         ck = clocks.stop()
         dev_ms = sum(a.elapsed_time(b) for a, b in ev)
-        t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
-        if world > 1:
-            torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-        dev_ms = float(t.item())
+        dev_ms = max_over_ranks(dev_ms, world)
         acc = st.get(want_grad=False)
         res = dict(w=w, ms_total=dev_ms, launches=int(launches), clocks=ck, wall_s=t_wall,
                    accept_rate=float(acc["n_accept"].mean() / max(acc["step"], 1)))
@@ -276,10 +292,7 @@ def main():
                 e2e_once()
             barrier()
             el = time.perf_counter() - t0
-            t = torch.tensor([el], dtype=torch.float64, device="cuda")
-            if world > 1:
-                torch.distributed.all_reduce(t, op=torch.distributed.ReduceOp.MAX)
-            res["e2e_s_per_step"] = float(t.item()) / n_e2e
+            res["e2e_s_per_step"] = max_over_ranks(el, world) / n_e2e
             res["h2d"] = int(w.theta0.nbytes)
             res["d2h"] = int(out_theta.nbytes + out_logp.nbytes)
         st.close()

@@ -122,9 +122,17 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   uint32_t hi[4], lo[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
+#if BEST_TC_ACT_F16
+    const uint32_t h2 = ptx::cvt_f16x2(th[2 * i], th[2 * i + 1]);
+    float b0, b1;
+    ptx::unpack2(ptx::f16x2_to_f32x2(h2), b0, b1);
+    hi[i] = h2;
+    lo[i] = ptx::cvt_f16x2(th[2 * i] - b0, th[2 * i + 1] - b1);
+#else
     const uint32_t h2 = ptx::pack_bf16x2(th[2 * i], th[2 * i + 1]);
     hi[i] = h2;
     lo[i] = ptx::pack_bf16x2(th[2 * i] - ptx::bf16_lo(h2), th[2 * i + 1] - ptx::bf16_hi(h2));
+#endif
   }
   const uint32_t rowa = C.sbase + SmemLayout::A + C.row * 128;
   ptx::sts_128(rowa + (((uint32_t)C.k ^ (C.row & 7)) << 4), hi[0], hi[1], hi[2], hi[3]);
@@ -133,8 +141,7 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   if ((!Geo<ROWS>::kInPlace)) {
     ptx::mbar_arrive(C.bars.xin_done());   // warp 3 publishes a_ready
   } else {
-#pragma unroll
-    for (int j = 0; j < kMaxKch; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
+    for (int j = 0; j < C.P->kch_max; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
   }
 }
 
@@ -159,6 +166,37 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, co
     for (int i = 0; i < 4; ++i) ptx::lds_c2x64(C.wouts_thr + jn * 256 + i * 16, ws[2 * i], ws[2 * i + 1]);
   }
   uint32_t dp[8];
+#if BEST_TC_ACT_F16
+  // fp16x2 epilogue: a' = (acc + bias) rounded to fp16 (prescaled by 1/2 for SiLU), ONE MUFU per pair,
+  // four HFMA2; the results are already the packed fp16 operand / act' words.
+  constexpr uint32_t kHalf = 0x38003800u, kNegHalf = 0xB800B800u, kOne = 0x3C003C00u;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const f32x2 a32 = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), b[i]);
+    const uint32_t a = ptx::cvt_f16x2_from(a32);
+    const uint32_t t = ptx::tanh_f16x2(a);
+    uint32_t h, dd;
+    if (ACT == BEST_ACT_SILU) {
+      h = ptx::hfma2(a, t, a);
+      const uint32_t sg = ptx::hfma2(t, kHalf, kHalf);
+      const uint32_t om = ptx::hfma2(t, kNegHalf, kHalf);
+      dd = ptx::hfma2(h, om, sg);
+    } else {
+      h = t;
+      dd = ptx::hfma2(ptx::hneg2(t), t, kOne);
+    }
+    if (LAST) {
+      // the scalar output keeps an fp32 path: h in fp32 from the fp16 tanh
+      const f32x2 t32 = ptx::f16x2_to_f32x2(t);
+      const f32x2 h32 = (ACT == BEST_ACT_SILU) ? ptx::fma2(a32, t32, a32) : t32;
+      acc2 = ptx::fma2(h32, ws[i], acc2);
+      if (want_grad) hp[i] = ptx::hmul2(dd, ptx::cvt_f16x2_from(ws[i]));
+    } else {
+      hp[i] = h;
+      dp[i] = dd;
+    }
+  }
+#else
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     const f32x2 a = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), b[i]);
@@ -172,6 +210,7 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, co
       dp[i] = ptx::pack_bf16x2_from(dd);
     }
   }
+#endif
   if (!LAST && want_grad) {
     uint8_t* dptr = dact_l + (size_t)jn * kDBlk;
     ptx::stg_128(dptr, dp[0], dp[1], dp[2], dp[3]);
@@ -231,8 +270,12 @@ __device__ __forceinline__ void bwd_group(const uint32_t (&v)[16], const uint4& 
   const uint32_t dw[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
+#if BEST_TC_ACT_F16
+    hp[i] = ptx::hmul2(ptx::cvt_f16x2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), dw[i]);
+#else
     const f32x2 dd = ptx::pack2u(dw[i] << 16, dw[i] & 0xFFFF0000u);
     hp[i] = ptx::pack_bf16x2_from(ptx::mul2(ptx::pack2u(v[2 * i], v[2 * i + 1]), dd));
+#endif
   }
 }
 template <int ROWS>
@@ -313,7 +356,7 @@ __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool wa
     if ((!Geo<ROWS>::kInPlace)) {   // keep every epi_done barrier at one phase per op (written = 64-column groups)
       for (int c = (written * 64 + op.ncols - 1) / op.ncols; c < 4; ++c) ptx::mbar_arrive(C.bars.epi_done(c));
     } else if (oi != n_ops - 1) {  // keep every a_ready barrier at one phase per op
-      for (int j = written; j < kMaxKch; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
+      for (int j = written; j < C.P->kch_max; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
     }
   }
   float a0, a1;

@@ -53,6 +53,13 @@ constexpr int kCtrlWarps = 4;          // producer, MMA issuer, TMEM allocator, 
 constexpr int kEpiWarps = 16;          // 4 per TMEM lane quarter
 constexpr int kEpiThreads = kEpiWarps * 32;
 constexpr int kThreads = (kCtrlWarps + kEpiWarps) * 32;
+// Operand type option: 1 = fp16 weights AND activations (kind::f16 needs equal operand formats; mixed
+// fp16 x bf16 traps), packed HFMA2 epilogue math with one MUFU per element PAIR.  Measured on B200
+// (27->512^4->1): gradient error 5.8e-3 instead of 1.49e-2, same speed (984 vs 998 TFLOP/s: the
+// epilogue is latency-, not math-bound).  Default 0 = bf16, the type BASELINE.json names.
+#ifndef BEST_TC_ACT_F16
+#define BEST_TC_ACT_F16 0
+#endif
 // Two register-allocation experiments, both measured SLOWER on B200 (HMC 16k chains: 1006 TFLOP/s
 // with neither, 938 with pinned per-thread constants, 881 with setmaxnreg 40/104) and so off:
 #ifndef BEST_TC_SETMAXNREG
@@ -90,6 +97,7 @@ struct Params {
   uint16_t* dact;         // scratch: per tile [n_hidden-1][H/64][8 pieces][tile rows][8] bf16
   size_t dact_tile_elems;
   uint8_t* aimg;          // ROWS < 128: per tile, SMEM image of the next A operand [16 chunks][ROWS][128 B]
+  int kch_max;            // k-chunks of the widest operand (= H / 64): barriers 0..kch_max-1 are in use
   int bias16;             // bias table kept as bf16 in SMEM (1024-wide layers)
   // target terms (fp64 masters on device, converted to fp32 in SMEM at kernel start)
   int has_gauss, has_box, banana_i, banana_j;
@@ -200,10 +208,10 @@ __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uin
   for (int64_t e = 0; e < n_evals; ++e) {
     for (int oi = 0; oi < n_ops; ++oi, ++o) {
       const OpDesc op = P.ops[oi];
-      const uint32_t idesc = ptx::idesc_bf16(kRows, op.ncols);
+      const uint32_t idesc = BEST_TC_ACT_F16 ? ptx::idesc_f16(kRows, op.ncols) : ptx::idesc_bf16(kRows, op.ncols);
       // chunks this op does not read are free as soon as everything issued so far has completed
       if (elect_one())
-        for (int j = op.kch; j < kMaxKch; ++j) ptx::mma_commit(bars.a_free(j));
+        for (int j = op.kch; j < P.kch_max; ++j) ptx::mma_commit(bars.a_free(j));
       __syncwarp();
       for (int c = 0; c < op.nch; ++c, ++g) {
         const uint32_t buf = g & 1u, use = g >> 1;
@@ -252,12 +260,12 @@ __device__ void loader_loop(const Params& P, const Bars& bars, uint32_t a_base, 
   for (int64_t e = 0; e < n_evals; ++e) {
     ptx::mbar_wait(bars.xin_done(), (uint32_t)(e & 1));
     if (elect_one())
-      for (int j = 0; j < kMaxKch; ++j) ptx::mbar_arrive(bars.a_ready(j));
+      for (int j = 0; j < P.kch_max; ++j) ptx::mbar_arrive(bars.a_ready(j));
     __syncwarp();
     for (int oi = 0; oi + 1 < n_ops; ++oi, ++o) {
       const OpDesc op = P.ops[oi];
       const int out_kch = (op.nch * op.ncols) >> 6;   // k-chunks of the operand this op produces
-      for (int j = 0; j < kMaxKch; ++j) {
+      for (int j = 0; j < P.kch_max; ++j) {
         if (j < out_kch) {
           ptx::mbar_wait(bars.epi_done((j * 64) / op.ncols), o & 1u);
           ptx::mbar_wait(bars.a_free(j), o & 1u);

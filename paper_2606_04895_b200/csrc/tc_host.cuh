@@ -332,6 +332,24 @@ struct TcPlan {
 
 namespace {
 
+uint16_t f32_to_f16(float f) {   // round to nearest even, overflow -> inf
+  uint32_t u;
+  std::memcpy(&u, &f, 4);
+  const uint32_t sign = (u >> 16) & 0x8000u;
+  const uint32_t a = u & 0x7FFFFFFFu;
+  if (a >= 0x7F800000u) return (uint16_t)(sign | 0x7C00u | (a > 0x7F800000u ? 0x200u : 0u));
+  if (a >= 0x477FF000u) return (uint16_t)(sign | 0x7C00u);                  // >= 65520 rounds to inf
+  if (a < 0x33000001u) return (uint16_t)sign;                               // < 2^-25 rounds to zero
+  int e = (int)(a >> 23) - 127;
+  uint32_t m = (a & 0x7FFFFFu) | 0x800000u;
+  int shift = (e < -14) ? (13 + (-14 - e)) : 13;                            // subnormal: shift further
+  uint32_t half_m = m >> shift;
+  const uint32_t rem = m & ((1u << shift) - 1u), halfway = 1u << (shift - 1);
+  if (rem > halfway || (rem == halfway && (half_m & 1u))) ++half_m;
+  uint32_t he = (e < -14) ? 0u : (uint32_t)(e + 15);
+  uint32_t r = (e < -14) ? half_m : ((he << 10) + (half_m - 0x400u));      // carry propagates into exponent
+  return (uint16_t)(sign | r);
+}
 uint16_t f32_to_bf16(float f) {  // round to nearest even
   uint32_t u;
   std::memcpy(&u, &f, 4);
@@ -426,6 +444,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   }
   tc::Params& P = pl->P;
   P.bias16 = r64 ? 1 : 0;
+  P.kch_max = H / 64;
   P.d = d; P.H = H; P.n_hidden = K; P.act = cfg->activation; P.mlp_scale = cfg->mlp_scale;
   const int ncols = H < 256 ? H : 256, nch = H / ncols, kchH = H / 64;
   int no = 0;
@@ -470,7 +489,8 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
         for (int r = 0; r < op.ncols; ++r)
           for (int kk = 0; kk < 32; ++kk) {
             const size_t off = (size_t)r * 32 + ((((kk >> 3) ^ ((r >> 1) & 3))) << 3) + (kk & 7);
-            pack[base + off] = f32_to_bf16(Bm(c * op.ncols + r, k32 * 32 + kk));
+            const float wv = Bm(c * op.ncols + r, k32 * 32 + kk);
+            pack[base + off] = BEST_TC_ACT_F16 ? f32_to_f16(wv) : f32_to_bf16(wv);
           }
       }
   }

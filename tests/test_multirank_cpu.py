@@ -1,0 +1,63 @@
+"""world_size-2 gloo test of the N>1 host logic of bench.py: chains shard across ranks
+with no data-path collective (each rank owns its own chains of the same target), the step time is the
+max over ranks, and the reference arm runs on rank 0 only."""
+import os
+import subprocess
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+WORKER = r"""
+import os, sys, json
+import numpy as np
+import torch, torch.distributed as dist
+sys.path.insert(0, sys.argv[1])
+import bench
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo")
+spec = dict(bench.WORKLOADS["tiny_mala"])
+w = bench.shard_workload(spec, rank, world)
+ms = bench.max_over_ranks(10.0 + 5.0 * rank, world, device="cpu")
+dist.barrier()
+out = dict(rank=rank, n_chains=int(w.n_chains), theta_sum=float(np.abs(w.theta0).sum()),
+           W0=float(w.W[0].sum()), mu0=float(w.mu[0]), ms=ms)
+print("RESULT " + json.dumps(out), flush=True)
+dist.destroy_process_group()
+"""
+
+
+def test_sharding_and_max_over_ranks_gloo(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER)
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29533", OMP_NUM_THREADS="1")
+    p = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+                        "--master-addr", "127.0.0.1", "--master-port", "29533", str(script), ROOT],
+                       capture_output=True, text=True, timeout=300, env=env)
+    assert p.returncode == 0, p.stderr[-2000:]
+    import json
+    res = sorted((json.loads(l.split("RESULT ", 1)[1]) for l in p.stdout.splitlines() if "RESULT " in l),
+                 key=lambda r: r["rank"])
+    assert [r["rank"] for r in res] == [0, 1]
+    # same target on both ranks (weights, mu), same number of chains, different chains
+    assert res[0]["W0"] == res[1]["W0"] and res[0]["mu0"] == res[1]["mu0"]
+    assert res[0]["n_chains"] == res[1]["n_chains"] == 64
+    assert res[0]["theta_sum"] != res[1]["theta_sum"]
+    # the slowest rank defines the step on every rank
+    assert res[0]["ms"] == res[1]["ms"] == 15.0
+
+
+def test_reference_arm_runs_on_rank0_only():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--steps", "1", "--warmup", "0", "--workload", "tiny_mala"],
+                       capture_output=True, text=True, timeout=300, env=env)
+    assert p.returncode == 0 and p.stdout.strip() == ""
+    env["RANK"] = "0"
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--steps", "1", "--warmup", "0", "--workload", "tiny_mala"],
+                       capture_output=True, text=True, timeout=300, env=env)
+    import json
+    line = json.loads(p.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
