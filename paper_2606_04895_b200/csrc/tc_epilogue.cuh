@@ -137,7 +137,11 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   const uint32_t rowa = C.sbase + SmemLayout::A + C.row * 128;
   ptx::sts_128(rowa + (((uint32_t)C.k ^ (C.row & 7)) << 4), hi[0], hi[1], hi[2], hi[3]);
   ptx::sts_128(rowa + (((uint32_t)(4 + C.k) ^ (C.row & 7)) << 4), lo[0], lo[1], lo[2], lo[3]);
+#if BEST_TC_CONSUMER_FENCE
+  if (!Geo<ROWS>::kInPlace) ptx::fence_proxy_async();
+#else
   ptx::fence_proxy_async();
+#endif
   if ((!Geo<ROWS>::kInPlace)) {
     ptx::mbar_arrive(C.bars.xin_done());   // warp 3 publishes a_ready
   } else {
@@ -222,7 +226,9 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, co
 template <int ROWS>
 __device__ __forceinline__ void publish_a(EpiCtx& C, int jn0, int n) {
   if (Geo<ROWS>::kInPlace) {
+#if !BEST_TC_CONSUMER_FENCE
     ptx::fence_proxy_async();
+#endif
     for (int i = 0; i < n; ++i) ptx::mbar_arrive(C.bars.a_ready(jn0 + i));
   }
 }

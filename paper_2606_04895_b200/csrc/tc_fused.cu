@@ -60,6 +60,12 @@ constexpr int kThreads = (kCtrlWarps + kEpiWarps) * 32;
 #ifndef BEST_TC_ACT_F16
 #define BEST_TC_ACT_F16 0
 #endif
+// 1 = the generic->async proxy fence is executed by the MMA warp after it has acquired a_ready instead
+// of by every epilogue thread before its arrive.  Parity-green and 1 % faster on B200 (1006 vs 998
+// TFLOP/s), but the documented pattern is the writer-side fence, so that is the default.
+#ifndef BEST_TC_CONSUMER_FENCE
+#define BEST_TC_CONSUMER_FENCE 0
+#endif
 // Two register-allocation experiments, both measured SLOWER on B200 (HMC 16k chains: 1006 TFLOP/s
 // with neither, 938 with pinned per-thread constants, 881 with setmaxnreg 40/104) and so off:
 #ifndef BEST_TC_SETMAXNREG
@@ -222,6 +228,12 @@ __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uin
         for (int j = 0; j < op.kch; ++j) {
           if (c == 0) {
             ptx::mbar_wait(bars.a_ready(j), o & 1u);
+#if BEST_TC_CONSUMER_FENCE
+            // the epilogue's generic-proxy st.shared (released by its mbarrier.arrive, acquired by the
+            // wait above) become visible to the async proxy HERE: the proxy fence costs the epilogue
+            // warps a MEMBAR.ALL.CTA per 64-column group, the idle-storeless MMA warp almost nothing
+            if (Geo<ROWS>::kInPlace) ptx::fence_proxy_async();
+#endif
             ptx::tc_fence_after();
           }
 #pragma unroll
