@@ -23,6 +23,8 @@ struct EpiCtx {
   uint32_t tmem_lane;   // tmem base + (lane quarter << 16)
   int row;              // 0..127
   int k;                // 0..3
+  int to_leader;        // CTA pair, rank 1: a_ready / d_free arrivals go to the leader CTA's barriers
+  int half;             // CTA pair: 0 = lanes 0..63 (lower N half, runs the sampler), 1 = lanes 64..127
   uint32_t o, g;        // op / n-chunk counters (mirror the MMA issuer)
   uint32_t vslot, pslot;  // rotating scratch slots
   // per-thread constants
@@ -33,6 +35,12 @@ struct EpiCtx {
   uint8_t* dact_thr;        // global: this thread's 16 bytes inside act' block (layer 0, chunk 0)
   uint8_t* aimg_thr;        // L2-image tiles: global image of the next A operand, this thread's first 16-B piece
 };
+
+// arrive on a barrier the MMA issuer waits on: the CTA's own, or (second CTA of a pair) the leader's
+__device__ __forceinline__ void arrive_mma(const EpiCtx& C, uint32_t bar) {
+  if (C.to_leader) ptx::mbar_arrive_leader(bar);
+  else ptx::mbar_arrive(bar);
+}
 
 // bias of the thread's 16 columns of group jn as 8 fp32 pairs
 template <int ROWS>
@@ -59,8 +67,8 @@ __device__ __forceinline__ void load_bias(const EpiCtx& C, int layer, int jn, f3
 template <int ROWS>
 __device__ __forceinline__ void store_a(const EpiCtx& C, int jn, const uint32_t (&hp)[8]) {
   if (Geo<ROWS>::kInPlace) {
-    ptx::sts_128(C.a_thr0 + jn * kAChunkBytes, hp[0], hp[1], hp[2], hp[3]);
-    ptx::sts_128(C.a_thr1 + jn * kAChunkBytes, hp[4], hp[5], hp[6], hp[7]);
+    ptx::sts_128(C.a_thr0 + jn * Geo<ROWS>::kAChunk, hp[0], hp[1], hp[2], hp[3]);
+    ptx::sts_128(C.a_thr1 + jn * Geo<ROWS>::kAChunk, hp[4], hp[5], hp[6], hp[7]);
   } else {
     uint8_t* p0 = C.aimg_thr + (size_t)jn * Geo<ROWS>::kAChunk;
     uint8_t* p1 = reinterpret_cast<uint8_t*>(reinterpret_cast<uintptr_t>(p0) ^ (uintptr_t)16);
@@ -118,6 +126,7 @@ __device__ __forceinline__ void tanh_pair(f32x2 a, f32x2& h, f32x2& dact) {
 // ---- first A operand: theta split into bf16 hi | lo (own 8 dims -> pieces k and 4+k) ------------
 template <int ROWS>
 __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
+  if (Geo<ROWS>::kPair && C.half != 0) return;   // the upper lane half only takes part in the MLP epilogues
   ptx::mbar_wait(C.bars.a_free(0), (C.o & 1u) ^ 1u);
   uint32_t hi[4], lo[4];
 #pragma unroll
@@ -145,7 +154,7 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   if ((!Geo<ROWS>::kInPlace)) {
     ptx::mbar_arrive(C.bars.xin_done());   // warp 3 publishes a_ready
   } else {
-    for (int j = 0; j < C.P->kch_max; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
+    for (int j = 0; j < C.P->kch_max; ++j) arrive_mma(C, C.bars.a_ready(j));
   }
 }
 
@@ -229,7 +238,7 @@ __device__ __forceinline__ void publish_a(EpiCtx& C, int jn0, int n) {
 #if !BEST_TC_CONSUMER_FENCE
     ptx::fence_proxy_async();
 #endif
-    for (int i = 0; i < n; ++i) ptx::mbar_arrive(C.bars.a_ready(jn0 + i));
+    for (int i = 0; i < n; ++i) arrive_mma(C, C.bars.a_ready(jn0 + i));
   }
 }
 
@@ -238,17 +247,18 @@ template <int ACT, bool LAST, int ROWS>
 __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_grad, f32x2& acc2,
                                         int& written) {
   const bool writes_a = !(LAST && !want_grad);
-  const int ngrp = op.ncols >> 6;
+  // 64-column groups of this thread per N-chunk (CTA pair: the lane half owns half of the chunk)
+  const int ngrp = Geo<ROWS>::kPair ? (op.ncols >> 7) : (op.ncols >> 6);
   constexpr uint32_t kDBlk = Geo<ROWS>::kTileRows * 128;
   uint8_t* dact_l = C.dact_thr + (size_t)(op.layer * (C.P->H >> 6)) * kDBlk;
   for (int c = 0; c < op.nch; ++c, ++C.g) {
-    const uint32_t buf = C.g & 1u, use = C.g >> 1;
+    const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
-    const uint32_t tcol = C.tmem_lane + buf * 256u + C.k * 16;
+    const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
     const bool gate = Geo<ROWS>::kInPlace && writes_a && (c != op.nch - 1);
     for (int grp = 0; grp < ngrp; ++grp) {
-      const int jn = c * ngrp + grp;
+      const int jn = Geo<ROWS>::kPair ? c * (op.ncols >> 6) + C.half * ngrp + grp : c * ngrp + grp;
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
       ptx::tmem_ld_wait();
@@ -265,7 +275,7 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
       ptx::mbar_arrive(C.bars.epi_done(c));
     }
     ptx::tc_fence_before();
-    ptx::mbar_arrive(C.bars.d_free(buf));
+    arrive_mma(C, C.bars.d_free(buf));
   }
 }
 
@@ -286,20 +296,22 @@ __device__ __forceinline__ void bwd_group(const uint32_t (&v)[16], const uint4& 
 }
 template <int ROWS>
 __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& written) {
-  const int ngrp = op.ncols >> 6;
+  // 64-column groups of this thread per N-chunk (CTA pair: the lane half owns half of the chunk)
+  const int ngrp = Geo<ROWS>::kPair ? (op.ncols >> 7) : (op.ncols >> 6);
   constexpr uint32_t kDBlk = Geo<ROWS>::kTileRows * 128, kDPiece = Geo<ROWS>::kTileRows * 16;
   const uint8_t* dact_l = C.dact_thr + (size_t)(op.layer * (C.P->H >> 6)) * kDBlk;
   for (int c = 0; c < op.nch; ++c, ++C.g) {
-    const uint32_t buf = C.g & 1u, use = C.g >> 1;
+    const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
     const bool gate = Geo<ROWS>::kInPlace && (c != op.nch - 1);
     // act' of the first group can be fetched before the accumulator is complete
-    const uint8_t* dp = dact_l + (size_t)(c * ngrp) * kDBlk;
+    const int jn0 = Geo<ROWS>::kPair ? c * (op.ncols >> 6) + C.half * ngrp : c * ngrp;
+    const uint8_t* dp = dact_l + (size_t)jn0 * kDBlk;
     uint4 a0 = ptx::ldg_128(dp), a1 = ptx::ldg_128(dp + kDPiece);
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
-    const uint32_t tcol = C.tmem_lane + buf * 256u + C.k * 16;
+    const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
     for (int grp = 0; grp < ngrp; ++grp) {
-      const int jn = c * ngrp + grp;
+      const int jn = Geo<ROWS>::kPair ? c * (op.ncols >> 6) + C.half * ngrp + grp : c * ngrp + grp;
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
       const uint4 d0 = a0, d1 = a1;
@@ -319,7 +331,7 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
       ptx::mbar_arrive(C.bars.epi_done(c));
     }
     ptx::tc_fence_before();
-    ptx::mbar_arrive(C.bars.d_free(buf));
+    arrive_mma(C, C.bars.d_free(buf));
   }
 }
 
@@ -347,27 +359,57 @@ __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool wa
     } else if (op.epi == EPI_BWD_HID) {
       epi_bwd<ROWS>(C, op, written);
     } else {  // EPI_BWD_FINAL: D[128][32] -> own 8 columns
-      const uint32_t buf = C.g & 1u, use = C.g >> 1;
+      const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
       ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
       ptx::tc_fence_after();
-      uint32_t v[8];
-      ptx::tmem_ld8(C.tmem_lane + buf * 256u + C.k * 8, v);
-      ptx::tmem_ld_wait();
+      if (!Geo<ROWS>::kPair) {
+        uint32_t v[8];
+        ptx::tmem_ld8(C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 8, v);
+        ptx::tmem_ld_wait();
 #pragma unroll
-      for (int i = 0; i < 8; ++i) gm[i] = __uint_as_float(v[i]);
+        for (int i = 0; i < 8; ++i) gm[i] = __uint_as_float(v[i]);
+      } else {
+        // pair layout: lanes 0..63 hold gradient dims 0..15, lanes 64..127 dims 16..31 (TMEM columns
+        // 0..15 each); the k == 0 thread of each lane half hands them to the chain's sampler threads
+        // through SMEM [32 dims][64 rows] (chunk 6 of the operand buffer: every MMA has completed)
+        const uint32_t GX = C.sbase + SmemLayout::A + 49152u + (uint32_t)C.row * 4u;
+        if (C.k == 0) {
+          uint32_t v[16];
+          ptx::tmem_ld16(C.tmem_lane + buf * Geo<ROWS>::kBufCols, v);
+          ptx::tmem_ld_wait();
+#pragma unroll
+          for (int i = 0; i < 16; ++i) ptx::sts_32(GX + (uint32_t)(C.half * 16 + i) * 256u, __uint_as_float(v[i]));
+        }
+        ptx::named_bar_sync(5 + (C.row >> 5), 256);
+        if (C.half == 0) {
+#pragma unroll
+          for (int i = 0; i < 8; ++i) gm[i] = ptx::lds_32(GX + (uint32_t)(8 * C.k + i) * 256u);
+        }
+      }
       ptx::tc_fence_before();
-      ptx::mbar_arrive(C.bars.d_free(buf));
+      arrive_mma(C, C.bars.d_free(buf));
       ++C.g;
     }
     if ((!Geo<ROWS>::kInPlace)) {   // keep every epi_done barrier at one phase per op (written = 64-column groups)
       for (int c = (written * 64 + op.ncols - 1) / op.ncols; c < 4; ++c) ptx::mbar_arrive(C.bars.epi_done(c));
     } else if (oi != n_ops - 1) {  // keep every a_ready barrier at one phase per op
-      for (int j = written; j < C.P->kch_max; ++j) ptx::mbar_arrive(C.bars.a_ready(j));
+      if (!Geo<ROWS>::kPair) {
+        for (int j = written; j < C.P->kch_max; ++j) arrive_mma(C, C.bars.a_ready(j));
+      } else if (written == 0 && C.half == 0) {   // pair: an op writes all k-chunks or none
+        for (int j = 0; j < C.P->kch_max; ++j) arrive_mma(C, C.bars.a_ready(j));
+      }
     }
   }
   float a0, a1;
   ptx::unpack2(acc2, a0, a1);
   out_part = a0 + a1;
+  if (Geo<ROWS>::kPair) {   // the output dot product is split over both lane halves
+    const uint32_t PX = C.sbase + SmemLayout::PART + 1024u + (uint32_t)C.row * 16u + (uint32_t)C.k * 4u;
+    if (C.half == 1) ptx::sts_32(PX, out_part);
+    ptx::named_bar_sync(5 + (C.row >> 5), 256);
+    if (C.half == 0) out_part += ptx::lds_32(PX);
+    ptx::named_bar_sync(5 + (C.row >> 5), 256);   // PX may be rewritten by the next evaluation
+  }
 }
 
 // ---- cooperative per-chain algebra: each thread owns dims [8k, 8k+8) ---------------------------

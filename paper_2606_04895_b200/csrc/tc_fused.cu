@@ -14,6 +14,8 @@
 // The MLP forward and its input-gradient backprop (A1b, A1c) are a chain of GEMMs whose
 // activations never leave the SM; only act' (bf16) is parked in an L2-resident scratch between
 // the forward and backward sweeps.  See DESIGN.md §"tensor-core kernel".
+#include <cuda.h>
+
 #include <cstdlib>
 #include <cstring>
 
@@ -37,12 +39,22 @@ constexpr int kRows = 128;           // TMEM lanes == MMA M
 //                accumulators (1024 columns) no longer fits TMEM, so the epilogue writes the
 //                next operand to an L2-resident image and warp 3 copies it back chunk by chunk
 //                (cp.async.bulk) as soon as the last N-chunk's MMAs have released the chunk.
+//   ROWS = 264 : CTA PAIR for 1024-wide layers (cluster of 2, tcgen05 cta_group::2): 64 chains per CTA,
+//                the leader CTA issues M = 128 MMAs over both CTAs' rows, each CTA streams HALF of
+//                every weight tile, and an N = 256 accumulator chunk takes only 128 TMEM columns per
+//                CTA (lanes 64..127 hold the upper half of N for the same 64 rows), so a whole
+//                1024-wide layer of accumulators fits TMEM and the operand is rewritten in place.
 template <int ROWS> struct Geo {
-  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32, "tile rows");
-  static constexpr bool kInPlace = (ROWS == 128);
-  static constexpr int kTileRows = ROWS;
-  static constexpr int kAChunk = ROWS * 128;           // bytes of one 64-column k-chunk
-  static constexpr int kEpiActive = ROWS * 4;          // epilogue threads that own a real chain
+  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32 || ROWS == 264, "tile geometry");
+  static constexpr bool kPair = (ROWS == 264);
+  static constexpr bool kInPlace = (ROWS == 128 || ROWS == 264);
+  static constexpr int kTileRows = kPair ? 64 : ROWS;
+  static constexpr int kAChunk = kTileRows * 128;      // bytes of one 64-column k-chunk
+  static constexpr int kEpiActive = kPair ? 512 : ROWS * 4;   // epilogue threads with MLP epilogue work
+  static constexpr int kNBuf = kPair ? 4 : 2;          // accumulator buffers
+  static constexpr int kBufCols = kPair ? 128 : 256;   // TMEM columns per buffer
+  static constexpr int kStagesG = 4;                   // weight ring: stages
+  static constexpr int kStageBytesG = 16384;           // ... of this many bytes per CTA (pair: one K = 64 slice)
 };
 constexpr int kAChunkBytes = 16384;  // R64 = false chunk pitch (also the exchange-slot size)
 constexpr int kMaxKch = 16;          // hidden width <= 1024
@@ -93,6 +105,8 @@ struct OpDesc {
 };
 
 struct Params {
+  // CTA-pair kernel: the weight pack as a 2-D byte tensor [rows][256 B], boxes of 32 rows (8 KB) / 4 rows (1 KB)
+  CUtensorMap wmap8, wmap1;
   int d, H, n_hidden, act;
   float mlp_scale, b_out;
   int n_ops_fwd, n_ops_all;
@@ -141,8 +155,9 @@ struct SmemLayout {
   static constexpr int VECS = RTMAT + 1024 * 4;                      // mu, lo, hi, 1/width: 4x32 floats
   static constexpr int PART = VECS + 4 * 32 * 4;                     // partial sums [2][4][128] floats
   static constexpr int BARS = PART + 2 * 4 * 128 * 4;
-  // barriers: full[4] empty[4] a_ready[16] a_free[16] d_full[2] d_free[2] epi_done[4] xin_done
-  static constexpr int NBARS = 2 * kStages + 2 * kMaxKch + 4 + 5;
+  // barriers: full[8] empty[8] a_ready[16] a_free[16] d_full[4] d_free[4] epi_done[4] xin_done and, for
+  // the CTA-pair kernel, the leader's copies of the peer's full[8] a_ready[16] d_free[4]
+  static constexpr int NBARS = 89;
   static constexpr int TMEMPTR = BARS + NBARS * 8;
   static constexpr int TOTAL = TMEMPTR + 16;
 };
@@ -151,13 +166,16 @@ static_assert(SmemLayout::TOTAL + 1024 <= 232448, "shared memory budget");
 struct Bars {  // mbarrier addresses are computed, never looked up (keeps them out of local memory)
   uint32_t base;
   __device__ __forceinline__ uint32_t full(int i) const { return base + 8u * i; }
-  __device__ __forceinline__ uint32_t empty(int i) const { return base + 8u * (kStages + i); }
-  __device__ __forceinline__ uint32_t a_ready(int j) const { return base + 8u * (2 * kStages + j); }
-  __device__ __forceinline__ uint32_t a_free(int j) const { return base + 8u * (2 * kStages + kMaxKch + j); }
-  __device__ __forceinline__ uint32_t d_full(int b) const { return base + 8u * (2 * kStages + 2 * kMaxKch + b); }
-  __device__ __forceinline__ uint32_t d_free(int b) const { return base + 8u * (2 * kStages + 2 * kMaxKch + 2 + b); }
-  __device__ __forceinline__ uint32_t epi_done(int c) const { return base + 8u * (2 * kStages + 2 * kMaxKch + 4 + c); }
-  __device__ __forceinline__ uint32_t xin_done() const { return base + 8u * (2 * kStages + 2 * kMaxKch + 8); }
+  __device__ __forceinline__ uint32_t empty(int i) const { return base + 8u * (8 + i); }
+  __device__ __forceinline__ uint32_t a_ready(int j) const { return base + 8u * (16 + j); }
+  __device__ __forceinline__ uint32_t a_free(int j) const { return base + 8u * (32 + j); }
+  __device__ __forceinline__ uint32_t d_full(int b) const { return base + 8u * (48 + b); }
+  __device__ __forceinline__ uint32_t d_free(int b) const { return base + 8u * (52 + b); }
+  __device__ __forceinline__ uint32_t epi_done(int c) const { return base + 8u * (56 + c); }
+  __device__ __forceinline__ uint32_t xin_done() const { return base + 8u * 60; }
+  __device__ __forceinline__ uint32_t full_peer(int i) const { return base + 8u * (61 + i); }
+  __device__ __forceinline__ uint32_t a_ready_peer(int j) const { return base + 8u * (69 + j); }
+  __device__ __forceinline__ uint32_t d_free_peer(int b) const { return base + 8u * (85 + b); }
 };
 __device__ __forceinline__ Bars make_bars(uint32_t base) { Bars b; b.base = base; return b; }
 
@@ -292,6 +310,91 @@ __device__ void loader_loop(const Params& P, const Bars& bars, uint32_t a_base, 
       }
     }
     ++o;   // the last op of the evaluation produces no operand
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// CTA-pair roles (Geo<264>).  Both CTAs run the producer (own half of every weight tile, own 8 x 8 KB
+// ring) and the epilogue; the leader (cluster rank 0) issues the MMAs, the other CTA's warp 1 relays
+// the completion of ITS full / a_ready / d_free barriers to the leader's *_peer copies.
+// ------------------------------------------------------------------------------------------------
+__device__ void producer_loop_pair(const Params& P, const Bars& bars, uint32_t stage_base, uint32_t rank,
+                                   int64_t n_evals, int n_ops) {
+  constexpr uint32_t NS = Geo<264>::kStagesG, SB = Geo<264>::kStageBytesG;
+  uint32_t t = 0;   // stage counter: one stage = one 64-wide k-chunk = two K32 tiles (this CTA's halves)
+  for (int64_t e = 0; e < n_evals; ++e) {
+    uint32_t src = 0;   // byte offset inside the pack
+    for (int oi = 0; oi < n_ops; ++oi) {
+      const OpDesc op = P.ops[oi];
+      const uint32_t bytes = (uint32_t)op.ncols * 64u, half = bytes >> 1;   // rows [rank N/2, +N/2) of a tile
+      const void* tmap = (half == 8192u) ? (const void*)&P.wmap8 : (const void*)&P.wmap1;
+      const int nst = op.nch * op.kch;
+      for (int i = 0; i < nst; ++i, ++t) {
+        const uint32_t s = t % NS, use = t / NS;
+        ptx::mbar_wait(bars.empty(s), (use & 1u) ^ 1u);
+        if (elect_one()) {
+          // all four halves' bytes land on the LEADER's full barrier; only the leader arrives on it
+          if (rank == 0) ptx::mbar_arrive_expect_tx(bars.full(s), 2u * bytes);
+          ptx::tma_2sm_load_2d(stage_base + s * SB, tmap, bars.full(s), 0, (int)((src + rank * half) >> 8));
+          ptx::tma_2sm_load_2d(stage_base + s * SB + half, tmap, bars.full(s), 0, (int)((src + bytes + rank * half) >> 8));
+        }
+        __syncwarp();
+        src += 2u * bytes;
+      }
+    }
+  }
+}
+
+template <bool LEADER>
+__device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base, uint32_t stage_base,
+                              uint32_t tmem_base, int64_t n_evals, int n_ops) {
+  constexpr uint32_t NS = Geo<264>::kStagesG, SB = Geo<264>::kStageBytesG, NB = Geo<264>::kNBuf;
+  uint32_t t = 0, g = 0, o = 0;
+  const uint64_t adesc0 = ptx::smem_desc_sw128(a_base);
+  const uint64_t bdesc0 = ptx::smem_desc_sw64(stage_base);
+  for (int64_t e = 0; e < n_evals; ++e) {
+    for (int oi = 0; oi < n_ops; ++oi, ++o) {
+      const OpDesc op = P.ops[oi];
+      const uint32_t idesc = ptx::idesc_bf16(kRows, op.ncols);
+      const uint32_t half16 = ((uint32_t)op.ncols * 32u) >> 4;   // one K32 tile half, in descriptor units
+      if (LEADER) {
+        if (elect_one())
+          for (int j = op.kch; j < P.kch_max; ++j) ptx::mma_commit_2cta(bars.a_free(j));
+        __syncwarp();
+      }
+      for (int c = 0; c < op.nch; ++c, ++g) {
+        const uint32_t buf = g % NB, use = g / NB;
+        if (LEADER) {
+          ptx::mbar_wait(bars.d_free(buf), (use & 1u) ^ 1u);   // both CTAs' epilogue threads arrive here
+          ptx::tc_fence_after();
+        }
+        const uint32_t d_tmem = tmem_base + buf * Geo<264>::kBufCols;
+        const bool last_c = (c == op.nch - 1);
+        for (int j = 0; j < op.kch; ++j, ++t) {
+          if (LEADER) {
+            if (c == 0) ptx::mbar_wait(bars.a_ready(j), o & 1u);   // both CTAs' k-chunk j
+            const uint32_t s = t % NS, use_s = t / NS;
+            ptx::mbar_wait(bars.full(s), use_s & 1u);   // both CTAs' halves of both K32 tiles
+            ptx::tc_fence_after();
+            const uint64_t ad = adesc0 + (uint64_t)((j * Geo<264>::kAChunk) >> 4);
+            const uint64_t bd = bdesc0 + (uint64_t)((s * SB) >> 4);
+            if (elect_one()) {
+              ptx::mma_bf16_ss_2cta(d_tmem, ad, bd, idesc, j != 0 ? 1u : 0u);
+              ptx::mma_bf16_ss_2cta(d_tmem, ad + 2, bd + 2, idesc, 1u);
+              ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
+              ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
+              ptx::mma_commit_2cta(bars.empty(s));
+              if (last_c) ptx::mma_commit_2cta(bars.a_free(j));
+            }
+            __syncwarp();
+          }
+        }
+        if (LEADER) {
+          if (elect_one()) ptx::mma_commit_2cta(bars.d_full(buf));
+          __syncwarp();
+        }
+      }
+    }
   }
 }
 

@@ -222,17 +222,29 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + SmemLayout::TMEMPTR);
 
   if (tid == 0) {
-    for (int i = 0; i < kStages; ++i) { ptx::mbar_init(bars.full(i), 1); ptx::mbar_init(bars.empty(i), 1); }
-    for (int i = 0; i < kMaxKch; ++i) {
-      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : kEpiThreads);   // ROWS < 128: warp 3 (+ bulk-copy bytes)
-      ptx::mbar_init(bars.a_free(i), 1);
+    for (int i = 0; i < 8; ++i) {
+      ptx::mbar_init(bars.full(i), 1); ptx::mbar_init(bars.empty(i), 1); ptx::mbar_init(bars.full_peer(i), 1);
     }
-    for (int i = 0; i < 2; ++i) { ptx::mbar_init(bars.d_full(i), 1); ptx::mbar_init(bars.d_free(i), Geo<ROWS>::kEpiActive); }
+    for (int i = 0; i < kMaxKch; ++i) {
+      // arrivals per phase: in place = every epilogue thread (pair: the 256 of the lane half that owns the
+      // k-chunk); L2-image tiles = warp 3 alone (+ the bulk copy's bytes)
+      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : kEpiThreads);   // pair: 256 of each CTA
+      ptx::mbar_init(bars.a_free(i), 1);
+      ptx::mbar_init(bars.a_ready_peer(i), 1);
+    }
+    for (int i = 0; i < 4; ++i) {
+      ptx::mbar_init(bars.d_full(i), 1);
+      ptx::mbar_init(bars.d_free(i), Geo<ROWS>::kPair ? 2 * kEpiThreads : Geo<ROWS>::kEpiActive);   // pair: both CTAs
+      ptx::mbar_init(bars.d_free_peer(i), 1);
+    }
     for (int i = 0; i < 4; ++i) ptx::mbar_init(bars.epi_done(i), Geo<ROWS>::kEpiActive);
     ptx::mbar_init(bars.xin_done(), Geo<ROWS>::kEpiActive);
     ptx::fence_mbar_init();
   }
-  if (warp == 2) ptx::tmem_alloc(sbase + SmemLayout::TMEMPTR, 512);
+  if (warp == 2) {
+    if (Geo<ROWS>::kPair) ptx::tmem_alloc_2cta(sbase + SmemLayout::TMEMPTR, 512);
+    else ptx::tmem_alloc(sbase + SmemLayout::TMEMPTR, 512);
+  }
   if (P.bias16) {   // bf16 bias table, two per word
     uint32_t* b16 = reinterpret_cast<uint32_t*>(bias_s);
     for (int i = tid; i < (P.n_hidden * P.H) >> 1; i += kThreads) b16[i] = ptx::pack_bf16x2(P.bias[2 * i], P.bias[2 * i + 1]);
@@ -259,6 +271,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   ptx::tc_fence_before();
   __syncthreads();
   ptx::tc_fence_after();
+  if (Geo<ROWS>::kPair) ptx::cluster_sync_all();   // both CTAs' barriers initialised, both TMEM allocations made
   const uint32_t tmem_base = *tmem_ptr;
 
   int64_t n_evals = 1;
@@ -271,7 +284,14 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
 #if BEST_TC_SETMAXNREG
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kCtrlRegs));
 #endif
-    if (warp == 0) {
+    if (Geo<ROWS>::kPair) {
+      const uint32_t rank = ptx::cluster_ctarank();
+      if (warp == 0) {
+        producer_loop_pair(P, bars, sbase + SmemLayout::STAGES, rank, n_evals, n_ops);
+      } else if (warp == 1) {
+        if (rank == 0) mma_loop_pair<true>(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
+      }
+    } else if (warp == 0) {
       producer_loop(P, bars, sbase + SmemLayout::STAGES, n_evals, n_ops);
     } else if (warp == 1) {
       mma_loop<ROWS>(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
@@ -287,7 +307,9 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     C.P = &P;
     C.bars = bars;
     C.sbase = sbase;
-    C.row = (warp & 3) * 32 + lane;
+    C.row = Geo<ROWS>::kPair ? ((warp & 1) * 32 + lane) : ((warp & 3) * 32 + lane);
+    C.half = Geo<ROWS>::kPair ? ((warp & 3) >> 1) : 0;
+    C.to_leader = (Geo<ROWS>::kPair && ptx::cluster_ctarank() != 0) ? 1 : 0;
     C.k = (warp - kCtrlWarps) >> 2;
     C.tmem_lane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
     C.o = 0; C.g = 0; C.vslot = 0; C.pslot = 0;
@@ -306,11 +328,22 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     asm volatile("" : "+r"(C.a_thr0), "+r"(C.a_thr1), "+r"(C.bias_thr), "+r"(C.wouts_thr), "+r"(C.v_thr),
                       "+r"(C.tmem_lane), "+r"(C.sbase), "+l"(C.dact_thr));
 #endif
-    if (C.row < ROWS) sampler_thread<METHOD, ROWS>(C, R);   // lanes ROWS..127 are phantom rows
+    if (Geo<ROWS>::kPair && C.half == 1) {
+      // upper lane half of a CTA pair: MLP epilogues only, in step with the sampler threads
+      const float th0[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+      float gm[8], op_;
+      for (int64_t e = 0; e < n_evals; ++e) tc_eval<ROWS>(C, th0, R.want_grad != 0, op_, gm);
+    } else if (C.row < Geo<ROWS>::kTileRows) {
+      sampler_thread<METHOD, ROWS>(C, R);   // lanes kTileRows..127 are phantom rows
+    }
   }
   ptx::tc_fence_before();
   __syncthreads();
-  if (warp == 2) ptx::tmem_dealloc(tmem_base, 512);
+  if (Geo<ROWS>::kPair) ptx::cluster_sync_all();   // the leader's MMAs wrote the peer's TMEM and read its SMEM
+  if (warp == 2) {
+    if (Geo<ROWS>::kPair) ptx::tmem_dealloc_2cta(tmem_base, 512);
+    else ptx::tmem_dealloc(tmem_base, 512);
+  }
 }
 
 }  // namespace tc
@@ -327,6 +360,7 @@ struct TcPlan {
   uint8_t* aimg = nullptr;
   size_t dact_cap = 0, aimg_cap = 0;
   int n_sm = 0;
+  bool no_pair = false;  // BEST_TC_ROWS=64|32 forces the single-CTA L2-image geometries
   int force_rows = 0;   // BEST_TC_ROWS=128|64|32 (environment, read at best_create): measurements only
 };
 
@@ -361,9 +395,11 @@ uint16_t f32_to_bf16(float f) {  // round to nearest even
 template <int METHOD, int ROWS>
 int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
   TcPlan* pl = ctx->tc;
-  const int64_t n_tiles = (rows + ROWS - 1) / ROWS;
+  constexpr int kTileRows = tc::Geo<ROWS>::kTileRows;
+  int64_t n_tiles = (rows + kTileRows - 1) / kTileRows;
+  if (tc::Geo<ROWS>::kPair) n_tiles = (n_tiles + 1) & ~(int64_t)1;   // whole CTA pairs
   // scratch: act' blocks (forward -> backward) and, for ROWS < 128, the next-operand image
-  pl->P.dact_tile_elems = (size_t)(pl->P.n_hidden - 1) * pl->P.H * ROWS;
+  pl->P.dact_tile_elems = (size_t)(pl->P.n_hidden - 1) * pl->P.H * kTileRows;
   const size_t dact_bytes = sizeof(uint16_t) * pl->P.dact_tile_elems * (size_t)n_tiles + 16;
   const size_t aimg_bytes = tc::Geo<ROWS>::kInPlace ? 16 : (size_t)16 * tc::Geo<ROWS>::kAChunk * (size_t)n_tiles;
   if (dact_bytes > pl->dact_cap || aimg_bytes > pl->aimg_cap) {
@@ -390,7 +426,20 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
     attr_set = true;
   }
   pl->P.L = ctx->L_dev;
-  tc::best_tc_kernel<METHOD, ROWS><<<(unsigned)n_tiles, tc::kThreads, smem_bytes, s>>>(pl->P, R);
+  if (tc::Geo<ROWS>::kPair) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)n_tiles);
+    cfg.blockDim = dim3(tc::kThreads);
+    cfg.dynamicSmemBytes = (size_t)smem_bytes;
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    BEST_CUDA(cudaLaunchKernelEx(&cfg, tc::best_tc_kernel<METHOD, ROWS>, pl->P, R));
+  } else {
+    tc::best_tc_kernel<METHOD, ROWS><<<(unsigned)n_tiles, tc::kThreads, smem_bytes, s>>>(pl->P, R);
+  }
   count_launch();
   BEST_CUDA(cudaGetLastError());
   return BEST_OK;
@@ -403,6 +452,7 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
 int pick_rows(const TcPlan* pl, int64_t rows, int n_sm) {
   if (pl->force_rows) return pl->force_rows;
   if (pl->P.H != 1024) return 128;
+  if (!pl->no_pair) return 264;   // CTA pairs (cta_group::2): the 1024-wide operand in place at full MMA rate
   return (rows + 63) / 64 >= n_sm ? 64 : ((rows + 31) / 32 > (rows + 63) / 64 && rows <= 32 * (int64_t)n_sm ? 32 : 64);
 }
 
@@ -416,12 +466,36 @@ int launch_tc(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
   }
   switch (pick_rows(pl, rows, pl->n_sm)) {
     case 128: return launch_tc_geo<METHOD, 128>(ctx, R, rows, s);
+    case 264: return launch_tc_geo<METHOD, 264>(ctx, R, rows, s);
     case 64: return launch_tc_geo<METHOD, 64>(ctx, R, rows, s);
     default: return launch_tc_geo<METHOD, 32>(ctx, R, rows, s);
   }
 }
 
 }  // namespace
+
+// the weight pack as a 2-D byte tensor for the CTA-pair kernel's 2-SM tensor copies
+static int make_wmap(CUtensorMap* m, void* base, size_t bytes, uint32_t box_rows) {
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_fn enc = nullptr;
+  if (!enc) {
+    void* fp = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    BEST_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qr));
+    if (!fp || qr != cudaDriverEntryPointSuccess) { set_error("cuTensorMapEncodeTiled not available"); return BEST_ERR_CUDA; }
+    enc = (encode_fn)fp;
+  }
+  const cuuint64_t dims[2] = {256, (cuuint64_t)(bytes / 256)};   // box dimensions are limited to 256 elements
+  const cuuint64_t strides[1] = {256};
+  const cuuint32_t box[2] = {256, box_rows};
+  const cuuint32_t es[2] = {1, 1};
+  const CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed"); return BEST_ERR_CUDA; }
+  return BEST_OK;
+}
 
 int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   const int K = cfg->n_affine - 1;  // hidden layers
@@ -440,7 +514,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   ctx->tc = pl;
   if (const char* e = std::getenv("BEST_TC_ROWS")) {
     const int v = std::atoi(e);
-    if ((v == 64 || v == 32 || (v == 128 && !r64))) pl->force_rows = v;
+    if ((v == 64 || v == 32 || (v == 128 && !r64) || (v == 264 && r64))) pl->force_rows = v;
   }
   tc::Params& P = pl->P;
   P.bias16 = r64 ? 1 : 0;
@@ -502,6 +576,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   }
   P.b_out = bvec[K][0];
   int rc;
+  pack.resize((pack.size() + 8191) / 8192 * 8192 + 8192, 0);   // whole 1 KB rows (+ slack) for the tensor maps
   if ((rc = dev_alloc(&pl->wpack, pack.size() * 2))) return rc;
   if ((rc = dev_alloc(&pl->bias, bias.size()))) return rc;
   if ((rc = dev_alloc(&pl->w_out, (size_t)H))) return rc;
@@ -509,6 +584,10 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   BEST_CUDA(cudaMemcpy(pl->bias, bias.data(), bias.size() * 4, cudaMemcpyHostToDevice));
   BEST_CUDA(cudaMemcpy(pl->w_out, W[K], sizeof(float) * H, cudaMemcpyHostToDevice));
   P.wpack = pl->wpack; P.bias = pl->bias; P.w_out = pl->w_out;
+  if (r64) {
+    if ((rc = make_wmap(&P.wmap8, pl->wpack, pack.size() * 2, 32))) return rc;
+    if ((rc = make_wmap(&P.wmap1, pl->wpack, pack.size() * 2, 4))) return rc;
+  }
   P.has_gauss = ctx->tgt.has_gauss; P.has_box = ctx->tgt.has_box;
   P.banana_i = ctx->tgt.banana_i; P.banana_j = ctx->tgt.banana_j;
   P.banana_sigma = (float)ctx->tgt.banana_sigma;
