@@ -23,6 +23,7 @@ struct EpiCtx {
   uint32_t tmem_lane;   // tmem base + (lane quarter << 16)
   int row;              // 0..127
   int k;                // 0..3
+  uint32_t a_wr;        // ping-pong geometry: byte offset of the operand buffer this op's epilogue writes
   int to_leader;        // CTA pair, rank 1: a_ready / d_free arrivals go to the leader CTA's barriers
   int half;             // CTA pair: 0 = lanes 0..63 (lower N half, runs the sampler), 1 = lanes 64..127
   uint32_t o, g;        // op / n-chunk counters (mirror the MMA issuer)
@@ -67,8 +68,9 @@ __device__ __forceinline__ void load_bias(const EpiCtx& C, int layer, int jn, f3
 template <int ROWS>
 __device__ __forceinline__ void store_a(const EpiCtx& C, int jn, const uint32_t (&hp)[8]) {
   if (Geo<ROWS>::kInPlace) {
-    ptx::sts_128(C.a_thr0 + jn * Geo<ROWS>::kAChunk, hp[0], hp[1], hp[2], hp[3]);
-    ptx::sts_128(C.a_thr1 + jn * Geo<ROWS>::kAChunk, hp[4], hp[5], hp[6], hp[7]);
+    const uint32_t off = jn * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? C.a_wr : 0u);
+    ptx::sts_128(C.a_thr0 + off, hp[0], hp[1], hp[2], hp[3]);
+    ptx::sts_128(C.a_thr1 + off, hp[4], hp[5], hp[6], hp[7]);
   } else {
     uint8_t* p0 = C.aimg_thr + (size_t)jn * Geo<ROWS>::kAChunk;
     uint8_t* p1 = reinterpret_cast<uint8_t*>(reinterpret_cast<uintptr_t>(p0) ^ (uintptr_t)16);
@@ -256,7 +258,7 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
-    const bool gate = Geo<ROWS>::kInPlace && writes_a && (c != op.nch - 1);
+    const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && writes_a && (c != op.nch - 1);
     for (int grp = 0; grp < ngrp; ++grp) {
       const int jn = Geo<ROWS>::kPair ? c * (op.ncols >> 6) + C.half * ngrp + grp : c * ngrp + grp;
       uint32_t v[16], hp[8];
@@ -302,7 +304,7 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
   const uint8_t* dact_l = C.dact_thr + (size_t)(op.layer * (C.P->H >> 6)) * kDBlk;
   for (int c = 0; c < op.nch; ++c, ++C.g) {
     const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
-    const bool gate = Geo<ROWS>::kInPlace && (c != op.nch - 1);
+    const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && (c != op.nch - 1);
     // act' of the first group can be fetched before the accumulator is complete
     const int jn0 = Geo<ROWS>::kPair ? c * (op.ncols >> 6) + C.half * ngrp : c * ngrp;
     const uint8_t* dp = dact_l + (size_t)jn0 * kDBlk;
@@ -350,6 +352,7 @@ __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool wa
   for (int oi = 0; oi < n_ops; ++oi, ++C.o) {
     const OpDesc op = P.ops[oi];
     int written = 0;
+    C.a_wr = (uint32_t)((oi + 1) & 1) * 65536u;   // (ping-pong) the buffer the NEXT op reads
     if (op.epi == EPI_FWD_HID) {
       if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, false, ROWS>(C, op, want_grad, acc2, written);
       else epi_fwd<BEST_ACT_TANH, false, ROWS>(C, op, want_grad, acc2, written);

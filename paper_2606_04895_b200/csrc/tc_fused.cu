@@ -45,9 +45,15 @@ constexpr int kRows = 128;           // TMEM lanes == MMA M
 //                CTA (lanes 64..127 hold the upper half of N for the same 64 rows), so a whole
 //                1024-wide layer of accumulators fits TMEM and the operand is rewritten in place.
 template <int ROWS> struct Geo {
-  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32 || ROWS == 264, "tile geometry");
-  static constexpr bool kPair = (ROWS == 264);
-  static constexpr bool kInPlace = (ROWS == 128 || ROWS == 264);
+  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32 || ROWS == 264 || ROWS == 265, "tile geometry");
+  static constexpr bool kPair = (ROWS == 264 || ROWS == 265);
+  // ROWS = 265: CTA pair for 512-wide layers.  64 chains per CTA need only 64 KB of operand and 256
+  // TMEM columns per layer, so BOTH are double-buffered: an op reads operand buffer (op & 1) and its
+  // epilogue writes the other one, accumulators alternate between two sets of TMEM columns.  No
+  // in-place hazard is left: the next op's MMAs start on the first finished k-chunk while this op's
+  // epilogue is still running.
+  static constexpr bool kPingPong = (ROWS == 265);
+  static constexpr bool kInPlace = (ROWS == 128 || ROWS == 264 || ROWS == 265);   // operand stays in SMEM
   static constexpr int kTileRows = kPair ? 64 : ROWS;
   static constexpr int kAChunk = kTileRows * 128;      // bytes of one 64-column k-chunk
   static constexpr int kEpiActive = kPair ? 512 : ROWS * 4;   // epilogue threads with MLP epilogue work
@@ -320,7 +326,7 @@ __device__ void loader_loop(const Params& P, const Bars& bars, uint32_t a_base, 
 // ------------------------------------------------------------------------------------------------
 __device__ void producer_loop_pair(const Params& P, const Bars& bars, uint32_t stage_base, uint32_t rank,
                                    int64_t n_evals, int n_ops) {
-  constexpr uint32_t NS = Geo<264>::kStagesG, SB = Geo<264>::kStageBytesG;
+  constexpr uint32_t NS = 4, SB = 16384;
   uint32_t t = 0;   // stage counter: one stage = one 64-wide k-chunk = two K32 tiles (this CTA's halves)
   for (int64_t e = 0; e < n_evals; ++e) {
     uint32_t src = 0;   // byte offset inside the pack
@@ -345,10 +351,10 @@ __device__ void producer_loop_pair(const Params& P, const Bars& bars, uint32_t s
   }
 }
 
-template <bool LEADER>
+template <bool LEADER, int ROWS>
 __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base, uint32_t stage_base,
                               uint32_t tmem_base, int64_t n_evals, int n_ops) {
-  constexpr uint32_t NS = Geo<264>::kStagesG, SB = Geo<264>::kStageBytesG, NB = Geo<264>::kNBuf;
+  constexpr uint32_t NS = Geo<ROWS>::kStagesG, SB = Geo<ROWS>::kStageBytesG, NB = Geo<ROWS>::kNBuf;
   uint32_t t = 0, g = 0, o = 0;
   const uint64_t adesc0 = ptx::smem_desc_sw128(a_base);
   const uint64_t bdesc0 = ptx::smem_desc_sw64(stage_base);
@@ -368,7 +374,7 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
           ptx::mbar_wait(bars.d_free(buf), (use & 1u) ^ 1u);   // both CTAs' epilogue threads arrive here
           ptx::tc_fence_after();
         }
-        const uint32_t d_tmem = tmem_base + buf * Geo<264>::kBufCols;
+        const uint32_t d_tmem = tmem_base + buf * Geo<ROWS>::kBufCols;
         const bool last_c = (c == op.nch - 1);
         for (int j = 0; j < op.kch; ++j, ++t) {
           if (LEADER) {
@@ -376,7 +382,7 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
             const uint32_t s = t % NS, use_s = t / NS;
             ptx::mbar_wait(bars.full(s), use_s & 1u);   // both CTAs' halves of both K32 tiles
             ptx::tc_fence_after();
-            const uint64_t ad = adesc0 + (uint64_t)((j * Geo<264>::kAChunk) >> 4);
+            const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? (oi & 1) * 65536 : 0)) >> 4);
             const uint64_t bd = bdesc0 + (uint64_t)((s * SB) >> 4);
             if (elect_one()) {
               ptx::mma_bf16_ss_2cta(d_tmem, ad, bd, idesc, j != 0 ? 1u : 0u);

@@ -289,7 +289,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
       if (warp == 0) {
         producer_loop_pair(P, bars, sbase + SmemLayout::STAGES, rank, n_evals, n_ops);
       } else if (warp == 1) {
-        if (rank == 0) mma_loop_pair<true>(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
+        if (rank == 0) mma_loop_pair<true, ROWS>(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
       }
     } else if (warp == 0) {
       producer_loop(P, bars, sbase + SmemLayout::STAGES, n_evals, n_ops);
@@ -451,6 +451,14 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
 // 1024-wide layers (whose operand does not fit in place) use 64, or 32 when that fills more SMs.
 int pick_rows(const TcPlan* pl, int64_t rows, int n_sm) {
   if (pl->force_rows) return pl->force_rows;
+  if (pl->P.H == 512 && !pl->no_pair) {
+    // 512-wide: 128-chain single-CTA tiles or 64-chain CTA pairs (operand + accumulators double-buffered).
+    // Measured per evaluation of one tile (HMC, B200): 52 us against 33 us, so the pairs win whenever
+    // they do not need more waves of CTAs: the 4096-chain config, the small points of the sweep.
+    const int64_t t128 = (rows + 127) / 128, t64 = ((rows + 63) / 64 + 1) & ~(int64_t)1;
+    const double c128 = (double)((t128 + n_sm - 1) / n_sm) * 52.0, c265 = (double)((t64 + n_sm - 1) / n_sm) * 33.0;
+    return c265 < c128 ? 265 : 128;
+  }
   if (pl->P.H != 1024) return 128;
   if (!pl->no_pair) return 264;   // CTA pairs (cta_group::2): the 1024-wide operand in place at full MMA rate
   return (rows + 63) / 64 >= n_sm ? 64 : ((rows + 31) / 32 > (rows + 63) / 64 && rows <= 32 * (int64_t)n_sm ? 32 : 64);
@@ -467,6 +475,7 @@ int launch_tc(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
   switch (pick_rows(pl, rows, pl->n_sm)) {
     case 128: return launch_tc_geo<METHOD, 128>(ctx, R, rows, s);
     case 264: return launch_tc_geo<METHOD, 264>(ctx, R, rows, s);
+    case 265: return launch_tc_geo<METHOD, 265>(ctx, R, rows, s);
     case 64: return launch_tc_geo<METHOD, 64>(ctx, R, rows, s);
     default: return launch_tc_geo<METHOD, 32>(ctx, R, rows, s);
   }
@@ -514,7 +523,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   ctx->tc = pl;
   if (const char* e = std::getenv("BEST_TC_ROWS")) {
     const int v = std::atoi(e);
-    if ((v == 64 || v == 32 || (v == 128 && !r64) || (v == 264 && r64))) pl->force_rows = v;
+    if ((v == 64 || v == 32 || (v == 128 && !r64) || (v == 264 && r64) || (v == 265 && H == 512))) pl->force_rows = v;
   }
   tc::Params& P = pl->P;
   P.bias16 = r64 ? 1 : 0;
@@ -584,7 +593,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   BEST_CUDA(cudaMemcpy(pl->bias, bias.data(), bias.size() * 4, cudaMemcpyHostToDevice));
   BEST_CUDA(cudaMemcpy(pl->w_out, W[K], sizeof(float) * H, cudaMemcpyHostToDevice));
   P.wpack = pl->wpack; P.bias = pl->bias; P.w_out = pl->w_out;
-  if (r64) {
+  if (r64 || H == 512) {
     if ((rc = make_wmap(&P.wmap8, pl->wpack, pack.size() * 2, 32))) return rc;
     if ((rc = make_wmap(&P.wmap1, pl->wpack, pack.size() * 2, 4))) return rc;
   }
