@@ -108,6 +108,7 @@ struct OpDesc {
   int ncols;  // columns per n-chunk (MMA N)
   int epi;
   int layer;  // FWD: hidden layer index (0-based) whose bias/act is applied; BWD_HID: layer whose act' multiplies
+  int paired; // CTA-pair kernel, 1024-wide: N-chunks are issued two at a time, k-chunk outer (see mma_loop_pair)
 };
 
 struct Params {
@@ -367,6 +368,44 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
         if (elect_one())
           for (int j = op.kch; j < P.kch_max; ++j) ptx::mma_commit_2cta(bars.a_free(j));
         __syncwarp();
+      }
+      if (op.paired) {
+        // Two N-chunks at a time, k-chunk outer: a_free(j) of the LAST pass then fires while that pass is
+        // still running (k-chunk by k-chunk) and the first pass's epilogue overlaps it, instead of every
+        // epilogue store waiting for the last N-chunk's sweep over K.
+        for (int c = 0; c < op.nch; c += 2, g += 2) {
+          const uint32_t b0 = g % NB, b1 = (g + 1) % NB, u0 = g / NB, u1 = (g + 1) / NB;
+          const bool last_p = (c + 2 >= op.nch);
+          if (LEADER) {
+            ptx::mbar_wait(bars.d_free(b0), (u0 & 1u) ^ 1u);
+            ptx::mbar_wait(bars.d_free(b1), (u1 & 1u) ^ 1u);
+            ptx::tc_fence_after();
+            for (int j = 0; j < op.kch; ++j) {
+              if (c == 0) ptx::mbar_wait(bars.a_ready(j), o & 1u);
+              const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk) >> 4);
+#pragma unroll
+              for (int q = 0; q < 2; ++q, ++t) {
+                const uint32_t s = t % NS, use_s = t / NS;
+                ptx::mbar_wait(bars.full(s), use_s & 1u);
+                ptx::tc_fence_after();
+                const uint64_t bd = bdesc0 + (uint64_t)((s * SB) >> 4);
+                const uint32_t d_tmem = tmem_base + (q ? b1 : b0) * Geo<ROWS>::kBufCols;
+                if (elect_one()) {
+                  ptx::mma_bf16_ss_2cta(d_tmem, ad, bd, idesc, j != 0 ? 1u : 0u);
+                  ptx::mma_bf16_ss_2cta(d_tmem, ad + 2, bd + 2, idesc, 1u);
+                  ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
+                  ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
+                  ptx::mma_commit_2cta(bars.empty(s));
+                  if (last_p && q == 1) ptx::mma_commit_2cta(bars.a_free(j));
+                }
+                __syncwarp();
+              }
+            }
+            if (elect_one()) { ptx::mma_commit_2cta(bars.d_full(b0)); ptx::mma_commit_2cta(bars.d_full(b1)); }
+            __syncwarp();
+          }
+        }
+        continue;
       }
       for (int c = 0; c < op.nch; ++c, ++g) {
         const uint32_t buf = g % NB, use = g / NB;

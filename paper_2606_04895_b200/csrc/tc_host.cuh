@@ -530,12 +530,14 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   P.kch_max = H / 64;
   P.d = d; P.H = H; P.n_hidden = K; P.act = cfg->activation; P.mlp_scale = cfg->mlp_scale;
   const int ncols = H < 256 ? H : 256, nch = H / ncols, kchH = H / 64;
+  // 1024-wide layers on the CTA-pair kernel: N-chunks issued two at a time (not for the forced fallbacks)
+  const int paired = (r64 && pl->force_rows != 64 && pl->force_rows != 32) ? 1 : 0;
   int no = 0;
   for (int l = 0; l < K; ++l)
-    P.ops[no++] = tc::OpDesc{l == 0 ? 1 : kchH, nch, ncols, l == K - 1 ? tc::EPI_FWD_LAST : tc::EPI_FWD_HID, l};
+    P.ops[no++] = tc::OpDesc{l == 0 ? 1 : kchH, nch, ncols, l == K - 1 ? tc::EPI_FWD_LAST : tc::EPI_FWD_HID, l, paired};
   P.n_ops_fwd = no;
-  for (int l = K - 1; l >= 1; --l) P.ops[no++] = tc::OpDesc{kchH, nch, ncols, tc::EPI_BWD_HID, l - 1};
-  P.ops[no++] = tc::OpDesc{kchH, 1, 32, tc::EPI_BWD_FINAL, 0};
+  for (int l = K - 1; l >= 1; --l) P.ops[no++] = tc::OpDesc{kchH, nch, ncols, tc::EPI_BWD_HID, l - 1, paired};
+  P.ops[no++] = tc::OpDesc{kchH, 1, 32, tc::EPI_BWD_FINAL, 0, 0};
   P.n_ops_all = no;
   P.dact_tile_elems = 0;   // set per launch (depends on the tile geometry)
 
@@ -565,8 +567,20 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
       if (op.epi == tc::EPI_BWD_HID) return W[op.layer + 1][(size_t)k * H + n];  // (W_l)^T, l = layer+1
       return n < d ? W[0][(size_t)k * d + n] : 0.0f;                             // (W_0)^T
     };
-    for (int c = 0; c < op.nch; ++c)
-      for (int k32 = 0; k32 < 2 * op.kch; ++k32) {
+    // consumption order of the K32 tiles: N-chunk outer, or (paired ops) two N-chunks at a time with the
+    // 64-wide k-chunk outer
+    std::vector<std::pair<int, int>> order;   // (c, k32)
+    if (op.paired) {
+      for (int c = 0; c < op.nch; c += 2)
+        for (int j = 0; j < op.kch; ++j)
+          for (int q = 0; q < 2; ++q) { order.push_back({c + q, 2 * j}); order.push_back({c + q, 2 * j + 1}); }
+    } else {
+      for (int c = 0; c < op.nch; ++c)
+        for (int k32 = 0; k32 < 2 * op.kch; ++k32) order.push_back({c, k32});
+    }
+    for (const auto& ck : order) {
+      const int c = ck.first, k32 = ck.second;
+      {
         const size_t base = pack.size();
         pack.resize(base + (size_t)op.ncols * 32, 0);
         for (int r = 0; r < op.ncols; ++r)
@@ -576,6 +590,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
             pack[base + off] = BEST_TC_ACT_F16 ? f32_to_f16(wv) : f32_to_bf16(wv);
           }
       }
+    }
   }
   std::vector<float> bias((size_t)K * H);
   {
