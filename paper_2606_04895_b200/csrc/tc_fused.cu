@@ -352,9 +352,14 @@ __device__ void producer_loop_pair(const Params& P, const Bars& bars, uint32_t s
   }
 }
 
+// Two warps of the leader CTA issue (wq = 0: warp 1, wq = 1: warp 3).  A pair MMA is only 64 cycles of
+// tensor work but costs ~50 cycles to issue (+ the stage wait / commit), so ONE issuer was measured at
+// ~450 cycles per 16 KB stage against the 256 the tensor pipe needs; in the paired order the two
+// N-chunks of a pass have their own accumulators and their own (alternating) stages, so each warp
+// takes one of them.  Ops that are not paired are issued by warp 1 alone.  a_free counts 2 arrivals.
 template <bool LEADER, int ROWS>
 __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base, uint32_t stage_base,
-                              uint32_t tmem_base, int64_t n_evals, int n_ops) {
+                              uint32_t tmem_base, int64_t n_evals, int n_ops, int wq) {
   constexpr uint32_t NS = Geo<ROWS>::kStagesG, SB = Geo<ROWS>::kStageBytesG, NB = Geo<ROWS>::kNBuf;
   uint32_t t = 0, g = 0, o = 0;
   const uint64_t adesc0 = ptx::smem_desc_sw128(a_base);
@@ -364,9 +369,9 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
       const OpDesc op = P.ops[oi];
       const uint32_t idesc = ptx::idesc_bf16(kRows, op.ncols);
       const uint32_t half16 = ((uint32_t)op.ncols * 32u) >> 4;   // one K32 tile half, in descriptor units
-      if (LEADER) {
+      if (LEADER && wq == 0) {
         if (elect_one())
-          for (int j = op.kch; j < P.kch_max; ++j) ptx::mma_commit_2cta(bars.a_free(j));
+          for (int j = op.kch; j < P.kch_max; ++j) { ptx::mma_commit_2cta(bars.a_free(j)); ptx::mma_commit_2cta(bars.a_free(j)); }
         __syncwarp();
       }
       if (op.paired) {
@@ -377,36 +382,35 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
           const uint32_t b0 = g % NB, b1 = (g + 1) % NB, u0 = g / NB, u1 = (g + 1) / NB;
           const bool last_p = (c + 2 >= op.nch);
           if (LEADER) {
-            ptx::mbar_wait(bars.d_free(b0), (u0 & 1u) ^ 1u);
-            ptx::mbar_wait(bars.d_free(b1), (u1 & 1u) ^ 1u);
+            const uint32_t bq = wq ? b1 : b0, uq = wq ? u1 : u0;
+            ptx::mbar_wait(bars.d_free(bq), (uq & 1u) ^ 1u);
             ptx::tc_fence_after();
+            const uint32_t d_tmem = tmem_base + bq * Geo<ROWS>::kBufCols;
             for (int j = 0; j < op.kch; ++j) {
               if (c == 0) ptx::mbar_wait(bars.a_ready(j), o & 1u);
               const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk) >> 4);
-#pragma unroll
-              for (int q = 0; q < 2; ++q, ++t) {
-                const uint32_t s = t % NS, use_s = t / NS;
-                ptx::mbar_wait(bars.full(s), use_s & 1u);
-                ptx::tc_fence_after();
-                const uint64_t bd = bdesc0 + (uint64_t)((s * SB) >> 4);
-                const uint32_t d_tmem = tmem_base + (q ? b1 : b0) * Geo<ROWS>::kBufCols;
-                if (elect_one()) {
-                  ptx::mma_bf16_ss_2cta(d_tmem, ad, bd, idesc, j != 0 ? 1u : 0u);
-                  ptx::mma_bf16_ss_2cta(d_tmem, ad + 2, bd + 2, idesc, 1u);
-                  ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
-                  ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
-                  ptx::mma_commit_2cta(bars.empty(s));
-                  if (last_p && q == 1) ptx::mma_commit_2cta(bars.a_free(j));
-                }
-                __syncwarp();
+              const uint32_t tt = t + 2u * (uint32_t)j + (uint32_t)wq, s = tt % NS, use_s = tt / NS;
+              ptx::mbar_wait(bars.full(s), use_s & 1u);
+              ptx::tc_fence_after();
+              const uint64_t bd = bdesc0 + (uint64_t)((s * SB) >> 4);
+              if (elect_one()) {
+                ptx::mma_bf16_ss_2cta(d_tmem, ad, bd, idesc, j != 0 ? 1u : 0u);
+                ptx::mma_bf16_ss_2cta(d_tmem, ad + 2, bd + 2, idesc, 1u);
+                ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
+                ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
+                ptx::mma_commit_2cta(bars.empty(s));
+                if (last_p) ptx::mma_commit_2cta(bars.a_free(j));   // one arrival per issuing warp
               }
+              __syncwarp();
             }
-            if (elect_one()) { ptx::mma_commit_2cta(bars.d_full(b0)); ptx::mma_commit_2cta(bars.d_full(b1)); }
+            if (elect_one()) ptx::mma_commit_2cta(bars.d_full(bq));
             __syncwarp();
           }
+          t += 2u * (uint32_t)op.kch;
         }
         continue;
       }
+      if (wq != 0) { t += (uint32_t)(op.nch * op.kch); g += (uint32_t)op.nch; continue; }
       for (int c = 0; c < op.nch; ++c, ++g) {
         const uint32_t buf = g % NB, use = g / NB;
         if (LEADER) {
@@ -429,7 +433,7 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
               ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
               ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
               ptx::mma_commit_2cta(bars.empty(s));
-              if (last_c) ptx::mma_commit_2cta(bars.a_free(j));
+              if (last_c) { ptx::mma_commit_2cta(bars.a_free(j)); ptx::mma_commit_2cta(bars.a_free(j)); }
             }
             __syncwarp();
           }

@@ -229,7 +229,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
       // arrivals per phase: in place = every epilogue thread (pair: the 256 of the lane half that owns the
       // k-chunk); L2-image tiles = warp 3 alone (+ the bulk copy's bytes)
       ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : kEpiThreads);   // pair: 256 of each CTA
-      ptx::mbar_init(bars.a_free(i), 1);
+      ptx::mbar_init(bars.a_free(i), Geo<ROWS>::kPair ? 2 : 1);   // pair kernels: two issuing warps
       ptx::mbar_init(bars.a_ready_peer(i), 1);
     }
     for (int i = 0; i < 4; ++i) {
@@ -288,8 +288,9 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
       const uint32_t rank = ptx::cluster_ctarank();
       if (warp == 0) {
         producer_loop_pair(P, bars, sbase + SmemLayout::STAGES, rank, n_evals, n_ops);
-      } else if (warp == 1) {
-        if (rank == 0) mma_loop_pair<true, ROWS>(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops);
+      } else if ((warp == 1 || warp == 3) && rank == 0) {
+        mma_loop_pair<true, ROWS>(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops,
+                                  warp == 3 ? 1 : 0);
       }
     } else if (warp == 0) {
       producer_loop(P, bars, sbase + SmemLayout::STAGES, n_evals, n_ops);
