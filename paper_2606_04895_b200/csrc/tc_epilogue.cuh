@@ -129,7 +129,7 @@ __device__ __forceinline__ void tanh_pair(f32x2 a, f32x2& h, f32x2& dact) {
 template <int ROWS>
 __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   if (Geo<ROWS>::kPair && C.half != 0) return;   // the upper lane half only takes part in the MLP epilogues
-  ptx::mbar_wait(C.bars.a_free(0), (C.o & 1u) ^ 1u);
+  if (!Geo<ROWS>::kPingPong) ptx::mbar_wait(C.bars.a_free(0), (C.o & 1u) ^ 1u);
   uint32_t hi[4], lo[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
@@ -244,6 +244,14 @@ __device__ __forceinline__ void publish_a(EpiCtx& C, int jn0, int n) {
   }
 }
 
+// CTA pair: the 64-column block of the layer that lane half `half` finds in its group `grp` of N-chunk c.
+// The hardware puts N columns [128 half, +128) of the chunk in that half's lanes; paired ops are packed
+// with the chunk's four 64-row blocks of B in the order 0,2,1,3, so that one round of the epilogue (both
+// halves, same grp) completes two CONSECUTIVE k-chunks of the next operand.
+__device__ __forceinline__ int pair_jn(const OpDesc& op, int c, int half, int grp, int ngrp) {
+  return op.paired ? c * (op.ncols >> 6) + grp * 2 + half : c * (op.ncols >> 6) + half * ngrp + grp;
+}
+
 // forward epilogue of one op
 template <int ACT, bool LAST, int ROWS>
 __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_grad, f32x2& acc2,
@@ -260,7 +268,7 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
     const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && writes_a && (c != op.nch - 1);
     for (int grp = 0; grp < ngrp; ++grp) {
-      const int jn = Geo<ROWS>::kPair ? c * (op.ncols >> 6) + C.half * ngrp + grp : c * ngrp + grp;
+      const int jn = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, grp, ngrp) : c * ngrp + grp;
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
       ptx::tmem_ld_wait();
@@ -306,19 +314,20 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
     const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
     const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && (c != op.nch - 1);
     // act' of the first group can be fetched before the accumulator is complete
-    const int jn0 = Geo<ROWS>::kPair ? c * (op.ncols >> 6) + C.half * ngrp : c * ngrp;
+    const int jn0 = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, 0, ngrp) : c * ngrp;
+    const int jstep = (Geo<ROWS>::kPair && op.paired) ? 2 : 1;
     const uint8_t* dp = dact_l + (size_t)jn0 * kDBlk;
     uint4 a0 = ptx::ldg_128(dp), a1 = ptx::ldg_128(dp + kDPiece);
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
     for (int grp = 0; grp < ngrp; ++grp) {
-      const int jn = Geo<ROWS>::kPair ? c * (op.ncols >> 6) + C.half * ngrp + grp : c * ngrp + grp;
+      const int jn = jn0 + grp * jstep;
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
       const uint4 d0 = a0, d1 = a1;
       if (grp + 1 < ngrp) {   // prefetch the next group's act'
-        const uint8_t* dn = dact_l + (size_t)(jn + 1) * kDBlk;
+        const uint8_t* dn = dact_l + (size_t)(jn + jstep) * kDBlk;
         a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
       }
       ptx::tmem_ld_wait();

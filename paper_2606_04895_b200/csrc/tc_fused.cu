@@ -369,7 +369,7 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
       const OpDesc op = P.ops[oi];
       const uint32_t idesc = ptx::idesc_bf16(kRows, op.ncols);
       const uint32_t half16 = ((uint32_t)op.ncols * 32u) >> 4;   // one K32 tile half, in descriptor units
-      if (LEADER && wq == 0) {
+      if (LEADER && wq == 0 && !Geo<ROWS>::kPingPong) {   // (ping-pong: nothing is overwritten in place, a_free unused)
         if (elect_one())
           for (int j = op.kch; j < P.kch_max; ++j) { ptx::mma_commit_2cta(bars.a_free(j)); ptx::mma_commit_2cta(bars.a_free(j)); }
         __syncwarp();
@@ -388,7 +388,7 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
             const uint32_t d_tmem = tmem_base + bq * Geo<ROWS>::kBufCols;
             for (int j = 0; j < op.kch; ++j) {
               if (c == 0) ptx::mbar_wait(bars.a_ready(j), o & 1u);
-              const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk) >> 4);
+              const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? (oi & 1) * 65536 : 0)) >> 4);
               const uint32_t tt = t + 2u * (uint32_t)j + (uint32_t)wq, s = tt % NS, use_s = tt / NS;
               ptx::mbar_wait(bars.full(s), use_s & 1u);
               ptx::tc_fence_after();
@@ -399,7 +399,7 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
                 ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
                 ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
                 ptx::mma_commit_2cta(bars.empty(s));
-                if (last_p) ptx::mma_commit_2cta(bars.a_free(j));   // one arrival per issuing warp
+                if (last_p && !Geo<ROWS>::kPingPong) ptx::mma_commit_2cta(bars.a_free(j));   // one arrival per issuing warp
               }
               __syncwarp();
             }
@@ -410,7 +410,11 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
         }
         continue;
       }
-      if (wq != 0) { t += (uint32_t)(op.nch * op.kch); g += (uint32_t)op.nch; continue; }
+      if (wq != 0) {   // not this warp's op: only keep in step with the operand barrier's phases
+        if (LEADER) ptx::mbar_wait(bars.a_ready(0), o & 1u);
+        t += (uint32_t)(op.nch * op.kch); g += (uint32_t)op.nch;
+        continue;
+      }
       for (int c = 0; c < op.nch; ++c, ++g) {
         const uint32_t buf = g % NB, use = g / NB;
         if (LEADER) {
@@ -433,7 +437,7 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
               ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
               ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
               ptx::mma_commit_2cta(bars.empty(s));
-              if (last_c) { ptx::mma_commit_2cta(bars.a_free(j)); ptx::mma_commit_2cta(bars.a_free(j)); }
+              if (last_c && !Geo<ROWS>::kPingPong) { ptx::mma_commit_2cta(bars.a_free(j)); ptx::mma_commit_2cta(bars.a_free(j)); }
             }
             __syncwarp();
           }

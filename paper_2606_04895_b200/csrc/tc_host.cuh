@@ -354,7 +354,10 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
 // =================================================================================================
 struct TcPlan {
   tc::Params P{};
+  tc::Params Pp{};           // 512-wide ping-pong pairs (geometry 265): the same ops in the paired order, own weight pack
+  bool has_pp = false;
   uint8_t* wpack = nullptr;
+  uint8_t* wpack_p = nullptr;
   float* bias = nullptr;
   float* w_out = nullptr;
   uint16_t* dact = nullptr;
@@ -396,12 +399,13 @@ uint16_t f32_to_bf16(float f) {  // round to nearest even
 template <int METHOD, int ROWS>
 int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
   TcPlan* pl = ctx->tc;
+  tc::Params& P = (ROWS == 265 && pl->has_pp) ? pl->Pp : pl->P;
   constexpr int kTileRows = tc::Geo<ROWS>::kTileRows;
   int64_t n_tiles = (rows + kTileRows - 1) / kTileRows;
   if (tc::Geo<ROWS>::kPair) n_tiles = (n_tiles + 1) & ~(int64_t)1;   // whole CTA pairs
   // scratch: act' blocks (forward -> backward) and, for ROWS < 128, the next-operand image
-  pl->P.dact_tile_elems = (size_t)(pl->P.n_hidden - 1) * pl->P.H * kTileRows;
-  const size_t dact_bytes = sizeof(uint16_t) * pl->P.dact_tile_elems * (size_t)n_tiles + 16;
+  P.dact_tile_elems = (size_t)(P.n_hidden - 1) * P.H * kTileRows;
+  const size_t dact_bytes = sizeof(uint16_t) * P.dact_tile_elems * (size_t)n_tiles + 16;
   const size_t aimg_bytes = tc::Geo<ROWS>::kInPlace ? 16 : (size_t)16 * tc::Geo<ROWS>::kAChunk * (size_t)n_tiles;
   if (dact_bytes > pl->dact_cap || aimg_bytes > pl->aimg_cap) {
     BEST_CUDA(cudaStreamSynchronize(s));
@@ -418,15 +422,15 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
       pl->aimg_cap = aimg_bytes;
     }
   }
-  pl->P.dact = pl->dact;
-  pl->P.aimg = pl->aimg;
+  P.dact = pl->dact;
+  P.aimg = pl->aimg;
   static bool attr_set = false;
   const int smem_bytes = tc::SmemLayout::TOTAL + 1024;
   if (!attr_set) {
     BEST_CUDA(cudaFuncSetAttribute(tc::best_tc_kernel<METHOD, ROWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
     attr_set = true;
   }
-  pl->P.L = ctx->L_dev;
+  P.L = ctx->L_dev;
   if (tc::Geo<ROWS>::kPair) {
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)n_tiles);
@@ -437,9 +441,9 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    BEST_CUDA(cudaLaunchKernelEx(&cfg, tc::best_tc_kernel<METHOD, ROWS>, pl->P, R));
+    BEST_CUDA(cudaLaunchKernelEx(&cfg, tc::best_tc_kernel<METHOD, ROWS>, P, R));
   } else {
-    tc::best_tc_kernel<METHOD, ROWS><<<(unsigned)n_tiles, tc::kThreads, smem_bytes, s>>>(pl->P, R);
+    tc::best_tc_kernel<METHOD, ROWS><<<(unsigned)n_tiles, tc::kThreads, smem_bytes, s>>>(P, R);
   }
   count_launch();
   BEST_CUDA(cudaGetLastError());
@@ -555,9 +559,10 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
     }
   }
   // B operand of every op as a logical [N][Ktot] bf16 matrix, cut into pre-swizzled stage tiles
+  auto build_pack = [&](const tc::Params& PP) {
   std::vector<uint16_t> pack;
-  for (int oi = 0; oi < P.n_ops_all; ++oi) {
-    const tc::OpDesc op = P.ops[oi];
+  for (int oi = 0; oi < PP.n_ops_all; ++oi) {
+    const tc::OpDesc op = PP.ops[oi];
     // forward SiLU layers are packed pre-scaled by 1/2 (exact), see silu_pair()
     const float fs = (tc::kSiluHalfPrescale && cfg->activation == BEST_ACT_SILU) ? 0.5f : 1.0f;
     auto Bm = [&](int n, int k) -> float {
@@ -587,12 +592,18 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
         for (int r = 0; r < op.ncols; ++r)
           for (int kk = 0; kk < 32; ++kk) {
             const size_t off = (size_t)r * 32 + ((((kk >> 3) ^ ((r >> 1) & 3))) << 3) + (kk & 7);
-            const float wv = Bm(c * op.ncols + r, k32 * 32 + kk);
+            // paired ops (CTA-pair kernels): B row blocks in the order 0,2,1,3, see pair_jn()
+            const int rl = (op.paired && op.ncols == 256) ? ((((r >> 6) & 1) * 2 + (r >> 7)) << 6) + (r & 63) : r;
+            const float wv = Bm(c * op.ncols + rl, k32 * 32 + kk);
             pack[base + off] = BEST_TC_ACT_F16 ? f32_to_f16(wv) : f32_to_bf16(wv);
           }
       }
     }
   }
+  pack.resize((pack.size() + 8191) / 8192 * 8192 + 8192, 0);   // whole 1 KB rows (+ slack) for the tensor maps
+  return pack;
+  };
+  const std::vector<uint16_t> pack = build_pack(P);
   std::vector<float> bias((size_t)K * H);
   {
     const float fs = (tc::kSiluHalfPrescale && cfg->activation == BEST_ACT_SILU) ? 0.5f : 1.0f;
@@ -601,7 +612,6 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   }
   P.b_out = bvec[K][0];
   int rc;
-  pack.resize((pack.size() + 8191) / 8192 * 8192 + 8192, 0);   // whole 1 KB rows (+ slack) for the tensor maps
   if ((rc = dev_alloc(&pl->wpack, pack.size() * 2))) return rc;
   if ((rc = dev_alloc(&pl->bias, bias.size()))) return rc;
   if ((rc = dev_alloc(&pl->w_out, (size_t)H))) return rc;
@@ -618,13 +628,25 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   P.banana_sigma = (float)ctx->tgt.banana_sigma;
   P.pen_kappa = (float)ctx->tgt.pen_kappa; P.pen_gamma = (float)ctx->tgt.pen_gamma;
   P.mu = ctx->tgt.mu; P.R = ctx->tgt.R; P.lo = ctx->tgt.lo; P.hi = ctx->tgt.hi; P.L = ctx->L_dev;
+  if (H == 512 && !(std::getenv("BEST_TC_PP_NOUTER"))) {
+    // geometry 265 issues the two N-chunks of a layer from two warps (k-chunk outer): same ops, paired order
+    pl->Pp = P;
+    for (int oi = 0; oi + 1 < P.n_ops_all; ++oi) pl->Pp.ops[oi].paired = 1;
+    const std::vector<uint16_t> pack_p = build_pack(pl->Pp);
+    if ((rc = dev_alloc(&pl->wpack_p, pack_p.size() * 2))) return rc;
+    BEST_CUDA(cudaMemcpy(pl->wpack_p, pack_p.data(), pack_p.size() * 2, cudaMemcpyHostToDevice));
+    pl->Pp.wpack = pl->wpack_p;
+    if ((rc = make_wmap(&pl->Pp.wmap8, pl->wpack_p, pack_p.size() * 2, 32))) return rc;
+    if ((rc = make_wmap(&pl->Pp.wmap1, pl->wpack_p, pack_p.size() * 2, 4))) return rc;
+    pl->has_pp = true;
+  }
   return BEST_OK;
 }
 
 void tc_plan_destroy(best_ctx* ctx) {
   TcPlan* pl = ctx->tc;
   if (!pl) return;
-  cudaFree(pl->wpack); cudaFree(pl->bias); cudaFree(pl->w_out); cudaFree(pl->dact); cudaFree(pl->aimg);
+  cudaFree(pl->wpack); cudaFree(pl->wpack_p); cudaFree(pl->bias); cudaFree(pl->w_out); cudaFree(pl->dact); cudaFree(pl->aimg);
   delete pl;
   ctx->tc = nullptr;
 }
