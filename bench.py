@@ -23,10 +23,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/r1c_ncu_full.md, r1d_ncu_full.md); None where no capture exists.
-NCU_TRAFFIC_BYTES = {("lcdm_mala", 100, "bf16"): 5.249792e6 + 0.164608e6,      # r1d, best_tc_kernel<1,265>
+# `ncu --set full` captures (profiles/r1c_ncu_full.md, r1e_ncu_full.md); None where no capture exists.
+NCU_TRAFFIC_BYTES = {("lcdm_mala", 100, "bf16"): 5.255424e6 + 0.453888e6,      # r1e, best_tc_kernel<1,265>
                      ("hmc", 1, "bf16"): 10.798848e6 + 9.035520e6,           # r1c, best_tc_kernel<2,128>
-                     ("aies", 1, "bf16"): 14.429184e6 + 256.0}               # r1d, per half-ensemble launch
+                     ("aies", 1, "bf16"): 14.427904e6 + 0.0}                 # r1e, per half-ensemble launch
 
 WORKLOADS = {
     # name: (maker kwargs, method, sampler kwargs, inner steps per bench step, config index)
@@ -335,7 +335,7 @@ def main():
         "roofline": {"bound": "tensor" if args.precision == "bf16" else "alu", "achieved": achieved_tf,
                      "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
                      "traffic": NCU_TRAFFIC_BYTES.get((args.workload, inner, args.precision)) if spec["n_chains"] == WORKLOADS[args.workload]["n_chains"] else None,
-                     "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1d_ncu_full.md)",
+                     "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1e_ncu_full.md)",
                      "peak_source": peak_src,
                      "frac_of_sustained": (achieved_tf / peaks["bf16_tflops_sustained"]) if peaks and args.precision == "bf16" else None,
                      "kernel": "best_tc_kernel<%s>" % spec["method"], "flops_per_launch": flops_per_launch},
