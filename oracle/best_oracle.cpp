@@ -118,6 +118,10 @@ struct Oracle {
   int banana_i = -1, banana_j = -1;
   double banana_sigma = 0.1;
   std::vector<double> L;  // lower-triangular whitening factor, row-major d*d
+  // SURVEY 8(f)#1 (a larger step for some parameters): per-dimension step factors s_i
+  // in whitened space (reading R20) and the hard-box option (reading R21)
+  std::vector<double> step_scale;  // [d], all 1 by default
+  bool hard_box = false;
   // covariance adaptation (O6)
   int64_t adapt_every = 0;
   double jitter = 1e-6;
@@ -226,7 +230,10 @@ double target_eval(const Oracle& o, const double* theta, double* grad) {
       grad[o.banana_i] += 2.0 * ti * t / s2;
     }
   }
-  if (o.has_box) {  // A1e
+  if (o.has_box && o.hard_box) {  // reading R21: log pi = -inf outside [lo, hi] (no penalty term)
+    for (int i = 0; i < d; ++i)
+      if (theta[i] < o.lo[i] || theta[i] > o.hi[i]) logp = -INFINITY;
+  } else if (o.has_box) {  // A1e
     double pen = 0.0;
     for (int i = 0; i < d; ++i) {
       const double width = o.hi[i] - o.lo[i];
@@ -269,12 +276,15 @@ bool accept_rule(double u, double log_alpha) { return std::log(u) < log_alpha; }
 // random numbers and call these; the detailed-balance / closed-form pins call these directly.
 // ---------------------------------------------------------------------------------------------
 
+// Per-dimension steps (reading R20): coordinate i of the whitened space moves with eps_i = eps s_i in MH
+// and in the HMC leap-frog (drift and kick); MALA, the one-step limit, has drift eps s_i^2 g_i and noise
+// sqrt(2 eps) s_i xi_i, i.e. eq (2.3) with eps_i = eps s_i^2 and q(.|z) = N(z + E g_z, 2E), E = diag(eps_i).
 // O2 MH (reading R5): theta' = theta + eps L xi; log alpha = logpi' - logpi
 void mh_map(const Oracle& o, const double* theta, double logp, const double* xi, double eps,
             double* theta_p, double* logp_p, double* log_alpha) {
   const int d = o.d;
   std::vector<double> dz(d), dx(d);
-  for (int i = 0; i < d; ++i) dz[i] = eps * xi[i];
+  for (int i = 0; i < d; ++i) dz[i] = eps * o.step_scale[i] * xi[i];
   L_apply(o, dz.data(), dx.data());
   for (int i = 0; i < d; ++i) theta_p[i] = theta[i] + dx[i];
   *logp_p = target_eval(o, theta_p, nullptr);
@@ -292,20 +302,24 @@ void mala_map(const Oracle& o, const double* theta, double logp, const double* g
   const int d = o.d;
   std::vector<double> gz(d), dz(d), dx(d), gzp(d);
   Lt_apply(o, grad, gz.data());
-  const double sq = std::sqrt(2.0 * eps);
-  for (int i = 0; i < d; ++i) dz[i] = eps * gz[i] + sq * xi[i];
+  std::vector<double> ei(d), sq(d);
+  for (int i = 0; i < d; ++i) {
+    ei[i] = eps * o.step_scale[i] * o.step_scale[i];
+    sq[i] = std::sqrt(2.0 * ei[i]);
+  }
+  for (int i = 0; i < d; ++i) dz[i] = ei[i] * gz[i] + sq[i] * xi[i];
   L_apply(o, dz.data(), dx.data());
   for (int i = 0; i < d; ++i) theta_p[i] = theta[i] + dx[i];
   *logp_p = target_eval(o, theta_p, grad_p);
   Lt_apply(o, grad_p, gzp.data());
   double fwd = 0.0, bwd = 0.0;
   for (int i = 0; i < d; ++i) {
-    const double f = sq * xi[i];                          // z' - z - eps g_z
-    const double r = -(eps * (gz[i] + gzp[i]) + sq * xi[i]);  // z - z' - eps g_z'
-    fwd += f * f;
-    bwd += r * r;
+    const double f = sq[i] * xi[i];                              // z' - z - eps_i g_z
+    const double r = -(ei[i] * (gz[i] + gzp[i]) + sq[i] * xi[i]);  // z - z' - eps_i g_z'
+    fwd += f * f / (4.0 * ei[i]);
+    bwd += r * r / (4.0 * ei[i]);
   }
-  *log_alpha = *logp_p - logp + (-bwd / (4.0 * eps)) - (-fwd / (4.0 * eps));
+  *log_alpha = *logp_p - logp + (-bwd) - (-fwd);
 }
 
 // O4 HMC: Hamiltonian eq (2.1)/(2.8) P:L56, L96 with identity mass after whitening;
@@ -319,16 +333,17 @@ void hmc_map(const Oracle& o, const double* theta, double logp, const double* gr
   for (int i = 0; i < d; ++i) kin0 += q[i] * q[i];
   const double H0 = -logp + 0.5 * kin0;
   Lt_apply(o, g.data(), gz.data());
-  for (int i = 0; i < d; ++i) q[i] += 0.5 * eps * gz[i];  // half kick
+  const std::vector<double>& sc = o.step_scale;
+  for (int i = 0; i < d; ++i) q[i] += 0.5 * eps * sc[i] * gz[i];  // half kick
   double lp = logp;
   for (int l = 1; l <= n_leapfrog; ++l) {
-    for (int i = 0; i < d; ++i) dz[i] = eps * q[i];       // drift: z += eps q  <=>  theta += eps L q
+    for (int i = 0; i < d; ++i) dz[i] = eps * sc[i] * q[i];  // drift: z += eps q  <=>  theta += eps L q
     L_apply(o, dz.data(), dx.data());
     for (int i = 0; i < d; ++i) th[i] += dx[i];
     lp = target_eval(o, th.data(), g.data());
     Lt_apply(o, g.data(), gz.data());
     const double c = (l < n_leapfrog) ? eps : 0.5 * eps;  // full kick inside, half kick at the end
-    for (int i = 0; i < d; ++i) q[i] += c * gz[i];
+    for (int i = 0; i < d; ++i) q[i] += c * sc[i] * gz[i];
   }
   double kin1 = 0.0;
   for (int i = 0; i < d; ++i) kin1 += q[i] * q[i];
@@ -513,9 +528,16 @@ void* oracle_create(const oracle_config* c) {
   for (int i = 0; i < c->d; ++i)
     for (int j = 0; j <= i; ++j)
       o->L[(size_t)i * c->d + j] = c->L ? c->L[(size_t)i * c->d + j] : (i == j ? 1.0 : 0.0);
+  o->step_scale.assign((size_t)c->d, 1.0);
   cov_reset(*o);
   return o;
 }
+// readings R20 / R21
+void oracle_set_step_scale(void* h, const double* s) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  for (int i = 0; i < o.d; ++i) o.step_scale[i] = s ? s[i] : 1.0;
+}
+void oracle_set_hard_box(void* h, int32_t on) { static_cast<Oracle*>(h)->hard_box = (on != 0); }
 void oracle_destroy(void* h) { delete static_cast<Oracle*>(h); }
 
 void oracle_set_whitening(void* h, const double* L) {

@@ -54,6 +54,8 @@ def lib():
         L.oracle_get_whitening.argtypes = [vp, dp]
         L.oracle_log_det_L.restype = C.c_double
         L.oracle_log_det_L.argtypes = [vp]
+        L.oracle_set_step_scale.argtypes = [vp, dp]
+        L.oracle_set_hard_box.argtypes = [vp, i32]
         L.oracle_set_adaptation.argtypes = [vp, i64, C.c_double]
         L.oracle_adapt_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
         L.oracle_cov_chol.restype = i32
@@ -189,6 +191,13 @@ class Oracle:
 
     def log_det_L(self):
         return lib().oracle_log_det_L(self._h)
+
+    # ---- per-dimension step factors (R20), hard box (R21) -----------------------
+    def set_step_scale(self, s):
+        lib().oracle_set_step_scale(self._h, None if s is None else _dp(_f64(s)))
+
+    def set_hard_box(self, on: bool):
+        lib().oracle_set_hard_box(self._h, 1 if on else 0)
 
     def set_adaptation(self, adapt_every: int, jitter: float = 1e-6):
         lib().oracle_set_adaptation(self._h, adapt_every, jitter)
