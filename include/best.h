@@ -131,6 +131,23 @@ int best_adapt_stats(best_ctx* ctx, int64_t* n_updates, int64_t* n_failures);
 int best_get_whitening(best_ctx* ctx, double* L_host);
 int best_set_whitening(best_ctx* ctx, const double* L_host);
 
+/* per-dimension step sizes (sec. 5.2: "a step size 10 times larger for the
+ * extension parameters") and the hard-box prior option; readings R20, R21.
+ *
+ * best_set_step_scale: s_host [d] (host, copied; NULL = all ones), every s_i positive and finite else
+ * BEST_ERR_ARG.  Coordinate i of the whitened space then moves with eps_i = eps * s_i in MH and in the
+ * HMC leap-frog (drift and kick, i.e. a diagonal mass matrix diag(s)^-2); MALA, the one-step limit, uses
+ * eq (2.3) with eps_i = eps * s_i^2 (drift eps_i g_i, noise sqrt(2 eps_i)).  AIES does not whiten and is
+ * not affected.  The factors persist across best_set_whitening and covariance adaptation (A9), which
+ * keep updating the unscaled factor that best_get_whitening returns.  Synchronises the device.
+ *
+ * best_set_hard_box: on != 0 replaces the smooth penalty (A1e) by log pi = -inf outside [lo, hi] (the
+ * boundary belongs to the box), so such proposals are rejected (accept rule R7); gradients are those of
+ * the remaining terms.  BEST_ERR_ARG if the context was created without a box.  Cached log pi of
+ * existing states is not recomputed: call it before best_state_create (or best_state_set afterwards). */
+int best_set_step_scale(best_ctx* ctx, const double* s_host);
+int best_set_hard_box(best_ctx* ctx, int32_t on);
+
 /* Read the state back (all pointers host, each nullable): theta [B*d], logp [B], grad [B*d]
  * (float, original space), global step counter, per-chain accept counters [B], total emulator
  * evaluations.  Synchronises `stream`.                                                          */

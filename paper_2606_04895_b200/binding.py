@@ -23,7 +23,7 @@ EXPORTS = [
     "best_step_mh", "best_step_mala", "best_step_hmc", "best_step_aies", "best_set_adaptation",
     "best_adapt_stats", "best_get_whitening", "best_set_whitening", "best_state_get",
     "best_state_get_f64", "best_state_last_log_alpha", "best_state_set", "best_launch_count",
-    "best_last_error", "best_version",
+    "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box",
 ]
 
 
@@ -75,6 +75,8 @@ def lib():
     L.best_adapt_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     L.best_get_whitening.argtypes = [vp, vp]
     L.best_set_whitening.argtypes = [vp, vp]
+    L.best_set_step_scale.argtypes = [vp, vp]
+    L.best_set_hard_box.argtypes = [vp, i32]
     L.best_state_get.argtypes = [vp, vp, vp, vp, C.POINTER(u64), vp, C.POINTER(u64), vp]
     L.best_state_get_f64.argtypes = [vp, vp, vp, vp, vp]
     L.best_state_last_log_alpha.argtypes = [vp, vp, vp]
@@ -170,6 +172,18 @@ class Context:
     def set_whitening(self, L):
         L = np.ascontiguousarray(L, dtype=np.float64)
         _check(lib().best_set_whitening(self._h, L.ctypes.data))
+
+    def set_step_scale(self, s):
+        if s is None:
+            _check(lib().best_set_step_scale(self._h, None))
+            return
+        s = np.ascontiguousarray(s, dtype=np.float64)
+        if s.shape != (self.d,):
+            raise ValueError("step scale must have shape (d,)")
+        _check(lib().best_set_step_scale(self._h, s.ctypes.data))
+
+    def set_hard_box(self, on: bool):
+        _check(lib().best_set_hard_box(self._h, 1 if on else 0))
 
     def adapt_stats(self):
         a, b = C.c_int64(), C.c_int64()

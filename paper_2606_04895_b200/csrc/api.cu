@@ -128,6 +128,16 @@ int best_create(const best_config* cfg, best_ctx** out) {
     return fail(BEST_ERR_CUDA);
   }
   ctx->L_dev = ctx->dev_consts + 4 * d * d;
+  if ((rc = dev_alloc(&ctx->Lraw_dev, (size_t)d * d + d))) return fail(rc);
+  ctx->scale_dev = ctx->Lraw_dev + (size_t)d * d;
+  {
+    std::vector<double> ones((size_t)d, 1.0);
+    if (cudaMemcpy(ctx->Lraw_dev, ctx->L_dev, sizeof(double) * d * d, cudaMemcpyDeviceToDevice) != cudaSuccess ||
+        cudaMemcpy(ctx->scale_dev, ones.data(), sizeof(double) * d, cudaMemcpyHostToDevice) != cudaSuccess) {
+      set_error("best_create: upload failed");
+      return fail(BEST_ERR_CUDA);
+    }
+  }
   if ((rc = dev_alloc(&ctx->cov_ref, d))) return fail(rc);
   if ((rc = dev_alloc(&ctx->adapt_counts, 2))) return fail(rc);
   cudaMemset(ctx->adapt_counts, 0, sizeof(int64_t) * 2);
@@ -147,6 +157,7 @@ int best_create(const best_config* cfg, best_ctx** out) {
   T.banana_sigma = cfg->banana_sigma;
   T.mlp_scale = cfg->mlp_scale;
   T.has_mlp = (cfg->n_affine > 0 && cfg->mlp_scale != 0.0f) ? 1 : 0;
+  T.hard_box = 0;
 
   if (cfg->n_affine > 0) {
     ctx->widths.assign(cfg->widths, cfg->widths + cfg->n_affine + 1);
@@ -190,7 +201,7 @@ void best_destroy(best_ctx* ctx) {
   for (auto p : ctx->Dact) cudaFree(p);
   cudaFree(ctx->X0); cudaFree(ctx->delta[0]); cudaFree(ctx->delta[1]);
   cudaFree(ctx->mlp_out); cudaFree(ctx->mlp_grad);
-  cudaFree(ctx->dev_consts); cudaFree(ctx->cov_acc); cudaFree(ctx->cov_ref); cudaFree(ctx->adapt_counts);
+  cudaFree(ctx->dev_consts); cudaFree(ctx->cov_acc); cudaFree(ctx->cov_ref); cudaFree(ctx->adapt_counts); cudaFree(ctx->Lraw_dev);
   delete ctx;
 }
 

@@ -1,4 +1,5 @@
 // C-ABI entry points, part 2: best_logp_grad, chain state, sampler dispatch, whitening, adaptation.
+#include <cmath>
 #include <cstring>
 
 #include "best_internal.h"
@@ -276,7 +277,44 @@ int best_adapt_stats(best_ctx* ctx, int64_t* n_updates, int64_t* n_failures) {
 int best_get_whitening(best_ctx* ctx, double* L_host) {
   if (!ctx || !L_host) { set_error("best_get_whitening: bad argument"); return BEST_ERR_ARG; }
   BEST_CUDA(cudaDeviceSynchronize());
-  BEST_CUDA(cudaMemcpy(L_host, ctx->L_dev, sizeof(double) * ctx->d * ctx->d, cudaMemcpyDeviceToHost));
+  BEST_CUDA(cudaMemcpy(L_host, ctx->Lraw_dev, sizeof(double) * ctx->d * ctx->d, cudaMemcpyDeviceToHost));
+  return BEST_OK;
+}
+
+// L_dev = L_raw diag(s): the factor every step kernel applies (columns scaled, still lower triangular)
+static int refresh_scaled_whitening(best_ctx* ctx) {
+  const int d = ctx->d;
+  std::vector<double> L((size_t)d * d), s((size_t)d);
+  BEST_CUDA(cudaMemcpy(L.data(), ctx->Lraw_dev, sizeof(double) * d * d, cudaMemcpyDeviceToHost));
+  BEST_CUDA(cudaMemcpy(s.data(), ctx->scale_dev, sizeof(double) * d, cudaMemcpyDeviceToHost));
+  for (int i = 0; i < d; ++i)
+    for (int j = 0; j < d; ++j) L[(size_t)i * d + j] *= s[j];
+  BEST_CUDA(cudaMemcpy(ctx->L_dev, L.data(), sizeof(double) * d * d, cudaMemcpyHostToDevice));
+  return BEST_OK;
+}
+
+int best_set_step_scale(best_ctx* ctx, const double* s_host) {
+  if (!ctx) { set_error("best_set_step_scale: NULL ctx"); return BEST_ERR_ARG; }
+  const int d = ctx->d;
+  std::vector<double> s((size_t)d, 1.0);
+  if (s_host)
+    for (int i = 0; i < d; ++i) {
+      if (!(s_host[i] > 0.0) || !std::isfinite(s_host[i])) {
+        set_error("best_set_step_scale: factors must be positive and finite");
+        return BEST_ERR_ARG;
+      }
+      s[i] = s_host[i];
+    }
+  BEST_CUDA(cudaDeviceSynchronize());
+  BEST_CUDA(cudaMemcpy(ctx->scale_dev, s.data(), sizeof(double) * d, cudaMemcpyHostToDevice));
+  return refresh_scaled_whitening(ctx);
+}
+
+int best_set_hard_box(best_ctx* ctx, int32_t on) {
+  if (!ctx) { set_error("best_set_hard_box: NULL ctx"); return BEST_ERR_ARG; }
+  if (on && !ctx->tgt.has_box) { set_error("best_set_hard_box: the target has no box"); return BEST_ERR_ARG; }
+  BEST_CUDA(cudaDeviceSynchronize());
+  ctx->tgt.hard_box = on ? 1 : 0;
   return BEST_OK;
 }
 
@@ -293,8 +331,8 @@ int best_set_whitening(best_ctx* ctx, const double* L_host) {
       }
     }
   BEST_CUDA(cudaDeviceSynchronize());
-  BEST_CUDA(cudaMemcpy(ctx->L_dev, L.data(), sizeof(double) * d * d, cudaMemcpyHostToDevice));
-  return BEST_OK;
+  BEST_CUDA(cudaMemcpy(ctx->Lraw_dev, L.data(), sizeof(double) * d * d, cudaMemcpyHostToDevice));
+  return refresh_scaled_whitening(ctx);
 }
 
 }  // extern "C"

@@ -66,6 +66,7 @@ struct TargetDev {
   double banana_sigma;
   double mlp_scale;
   int has_mlp;
+  int hard_box;  // 8(f)#1: log pi = -inf outside [lo, hi] instead of the smooth penalty
 };
 
 struct TcPlan;  // bf16 tensor-core path (tc_fused.cu)
@@ -82,7 +83,9 @@ struct best_ctx {
   // fp32 emulator weights, zero padded: W[k] [wp[k+1]][wp[k]], b[k] [wp[k+1]]
   std::vector<float*> W, b;
   double* dev_consts = nullptr;  // mu | R | lo | hi | L  (5 blocks)
-  double* L_dev = nullptr;       // [d*d] lower triangular, updated on device by adaptation
+  double* L_dev = nullptr;       // [d*d] lower triangular, updated on device by adaptation: L_raw * diag(step scale)
+  double* Lraw_dev = nullptr;    // [d*d] the whitening factor itself | [d] per-dimension step factors (8(f)#1)
+  double* scale_dev = nullptr;   // = Lraw_dev + d*d
   // fp32 emulator scratch (sized for scratch_n chains)
   int64_t scratch_n = 0;
   float* X0 = nullptr;            // [n][dp]

@@ -80,7 +80,10 @@ __global__ void k_finish_target(TargetDev T, const double* __restrict__ theta, i
     g[T.banana_j] += -t / s2;
     g[T.banana_i] += 2.0 * ti * t / s2;
   }
-  if (T.has_box) {
+  if (T.has_box && T.hard_box) {  // 8(f)#1: -inf outside the box, no penalty term
+    for (int i = 0; i < d; ++i)
+      if (th[i] < T.lo[i] || th[i] > T.hi[i]) lp = -INFINITY;
+  } else if (T.has_box) {
     double pen = 0.0;
     for (int i = 0; i < d; ++i) {
       const double lo = T.lo[i], hi = T.hi[i], width = hi - lo;

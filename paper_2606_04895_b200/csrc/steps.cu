@@ -225,7 +225,8 @@ k_cov_accumulate(const double* __restrict__ theta, int64_t B, int d, const doubl
 
 // C = scatter/(n-1), C_ii *= (1+jitter), L = chol(C) with jitter x10 retries; swap L on success.
 __global__ void k_cov_finalize(double* __restrict__ acc, int nblk, int d, double jitter,
-                               double* __restrict__ L, long long* __restrict__ counts) {
+                               double* __restrict__ L, double* __restrict__ Lraw,
+                               const double* __restrict__ scale, long long* __restrict__ counts) {
   __shared__ double S[1 + kMaxD + kMaxD * kMaxD];
   __shared__ double Cm[kMaxD * kMaxD], Lt[kMaxD * kMaxD];
   const int ne = 1 + d + d * d;
@@ -265,7 +266,11 @@ __global__ void k_cov_finalize(double* __restrict__ acc, int nblk, int d, double
   }
   if (ok) {
     for (int i = 0; i < d; ++i)
-      for (int j = 0; j < d; ++j) L[i * d + j] = (j <= i) ? Lt[i * d + j] : 0.0;
+      for (int j = 0; j < d; ++j) {
+        const double v = (j <= i) ? Lt[i * d + j] : 0.0;
+        Lraw[i * d + j] = v;
+        L[i * d + j] = v * scale[j];   // per-dimension step factors (8(f)#1) survive the update
+      }
     counts[0] += 1;
   } else {
     counts[1] += 1;
@@ -298,7 +303,7 @@ int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin,
     count_launch();
     if (++ctx->win_steps >= ctx->adapt_every) {
       k_cov_finalize<<<1, 256, 0, s>>>(ctx->cov_acc, nblk, ctx->d, ctx->jitter, ctx->L_dev,
-                                       (long long*)ctx->adapt_counts);
+                                       ctx->Lraw_dev, ctx->scale_dev, (long long*)ctx->adapt_counts);
       count_launch();
       ctx->win_steps = 0;
     }

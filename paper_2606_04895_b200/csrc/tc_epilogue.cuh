@@ -519,7 +519,9 @@ __device__ __forceinline__ void finish_target(EpiCtx& C, const float (&th)[8], f
       const uint32_t gi = (uint32_t)(8 * C.k + i) * 4u;
       const float lo = ptx::lds_c32(vecs + 128u + gi), hi = ptx::lds_c32(vecs + 256u + gi);
       const float ex = fmaxf(fmaxf(lo - th[i], th[i] - hi), 0.0f);
-      if (ex > 0.0f) {
+      if (ex > 0.0f && P.hard_box) {
+        part = -INFINITY;   // 8(f)#1: outside the hard box
+      } else if (ex > 0.0f) {
         const float iw = ptx::lds_c32(vecs + 384u + gi);
         const float t = P.pen_gamma * ex * iw;
         float f, df;

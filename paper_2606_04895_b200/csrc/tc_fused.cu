@@ -128,6 +128,7 @@ struct Params {
   int bias16;             // bias table kept as bf16 in SMEM (1024-wide layers)
   // target terms (fp64 masters on device, converted to fp32 in SMEM at kernel start)
   int has_gauss, has_box, banana_i, banana_j;
+  int hard_box;   // set per launch from the context (8(f)#1)
   float banana_sigma, pen_kappa, pen_gamma;
   const double *mu, *R, *lo, *hi, *L;
 };

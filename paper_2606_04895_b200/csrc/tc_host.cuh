@@ -431,6 +431,7 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
     attr_set = true;
   }
   P.L = ctx->L_dev;
+  P.hard_box = ctx->tgt.hard_box;
   if (tc::Geo<ROWS>::kPair) {
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)n_tiles);

@@ -154,11 +154,14 @@ def test_unsupported_shapes(B):
         assert e.value.code == B.BEST_ERR_UNSUPPORTED
 
 
-def _single_step_stat(B, O, w, method, seed, **kw):
+def _single_step_stat(B, O, w, method, seed, setup=None, **kw):
     kw = {k: (f32(v) if isinstance(v, float) else v) for k, v in kw.items()}
     ctx = B.Context(w, B.PREC_BF16)
+    orc = O.Oracle(w)
+    if setup is not None:
+        setup(ctx, orc)
     st = ctx.new_state(w.theta0)
-    ost = O.Oracle(w).new_state(w.theta0)
+    ost = orc.new_state(w.theta0)
     th0 = ost.theta.copy()
     getattr(st, "step_" + method)(1, seed, **kw)
     getattr(ost, "step_" + method)(1, seed, **kw)
@@ -166,7 +169,8 @@ def _single_step_stat(B, O, w, method, seed, **kw):
     out = st.get(want_grad=(method in ("mala", "hmc")))
     acc, acc_ref = out["n_accept"].astype(np.int64), ost.n_accept.astype(np.int64)
     m = accept_margins(O, seed, 0, w.n_chains, ost.last_log_alpha)
-    dla = np.abs(la - ost.last_log_alpha)
+    with np.errstate(invalid="ignore"):      # hard box: (-inf) - (-inf), masked by the where
+        dla = np.abs(np.where(la == ost.last_log_alpha, 0.0, la - ost.last_log_alpha))
     mism = acc != acc_ref
     info = dict(n=w.n_chains, mismatch_rate=float(mism.mean()), max_dla=float(dla.max()),
                 median_dla=float(np.median(dla)), accept_rate=float(acc_ref.mean()))
@@ -196,6 +200,38 @@ def test_T2_single_step_statistical(B, O, method, kw):
 def test_T2_sterile_1024_single_step(B, O, method, kw):
     """single-step maps on the 29→1024⁴→1 banana target (64-chain tiles), 1024 + 38 chains"""
     _single_step_stat(B, O, WL.sterile(n_chains=1062), method, seed=31, **kw)
+
+
+# ---- SURVEY 8(f)#1 on the tensor-core path: per-dimension step factors (R20), hard box (R21) ------
+@pytest.mark.parametrize("net,method,kw", [("lcdm", "mh", dict(eps=0.1)), ("lcdm", "mala", dict(eps=0.02)),
+                                           ("lcdm", "hmc", dict(eps=0.03, n_leapfrog=4)),
+                                           ("sterile", "mala", dict(eps=0.003)), ("sterile", "hmc", dict(eps=0.01, n_leapfrog=4))])
+def test_N1_step_scale_single_step(B, O, net, method, kw):
+    w = WL.lcdm(n_chains=1024 + 40, mlp_scale=3.0 if method == "hmc" else 1.0) if net == "lcdm" else WL.sterile(n_chains=600)
+    s = np.exp(np.random.default_rng(3).uniform(np.log(0.3), np.log(3.0), w.d))
+    s[-2:] = 10.0 if net == "lcdm" else 3.0
+    info = _single_step_stat(B, O, w, method, seed=91, setup=lambda c, o: (c.set_step_scale(s), o.set_step_scale(s)), **kw)
+    assert 0.02 < info["accept_rate"] < 0.999, info
+
+
+@pytest.mark.parametrize("method,kw", [("mh", dict(eps=0.2)), ("mala", dict(eps=0.1)), ("aies", dict(a=2.0))])
+def test_N1_hard_box_single_step(B, O, method, kw):
+    w = WL.lcdm(n_chains=1024 + 40)
+    sig = np.sqrt(np.diag(w.Sigma))
+    w.lo, w.hi = w.mu - 1.6 * sig, w.mu + 1.6 * sig
+    w.theta0 = np.clip(w.theta0, (w.lo + 1e-3 * sig).astype(np.float32), (w.hi - 1e-3 * sig).astype(np.float32))
+    ctxs = []
+    info = _single_step_stat(B, O, w, method, seed=17,
+                             setup=lambda c, o: (c.set_hard_box(True), o.set_hard_box(True), ctxs.append(c)), **kw)
+    assert info["accept_rate"] < 0.9, info
+    # invariant: no chain ever leaves the box
+    ctx = B.Context(w, B.PREC_BF16)
+    ctx.set_hard_box(True)
+    st = ctx.new_state(w.theta0)
+    getattr(st, "step_" + method)(10, 5, *[f32(v) if isinstance(v, float) else v for v in kw.values()])
+    th = st.get(want_grad=False)["theta"].astype(np.float64)
+    assert (th >= w.lo - 1e-5 * sig - 1e-6).all() and (th <= w.hi + 1e-5 * sig + 1e-6).all()   # fp32 read-back
+    ctx.close()
 
 
 def test_T4_split_invariance_1024(B):

@@ -74,11 +74,14 @@ def f32(x):
     return float(np.float32(x))
 
 
-def _single_step(B, O, w, method, seed, **kw):
+def _single_step(B, O, w, method, seed, setup=None, **kw):
     kw = {k: (f32(v) if isinstance(v, float) else v) for k, v in kw.items()}
     ctx = B.Context(w, B.PREC_FP32)
+    orc = O.Oracle(w)
+    if setup is not None:
+        setup(ctx, orc)
     st = ctx.new_state(w.theta0)
-    ost = O.Oracle(w).new_state(w.theta0)
+    ost = orc.new_state(w.theta0)
     th0 = ost.theta.copy()
     getattr(st, "step_" + method)(1, seed, **kw)
     getattr(ost, "step_" + method)(1, seed, **kw)
@@ -88,9 +91,11 @@ def _single_step(B, O, w, method, seed, **kw):
     acc_ref = ost.n_accept.astype(np.int64)
     m = accept_margins(O, seed, 0, w.n_chains, ost.last_log_alpha)
     mism = acc != acc_ref
+    with np.errstate(invalid="ignore"):      # hard box: (-inf) - (-inf), masked by the where
+        dla = np.abs(np.where(la == ost.last_log_alpha, 0.0, la - ost.last_log_alpha))
     info = dict(n=w.n_chains, mismatches=int(mism.sum()),
                 max_margin_of_mismatch=float(m[mism].max()) if mism.any() else 0.0,
-                max_dla=float(np.nanmax(np.abs(la - ost.last_log_alpha))),
+                max_dla=float(np.nanmax(dla)),
                 accept_rate=float(acc_ref.mean()))
     print(f"[T2] {w.name}/{method}: {info}")
     # accept bits identical outside the logged margin set |log u − log α| < 1e-6 (north_star)
@@ -264,6 +269,114 @@ def test_T6_adaptation_matches_oracle_driver(B, O):
     np.testing.assert_allclose(ctx.get_whitening(), o.get_whitening(), rtol=1e-9, atol=1e-11)
     th, _, _ = st.get_f64(want_grad=False)
     np.testing.assert_allclose(th, ost.theta, rtol=1e-9, atol=1e-9)
+    ctx.close()
+
+
+# ---- per-dimension step factors (R20) and hard box (R21) --------------------------
+def _step_factors(d, seed):
+    s = np.exp(np.random.default_rng(seed).uniform(np.log(0.3), np.log(3.0), d))
+    s[-2:] = 10.0                                   # the paper's "10 times larger for the extension parameters"
+    return s
+
+
+@pytest.mark.parametrize("method,kw", [("mh", dict(eps=0.1)), ("mala", dict(eps=0.02)),
+                                       ("hmc", dict(eps=0.03, n_leapfrog=4))])
+def test_N1_step_scale_single_step(B, O, method, kw):
+    w = WL.lcdm(n_chains=1024, mlp_scale=3.0 if method == "hmc" else 1.0)
+    s = _step_factors(w.d, 3)
+    info = _single_step(B, O, w, method, seed=91, setup=lambda c, o: (c.set_step_scale(s), o.set_step_scale(s)), **kw)
+    assert 0.02 < info["accept_rate"] < 0.999, info     # both branches of the accept rule are exercised
+
+
+def test_N1_step_scale_api(B, O):
+    """Factors persist across set_whitening and adaptation; get_whitening returns the unscaled factor;
+    NULL resets; bad factors are refused."""
+    w = WL.gaussian(5, 256, seed=81)
+    w.L = np.diag(np.sqrt(np.diag(w.Sigma)))
+    s = np.array([0.5, 2.0, 1.0, 3.0, 0.7])
+    ctx = B.Context(w, B.PREC_FP32)
+    ctx.set_step_scale(s)
+    np.testing.assert_array_equal(ctx.get_whitening(), w.L)
+    L2 = np.linalg.cholesky(w.Sigma)
+    ctx.set_whitening(L2)
+    np.testing.assert_array_equal(ctx.get_whitening(), np.tril(L2))
+    st = ctx.new_state(w.theta0)
+    st.set_adaptation(50, 1e-6)
+    o = O.Oracle(w)
+    o.set_whitening(L2)
+    o.set_step_scale(s)
+    o.set_adaptation(50, 1e-6)
+    ost = o.new_state(w.theta0)
+    st.step_mala(100, 4, 0.2)
+    ost.step_mala(100, 4, f32(0.2))
+    np.testing.assert_allclose(ctx.get_whitening(), o.get_whitening(), rtol=1e-9, atol=1e-11)
+    th, _, _ = st.get_f64(want_grad=False)
+    np.testing.assert_allclose(th, ost.theta, rtol=1e-9, atol=1e-9)
+    for bad in (np.array([1.0, 0.0, 1, 1, 1]), np.array([1.0, -2.0, 1, 1, 1]), np.array([1.0, np.inf, 1, 1, 1]),
+                np.array([1.0, np.nan, 1, 1, 1])):
+        with pytest.raises(B.BestError) as e:
+            ctx.set_step_scale(bad)
+        assert e.value.code == B.BEST_ERR_ARG
+    st.set_adaptation(0)
+    ctx.set_step_scale(None)
+    ost2 = O.Oracle(w)
+    ost2.set_whitening(ctx.get_whitening())
+    a, b2 = ctx.new_state(w.theta0), ost2.new_state(w.theta0)
+    a.step_mh(3, 8, 0.3)
+    b2.step_mh(3, 8, f32(0.3))
+    np.testing.assert_allclose(a.get_f64(want_grad=False)[0], b2.theta, rtol=1e-9, atol=1e-9)
+    ctx.close()
+
+
+def _narrow_box(w, nsig):
+    """box = μ ± nsig·σ per coordinate, starting points clipped into it"""
+    sig = np.sqrt(np.diag(w.Sigma))
+    w.lo, w.hi = w.mu - nsig * sig, w.mu + nsig * sig
+    w.theta0 = np.clip(w.theta0, (w.lo + 1e-3 * sig).astype(np.float32), (w.hi - 1e-3 * sig).astype(np.float32))
+    return w
+
+
+@pytest.mark.parametrize("method,kw", [("mh", dict(eps=0.5)), ("mala", dict(eps=0.3)), ("hmc", dict(eps=0.3, n_leapfrog=4)),
+                                       ("aies", dict(a=2.0))])
+def test_N1_hard_box_single_step(B, O, method, kw):
+    w = _narrow_box(WL.tiny().with_chains(8192, seed=12), 1.2)
+    info = _single_step(B, O, w, method, seed=17, setup=lambda c, o: (c.set_hard_box(True), o.set_hard_box(True)), **kw)
+    assert info["accept_rate"] < 0.9, info              # a visible share of the proposals leaves the box
+
+
+def test_N1_hard_box_values_and_invariant(B, O):
+    w = _narrow_box(WL.tiny().with_chains(4096, seed=13), 1.0)
+    ctx = B.Context(w, B.PREC_FP32)
+    o = O.Oracle(w)
+    ctx.set_hard_box(True)
+    o.set_hard_box(True)
+    pts = WL.probe_points(w, 600, seed=3)
+    lp = np.zeros(600, np.float32)
+    g = np.zeros((600, w.d), np.float32)
+    ctx.logp_grad(pts, 600, lp, g)
+    lp_ref, g_ref = o.logp_grad(pts)
+    outside = np.isneginf(lp_ref)
+    assert 50 < outside.sum() < 550
+    assert np.array_equal(np.isneginf(lp), outside)
+    ins = ~outside
+    assert np.abs(lp[ins] - lp_ref[ins]).max() <= TOL[0] * np.abs(lp_ref[ins]).max()
+    num = np.linalg.norm(g - g_ref, axis=1)
+    assert (num <= TOL[0] * np.linalg.norm(g_ref, axis=1)).all()     # gradient of the remaining terms everywhere
+    st = ctx.new_state(w.theta0)
+    for step in (lambda: st.step_mh(20, 5, 0.6), lambda: st.step_mala(20, 6, 0.3), lambda: st.step_hmc(5, 7, 0.3, 4),
+                 lambda: st.step_aies(10, 8, 2.0)):
+        step()
+        th = st.get_f64(want_grad=False)[0]
+        assert (th >= w.lo).all() and (th <= w.hi).all()
+    acc = st.get(want_grad=False)["n_accept"]
+    assert acc.min() >= 1
+    wf = WL.tiny().with_chains(16, seed=13)
+    wf.lo = wf.hi = None
+    c2 = B.Context(wf, B.PREC_FP32)
+    with pytest.raises(B.BestError) as e:
+        c2.set_hard_box(True)
+    assert e.value.code == B.BEST_ERR_ARG
+    c2.close()
     ctx.close()
 
 
