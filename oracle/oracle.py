@@ -292,6 +292,60 @@ class OracleState:
         self.n_evals += self.B * n_traj * n_leapfrog
         return tr
 
+    # ---- burn-in loop (reading R22) ----------------------
+    def _step(self, method, n, seed, eps, n_leapfrog):
+        if method == "mh":
+            self.step_mh(n, seed, eps)
+        elif method == "mala":
+            self.step_mala(n, seed, eps)
+        elif method == "hmc":
+            self.step_hmc(n, seed, eps, n_leapfrog)
+        else:
+            raise ValueError("burn-in loop: mh, mala or hmc (the paper runs none for AIES, P:L260)")
+
+    def burn_in(self, method, n_iter, n_steps, n_adapt, block, seed, eps0, target_accept,
+                n_leapfrog=1, jitter=1e-6):
+        """n_iter burn-in iterations of n_steps steps each.  In every iteration the first
+        n_adapt steps adapt the step size and are then discarded; the covariance of all chains
+        over the remaining n_steps − n_adapt steps replaces the whitening factor (O6), and
+        the best-fit point (largest log π over the ensemble, kept over iterations) is updated.
+        The paper gives no adaptation rule: reading R22 = Nesterov dual averaging as in Hoffman & Gelman
+        (2014, Alg. 5; γ = 0.05, t₀ = 10, κ = 0.75, μ = log 10ε) on the acceptance FRACTION of the whole
+        ensemble over blocks of `block` steps, restarted in each iteration from the current ε.
+        ε crosses the sampler interface as float32, like on the C-ABI.  Returns (ε, θ_best, log π_best,
+        [ε used in each block])."""
+        GAMMA, T0, KAPPA = 0.05, 10.0, 0.75
+        import math
+        eps = float(np.float32(eps0))
+        best_lp, best_th, hist = -math.inf, None, []
+        for _ in range(n_iter):
+            if n_adapt > 0:
+                mu, hbar, logeps_bar, m, cur, done = math.log(10.0 * eps), 0.0, 0.0, 0, eps, 0
+                while done < n_adapt:
+                    nb = min(block, n_adapt - done)
+                    a0 = int(self.n_accept.sum())
+                    cur32 = float(np.float32(cur))
+                    hist.append(cur32)
+                    self._step(method, nb, seed, cur32, n_leapfrog)
+                    alpha = (int(self.n_accept.sum()) - a0) / float(self.B * nb)
+                    m += 1
+                    hbar = (1.0 - 1.0 / (m + T0)) * hbar + (target_accept - alpha) / (m + T0)
+                    logeps = mu - math.sqrt(m) / GAMMA * hbar
+                    eta = math.pow(m, -KAPPA)
+                    logeps_bar = eta * logeps + (1.0 - eta) * logeps_bar
+                    cur = math.exp(logeps)
+                    done += nb
+                eps = float(np.float32(math.exp(logeps_bar)))
+            win = n_steps - n_adapt
+            if win > 0:
+                self.o.set_adaptation(win, jitter)
+                self._step(method, win, seed, eps, n_leapfrog)
+                self.o.set_adaptation(0, jitter)
+            i = int(np.argmax(self.logp))
+            if self.logp[i] > best_lp:
+                best_lp, best_th = float(self.logp[i]), self.theta[i].copy()
+        return eps, best_th, best_lp, hist
+
     def step_aies(self, n_steps, seed, a=2.0, thin=0):
         tr = self._trace(n_steps, thin)
         rc = lib().oracle_step_aies(self.o._h, self.B, _dp(self.theta), _dp(self.logp), self.step,

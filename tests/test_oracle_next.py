@@ -173,3 +173,66 @@ def test_hard_box_value_and_uniform_law(oracle_mod):
     v = ((tr - 0.5 * (wu.lo + wu.hi)) ** 2).mean(axis=0)
     se_v = v.std(axis=0, ddof=1) / math.sqrt(v.shape[0])
     assert np.all(np.abs(v.mean(axis=0) - (wu.hi - wu.lo) ** 2 / 12.0) < 4.0 * se_v)
+
+
+# ---- burn-in loop (reading R22) -------------------------------------------------------
+class _FakeState:
+    """Feeds the dual-averaging recursion a prescribed acceptance fraction per block."""
+
+    def __init__(self, oracle_mod, alphas, B=1000):
+        self._alphas, self.B, self.k = list(alphas), B, 0
+        self.n_accept = np.zeros(B, dtype=np.uint64)
+        self.logp, self.theta = np.zeros(B), np.zeros((B, 1))
+        self.eps_seen = []
+        self.o = type("O", (), {"set_adaptation": lambda self, *a: None})()
+        self._burn = oracle_mod.OracleState.burn_in.__get__(self)
+
+    def _step(self, method, n, seed, eps, nl):
+        self.eps_seen.append(eps)
+        k = int(round(self._alphas[self.k] * self.B * n))
+        self.n_accept[0] += np.uint64(k)
+        self.k += 1
+
+
+def test_dual_averaging_closed_form(oracle_mod):
+    """Constant acceptance α: H̄_m = (δ−α)·m/(m+t₀) ⇒ log ε_m = μ − √m/γ·(δ−α)·m/(m+t₀), μ = log 10ε₀;
+    α ≡ δ ⇒ every ε_m = 10 ε₀ (Hoffman & Gelman 2014, Alg. 5)."""
+    eps0, delta, nblk = 0.25, 0.574, 12
+    for alpha in (0.574, 0.2, 0.9):
+        fs = _FakeState(oracle_mod, [alpha] * nblk)
+        eps, _, _, hist = fs._burn("mala", 1, 10 * nblk, 10 * nblk, 10, 1, eps0, delta)
+        assert len(hist) == nblk and hist[0] == float(np.float32(eps0))
+        m = np.arange(1, nblk)
+        ref = np.log(10 * eps0) - np.sqrt(m) / 0.05 * (delta - alpha) * m / (m + 10.0)
+        np.testing.assert_allclose(np.log(hist[1:]), ref, rtol=0, atol=2e-6)     # float32 ε at the interface
+        # the returned ε is the weighted average log ε̄ = Σ-recursion with weights m^-0.75
+        m_all = np.arange(1, nblk + 1)
+        le = np.log(10 * eps0) - np.sqrt(m_all) / 0.05 * (delta - alpha) * m_all / (m_all + 10.0)
+        bar = 0.0
+        for mm, l in zip(m_all, le):
+            bar = mm ** -0.75 * l + (1 - mm ** -0.75) * bar
+        assert math.log(eps) == pytest.approx(bar, abs=2e-6)
+
+
+def test_burn_in_finds_optimal_mh_scale_and_covariance(oracle_mod):
+    """Anisotropic Gaussian, diagonal initial whitening: after 3 iterations L Lᵀ ≈ Σ, the MH step adapted
+    toward acceptance 0.234 is the textbook optimal 2.38/√d (Roberts, Gelman & Gilks 1997; asymptotic in d: ±15 % at d = 30),
+    the acceptance of a fresh run sits at the target, and the best-fit point is near μ."""
+    d = 30
+    w = WL.gaussian(d, 512, seed=44, cond=50.0)
+    w.lo = w.hi = None
+    w.L = np.diag(np.sqrt(np.diag(w.Sigma)))
+    o = oracle_mod.Oracle(w)
+    st = o.new_state(w.theta0)
+    eps, th_best, lp_best, hist = st.burn_in("mh", 3, 390, 240, 4, 5, 0.05, 0.234)   # 60 blocks per iteration: ε̄ forgets the 10 ε₀ start
+    C = o.get_whitening() @ o.get_whitening().T
+    dscale = np.sqrt(np.outer(np.diag(w.Sigma), np.diag(w.Sigma)))
+    assert np.abs(C - w.Sigma).max() / dscale.max() < 0.08          # 512 chains x 150 steps per window
+    assert 0.85 * 2.38 / math.sqrt(d) < eps < 1.15 * 2.38 / math.sqrt(d), eps
+    a0 = st.n_accept.sum()
+    st.step_mh(100, 5, eps)
+    rate = (st.n_accept.sum() - a0) / (512 * 100)
+    assert abs(rate - 0.234) < 0.05, rate
+    z = np.linalg.solve(np.linalg.cholesky(w.Sigma), th_best - w.mu)
+    assert lp_best == pytest.approx(-0.5 * z @ z, abs=1e-9) and z @ z < 0.5 * d   # the best of 512 chains lies well inside the typical set (E z.z = d)
+    assert o.adapt_stats() == (3, 0)
