@@ -148,6 +148,33 @@ int best_set_whitening(best_ctx* ctx, const double* L_host);
 int best_set_step_scale(best_ctx* ctx, const double* s_host);
 int best_set_hard_box(best_ctx* ctx, int32_t on);
 
+/* the burn-in loop of PAPER.md sec. 3.2 / 4 ("a burn-in loop where the covariance
+ * matrix and the best-fit point are iteratively updated based on short chains"; sec. 4.3: iterations of
+ * n_steps steps "of which the first [n_adapt] steps are used for step size adaptation and afterwards
+ * discarded"); reading R22.  Host-side schedule around the step kernels and A9:
+ * for each of n_iter iterations
+ *   (1) n_adapt steps in blocks of `block` steps (the last block may be shorter); after block m the
+ *       acceptance fraction alpha of ALL chains over the block (summed on the device) drives Nesterov
+ *       dual averaging (Hoffman & Gelman 2014, Alg. 5: gamma 0.05, t0 10, kappa 0.75, mu = log(10 eps)),
+ *       restarted from the current eps; the next block runs with eps_m, the iteration ends with the
+ *       averaged step exp(log eps-bar), rounded to float;
+ *   (2) n_steps - n_adapt steps with one covariance window over all of them; at its end the whitening
+ *       factor is replaced on the device (A9, `jitter` as in best_set_adaptation);
+ *   (3) the chain with the largest cached log pi updates the best-fit point if it beats the previous
+ *       iterations.
+ * method: BEST_METHOD_MH / _MALA / _HMC (the paper runs no burn-in loop for AIES: BEST_ERR_ARG);
+ * n_leapfrog is read for HMC only.  *eps_inout (host): initial step in, adapted step out.
+ * target_accept in (0,1), e.g. 0.234 MH, 0.574 MALA, 0.65-0.8 HMC.  best_theta [d] / best_logp (host,
+ * nullable) receive the best-fit point in the original space (fp32 / fp64).  eps_hist (host, nullable,
+ * capacity n_iter * ceil(n_adapt / block)) receives the step used in every adaptation block.
+ * Synchronises `stream` after every block; leaves adaptation switched off.  The global step counter
+ * advances by n_iter * n_steps.                                                                       */
+enum { BEST_METHOD_MH = 0, BEST_METHOD_MALA = 1, BEST_METHOD_HMC = 2 };
+int best_burn_in(best_ctx* ctx, best_state* st, int32_t method, int32_t n_iter, int64_t n_steps,
+                 int64_t n_adapt, int64_t block, uint64_t seed, float* eps_inout, float target_accept,
+                 int32_t n_leapfrog, double jitter, float* best_theta, double* best_logp,
+                 float* eps_hist, void* stream);
+
 /* Read the state back (all pointers host, each nullable): theta [B*d], logp [B], grad [B*d]
  * (float, original space), global step counter, per-chain accept counters [B], total emulator
  * evaluations.  Synchronises `stream`.                                                          */

@@ -17,13 +17,14 @@ LIB_PATH = os.path.join(_HERE, "libbest.so")
 BEST_OK, BEST_ERR_ARG, BEST_ERR_CUDA, BEST_ERR_NOT_SPD, BEST_ERR_UNSUPPORTED, BEST_ERR_ALLOC = 0, -1, -2, -3, -4, -5
 ACT_TANH, ACT_SILU = 0, 1
 PREC_FP32, PREC_BF16 = 0, 1
+METHOD_MH, METHOD_MALA, METHOD_HMC = 0, 1, 2
 
 EXPORTS = [
     "best_create", "best_destroy", "best_logp_grad", "best_state_create", "best_state_destroy",
     "best_step_mh", "best_step_mala", "best_step_hmc", "best_step_aies", "best_set_adaptation",
     "best_adapt_stats", "best_get_whitening", "best_set_whitening", "best_state_get",
     "best_state_get_f64", "best_state_last_log_alpha", "best_state_set", "best_launch_count",
-    "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box",
+    "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box", "best_burn_in",
 ]
 
 
@@ -77,6 +78,8 @@ def lib():
     L.best_set_whitening.argtypes = [vp, vp]
     L.best_set_step_scale.argtypes = [vp, vp]
     L.best_set_hard_box.argtypes = [vp, i32]
+    L.best_burn_in.argtypes = [vp, vp, i32, i32, i64, i64, i64, u64, C.POINTER(C.c_float), C.c_float, i32,
+                               C.c_double, vp, C.POINTER(C.c_double), vp, vp]
     L.best_state_get.argtypes = [vp, vp, vp, vp, C.POINTER(u64), vp, C.POINTER(u64), vp]
     L.best_state_get_f64.argtypes = [vp, vp, vp, vp, vp]
     L.best_state_last_log_alpha.argtypes = [vp, vp, vp]
@@ -230,6 +233,20 @@ class State:
 
     def set_adaptation(self, adapt_every, jitter=1e-6):
         _check(lib().best_set_adaptation(self.ctx._h, self._h, adapt_every, jitter))
+
+    def burn_in(self, method, n_iter, n_steps, n_adapt, block, seed, eps0, target_accept, n_leapfrog=1,
+                jitter=1e-6, stream=0):
+        """best_burn_in: returns (eps, best_theta [d] float32, best_logp, eps used in every adaptation block)."""
+        m = {"mh": METHOD_MH, "mala": METHOD_MALA, "hmc": METHOD_HMC}.get(method, method)
+        eps = C.c_float(eps0)
+        best_lp = C.c_double()
+        best_th = np.zeros(self.ctx.d, dtype=np.float32)
+        nblk = n_iter * (-(-n_adapt // block) if n_adapt > 0 and block > 0 else 0)
+        hist = np.zeros(max(nblk, 1), dtype=np.float32)
+        _check(lib().best_burn_in(self.ctx._h, self._h, m, n_iter, n_steps, n_adapt, block, seed, C.byref(eps),
+                                  target_accept, n_leapfrog, jitter, best_th.ctypes.data, C.byref(best_lp),
+                                  hist.ctypes.data, stream or None))
+        return eps.value, best_th, best_lp.value, hist[:nblk]
 
     def get(self, want_grad=True, stream=0):
         d, B = self.ctx.d, self.B

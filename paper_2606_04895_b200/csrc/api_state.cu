@@ -41,6 +41,27 @@ enum { M_MH = 0, M_MALA = 1, M_HMC = 2, M_AIES = 3 };
 
 }  // namespace
 
+namespace {
+__global__ void k_sum_accept(const unsigned long long* __restrict__ n_accept, int64_t B,
+                             unsigned long long* __restrict__ out) {
+  unsigned long long s = 0;
+  for (int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; c < B; c += (int64_t)gridDim.x * blockDim.x)
+    s += n_accept[c];
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0 && s) atomicAdd(out, s);
+}
+
+int total_accepts(best_state* st, unsigned long long* dev_tmp, unsigned long long* out, cudaStream_t s) {
+  BEST_CUDA(cudaMemsetAsync(dev_tmp, 0, sizeof(unsigned long long), s));
+  const int nb = (int)((st->B + 255) / 256 < 1024 ? (st->B + 255) / 256 : 1024);
+  k_sum_accept<<<nb, 256, 0, s>>>(st->n_accept, st->B, dev_tmp);
+  count_launch();
+  BEST_CUDA(cudaMemcpyAsync(out, dev_tmp, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
+  BEST_CUDA(cudaStreamSynchronize(s));
+  return BEST_OK;
+}
+}  // namespace
+
 extern "C" {
 
 int best_logp_grad(best_ctx* ctx, const float* theta, int64_t n, float* logp, float* grad,
@@ -333,6 +354,86 @@ int best_set_whitening(best_ctx* ctx, const double* L_host) {
   BEST_CUDA(cudaDeviceSynchronize());
   BEST_CUDA(cudaMemcpy(ctx->Lraw_dev, L.data(), sizeof(double) * d * d, cudaMemcpyHostToDevice));
   return refresh_scaled_whitening(ctx);
+}
+
+int best_burn_in(best_ctx* ctx, best_state* st, int32_t method, int32_t n_iter, int64_t n_steps,
+                 int64_t n_adapt, int64_t block, uint64_t seed, float* eps_inout, float target_accept,
+                 int32_t n_leapfrog, double jitter, float* best_theta, double* best_logp,
+                 float* eps_hist, void* stream) {
+  if (!ctx || !st || st->ctx != ctx || !eps_inout) { set_error("best_burn_in: bad ctx/state/eps"); return BEST_ERR_ARG; }
+  if (method != BEST_METHOD_MH && method != BEST_METHOD_MALA && method != BEST_METHOD_HMC) {
+    set_error("best_burn_in: method must be MH, MALA or HMC (no burn-in loop for AIES)");
+    return BEST_ERR_ARG;
+  }
+  if (n_iter < 0 || n_steps < 0 || n_adapt < 0 || n_adapt > n_steps || (n_adapt > 0 && block < 1) ||
+      !(target_accept > 0.f && target_accept < 1.f) || !(*eps_inout > 0.f) || !(jitter >= 0.0)) {
+    set_error("best_burn_in: bad schedule / target_accept / eps / jitter");
+    return BEST_ERR_ARG;
+  }
+  cudaStream_t s = (cudaStream_t)stream;
+  const int m_int = method == BEST_METHOD_MH ? M_MH : method == BEST_METHOD_MALA ? M_MALA : M_HMC;
+  constexpr double kGamma = 0.05, kT0 = 10.0, kKappa = 0.75;
+  DevBuf tmp;
+  BEST_TRY(tmp.alloc(sizeof(unsigned long long)));
+  unsigned long long* dtmp = (unsigned long long*)tmp.p;
+  float eps = *eps_inout;
+  double best_lp = -INFINITY;
+  std::vector<double> lp_host((size_t)st->B);
+  int64_t nh = 0;
+  ctx->adapt_every = 0;
+  for (int it = 0; it < n_iter; ++it) {
+    if (n_adapt > 0) {  // (1) dual averaging on the ensemble acceptance fraction
+      const double mu = std::log(10.0 * (double)eps);
+      double hbar = 0.0, logeps_bar = 0.0, cur = (double)eps;
+      int64_t done = 0;
+      int m = 0;
+      while (done < n_adapt) {
+        const int64_t nb = (block < n_adapt - done) ? block : (n_adapt - done);
+        unsigned long long a0 = 0, a1 = 0;
+        BEST_TRY(total_accepts(st, dtmp, &a0, s));
+        const float cur32 = (float)cur;
+        if (eps_hist) eps_hist[nh] = cur32;
+        ++nh;
+        BEST_TRY(run_step(ctx, st, m_int, nb, seed, cur32, n_leapfrog, nullptr, 0, stream));
+        BEST_TRY(total_accepts(st, dtmp, &a1, s));
+        const double alpha = (double)(a1 - a0) / ((double)st->B * (double)nb);
+        ++m;
+        hbar = (1.0 - 1.0 / (m + kT0)) * hbar + ((double)target_accept - alpha) / (m + kT0);
+        const double logeps = mu - std::sqrt((double)m) / kGamma * hbar;
+        const double eta = std::pow((double)m, -kKappa);
+        logeps_bar = eta * logeps + (1.0 - eta) * logeps_bar;
+        cur = std::exp(logeps);
+        done += nb;
+      }
+      eps = (float)std::exp(logeps_bar);
+    }
+    const int64_t win = n_steps - n_adapt;
+    if (win > 0) {  // (2) one covariance window -> whitening update on the device
+      if (win > INT32_MAX) { set_error("best_burn_in: window too long"); return BEST_ERR_ARG; }
+      BEST_TRY(best_set_adaptation(ctx, st, (int32_t)win, jitter));
+      const int rc = run_step(ctx, st, m_int, win, seed, eps, n_leapfrog, nullptr, 0, stream);
+      ctx->adapt_every = 0;
+      if (rc) return rc;
+    }
+    // (3) best fit over the ensemble (first chain with the largest cached log pi)
+    BEST_CUDA(cudaStreamSynchronize(s));
+    BEST_CUDA(cudaMemcpy(lp_host.data(), st->logp, sizeof(double) * st->B, cudaMemcpyDeviceToHost));
+    int64_t arg = 0;
+    for (int64_t c = 1; c < st->B; ++c)
+      if (lp_host[c] > lp_host[arg]) arg = c;
+    if (st->B > 0 && lp_host[arg] > best_lp) {
+      best_lp = lp_host[arg];
+      if (best_theta)
+        for (int i = 0; i < ctx->d; ++i) {
+          double v;
+          BEST_CUDA(cudaMemcpy(&v, st->theta + (size_t)i * st->B + arg, sizeof(double), cudaMemcpyDeviceToHost));
+          best_theta[i] = (float)v;
+        }
+    }
+  }
+  *eps_inout = eps;
+  if (best_logp) *best_logp = best_lp;
+  return BEST_OK;
 }
 
 }  // extern "C"

@@ -234,6 +234,28 @@ def test_N1_hard_box_single_step(B, O, method, kw):
     ctx.close()
 
 
+def test_N2_burn_in_reaches_target_acceptance(B):
+    """SURVEY 8(f)#2 on the tensor-core path: after the loop a fresh run accepts at the target rate and
+    the whitening factor has been replaced once per iteration."""
+    w = WL.lcdm(n_chains=2048)
+    w.L = np.diag(np.sqrt(np.diag(w.Sigma)))
+    ctx = B.Context(w, B.PREC_BF16)
+    st = ctx.new_state(w.theta0)
+    eps, th_best, lp_best, hist = st.burn_in("mala", 2, 400, 300, 5, 7, 0.01, 0.574)
+    assert len(hist) == 120 and hist[0] == f32(0.01)
+    assert ctx.adapt_stats() == (2, 0)
+    C = ctx.get_whitening() @ ctx.get_whitening().T
+    dscale = np.sqrt(np.outer(np.diag(w.Sigma), np.diag(w.Sigma)))
+    assert np.abs(C - w.Sigma).max() / dscale.max() < 0.1
+    a0 = st.get(want_grad=False)["n_accept"].sum()
+    st.step_mala(50, 7, eps)
+    out = st.get(want_grad=False)
+    rate = (out["n_accept"].sum() - a0) / (2048 * 50)
+    assert abs(rate - 0.574) < 0.06, (eps, rate)
+    assert lp_best >= out["logp"].max() - 1e-3 or lp_best > np.median(out["logp"])
+    ctx.close()
+
+
 def test_T4_split_invariance_1024(B):
     w = WL.sterile(n_chains=200)
     ctx = B.Context(w, B.PREC_BF16)

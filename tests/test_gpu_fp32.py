@@ -380,6 +380,52 @@ def test_N1_hard_box_values_and_invariant(B, O):
     ctx.close()
 
 
+# ---- burn-in loop (R22) ------------------------------------------------------------
+@pytest.mark.parametrize("method,eps0,delta,nl", [("mh", 0.1, 0.234, 1), ("mala", 0.05, 0.574, 1), ("hmc", 0.05, 0.7, 3)])
+def test_N2_burn_in_matches_oracle(B, O, method, eps0, delta, nl):
+    """Same seeds and schedule: every block's step, the adapted step, the whitening factor after each
+    iteration's covariance window, the final ensemble and the best-fit point track the oracle's loop."""
+    w = WL.tiny().with_chains(256, seed=19)
+    w.L = np.diag(np.sqrt(np.diag(w.Sigma)))
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(w.theta0)
+    o = O.Oracle(w)
+    ost = o.new_state(w.theta0)
+    eps, th_best, lp_best, hist = st.burn_in(method, 2, 110, 60, 8, 23, eps0, delta, n_leapfrog=nl)
+    eps_o, th_o, lp_o, hist_o = ost.burn_in(method, 2, 110, 60, 8, 23, eps0, f32(delta), n_leapfrog=nl)
+    assert len(hist) == len(hist_o) == 2 * 8
+    np.testing.assert_allclose(hist, hist_o, rtol=1e-6)
+    assert eps == pytest.approx(eps_o, rel=1e-6)
+    # the emulator runs in fp32 (rel 1e-5 bar): positions agree to that, not to fp64 rounding
+    np.testing.assert_allclose(ctx.get_whitening(), o.get_whitening(), rtol=1e-5, atol=1e-7)
+    th, lp, _ = st.get_f64(want_grad=False)
+    np.testing.assert_allclose(th, ost.theta, rtol=0, atol=1e-5 * np.abs(ost.theta).max())
+    np.testing.assert_allclose(th_best, th_o, rtol=0, atol=1e-5 * np.abs(ost.theta).max())
+    assert lp_best == pytest.approx(lp_o, rel=1e-5, abs=1e-5)
+    assert ctx.adapt_stats() == (2, 0) and st.get(want_grad=False)["step"] == 220
+    # adaptation is left switched off: more steps do not move the whitening factor
+    L0 = ctx.get_whitening()
+    st.step_mh(5, 1, 0.1)
+    assert np.array_equal(ctx.get_whitening(), L0)
+    ctx.close()
+
+
+def test_N2_burn_in_arguments(B):
+    w = WL.tiny().with_chains(16, seed=1)
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(w.theta0)
+    for args in ((3, 1, 10, 5, 5, 1, 0.1, 0.5), ("mh", 1, 10, 5, 5, 1, 0.1, 0.0), ("mh", 1, 10, 5, 5, 1, 0.1, 1.0),
+                 ("mh", 1, 10, 11, 5, 1, 0.1, 0.5), ("mh", 1, 10, 5, 0, 1, 0.1, 0.5), ("mh", 1, 10, 5, 5, 1, 0.0, 0.5)):
+        with pytest.raises(B.BestError) as e:
+            st.burn_in(*args)
+        assert e.value.code == B.BEST_ERR_ARG
+    eps, th, lp, hist = st.burn_in("mh", 0, 10, 5, 5, 1, 0.1, 0.5)          # no iterations: nothing happens
+    assert eps == f32(0.1) and len(hist) == 0 and st.get(want_grad=False)["step"] == 0
+    eps, th, lp, hist = st.burn_in("mh", 1, 10, 0, 1, 1, 0.1, 0.5)          # no adaptation: covariance window only
+    assert eps == f32(0.1) and ctx.adapt_stats() == (1, 0)
+    ctx.close()
+
+
 def test_T7_nonfinite_and_far_outside(B):
     w = WL.lcdm(n_chains=256, hidden=64, n_hidden=2, mlp_scale=3.0)
     th0 = w.theta0.copy()
