@@ -32,13 +32,16 @@ def test_sharding_and_max_over_ranks_gloo(tmp_path):
     script = tmp_path / "worker.py"
     script.write_text(WORKER)
     import socket
-    with socket.socket() as sk:          # a free port: back-to-back runs must not collide
-        sk.bind(("127.0.0.1", 0))
-        port = str(sk.getsockname()[1])
-    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=port, OMP_NUM_THREADS="1")
-    p = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
-                        "--master-addr", "127.0.0.1", "--master-port", port, str(script), ROOT],
-                       capture_output=True, text=True, timeout=300, env=env)
+    for attempt in range(3):             # the rendezvous port can be taken between probing and binding: retry
+        with socket.socket() as sk:      # a free port: back-to-back runs must not collide
+            sk.bind(("127.0.0.1", 0))
+            port = str(sk.getsockname()[1])
+        env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=port, OMP_NUM_THREADS="1")
+        p = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2",
+                            "--master-addr", "127.0.0.1", "--master-port", port, str(script), ROOT],
+                           capture_output=True, text=True, timeout=300, env=env)
+        if p.returncode == 0:
+            break
     assert p.returncode == 0, p.stderr[-2000:]
     import json
     res = sorted((json.loads(l.split("RESULT ", 1)[1]) for l in p.stdout.splitlines() if "RESULT " in l),
