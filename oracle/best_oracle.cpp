@@ -365,6 +365,18 @@ void aies_map(const Oracle& o, const double* theta_i, double logp_i, const doubl
   *log_alpha = (double)(d - 1) * std::log(z) + *logp_p - logp_i;
 }
 
+// Differential-evolution move, eq (2.16) P:L170-176 (reading R23):
+//   x_i' = x_i + gamma (x_j - x_k),  gamma = (1 + eta) 2.38 / sqrt(2 d),  eta ~ N(0, sigma_gamma).
+// j and k are two DIFFERENT walkers; swapping them flips the displacement, so the proposal is symmetric
+// and log alpha = log pi(x') - log pi(x_i) with no extra factor.
+void de_map(const Oracle& o, const double* theta_i, double logp_i, const double* theta_j,
+            const double* theta_k, double gamma, double* theta_p, double* logp_p, double* log_alpha) {
+  const int d = o.d;
+  for (int q = 0; q < d; ++q) theta_p[q] = theta_i[q] + gamma * (theta_j[q] - theta_k[q]);
+  *logp_p = target_eval(o, theta_p, nullptr);
+  *log_alpha = *logp_p - logp_i;
+}
+
 // ---------------------------------------------------------------------------------------------
 // O6 covariance adaptation (reading R14)
 // ---------------------------------------------------------------------------------------------
@@ -735,6 +747,61 @@ int32_t oracle_step_aies(void* h, int64_t B, double* theta, double* logp, uint64
         const int64_t j = other0 + (int64_t)(((uint64_t)raw * (uint64_t)half) >> 32);
         const double z = stretch_z(uz, a);
         aies_map(o, theta + i * d, logp[i], theta + j * d, z, newth.data() + r * d, &lpp, &la);
+        newlp[r] = lpp;
+        if (last_log_alpha) last_log_alpha[i] = la;
+        acc[r] = accept_rule(u, la) ? 1 : 0;
+      }
+      for (int64_t r = 0; r < half; ++r)
+        if (acc[r]) {
+          const int64_t i = own0 + r;
+          std::memcpy(theta + i * d, newth.data() + r * d, sizeof(double) * d);
+          logp[i] = newlp[r];
+          n_accept[i] += 1;
+        }
+    }
+    write_trace(o, trace, thin, t, B, theta);
+  }
+  return 0;
+}
+
+// DE move with the ensemble split of R11 (reading R23): every i in half S_h draws j != k uniformly from
+// the OTHER half's current positions.  From the control block (slot 0): word0 -> accept uniform,
+// word2 -> j = other0 + floor(w2 (B/2) / 2^32), word3 -> k' = floor(w3 (B/2 - 1) / 2^32), k = other0 + k'
+// + (k' >= j - other0) (uniform over the B/2 - 1 walkers that are not j); eta = sigma_gamma * (first normal
+// of slot 1).
+void oracle_de_map(void* h, const double* theta_i, double logp_i, const double* theta_j,
+                   const double* theta_k, double gamma, double* theta_p, double* logp_p, double* log_alpha) {
+  de_map(*static_cast<Oracle*>(h), theta_i, logp_i, theta_j, theta_k, gamma, theta_p, logp_p, log_alpha);
+}
+int32_t oracle_step_aies_de(void* h, int64_t B, double* theta, double* logp, uint64_t step0,
+                            int64_t n_steps, uint64_t seed, double sigma_gamma, uint64_t* n_accept,
+                            double* last_log_alpha, double* trace, int32_t thin) {
+  Oracle& o = *static_cast<Oracle*>(h);
+  const int d = o.d;
+  if (B < 4 || (B % 2) != 0 || !(sigma_gamma >= 0.0)) return -1;
+  const int64_t half = B / 2;
+  const double gamma0 = 2.38 / std::sqrt(2.0 * (double)d);
+  for (int64_t t = 0; t < n_steps; ++t) {
+    const uint64_t step = step0 + (uint64_t)t;
+    for (int hh = 0; hh < 2; ++hh) {
+      const int64_t own0 = hh == 0 ? 0 : half, other0 = hh == 0 ? half : 0;
+      std::vector<double> newth((size_t)half * d), newlp(half);
+      std::vector<uint8_t> acc(half);
+#pragma omp parallel for schedule(dynamic, 1)
+      for (int64_t r = 0; r < half; ++r) {
+        const int64_t i = own0 + r;
+        uint32_t w[4];
+        philox_block(seed, (uint64_t)i, step, 0u, w);
+        const double u = u01(w[0]);
+        const int64_t jr = (int64_t)(((uint64_t)w[2] * (uint64_t)half) >> 32);
+        int64_t kr = (int64_t)(((uint64_t)w[3] * (uint64_t)(half - 1)) >> 32);
+        if (kr >= jr) kr += 1;
+        std::vector<double> xi(4 * ((d + 3) / 4));
+        draw_normals(seed, (uint64_t)i, step, d, xi.data());
+        const double gamma = (1.0 + sigma_gamma * xi[0]) * gamma0;
+        double lpp, la;
+        de_map(o, theta + i * d, logp[i], theta + (other0 + jr) * d, theta + (other0 + kr) * d, gamma,
+               newth.data() + r * d, &lpp, &la);
         newlp[r] = lpp;
         if (last_log_alpha) last_log_alpha[i] = la;
         acc[r] = accept_rule(u, la) ? 1 : 0;

@@ -71,6 +71,9 @@ def lib():
         L.oracle_step_mh.argtypes = [vp, i64, dp, dp, u64, i64, u64, C.c_double, u64p, dp, dp, i32]
         L.oracle_step_mala.argtypes = [vp, i64, dp, dp, dp, u64, i64, u64, C.c_double, u64p, dp, dp, i32]
         L.oracle_step_hmc.argtypes = [vp, i64, dp, dp, dp, u64, i64, u64, C.c_double, i32, u64p, dp, dp, i32]
+        L.oracle_de_map.argtypes = [vp, dp, C.c_double, dp, dp, C.c_double, dp, dp, dp]
+        L.oracle_step_aies_de.restype = i32
+        L.oracle_step_aies_de.argtypes = [vp, i64, dp, dp, u64, i64, u64, C.c_double, u64p, dp, dp, i32]
         L.oracle_step_aies.restype = i32
         L.oracle_step_aies.argtypes = [vp, i64, dp, dp, u64, i64, u64, C.c_double, u64p, dp, dp, i32]
         _LIB = L
@@ -240,6 +243,13 @@ class Oracle:
                               C.byref(lpp), C.byref(la))
         return thp, lpp.value, la.value
 
+    def de_map(self, theta_i, logp_i, theta_j, theta_k, gamma):
+        thp = np.zeros(self.d)
+        lpp, la = C.c_double(), C.c_double()
+        lib().oracle_de_map(self._h, _dp(_f64(theta_i)), logp_i, _dp(_f64(theta_j)), _dp(_f64(theta_k)), gamma,
+                            _dp(thp), C.byref(lpp), C.byref(la))
+        return thp, lpp.value, la.value
+
     # ---- chains -------------------------------------------------------------------------------
     def new_state(self, theta0):
         return OracleState(self, theta0)
@@ -353,6 +363,18 @@ class OracleState:
                                     _dp(tr), thin)
         if rc != 0:
             raise ValueError("oracle_step_aies: bad arguments")
+        self.step += n_steps
+        self.n_evals += self.B * n_steps
+        return tr
+
+    def step_aies_de(self, n_steps, seed, sigma_gamma=1e-5, thin=0):
+        """Differential-evolution move, eq (2.16) (SURVEY 8(f)#3, reading R23)."""
+        tr = self._trace(n_steps, thin)
+        rc = lib().oracle_step_aies_de(self.o._h, self.B, _dp(self.theta), _dp(self.logp), self.step,
+                                       n_steps, seed, sigma_gamma, self._u64p(), _dp(self.last_log_alpha),
+                                       _dp(tr), thin)
+        if rc != 0:
+            raise ValueError("oracle_step_aies_de: bad arguments")
         self.step += n_steps
         self.n_evals += self.B * n_steps
         return tr

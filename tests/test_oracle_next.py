@@ -236,3 +236,99 @@ def test_burn_in_finds_optimal_mh_scale_and_covariance(oracle_mod):
     z = np.linalg.solve(np.linalg.cholesky(w.Sigma), th_best - w.mu)
     assert lp_best == pytest.approx(-0.5 * z @ z, abs=1e-9) and z @ z < 0.5 * d   # the best of 512 chains lies well inside the typical set (E z.z = d)
     assert o.adapt_stats() == (3, 0)
+
+
+# ---- differential-evolution move, eq (2.16) (reading R23) -------------------------------
+def test_de_map_is_eq_2_16(oracle_mod):
+    w = WL.tiny(n_chains=8, seed=3, d=3, hidden=(8, 8), mlp_scale=0.7)
+    o = oracle_mod.Oracle(w)
+    xi, xj, xk = (w.theta0[n].astype(np.float64) for n in range(3))
+    lp = o.logp_grad(np.stack([xi]), want_grad=False)[0][0]
+    g = 0.61
+    thp, lpp, la = o.de_map(xi, lp, xj, xk, g)
+    np.testing.assert_allclose(thp, xi + g * (xj - xk), rtol=0, atol=1e-15)
+    assert lpp == pytest.approx(o.logp_grad(thp[None, :], want_grad=False)[0][0], abs=1e-13)
+    assert la == pytest.approx(lpp - lp, abs=1e-13)                       # symmetric proposal: no extra factor
+    # swapping j and k proposes the mirror image
+    thm, _, _ = o.de_map(xi, lp, xk, xj, g)
+    np.testing.assert_allclose(thm - xi, -(thp - xi), rtol=0, atol=1e-15)
+
+
+def test_de_partners_distinct_uniform_from_other_half(oracle_mod):
+    """σ_γ = 0 ⇒ x' − x_i = 2.38/√(2d)·(x_j − x_k) exactly: recover (j, k) of every walker by brute force over
+    all ordered pairs of the ensemble; they must be two different walkers of the complementary half, uniform."""
+    d, B = 2, 24
+    w = WL.gaussian(d, B, seed=6)
+    w.lo = w.hi = None
+    w.mu = w.Sigma_inv = None                      # flat target: every proposal is accepted
+    o = oracle_mod.Oracle(w)
+    g0 = 2.38 / math.sqrt(2 * d)
+    half = B // 2
+    counts = np.zeros((half, half), dtype=np.int64)
+    n_steps = 400
+    for step in range(n_steps):
+        st = o.new_state(w.theta0)
+        st.step = step
+        before = st.theta.copy()
+        st.step_aies_de(1, 99, sigma_gamma=0.0)
+        # half 0 moved against the untouched half 1
+        D = before[:, None, :] - before[None, :, :]                       # all ordered pairs x_j − x_k
+        for i in range(half):
+            disp = (st.theta[i] - before[i]) / g0
+            hit = np.abs(D - disp).max(axis=-1) < 1e-12
+            np.fill_diagonal(hit, False)
+            hits = np.argwhere(hit)
+            assert len(hits) == 1, (step, i, hits)
+            j, k = hits[0]
+            assert j >= half and k >= half
+            counts[j - half, k - half] += 1
+    assert np.all(np.diag(counts) == 0)
+    off = counts[~np.eye(half, dtype=bool)]
+    expect = n_steps * half / (half * (half - 1))
+    chi2 = float(((off - expect) ** 2 / expect).sum())
+    dof = half * (half - 1) - 1
+    assert abs(chi2 - dof) < 5.0 * math.sqrt(2.0 * dof), (chi2, dof)
+
+
+def test_de_gamma_distribution(oracle_mod):
+    """γ = (1 + η)·2.38/√(2d), η ~ N(0, σ_γ): ratio of the displacement to (x_j − x_k) has that mean and sd."""
+    d, B = 3, 8
+    w = WL.gaussian(d, B, seed=7)
+    w.lo = w.hi = None
+    w.mu = w.Sigma_inv = None
+    o = oracle_mod.Oracle(w)
+    g0, sg = 2.38 / math.sqrt(2 * d), 0.3
+    gam = []
+    for step in range(1500):
+        a, b = o.new_state(w.theta0), o.new_state(w.theta0)
+        a.step = b.step = step
+        a.step_aies_de(1, 5, sigma_gamma=0.0)
+        b.step_aies_de(1, 5, sigma_gamma=sg)
+        da, db = a.theta[:B // 2] - w.theta0[:B // 2], b.theta[:B // 2] - w.theta0[:B // 2]
+        gam.append(g0 * (db * da).sum(axis=1) / (da * da).sum(axis=1))      # same (j, k), different γ
+    gam = np.concatenate(gam)
+    n = gam.size
+    assert abs(gam.mean() - g0) < 4.0 * g0 * sg / math.sqrt(n)
+    assert abs(gam.std() - g0 * sg) < 4.0 * g0 * sg / math.sqrt(2 * n)
+
+
+def test_de_moments_anisotropic_gaussian(oracle_mod):
+    """Stationarity: closed-form Gaussian moments within 4 MC standard errors (a spurious Jacobian factor in
+    log α, or j = k allowed, biases the variance)."""
+    d, B = 4, 512
+    w = WL.gaussian(d, B, seed=15, cond=100.0)
+    w.lo = w.hi = None
+    o = oracle_mod.Oracle(w)
+    st = o.new_state(w.theta0)
+    st.step_aies_de(200, 8, sigma_gamma=0.1)
+    tr = st.step_aies_de(600, 8, sigma_gamma=0.1, thin=6)          # [100, B, d]
+    acc = st.n_accept.mean() / 800
+    assert 0.1 < acc < 0.7, acc
+    # walkers of one ensemble are not independent: blocks of time as the replicates
+    blocks = tr.reshape(10, 10 * B, d)
+    m = blocks.mean(axis=1)
+    se = m.std(axis=0, ddof=1) / math.sqrt(10)
+    assert np.all(np.abs(m.mean(axis=0) - w.mu) < 4.0 * se + 1e-12)
+    v = ((blocks - w.mu) ** 2).mean(axis=1)
+    se_v = v.std(axis=0, ddof=1) / math.sqrt(10)
+    assert np.all(np.abs(v.mean(axis=0) - np.diag(w.Sigma)) < 4.0 * se_v)
