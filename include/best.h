@@ -118,6 +118,17 @@ int best_step_hmc(best_ctx* ctx, best_state* st, int64_t n_traj, uint64_t seed, 
 int best_step_aies(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, float a,
                    float* trace_dev, int32_t thin, void* stream);
 
+/* the Differential Evolution move of the ensemble sampler, eq (2.16):
+ *   x_i' = x_i + gamma (x_j - x_k),  gamma = (1 + eta) 2.38 / sqrt(2 d),  eta ~ N(0, sigma_gamma).
+ * Same ensemble split, update order, state, trace and step counter as best_step_aies (half 0 against
+ * the current half 1, then half 1 against the updated half 0; one step = B forward evaluations).
+ * DESIGN.md reading R23: j != k are drawn uniformly from the OTHER half (control block words 2, 3),
+ * eta = sigma_gamma * (first normal of slot 1); the proposal is symmetric, so
+ * log alpha = log pi(x') - log pi(x_i).  No whitening.
+ * Errors: BEST_ERR_ARG for sigma_gamma < 0 (0 is allowed: fixed gamma), odd or < 4 walker count.     */
+int best_step_aies_de(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, float sigma_gamma,
+                      float* trace_dev, int32_t thin, void* stream);
+
 /* Running covariance adaptation (A9; reading R14).  While adapt_every > 0 the
  * MH/MALA/HMC steps of `st` accumulate n, Σθ, Σθθᵀ (fp64) of the post-accept states of all chains;
  * every adapt_every steps  C = scatter/(n−1),  C_ii *= (1+jitter),  L = chol(C)  is computed ON

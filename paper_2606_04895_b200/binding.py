@@ -24,7 +24,7 @@ EXPORTS = [
     "best_step_mh", "best_step_mala", "best_step_hmc", "best_step_aies", "best_set_adaptation",
     "best_adapt_stats", "best_get_whitening", "best_set_whitening", "best_state_get",
     "best_state_get_f64", "best_state_last_log_alpha", "best_state_set", "best_launch_count",
-    "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box", "best_burn_in",
+    "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box", "best_burn_in", "best_step_aies_de",
 ]
 
 
@@ -72,6 +72,7 @@ def lib():
     L.best_step_mala.argtypes = [vp, vp, i64, u64, f32, vp, i32, vp]
     L.best_step_hmc.argtypes = [vp, vp, i64, u64, f32, i32, vp, i32, vp]
     L.best_step_aies.argtypes = [vp, vp, i64, u64, f32, vp, i32, vp]
+    L.best_step_aies_de.argtypes = [vp, vp, i64, u64, f32, vp, i32, vp]
     L.best_set_adaptation.argtypes = [vp, vp, i32, C.c_double]
     L.best_adapt_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
     L.best_get_whitening.argtypes = [vp, vp]
@@ -230,6 +231,10 @@ class State:
 
     def step_aies(self, n_steps, seed, a=2.0, trace=None, thin=0, stream=0):
         _check(lib().best_step_aies(self.ctx._h, self._h, n_steps, seed, a, _ptr(trace), thin, stream or None))
+
+    def step_aies_de(self, n_steps, seed, sigma_gamma=1e-5, trace=None, thin=0, stream=0):
+        _check(lib().best_step_aies_de(self.ctx._h, self._h, n_steps, seed, sigma_gamma, _ptr(trace), thin,
+                                       stream or None))
 
     def set_adaptation(self, adapt_every, jitter=1e-6):
         _check(lib().best_set_adaptation(self.ctx._h, self._h, adapt_every, jitter))

@@ -226,19 +226,22 @@ int best_state_last_log_alpha(best_state* st, double* log_alpha, void* stream) {
 }
 
 static int run_step(best_ctx* ctx, best_state* st, int method, int64_t n, uint64_t seed, float eps,
-                    int nl, float* trace, int thin, void* stream) {
+                    int nl, float* trace, int thin, void* stream, bool de = false) {
   BEST_TRY(check_step_args(ctx, st, n, trace, thin));
   cudaStream_t s = (cudaStream_t)stream;
   if (method != M_AIES && !(eps > 0.f)) { set_error("step: eps must be > 0"); return BEST_ERR_ARG; }
   if (method == M_HMC && nl < 1) { set_error("hmc: n_leapfrog must be >= 1"); return BEST_ERR_ARG; }
-  if (method == M_AIES) {
+  if (method == M_AIES && de) {
+    if (!(eps >= 0.f)) { set_error("aies_de: sigma_gamma must be >= 0"); return BEST_ERR_ARG; }
+    if (st->B < 4 || (st->B & 1)) { set_error("aies_de: walker count must be even and >= 4"); return BEST_ERR_ARG; }
+  } else if (method == M_AIES) {
     if (!(eps > 1.f)) { set_error("aies: a must be > 1"); return BEST_ERR_ARG; }
     if (st->B < 2 || (st->B & 1)) { set_error("aies: walker count must be even and >= 2"); return BEST_ERR_ARG; }
   }
   if (n == 0) return BEST_OK;
   int rc;
   if (ctx->precision == BEST_PREC_BF16) {
-    rc = tc_step(ctx, st, method, n, seed, eps, nl, trace, thin, s);
+    rc = tc_step(ctx, st, method, n, seed, eps, nl, trace, thin, s, de);
   } else {
     if ((method == M_MALA || method == M_HMC) && !st->grad_valid) {
       BEST_TRY(eval_target_soa(ctx, st->theta, st->B, st->B, st->logp, st->grad, s));
@@ -248,7 +251,7 @@ static int run_step(best_ctx* ctx, best_state* st, int method, int64_t n, uint64
       case M_MH: rc = step_mh(ctx, st, n, seed, eps, trace, thin, s); st->grad_valid = false; break;
       case M_MALA: rc = step_mala(ctx, st, n, seed, eps, trace, thin, s); break;
       case M_HMC: rc = step_hmc(ctx, st, n, seed, eps, nl, trace, thin, s); break;
-      default: rc = step_aies(ctx, st, n, seed, eps, trace, thin, s); st->grad_valid = false; break;
+      default: rc = step_aies(ctx, st, n, seed, eps, trace, thin, s, de); st->grad_valid = false; break;
     }
   }
   if (rc) return rc;
@@ -272,6 +275,10 @@ int best_step_hmc(best_ctx* ctx, best_state* st, int64_t n_traj, uint64_t seed, 
 int best_step_aies(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, float a,
                    float* trace_dev, int32_t thin, void* stream) {
   return run_step(ctx, st, M_AIES, n_steps, seed, a, 0, trace_dev, thin, stream);
+}
+int best_step_aies_de(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, float sigma_gamma,
+                      float* trace_dev, int32_t thin, void* stream) {
+  return run_step(ctx, st, M_AIES, n_steps, seed, sigma_gamma, 0, trace_dev, thin, stream, true);
 }
 
 int best_set_adaptation(best_ctx* ctx, best_state* st, int32_t adapt_every, double jitter) {

@@ -132,7 +132,7 @@ int eval_target_soa(best_ctx* ctx, const double* theta, int64_t ld, int64_t n, d
 int step_mh(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cudaStream_t);
 int step_mala(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cudaStream_t);
 int step_hmc(best_ctx*, best_state*, int64_t, uint64_t, double, int, float*, int, cudaStream_t);
-int step_aies(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cudaStream_t);
+int step_aies(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cudaStream_t, bool de = false);
 int adapt_reset(best_ctx* ctx, best_state* st, cudaStream_t s);
 // after step index t of a call: trace slot (every `thin` steps) and covariance accumulation / update
 int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin, bool adapt, cudaStream_t s);

@@ -186,6 +186,41 @@ __global__ void k_aies_accept(Chains S, uint64_t seed, uint64_t step, double a, 
   }
 }
 
+// Differential-evolution move, eq (2.16) (reading R23): x' = x_i + gamma (x_j - x_k),
+// j != k from the other half (control words 2 and 3), gamma = (1 + sigma * n0) 2.38 / sqrt(2 d) with n0
+// the first normal of slot 1; symmetric proposal, log alpha = log pi(x') - log pi(x_i).
+__global__ void k_de_propose(Chains S, uint64_t seed, uint64_t step, double sigma, int64_t own0,
+                             int64_t oth0, int64_t half) {
+  const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (r >= half) return;
+  const int64_t i = own0 + r;
+  const uint4 w = philox4x32_10((uint32_t)i, step, 0u, seed);
+  const int64_t jr = (int64_t)__umulhi(w.z, (uint32_t)half);
+  int64_t kr = (int64_t)__umulhi(w.w, (uint32_t)(half - 1));
+  if (kr >= jr) kr += 1;
+  const uint4 wn = philox4x32_10((uint32_t)i, step, 1u, seed);
+  double n0, n1;
+  box_muller(wn.x, wn.y, n0, n1);
+  const double gamma = (1.0 + sigma * n0) * (2.38 / sqrt(2.0 * (double)S.d));
+  const int64_t j = oth0 + jr, k = oth0 + kr;
+  for (int q = 0; q < S.d; ++q)
+    S.p_theta[q * S.B + r] = S.theta[q * S.B + i] + gamma * (S.theta[q * S.B + j] - S.theta[q * S.B + k]);
+}
+
+__global__ void k_de_accept(Chains S, uint64_t seed, uint64_t step, int64_t own0, int64_t half) {
+  const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (r >= half) return;
+  const int64_t i = own0 + r;
+  const uint4 w = philox4x32_10((uint32_t)i, step, 0u, seed);
+  const double la = S.p_logp[r] - S.logp[i];
+  S.last_la[i] = la;
+  if (accept_rule<double>(u01<double>(w.x), la)) {
+    for (int q = 0; q < S.d; ++q) S.theta[q * S.B + i] = S.p_theta[q * S.B + r];
+    S.logp[i] = S.p_logp[r];
+    S.n_accept[i] += 1ull;
+  }
+}
+
 __global__ void k_trace(const double* __restrict__ theta, int64_t B, int d, float* __restrict__ out) {
   const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (c >= B) return;
@@ -385,7 +420,7 @@ int step_hmc(best_ctx* ctx, best_state* st, int64_t n_traj, uint64_t seed, doubl
 }
 
 int step_aies(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, double a, float* trace,
-              int thin, cudaStream_t s) {
+              int thin, cudaStream_t s, bool de) {
   Chains S = chains_of(st);
   const int64_t half = st->B / 2;
   const int nb = nblocks(half);
@@ -393,10 +428,12 @@ int step_aies(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, dou
     const uint64_t step = st->step + (uint64_t)t;
     for (int hh = 0; hh < 2; ++hh) {
       const int64_t own0 = hh == 0 ? 0 : half, oth0 = hh == 0 ? half : 0;
-      k_aies_propose<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, oth0, half);
+      if (de) k_de_propose<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, oth0, half);   // a = sigma_gamma
+      else k_aies_propose<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, oth0, half);
       count_launch();
       BEST_TRY(eval_target_soa(ctx, st->p_theta, st->B, half, st->p_logp, nullptr, s));
-      k_aies_accept<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, half);
+      if (de) k_de_accept<<<nb, TPB, 0, s>>>(S, seed, step, own0, half);
+      else k_aies_accept<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, half);
       count_launch();
     }
     BEST_TRY(after_step(ctx, st, t, trace, thin, false, s));

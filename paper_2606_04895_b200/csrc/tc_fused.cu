@@ -148,6 +148,7 @@ struct Run {
   const float* in_rows; float* out_logp; float* out_grad;
   // AIES
   int64_t own0, oth0;
+  int de;               // differential-evolution move (eq 2.16) instead of the stretch move; eps = sigma_gamma
 };
 
 // shared-memory carve-up (dynamic, 1024-byte aligned base)

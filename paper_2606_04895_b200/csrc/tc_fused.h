@@ -10,5 +10,5 @@ int tc_logp_grad(best_ctx* ctx, const float* theta_rows, int64_t n, float* logp,
                  cudaStream_t s);
 int tc_state_init(best_ctx* ctx, best_state* st, cudaStream_t s);
 int tc_step(best_ctx* ctx, best_state* st, int method, int64_t n_steps, uint64_t seed, float eps,
-            int n_leapfrog, float* trace, int thin, cudaStream_t s);
+            int n_leapfrog, float* trace, int thin, cudaStream_t s, bool de = false);
 }  // namespace best

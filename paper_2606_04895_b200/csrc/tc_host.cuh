@@ -51,7 +51,21 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
     const float t = u01<float>(w.y) * (a - 1.0f) + 1.0f;
     const float z = t * t / a;
     float thp[8], g[8], lpp;
-    {
+    if (R.de) {
+      // eq (2.16), reading R23: x' = x_i + gamma (x_j - x_k), k != j from the same half, R.eps = sigma_gamma
+      int64_t kr = (int64_t)__umulhi(w.w, (uint32_t)(R.B - 1));
+      if (kr >= j - R.oth0) kr += 1;
+      const uint4 wn = philox4x32_10((uint32_t)i, R.step0, 1u, R.seed);
+      float n0, n1;
+      box_muller(wn.x, wn.y, n0, n1);
+      const float gamma = (1.0f + R.eps * n0) * (2.38f / sqrtf(2.0f * (float)d));
+      float thi[8], thj[8], thk[8];
+      load_vec8(C, R.theta, R.ld, i, d, valid, thi);
+      load_vec8(C, R.theta, R.ld, j, d, valid, thj);
+      load_vec8(C, R.theta, R.ld, R.oth0 + kr, d, valid, thk);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) thp[q] = thi[q] + gamma * (thj[q] - thk[q]);
+    } else {
       float thi[8], thj[8];
       load_vec8(C, R.theta, R.ld, i, d, valid, thi);
       load_vec8(C, R.theta, R.ld, j, d, valid, thj);
@@ -59,7 +73,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
       for (int q = 0; q < 8; ++q) thp[q] = thj[q] + z * (thi[q] - thj[q]);
     }
     eval_target<ROWS>(C, thp, false, lpp, g);
-    const float la = (float)(d - 1) * logf(z) + lpp - (valid ? (float)R.logp[i] : 0.0f);
+    const float la = (R.de ? 0.0f : (float)(d - 1) * logf(z)) + lpp - (valid ? (float)R.logp[i] : 0.0f);
     const bool acc = valid && accept_rule<float>(u01<float>(w.x), la);
     qbar(C);   // (warp-uniform) every thread of the chain has read logp[i] before the leader overwrites it
     if (acc) store_vec8(C, R.theta, R.ld, i, d, thp);
@@ -672,12 +686,13 @@ int tc_state_init(best_ctx* ctx, best_state* st, cudaStream_t s) {
 }
 
 int tc_step(best_ctx* ctx, best_state* st, int method, int64_t n_steps, uint64_t seed, float eps,
-            int n_leapfrog, float* trace, int thin, cudaStream_t s) {
+            int n_leapfrog, float* trace, int thin, cudaStream_t s, bool de) {
   if ((method == tc::M_MALA || method == tc::M_HMC) && !st->grad_valid) BEST_TRY(tc_state_init(ctx, st, s));
   tc::Run R{};
   R.method = method; R.io_mode = tc::IO_SOA_F64;
   R.want_grad = (method == tc::M_MALA || method == tc::M_HMC) ? 1 : 0;
   R.B = st->B; R.ld = st->B; R.seed = seed; R.eps = eps; R.n_leapfrog = n_leapfrog;
+  R.de = de ? 1 : 0;
   R.theta = st->theta; R.grad = st->grad; R.logp = st->logp; R.last_la = st->last_la; R.n_accept = st->n_accept;
   const bool adapt = ctx->adapt_every > 0 && method != tc::M_AIES;
   int64_t t0 = 0;

@@ -234,6 +234,14 @@ def test_N1_hard_box_single_step(B, O, method, kw):
     ctx.close()
 
 
+@pytest.mark.parametrize("net", ["lcdm", "sterile"])
+def test_N3_de_single_step(B, O, net):
+    """SURVEY 8(f)#3, eq (2.16) on the tensor-core path (512-wide pairs / 1024-wide pairs)."""
+    w = WL.lcdm(n_chains=1024 + 40) if net == "lcdm" else WL.sterile(n_chains=1062)
+    info = _single_step_stat(B, O, w, "aies_de", seed=31, sigma_gamma=0.2)
+    assert 0.02 < info["accept_rate"] < 0.999, info
+
+
 def test_N2_burn_in_reaches_target_acceptance(B):
     """SURVEY 8(f)#2 on the tensor-core path: after the loop a fresh run accepts at the target rate and
     the whitening factor has been replaced once per iteration."""

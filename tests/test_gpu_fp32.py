@@ -178,24 +178,25 @@ def _moments_vs_exact(trace, mu, Sigma, nsig=4.0):
             assert abs(p.mean() - Sigma[i, j]) < nsig * p.std(ddof=1) / math.sqrt(Bn), (i, j)
 
 
-@pytest.mark.parametrize("method", ["mh", "mala", "hmc", "aies"])
+@pytest.mark.parametrize("method", ["mh", "mala", "hmc", "aies", "aies_de"])
 @pytest.mark.parametrize("d", [6, 27])
 def test_T5_gaussian_closed_form_moments(B, method, d):
     import torch
-    if method == "aies" and d == 27:
+    if method.startswith("aies") and d == 27:
         pytest.skip("AIES moment parity is tested at small d (slow mixing at d=27, SURVEY §8(c))")
     w = WL.gaussian(d, 512, seed=40 + d, cond=100.0 if d == 6 else 1e4)
     ctx = B.Context(w, B.PREC_FP32)
     st = ctx.new_state(w.theta0)
     plan = {"mh": (dict(eps=2.4 / math.sqrt(d)), 400, 2400, 4), "mala": (dict(eps=0.5 if d == 6 else 0.3), 100, 800, 2),
-            "hmc": (dict(eps=0.4 if d == 6 else 0.25, n_leapfrog=4), 30, 300, 1), "aies": (dict(a=2.0), 400, 3000, 5)}
+            "hmc": (dict(eps=0.4 if d == 6 else 0.25, n_leapfrog=4), 30, 300, 1), "aies": (dict(a=2.0), 400, 3000, 5),
+            "aies_de": (dict(sigma_gamma=0.1), 400, 3000, 5)}
     kw, burn, n, thin = plan[method]
     getattr(st, "step_" + method)(burn, 11, **kw)
     tr = torch.zeros(n // thin, 512, d, device="cuda")
     getattr(st, "step_" + method)(n, 11, trace=tr, thin=thin, **kw)
     torch.cuda.synchronize()
     trace = tr.cpu().numpy().astype(np.float64)
-    if method == "aies":       # walkers are coupled: batch means over time
+    if method.startswith("aies"):       # walkers are coupled: batch means over time
         xc = (trace - w.mu) / np.sqrt(np.diag(w.Sigma))
         v = (xc ** 2).mean(axis=1).reshape(30, -1, d).mean(axis=1)
         se = v.std(axis=0, ddof=1) / math.sqrt(30)
@@ -377,6 +378,32 @@ def test_N1_hard_box_values_and_invariant(B, O):
         c2.set_hard_box(True)
     assert e.value.code == B.BEST_ERR_ARG
     c2.close()
+    ctx.close()
+
+
+# ---- differential-evolution move, eq (2.16) (R23) ----------------------------------
+@pytest.mark.parametrize("sg", [0.0, 0.3])
+def test_N3_de_single_step(B, O, sg):
+    _single_step(B, O, WL.tiny().with_chains(65536, seed=5), "aies_de", seed=1234, sigma_gamma=sg)
+    _single_step(B, O, WL.sterile(n_chains=1024), "aies_de", seed=9, sigma_gamma=sg)
+
+
+def test_N3_de_split_invariance_and_errors(B):
+    w = WL.tiny().with_chains(300, seed=2)
+    ctx = B.Context(w, B.PREC_FP32)
+    a, b2 = ctx.new_state(w.theta0), ctx.new_state(w.theta0)
+    a.step_aies_de(6, 11, f32(0.2))
+    for _ in range(3):
+        b2.step_aies_de(2, 11, f32(0.2))
+    ga, gb = a.get(want_grad=False), b2.get(want_grad=False)
+    assert np.array_equal(ga["theta"], gb["theta"]) and np.array_equal(ga["n_accept"], gb["n_accept"])
+    assert ga["step"] == 6 and ga["n_accept"].sum() > 0
+    for bad in (lambda: a.step_aies_de(1, 1, -0.1), lambda: ctx.new_state(w.theta0[:2]).step_aies_de(1, 1, 0.1),
+                lambda: ctx.new_state(w.theta0[:7]).step_aies_de(1, 1, 0.1)):
+        with pytest.raises(B.BestError) as e:
+            bad()
+        assert e.value.code == B.BEST_ERR_ARG
+    ctx.new_state(w.theta0[:4]).step_aies_de(2, 1, 0.1)          # the smallest ensemble: two walkers per half
     ctx.close()
 
 
