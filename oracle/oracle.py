@@ -130,6 +130,26 @@ def num_threads() -> int:
     return int(lib().oracle_num_threads())
 
 
+def rminus1(trace) -> float:
+    """Gelman-Rubin type statistic R − 1 of eq (4.1)-(4.2), written out from the
+    text: trace [n][B][d] (n samples of each of B chains).  B = covariance of the chain means (unbiased,
+    over chains), W = mean over chains of the within-chain covariances (unbiased, over samples),
+    d_i = sqrt(B_ii), B~ = D^-1 B D^-1, W~ = D^-1 W D^-1, R − 1 = max_i |lambda_i(W~^-1 B~)|."""
+    x = np.asarray(trace, dtype=np.float64)
+    n, nb, d = x.shape
+    means = x.mean(axis=0)                                        # [B][d]
+    Bm = np.atleast_2d(np.cov(means, rowvar=False, ddof=1))
+    W = np.zeros((d, d))
+    for c in range(nb):
+        W += np.atleast_2d(np.cov(x[:, c, :], rowvar=False, ddof=1))
+    W /= nb
+    dd = np.sqrt(np.diag(Bm))
+    Bt = Bm / np.outer(dd, dd)
+    Wt = W / np.outer(dd, dd)
+    lam = np.linalg.eigvals(np.linalg.inv(Wt) @ Bt)
+    return float(np.max(np.abs(lam)))
+
+
 class Oracle:
     """One target (emulator + Gaussian + banana + box + whitening L) and the sampler steps."""
 

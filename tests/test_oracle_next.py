@@ -332,3 +332,49 @@ def test_de_moments_anisotropic_gaussian(oracle_mod):
     v = ((blocks - w.mu) ** 2).mean(axis=1)
     se_v = v.std(axis=0, ddof=1) / math.sqrt(10)
     assert np.all(np.abs(v.mean(axis=0) - np.diag(w.Sigma)) < 4.0 * se_v)
+
+
+# ---- R − 1 of eq (4.1)-(4.2) --------------------------------------------------------
+def _exact_chains(rng, n, nb, d, W0, c):
+    """Chains whose within-chain covariance is EXACTLY W0 each and whose means have covariance EXACTLY c·W0."""
+    def exact(m, C):
+        z = rng.standard_normal((m, d))
+        z -= z.mean(axis=0)
+        z = z @ np.linalg.inv(np.linalg.cholesky(np.cov(z, rowvar=False, ddof=1)).T)     # sample cov = I
+        return z @ np.linalg.cholesky(C).T
+    means = exact(nb, c * W0)
+    return np.stack([exact(n, W0) + means[k] for k in range(nb)], axis=1)                # [n][B][d]
+
+
+def test_rminus1_closed_forms(oracle_mod):
+    rng = np.random.default_rng(12)
+    d, n, nb = 4, 40, 12
+    A = rng.standard_normal((d, d))
+    W0 = A @ A.T + 0.5 * np.eye(d)
+    for c in (0.01, 0.3, 2.0):
+        tr = _exact_chains(rng, n, nb, d, W0, c)
+        assert oracle_mod.rminus1(tr) == pytest.approx(c, rel=1e-9)                      # B = c W ⇒ every λ = c
+        # affine reparametrisation leaves eig(W⁻¹B) unchanged (the D scaling is a similarity)
+        T = rng.standard_normal((d, d)) + 2.0 * np.eye(d)
+        assert oracle_mod.rminus1(tr @ T.T + rng.standard_normal(d)) == pytest.approx(c, rel=1e-8)
+    # d = 1: var(chain means) / mean(chain variances)
+    x = rng.standard_normal((50, 7, 1)) * np.linspace(0.5, 2.0, 7)[None, :, None] + rng.standard_normal((1, 7, 1))
+    ref = x.mean(axis=0)[:, 0].var(ddof=1) / x[:, :, 0].var(axis=0, ddof=1).mean()
+    assert oracle_mod.rminus1(x) == pytest.approx(ref, rel=1e-12)
+    # B and W diagonal in the same basis with different ratios: the largest ratio
+    ratios = np.array([0.05, 0.7, 0.2])
+    nb2 = 9
+    m = rng.standard_normal((nb2, 3)); m -= m.mean(axis=0)
+    m = m @ np.linalg.inv(np.linalg.cholesky(np.cov(m, rowvar=False, ddof=1)).T) * np.sqrt(ratios)
+    z = rng.standard_normal((30, 3)); z -= z.mean(axis=0)
+    z = z @ np.linalg.inv(np.linalg.cholesky(np.cov(z, rowvar=False, ddof=1)).T)
+    tr = np.stack([z + m[k] for k in range(nb2)], axis=1)
+    assert oracle_mod.rminus1(tr) == pytest.approx(ratios.max(), rel=1e-9)
+
+
+def test_rminus1_mixed_chains_small_unmixed_large(oracle_mod):
+    rng = np.random.default_rng(3)
+    iid = rng.standard_normal((2000, 16, 5))
+    assert oracle_mod.rminus1(iid) < 0.02                         # ~ (d + few)/n for independent draws
+    stuck = iid * 0.1 + 3.0 * rng.standard_normal((1, 16, 5))    # chains far apart relative to their spread
+    assert oracle_mod.rminus1(stuck) > 100.0
