@@ -180,6 +180,16 @@ int best_set_hard_box(best_ctx* ctx, int32_t on);
  * capacity n_iter * ceil(n_adapt / block)) receives the step used in every adaptation block.
  * Synchronises `stream` after every block; leaves adaptation switched off.  The global step counter
  * advances by n_iter * n_steps.                                                                       */
+/* the Gelman-Rubin type convergence statistic R - 1 of PAPER.md eq (4.1)-(4.2), on the
+ * device, from a trace as written by best_step_* (`trace_dev`: device, fp32, [n][B][d]: n samples of each
+ * of B chains).  B = covariance of the chain means, W = mean of the within-chain covariances (both
+ * unbiased), d_i = sqrt(B_ii), R - 1 = max |eig((D^-1 W D^-1)^-1 (D^-1 B D^-1))|.  fp64 accumulation with
+ * a fixed summation order (same trace => same bits).  `*rminus1_host` (host) receives the value.
+ * Synchronises `stream`.  Errors: BEST_ERR_ARG for n < 2, B < 2, d outside 1..32 or a host trace pointer;
+ * BEST_ERR_NOT_SPD (value NaN) if W, in units of the between-chain variance, is not positive definite to
+ * 1e-12 (e.g. a dimension in which no chain ever moved: R - 1 > 1e12 is not resolvable) or some B_ii = 0. */
+int best_rminus1(const float* trace_dev, int64_t n, int64_t B, int32_t d, double* rminus1_host, void* stream);
+
 enum { BEST_METHOD_MH = 0, BEST_METHOD_MALA = 1, BEST_METHOD_HMC = 2 };
 int best_burn_in(best_ctx* ctx, best_state* st, int32_t method, int32_t n_iter, int64_t n_steps,
                  int64_t n_adapt, int64_t block, uint64_t seed, float* eps_inout, float target_accept,

@@ -407,6 +407,56 @@ def test_N3_de_split_invariance_and_errors(B):
     ctx.close()
 
 
+# ---- R - 1 of eq (4.1)-(4.2) on the device ------------------------------------------
+def test_N4_rminus1_matches_oracle(B, O):
+    import torch
+    # (i) a real trace: tiny config, MALA, 256 chains x 200 samples
+    w = WL.tiny().with_chains(256, seed=4)
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(w.theta0)
+    tr = torch.zeros(200, 256, w.d, device="cuda")
+    st.step_mala(200, 3, 0.3, trace=tr, thin=1)
+    torch.cuda.synchronize()
+    r_gpu = B.rminus1(tr)
+    r_ref = O.rminus1(tr.cpu().numpy())
+    assert r_gpu == pytest.approx(r_ref, rel=1e-9) and 0.0 < r_gpu < 1.0
+    assert B.rminus1(tr) == r_gpu                                            # fixed summation order
+    ctx.close()
+    # (ii) sizes of the paper's runs: d = 29, ragged tails in every kernel (4099 chains x 67 samples), chains
+    # displaced by ~ their own spread, correlated dimensions
+    rng = np.random.default_rng(8)
+    d, nb, n = 29, 4099, 67
+    A = rng.standard_normal((d, d)) / math.sqrt(d) + np.eye(d)
+    x = (rng.standard_normal((n, nb, d)) + 0.7 * rng.standard_normal((1, nb, d))) @ A.T + 5.0
+    x32 = x.astype(np.float32)
+    r_gpu = B.rminus1(torch.from_numpy(x32).cuda())
+    assert r_gpu == pytest.approx(O.rminus1(x32), rel=1e-8)
+    # (iii) tiny shapes and d = 1, 32
+    for (n, nb, d) in ((2, 2, 1), (5, 3, 2), (40, 9, 32)):
+        x32 = (rng.standard_normal((n, nb, d)) + rng.standard_normal((1, nb, d))).astype(np.float32)
+        assert B.rminus1(torch.from_numpy(x32).cuda()) == pytest.approx(O.rminus1(x32), rel=1e-8), (n, nb, d)
+    # (iv) stuck ensemble: large value, still accurate
+    x32 = (0.01 * rng.standard_normal((50, 64, 6)) + rng.standard_normal((1, 64, 6))).astype(np.float32)
+    r = B.rminus1(torch.from_numpy(x32).cuda())
+    assert r > 1e3 and r == pytest.approx(O.rminus1(x32), rel=1e-6)
+
+
+def test_N4_rminus1_errors(B):
+    import ctypes as C
+    import torch
+    x = torch.randn(10, 8, 3, device="cuda")
+    for call in (lambda: B.lib().best_rminus1(x.data_ptr(), 1, 8, 3, C.byref(C.c_double()), None),
+                 lambda: B.lib().best_rminus1(x.data_ptr(), 10, 1, 3, C.byref(C.c_double()), None),
+                 lambda: B.lib().best_rminus1(x.data_ptr(), 10, 8, 33, C.byref(C.c_double()), None),
+                 lambda: B.lib().best_rminus1(x.cpu().numpy().ctypes.data, 10, 8, 3, C.byref(C.c_double()), None)):
+        assert call() == B.BEST_ERR_ARG
+    frozen = x.clone()
+    frozen[:, :, 1] = frozen[0:1, :, 1]                 # dimension 1 never moves inside a chain: W_11 = 0
+    with pytest.raises(B.BestError) as e:
+        B.rminus1(frozen)
+    assert e.value.code == B.BEST_ERR_NOT_SPD
+
+
 # ---- burn-in loop (R22) ------------------------------------------------------------
 @pytest.mark.parametrize("method,eps0,delta,nl", [("mh", 0.1, 0.234, 1), ("mala", 0.05, 0.574, 1), ("hmc", 0.05, 0.7, 3)])
 def test_N2_burn_in_matches_oracle(B, O, method, eps0, delta, nl):
