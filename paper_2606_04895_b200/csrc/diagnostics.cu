@@ -23,49 +23,75 @@ __global__ void k_chain_means(const float* __restrict__ trace, int64_t n, int64_
   means[e] = s / (double)n;
 }
 
-// gm[i] = (1/B) sum_c means[c][i]   (one block; thread i sums its dimension in chain order)
+// gm[i] = (1/B) sum_c means[c][i]   (one block of 32 x 32 threads: part p sums the chains c = p mod 32 in
+// order, the 32 parts are then added in order -- a fixed summation order)
 __global__ void k_grand_mean(const double* __restrict__ means, int64_t B, int d, double* __restrict__ gm) {
-  const int i = threadIdx.x;
-  if (i >= d) return;
+  __shared__ double part[32][33];
+  const int i = threadIdx.x & 31, p = threadIdx.x >> 5;
   double s = 0.0;
-  for (int64_t c = 0; c < B; ++c) s += means[c * d + i];
-  gm[i] = s / (double)B;
+  if (i < d)
+    for (int64_t c = p; c < B; c += 32) s += means[c * d + i];
+  part[p][i] = s;
+  __syncthreads();
+  if (p == 0 && i < d) {
+    double t = 0.0;
+    for (int q = 0; q < 32; ++q) t += part[q][i];
+    gm[i] = t / (double)B;
+  }
 }
 
-// acc[blk][i*d + j] = sum over the block's rows of (x_i - ref_i)(x_j - ref_j); rows are [nrows][d]
+// acc[blk][i*d + j] = sum over the block's rows of (x_i - ref_i)(x_j - ref_j); rows are [nrows][d].
+// The rows of a tile sit in SMEM padded to 32 columns (zeros); the 128 threads are two groups of 8 x 8
+// threads, each thread holding a 4 x 4 block of the 32 x 32 Gram matrix in registers (two 32-byte SMEM
+// reads, broadcast inside a warp, per 16 fp64 FMAs) and each group taking every other row of the tile.
+constexpr int G_ROWS = 64;
 template <typename T>
 __global__ void __launch_bounds__(G_TPB)
 k_gram_partial(const T* __restrict__ rows, int64_t nrows, int d, const double* __restrict__ ref,
                double* __restrict__ acc) {
-  extern __shared__ double xs[];  // [G_TPB][d + 1]
-  const int dd = d * d, pitch = d + 1;
-  double mine[(kMaxD * kMaxD + G_TPB - 1) / G_TPB];
+  __shared__ __align__(16) double xs[G_ROWS * kMaxD];
+  const int grp = threadIdx.x >> 6, u = threadIdx.x & 63, ti = u >> 3, tj = u & 7;
+  double a4[4][4];
 #pragma unroll
-  for (int q = 0; q < (kMaxD * kMaxD + G_TPB - 1) / G_TPB; ++q) mine[q] = 0.0;
-  for (int64_t r0 = blockIdx.x * (int64_t)G_TPB; r0 < nrows; r0 += (int64_t)gridDim.x * G_TPB) {
-    const int nv = (int)((nrows - r0 < G_TPB) ? (nrows - r0) : G_TPB);
+  for (int p = 0; p < 4; ++p)
+#pragma unroll
+    for (int q = 0; q < 4; ++q) a4[p][q] = 0.0;
+  for (int e = threadIdx.x; e < G_ROWS * kMaxD; e += G_TPB) xs[e] = 0.0;   // the padding columns stay zero
+  for (int64_t r0 = blockIdx.x * (int64_t)G_ROWS; r0 < nrows; r0 += (int64_t)gridDim.x * G_ROWS) {
+    const int nv = (int)((nrows - r0 < G_ROWS) ? (nrows - r0) : G_ROWS);
     __syncthreads();
-    for (int e = threadIdx.x; e < nv * d; e += G_TPB) {   // contiguous, coalesced
+    for (int e = threadIdx.x; e < G_ROWS * d; e += G_TPB) {   // contiguous, coalesced
       const int r = e / d, i = e - r * d;
-      xs[r * pitch + i] = (double)rows[r0 * d + e] - ref[i];
+      xs[r * kMaxD + i] = (r < nv) ? (double)rows[r0 * d + e] - ref[i] : 0.0;
     }
     __syncthreads();
+    for (int r = grp; r < nv; r += 2) {
+      const double2* pa = reinterpret_cast<const double2*>(xs + r * kMaxD + 4 * ti);
+      const double2* pb = reinterpret_cast<const double2*>(xs + r * kMaxD + 4 * tj);
+      const double2 a01 = pa[0], a23 = pa[1], b01 = pb[0], b23 = pb[1];
+      const double a[4] = {a01.x, a01.y, a23.x, a23.y}, b[4] = {b01.x, b01.y, b23.x, b23.y};
 #pragma unroll
-    for (int q = 0; q < (kMaxD * kMaxD + G_TPB - 1) / G_TPB; ++q) {
-      const int e = threadIdx.x + q * G_TPB;
-      if (e < dd) {
-        const int i = e / d, j = e - i * d;
-        double s = 0.0;
-        for (int r = 0; r < nv; ++r) s += xs[r * pitch + i] * xs[r * pitch + j];
-        mine[q] += s;
-      }
+      for (int p = 0; p < 4; ++p)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) a4[p][q] = fma(a[p], b[q], a4[p][q]);
     }
   }
+  // group 1 hands its block to group 0 through SMEM (fixed order: g0 + g1)
+  __syncthreads();
+  if (grp == 1)
 #pragma unroll
-  for (int q = 0; q < (kMaxD * kMaxD + G_TPB - 1) / G_TPB; ++q) {
-    const int e = threadIdx.x + q * G_TPB;
-    if (e < dd) acc[(size_t)blockIdx.x * dd + e] = mine[q];
-  }
+    for (int p = 0; p < 4; ++p)
+#pragma unroll
+      for (int q = 0; q < 4; ++q) xs[(4 * ti + p) * kMaxD + 4 * tj + q] = a4[p][q];
+  __syncthreads();
+  if (grp == 0)
+#pragma unroll
+    for (int p = 0; p < 4; ++p)
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int i = 4 * ti + p, j = 4 * tj + q;
+        if (i < d && j < d) acc[(size_t)blockIdx.x * d * d + i * d + j] = a4[p][q] + xs[i * kMaxD + j];
+      }
 }
 
 // out[0] = R - 1, out[1] = status (0 ok, 1 W~ not positive definite / B_ii = 0)
@@ -80,87 +106,108 @@ __global__ void k_rminus1_finalize(const double* __restrict__ accS, int nblkS, c
     S[e] = s; M[e] = m;
   }
   __syncthreads();
-  if (threadIdx.x != 0) return;
-  bool ok = true;
-  // W~ into S, B~ into M (symmetrised)
-  for (int i = 0; i < d; ++i)
-    for (int j = 0; j <= i; ++j) {
-      const double mij = 0.5 * (M[i * d + j] + M[j * d + i]), sij = 0.5 * (S[i * d + j] + S[j * d + i]);
-      const double bij = mij / (nb - 1.0), wij = (sij - n * mij) / (nb * (n - 1.0));
-      A[i * d + j] = A[j * d + i] = bij;
-      Lc[i * d + j] = Lc[j * d + i] = wij;
-    }
-  for (int i = 0; i < d; ++i) if (!(A[i * d + i] > 0.0)) ok = false;
-  if (ok) {
+  if (threadIdx.x >= 32) return;          // one warp does the dense d x d algebra (lane = row / column)
+  const int lane = threadIdx.x;
+  __shared__ int ok_s;
+  if (lane == 0) {
+    bool ok = true;
+    // B into A, W into Lc (symmetrised)
     for (int i = 0; i < d; ++i)
-      for (int j = 0; j < d; ++j) {
-        const double sc = sqrt(A[i * d + i]) * sqrt(A[j * d + j]);
-        M[i * d + j] = A[i * d + j] / sc;
-        S[i * d + j] = Lc[i * d + j] / sc;
+      for (int j = 0; j <= i; ++j) {
+        const double mij = 0.5 * (M[i * d + j] + M[j * d + i]), sij = 0.5 * (S[i * d + j] + S[j * d + i]);
+        const double bij = mij / (nb - 1.0), wij = (sij - n * mij) / (nb * (n - 1.0));
+        A[i * d + j] = A[j * d + i] = bij;
+        Lc[i * d + j] = Lc[j * d + i] = wij;
       }
-    // Cholesky W~ = L L^T (lower, in Lc)
-    for (int j = 0; j < d && ok; ++j) {
-      double s = S[j * d + j];
-      for (int k = 0; k < j; ++k) s -= Lc[j * d + k] * Lc[j * d + k];
-      // W~ is in units of the between-chain variance: a pivot below 1e-12 means R - 1 > 1e12, which the
-      // fp64 cancellation S - n M cannot resolve (a dimension in which no chain moved), or a singular W
-      if (!(s > 1e-12) || !(s > 1e-13 * S[j * d + j])) { ok = false; break; }
-      const double ljj = sqrt(s);
-      Lc[j * d + j] = ljj;
-      for (int i = j + 1; i < d; ++i) {
-        double t = S[i * d + j];
-        for (int k = 0; k < j; ++k) t -= Lc[i * d + k] * Lc[j * d + k];
-        Lc[i * d + j] = t / ljj;
+    for (int i = 0; i < d; ++i) if (!(A[i * d + i] > 0.0)) ok = false;
+    if (ok) {
+      for (int i = 0; i < d; ++i)
+        for (int j = 0; j < d; ++j) {
+          const double sc = sqrt(A[i * d + i]) * sqrt(A[j * d + j]);
+          M[i * d + j] = A[i * d + j] / sc;   // B~
+          S[i * d + j] = Lc[i * d + j] / sc;  // W~
+        }
+      // Cholesky W~ = L L^T (lower, in Lc)
+      for (int j = 0; j < d && ok; ++j) {
+        double s = S[j * d + j];
+        for (int k = 0; k < j; ++k) s -= Lc[j * d + k] * Lc[j * d + k];
+        // W~ is in units of the between-chain variance: a pivot below 1e-12 means R - 1 > 1e12, which the
+        // fp64 cancellation S - n M cannot resolve (a dimension in which no chain moved), or a singular W
+        if (!(s > 1e-12) || !(s > 1e-13 * S[j * d + j])) { ok = false; break; }
+        const double ljj = sqrt(s);
+        Lc[j * d + j] = ljj;
+        for (int i = j + 1; i < d; ++i) {
+          double t = S[i * d + j];
+          for (int k = 0; k < j; ++k) t -= Lc[i * d + k] * Lc[j * d + k];
+          Lc[i * d + j] = t / ljj;
+        }
       }
     }
+    ok_s = ok ? 1 : 0;
   }
-  if (!ok) { out[0] = nan(""); out[1] = 1.0; return; }
-  // A = L^-1 B~ L^-T : first Y = L^-1 B~ (columns), then A = Y L^-T  <=>  A^T = L^-1 Y^T
-  for (int c = 0; c < d; ++c)
+  __syncwarp();
+  if (!ok_s) {
+    if (lane == 0) { out[0] = nan(""); out[1] = 1.0; }
+    return;
+  }
+  // A = L^-1 B~ L^-T : Y = L^-1 B~ (lane = column), then row r of the result solves L z = Y[r][:]^T (lane = row)
+  if (lane < d) {
+    const int c = lane;
     for (int i = 0; i < d; ++i) {
       double t = M[i * d + c];
       for (int k = 0; k < i; ++k) t -= Lc[i * d + k] * A[k * d + c];
       A[i * d + c] = t / Lc[i * d + i];
     }
-  for (int r = 0; r < d; ++r)      // row r of Y: solve L z = Y[r][:]^T, store as row r of the result
+  }
+  __syncwarp();
+  if (lane < d) {
+    const int r = lane;
     for (int i = 0; i < d; ++i) {
       double t = A[r * d + i];
       for (int k = 0; k < i; ++k) t -= Lc[i * d + k] * S[r * d + k];
       S[r * d + i] = t / Lc[i * d + i];
     }
-  for (int i = 0; i < d; ++i)
-    for (int j = 0; j <= i; ++j) A[i * d + j] = A[j * d + i] = 0.5 * (S[i * d + j] + S[j * d + i]);
-  // cyclic Jacobi on the symmetric A
+  }
+  __syncwarp();
+  if (lane < d)
+    for (int j = 0; j < d; ++j) A[lane * d + j] = 0.5 * (S[lane * d + j] + S[j * d + lane]);
+  __syncwarp();
+  // cyclic Jacobi on the symmetric A; every lane computes the same rotation, lane k updates row / column k
   for (int sweep = 0; sweep < 60; ++sweep) {
     double off = 0.0, diag = 0.0;
-    for (int i = 0; i < d; ++i) {
+    for (int i = 0; i < d; ++i) {       // same fixed-order sums on every lane
       diag += A[i * d + i] * A[i * d + i];
       for (int j = 0; j < i; ++j) off += A[i * d + j] * A[i * d + j];
     }
     if (off <= 1e-30 * diag || off == 0.0) break;
     for (int p = 0; p < d - 1; ++p)
       for (int q = p + 1; q < d; ++q) {
-        const double apq = A[p * d + q];
+        const double apq = A[p * d + q], app = A[p * d + p], aqq = A[q * d + q];
+        __syncwarp();
         if (apq == 0.0) continue;
-        const double theta = (A[q * d + q] - A[p * d + p]) / (2.0 * apq);
+        const double theta = (aqq - app) / (2.0 * apq);
         const double t = (theta >= 0.0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
         const double cs = 1.0 / sqrt(t * t + 1.0), sn = t * cs;
-        for (int k = 0; k < d; ++k) {   // columns p, q
-          const double akp = A[k * d + p], akq = A[k * d + q];
-          A[k * d + p] = cs * akp - sn * akq;
-          A[k * d + q] = sn * akp + cs * akq;
+        if (lane < d) {   // columns p, q of row `lane`
+          const double akp = A[lane * d + p], akq = A[lane * d + q];
+          A[lane * d + p] = cs * akp - sn * akq;
+          A[lane * d + q] = sn * akp + cs * akq;
         }
-        for (int k = 0; k < d; ++k) {   // rows p, q
-          const double apk = A[p * d + k], aqk = A[q * d + k];
-          A[p * d + k] = cs * apk - sn * aqk;
-          A[q * d + k] = sn * apk + cs * aqk;
+        __syncwarp();
+        if (lane < d) {   // rows p, q of column `lane`
+          const double apk = A[p * d + lane], aqk = A[q * d + lane];
+          A[p * d + lane] = cs * apk - sn * aqk;
+          A[q * d + lane] = sn * apk + cs * aqk;
         }
+        __syncwarp();
       }
   }
-  double best = 0.0;
-  for (int i = 0; i < d; ++i) best = fmax(best, fabs(A[i * d + i]));
-  out[0] = best;
-  out[1] = 0.0;
+  if (lane == 0) {
+    double best = 0.0;
+    for (int i = 0; i < d; ++i) best = fmax(best, fabs(A[i * d + i]));
+    out[0] = best;
+    out[1] = 0.0;
+  }
 }
 
 }  // namespace
@@ -178,8 +225,8 @@ extern "C" int best_rminus1(const float* trace_dev, int64_t n, int64_t B, int32_
   cudaStream_t s = (cudaStream_t)stream;
   const int dd = d * d;
   const int64_t row = B * (int64_t)d;
-  const int nblkS = (int)std::min<int64_t>((n * B + G_TPB - 1) / G_TPB, 1184);
-  const int nblkM = (int)std::min<int64_t>((B + G_TPB - 1) / G_TPB, 148);
+  const int nblkS = (int)std::min<int64_t>((n * B + G_ROWS - 1) / G_ROWS, 592);   // 4 CTAs per SM
+  const int nblkM = (int)std::min<int64_t>((B + G_ROWS - 1) / G_ROWS, 148);
   double* buf = nullptr;
   const size_t n_means = (size_t)row, n_tot = n_means + (size_t)d + (size_t)(nblkS + nblkM) * dd + 2;
   BEST_TRY(dev_alloc(&buf, n_tot));
@@ -187,10 +234,9 @@ extern "C" int best_rminus1(const float* trace_dev, int64_t n, int64_t B, int32_
          *out = accM + (size_t)nblkM * dd;
   auto done = [&](int rc) { cudaFree(buf); return rc; };
   k_chain_means<<<(unsigned)((row + 255) / 256), 256, 0, s>>>(trace_dev, n, row, means);
-  k_grand_mean<<<1, 32, 0, s>>>(means, B, d, gm);
-  const size_t smem = sizeof(double) * G_TPB * (d + 1);
-  k_gram_partial<float><<<nblkS, G_TPB, smem, s>>>(trace_dev, n * B, d, gm, accS);
-  k_gram_partial<double><<<nblkM, G_TPB, smem, s>>>(means, B, d, gm, accM);
+  k_grand_mean<<<1, 1024, 0, s>>>(means, B, d, gm);
+  k_gram_partial<float><<<nblkS, G_TPB, 0, s>>>(trace_dev, n * B, d, gm, accS);
+  k_gram_partial<double><<<nblkM, G_TPB, 0, s>>>(means, B, d, gm, accM);
   k_rminus1_finalize<<<1, 256, 0, s>>>(accS, nblkS, accM, nblkM, d, (double)n, (double)B, out);
   count_launch(5);
   double h[2] = {0.0, 0.0};
