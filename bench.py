@@ -93,6 +93,8 @@ def run_steps(st, spec, n, seed, stream=0):
         st.step_mh(n, seed, spec["eps"], stream=stream)
     elif m == "hmc":
         st.step_hmc(n, seed, spec["eps"], spec["n_leapfrog"], stream=stream)
+    elif m == "aies_de":
+        st.step_aies_de(n, seed, spec.get("sigma_gamma", 0.1), stream=stream)
     else:
         st.step_aies(n, seed, spec.get("a", 2.0), stream=stream)
 
@@ -371,6 +373,38 @@ def main():
                                          "tflops": flops_per_chain_step(rr["w"], sp) * v / 1e12,
                                          "accept_rate": rr["accept_rate"], "sampler_steps": n_steps}
         extra["sweep_adapt500"] = sweep
+        # DE move on the AIES config, the burn-in loop on the default config, R - 1 of a trace
+        sp = dict(WORKLOADS["aies"], method="aies_de", sigma_gamma=0.1)
+        rr = measure(sp, n_x, 3, with_e2e=False)
+        v = sp["n_chains"] * sp["inner"] / (rr["ms_total"] / n_x * 1e-3)
+        extra["aies_de"] = {"chain_steps_per_s": v, "tflops": flops_per_chain_step(rr["w"], sp) * v / 1e12,
+                            "ms_per_step": rr["ms_total"] / n_x, "accept_rate": rr["accept_rate"], "inner": sp["inner"]}
+        w = make_workload(spec, spec["n_chains"])
+        w.L = np.diag(np.sqrt(np.diag(w.Sigma)))
+        ctx = B.Context(w, prec)
+        st = ctx.new_state(w.theta0)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        eps, _, _, hist = st.burn_in("mala", 3, 600, 200, 10, 7, 0.05, 0.574)
+        torch.cuda.synchronize()
+        el = time.perf_counter() - t0
+        tr = torch.zeros(500, w.n_chains, w.d, device="cuda")
+        a0 = st.get(want_grad=False)["n_accept"].sum()
+        st.step_mala(500, 7, eps, trace=tr, thin=1)
+        torch.cuda.synchronize()
+        acc = float((st.get(want_grad=False)["n_accept"].sum() - a0) / (500 * w.n_chains))
+        B.rminus1(tr)
+        t0 = time.perf_counter()
+        r1 = B.rminus1(tr)
+        t_r = time.perf_counter() - t0
+        extra["burn_in"] = {"config": "default workload from a diagonal whitening: 3 iterations x 600 MALA steps, "
+                                      "200 of them adapting the step in blocks of 10, target acceptance 0.574",
+                            "wall_s": el, "chain_steps_per_s": 3 * 600 * w.n_chains / el, "eps": eps,
+                            "adaptation_blocks": int(len(hist)), "accept_rate_after": acc}
+        extra["rminus1"] = {"trace": [500, int(w.n_chains), int(w.d)], "value": r1, "ms": 1e3 * t_r,
+                            "GB_per_s": tr.numel() * 4 / t_r / 1e9}
+        st.close()
+        ctx.close()
         line["extra"] = extra
     if rank == 0:
         print(json.dumps(line))
