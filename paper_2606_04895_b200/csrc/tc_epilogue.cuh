@@ -252,6 +252,21 @@ __device__ __forceinline__ int pair_jn(const OpDesc& op, int c, int half, int gr
   return op.paired ? c * (op.ncols >> 6) + grp * 2 + half : c * (op.ncols >> 6) + half * ngrp + grp;
 }
 
+// Order in which a thread walks the 64-column groups of an N-chunk.  BEST_TC_STAGGER (off): the warps of the
+// odd row quarters swap neighbouring groups, so that half of the epilogue warps are in their TMEM-load /
+// MUFU phase while the other half stores (single-CTA in-place tiles only; the pair kernels' issue order
+// relies on rounds completing consecutive k-chunks).  Measured A/B on B200, 16k chains on 27->512^4->1:
+// HMC -4 %, MALA -2 %, MH +0.7 % -- the first k-chunk of the next operand completes a round later, which
+// costs more than the phase overlap gains.
+#ifndef BEST_TC_STAGGER
+#define BEST_TC_STAGGER 0
+#endif
+template <int ROWS>
+__device__ __forceinline__ int stagger(const EpiCtx& C, int g0, int ngrp) {
+  if (BEST_TC_STAGGER && ROWS == 128 && (ngrp & 1) == 0) return g0 ^ (int)((C.row >> 5) & 1u);
+  return g0;
+}
+
 // forward epilogue of one op
 template <int ACT, bool LAST, int ROWS>
 __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_grad, f32x2& acc2,
@@ -267,7 +282,8 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
     const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && writes_a && (c != op.nch - 1);
-    for (int grp = 0; grp < ngrp; ++grp) {
+    for (int g0 = 0; g0 < ngrp; ++g0) {
+      const int grp = stagger<ROWS>(C, g0, ngrp);
       const int jn = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, grp, ngrp) : c * ngrp + grp;
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
@@ -277,7 +293,7 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
         if (gate) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
         store_a<ROWS>(C, jn, hp);
         publish_a<ROWS>(C, jn, 1);
-        written = jn + 1;
+        written = max(written, jn + 1);
       }
     }
     if ((!Geo<ROWS>::kInPlace) && writes_a) {   // this N-chunk of the next operand is in the L2 image
@@ -314,20 +330,22 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
     const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
     const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && (c != op.nch - 1);
     // act' of the first group can be fetched before the accumulator is complete
-    const int jn0 = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, 0, ngrp) : c * ngrp;
     const int jstep = (Geo<ROWS>::kPair && op.paired) ? 2 : 1;
+    const int jnc = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, 0, ngrp) : c * ngrp;   // group 0 of this chunk
+    const int jn0 = jnc + stagger<ROWS>(C, 0, ngrp) * jstep;
     const uint8_t* dp = dact_l + (size_t)jn0 * kDBlk;
     uint4 a0 = ptx::ldg_128(dp), a1 = ptx::ldg_128(dp + kDPiece);
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
-    for (int grp = 0; grp < ngrp; ++grp) {
-      const int jn = jn0 + grp * jstep;
+    for (int g0 = 0; g0 < ngrp; ++g0) {
+      const int grp = stagger<ROWS>(C, g0, ngrp);
+      const int jn = jnc + grp * jstep;
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
       const uint4 d0 = a0, d1 = a1;
-      if (grp + 1 < ngrp) {   // prefetch the next group's act'
-        const uint8_t* dn = dact_l + (size_t)(jn + jstep) * kDBlk;
+      if (g0 + 1 < ngrp) {   // prefetch the next group's act'
+        const uint8_t* dn = dact_l + (size_t)(jnc + stagger<ROWS>(C, g0 + 1, ngrp) * jstep) * kDBlk;
         a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
       }
       ptx::tmem_ld_wait();
@@ -335,7 +353,7 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
       if (gate) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
       store_a<ROWS>(C, jn, hp);
       publish_a<ROWS>(C, jn, 1);
-      written = jn + 1;
+      written = max(written, jn + 1);
     }
     if (!Geo<ROWS>::kInPlace) {
       ptx::fence_proxy_async_all();

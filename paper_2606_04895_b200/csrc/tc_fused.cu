@@ -164,9 +164,8 @@ struct SmemLayout {
   static constexpr int VECS = RTMAT + 1024 * 4;                      // mu, lo, hi, 1/width: 4x32 floats
   static constexpr int PART = VECS + 4 * 32 * 4;                     // partial sums [2][4][128] floats
   static constexpr int BARS = PART + 2 * 4 * 128 * 4;
-  // barriers: full[8] empty[8] a_ready[16] a_free[16] d_full[4] d_free[4] epi_done[4] xin_done and, for
-  // the CTA-pair kernel, the leader's copies of the peer's full[8] a_ready[16] d_free[4]
-  static constexpr int NBARS = 89;
+  // barriers: full[8] empty[8] a_ready[16] a_free[16] d_full[4] d_free[4] epi_done[4] xin_done
+  static constexpr int NBARS = 61;
   static constexpr int TMEMPTR = BARS + NBARS * 8;
   static constexpr int TOTAL = TMEMPTR + 16;
 };
@@ -182,9 +181,6 @@ struct Bars {  // mbarrier addresses are computed, never looked up (keeps them o
   __device__ __forceinline__ uint32_t d_free(int b) const { return base + 8u * (52 + b); }
   __device__ __forceinline__ uint32_t epi_done(int c) const { return base + 8u * (56 + c); }
   __device__ __forceinline__ uint32_t xin_done() const { return base + 8u * 60; }
-  __device__ __forceinline__ uint32_t full_peer(int i) const { return base + 8u * (61 + i); }
-  __device__ __forceinline__ uint32_t a_ready_peer(int j) const { return base + 8u * (69 + j); }
-  __device__ __forceinline__ uint32_t d_free_peer(int b) const { return base + 8u * (85 + b); }
 };
 __device__ __forceinline__ Bars make_bars(uint32_t base) { Bars b; b.base = base; return b; }
 
@@ -323,9 +319,11 @@ __device__ void loader_loop(const Params& P, const Bars& bars, uint32_t a_base, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// CTA-pair roles (Geo<264>).  Both CTAs run the producer (own half of every weight tile, own 8 x 8 KB
-// ring) and the epilogue; the leader (cluster rank 0) issues the MMAs, the other CTA's warp 1 relays
-// the completion of ITS full / a_ready / d_free barriers to the leader's *_peer copies.
+// CTA-pair roles (Geo<264>, Geo<265>).  Both CTAs run the producer and the epilogue; the leader (cluster
+// rank 0) issues the MMAs.  Every barrier the issuer waits on lives in the LEADER's shared memory: each
+// CTA's producer loads its own half of a weight stage with 2-SM tensor copies that credit the leader's
+// full barrier, and the peer's epilogue threads arrive on the leader's a_ready / d_free directly
+// (shared::cluster address with the rank bit cleared).
 // ------------------------------------------------------------------------------------------------
 __device__ void producer_loop_pair(const Params& P, const Bars& bars, uint32_t stage_base, uint32_t rank,
                                    int64_t n_evals, int n_ops) {

@@ -237,19 +237,17 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
 
   if (tid == 0) {
     for (int i = 0; i < 8; ++i) {
-      ptx::mbar_init(bars.full(i), 1); ptx::mbar_init(bars.empty(i), 1); ptx::mbar_init(bars.full_peer(i), 1);
+      ptx::mbar_init(bars.full(i), 1); ptx::mbar_init(bars.empty(i), 1);
     }
     for (int i = 0; i < kMaxKch; ++i) {
       // arrivals per phase: in place = every epilogue thread (pair: the 256 of the lane half that owns the
       // k-chunk); L2-image tiles = warp 3 alone (+ the bulk copy's bytes)
       ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : kEpiThreads);   // pair: 256 of each CTA
       ptx::mbar_init(bars.a_free(i), Geo<ROWS>::kPair ? 2 : 1);   // pair kernels: two issuing warps
-      ptx::mbar_init(bars.a_ready_peer(i), 1);
     }
     for (int i = 0; i < 4; ++i) {
       ptx::mbar_init(bars.d_full(i), 1);
       ptx::mbar_init(bars.d_free(i), Geo<ROWS>::kPair ? 2 * kEpiThreads : Geo<ROWS>::kEpiActive);   // pair: both CTAs
-      ptx::mbar_init(bars.d_free_peer(i), 1);
     }
     for (int i = 0; i < 4; ++i) ptx::mbar_init(bars.epi_done(i), Geo<ROWS>::kEpiActive);
     ptx::mbar_init(bars.xin_done(), Geo<ROWS>::kEpiActive);
