@@ -23,8 +23,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures (profiles/r1c_ncu_full.md, r1e_ncu_full.md); None where no capture exists.
-NCU_TRAFFIC_BYTES = {("lcdm_mala", 100, "bf16"): 5.255424e6 + 0.453888e6,      # r1e, best_tc_kernel<1,265>
+# `ncu --set full` captures (profiles/r1c_ncu_full.md, r1e_ncu_full.md, r1f_ncu_full.md); None where no capture exists.
+NCU_TRAFFIC_BYTES = {("lcdm_mala", 100, "bf16"): 5.281792e6 + 0.275968e6,      # r1f, best_tc_kernel<1,233>
                      ("hmc", 1, "bf16"): 10.798848e6 + 9.035520e6,           # r1c, best_tc_kernel<2,128>
                      ("aies", 1, "bf16"): 14.427904e6 + 0.0}                 # r1e, per half-ensemble launch
 
@@ -39,6 +39,9 @@ WORKLOADS = {
     "sterile_mh_16k": dict(cfg=4, make="sterile", n_chains=16384, mlp_scale=1.0, method="mh", eps=0.3, inner=20),
     "sterile_hmc_16k": dict(cfg=4, make="sterile", n_chains=16384, mlp_scale=1.0, method="hmc", eps=0.03, n_leapfrog=8, inner=4),
     "lcdm256_hmc": dict(cfg=2, make="lcdm", hidden=256, n_chains=16384, mlp_scale=3.0, method="hmc", eps=0.1, n_leapfrog=16, inner=8),
+    # small-batch (latency / L2-bound) points of configs[4], for the ncu captures in profiles/r1f_small_batch.md
+    "sterile_mala_1k": dict(cfg=4, make="sterile", n_chains=1024, mlp_scale=1.0, method="mala", eps=0.01, inner=100),
+    "sterile_mala_64": dict(cfg=4, make="sterile", n_chains=64, mlp_scale=1.0, method="mala", eps=0.01, inner=100),
     "tiny_mala": dict(cfg=0, make="tiny", n_chains=64, mlp_scale=0.1, method="mala", eps=0.3, inner=100),
 }
 
@@ -100,7 +103,7 @@ def run_steps(st, spec, n, seed, stream=0):
 
 
 class ClockSampler(threading.Thread):
-    """nvidia-smi clocks / throttle reasons while the timed region runs (B200_PROFILING.md)."""
+    """SM clocks / throttle reasons while the timed region runs (B200_PROFILING.md): NVML, else nvidia-smi."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -108,14 +111,38 @@ class ClockSampler(threading.Thread):
         super().__init__(daemon=True)
         self.index, self.rows, self._stop_evt = index, [], threading.Event()
 
+    def _nvml(self):
+        """NVML handle for fast sampling (a query takes < 1 ms; an nvidia-smi process ~100 ms, longer than
+        the whole timed region of a short run).  None when pynvml is not usable: nvidia-smi is then polled."""
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            return pynvml, pynvml.nvmlDeviceGetHandleByIndex(self.index)
+        except Exception:
+            return None
+
     def run(self):
+        nv = self._nvml()
         while not self._stop_evt.is_set():
             try:
+                if nv is not None:
+                    nvml, h = nv
+                    try:
+                        rs = nvml.nvmlDeviceGetCurrentClocksEventReasons(h)
+                    except Exception:
+                        rs = nvml.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                    bits = (nvml.nvmlClocksThrottleReasonHwSlowdown, nvml.nvmlClocksThrottleReasonHwThermalSlowdown,
+                            nvml.nvmlClocksThrottleReasonSwThermalSlowdown, nvml.nvmlClocksThrottleReasonSwPowerCap)
+                    self.rows.append([str(nvml.nvmlDeviceGetClockInfo(h, nvml.NVML_CLOCK_SM)),
+                                      str(nvml.nvmlDeviceGetMaxClockInfo(h, nvml.NVML_CLOCK_SM))]
+                                     + ["Active" if rs & b else "Not Active" for b in bits])
+                    self._stop_evt.wait(0.005)
+                    continue
                 out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
                                       "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
                 self.rows.append([x.strip() for x in out.strip().split(",")])
             except Exception:
-                pass
+                nv = None
             self._stop_evt.wait(0.1)
 
     def stop(self):
@@ -129,10 +156,11 @@ class ClockSampler(threading.Thread):
                 "reasons": reasons, "samples": len(sm)}
 
 
-def cpu_baseline(spec, budget_s=12.0):
+def cpu_baseline(spec, budget_s=12.0, n_sample=None):
     """The oracle as it stands, timed on the host cores on a bounded sample of the same workload."""
     from oracle import oracle as O
-    n_sample = 256 if spec["make"] != "tiny" else 64
+    if n_sample is None:
+        n_sample = 256 if spec["make"] != "tiny" else 64
     w = make_workload(spec, n_sample)
     o = O.Oracle(w)
     ost = o.new_state(w.theta0)
@@ -337,7 +365,7 @@ def main():
         "roofline": {"bound": "tensor" if args.precision == "bf16" else "alu", "achieved": achieved_tf,
                      "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
                      "traffic": NCU_TRAFFIC_BYTES.get((args.workload, inner, args.precision)) if spec["n_chains"] == WORKLOADS[args.workload]["n_chains"] else None,
-                     "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1e_ncu_full.md)",
+                     "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1f_ncu_full.md; hmc r1c, aies r1e)",
                      "peak_source": peak_src,
                      "frac_of_sustained": (achieved_tf / peaks["bf16_tflops_sustained"]) if peaks and args.precision == "bf16" else None,
                      "kernel": "best_tc_kernel<%s>" % spec["method"], "flops_per_launch": flops_per_launch},
@@ -372,7 +400,34 @@ def main():
                 sweep[f"{meth}_{nb}"] = {"chain_steps_per_s": v, "ms_per_sampler_step": rr["ms_total"] / n_steps,
                                          "tflops": flops_per_chain_step(rr["w"], sp) * v / 1e12,
                                          "accept_rate": rr["accept_rate"], "sampler_steps": n_steps}
+        # the oracle beside the curve (north_star: "a chain-steps/s vs batch-size curve reported against the
+        # oracle"): B = 1 and 64 chains in full for ~1.5 s each, and 256 chains for MH / MALA -- OpenMP over
+        # chains saturates the host cores well before that, so the 256-chain figure also stands for 1k..65k
+        if not args.no_cpu_baseline:
+            orc = {}
+            for meth, kw, nbs in (("mh", dict(eps=0.3), (1, 64, 256)), ("mala", dict(eps=0.01), (1, 64, 256)),
+                                  ("hmc", dict(eps=0.03, n_leapfrog=8), (1, 64))):
+                for nb in nbs:
+                    sp = dict(cfg=4, make="sterile", n_chains=nb, mlp_scale=1.0, method=meth, **kw)
+                    cb = cpu_baseline(sp, budget_s=1.5, n_sample=nb)
+                    orc[f"{meth}_{nb}"] = {"chain_steps_per_s": cb["value"], "sample": cb["sample"]}
+            orc["cores"] = cb["cores"]
+            sweep["oracle"] = orc
         extra["sweep_adapt500"] = sweep
+        # Small-batch path: every 128-chain tile (one CTA pair) streams the forward and the
+        # backward weight pack from L2 once per evaluation: algorithmic bytes = tiles x 2|W| per MALA step,
+        # |W| = 2 B x MACs (bf16, unpadded).  Denominator: best_probe_l2_read (148 CTAs re-reading a 32 MiB
+        # buffer that stays in the 126 MB L2, 16-byte loads, 20 passes, best of 3).
+        l2_gbs = max(B.probe_l2_read(32 << 20, 20) for _ in range(3))
+        small = {"l2_resident_read_GB_per_s": l2_gbs, "hbm_copy_GB_per_s": peaks.get("hbm_gbs")}
+        for nb in (1, 64, 1024):
+            k = sweep[f"mala_{nb}"]
+            tiles = (nb + 127) // 128
+            by = tiles * 2 * 2 * rr["w"].macs
+            gbs = by / (k["ms_per_sampler_step"] * 1e-3) / 1e9
+            small[f"mala_{nb}"] = {"tiles": tiles, "weight_bytes_per_step": by, "ms_per_sampler_step": k["ms_per_sampler_step"],
+                                   "achieved_l2_GB_per_s": gbs, "frac_of_l2_read": gbs / l2_gbs}
+        extra["small_batch"] = small
         # DE move on the AIES config, the burn-in loop on the default config, R - 1 of a trace
         sp = dict(WORKLOADS["aies"], method="aies_de", sigma_gamma=0.1)
         rr = measure(sp, n_x, 3, with_e2e=False)

@@ -190,6 +190,15 @@ int best_set_hard_box(best_ctx* ctx, int32_t on);
  * 1e-12 (e.g. a dimension in which no chain ever moved: R - 1 > 1e12 is not resolvable) or some B_ii = 0. */
 int best_rminus1(const float* trace_dev, int64_t n, int64_t B, int32_t d, double* rminus1_host, void* stream);
 
+/* Measurement aid for the small-batch roofline ("measure the box's L2 bandwidth with a
+ * resident-copy microbenchmark"; the small-batch path streams the weight packs from L2, sec. 3.1
+ * "evaluating the emulator for up to 100 points simultaneously does not affect the evaluation time").
+ * One CTA of 512 threads per SM reads a freshly allocated device buffer of `bytes` (1 MiB..96 MiB, multiple
+ * of 8 KiB: resident in the 126 MB L2 after an untimed first pass) `passes` times with 16-byte loads;
+ * `*gb_per_s_host` (host) receives bytes * passes * CTAs / CUDA-event time.  Allocates and frees its buffer,
+ * synchronises `stream`.  Errors: BEST_ERR_ARG (sizes), BEST_ERR_CUDA.                                    */
+int best_probe_l2_read(int64_t bytes, int32_t passes, double* gb_per_s_host, void* stream);
+
 enum { BEST_METHOD_MH = 0, BEST_METHOD_MALA = 1, BEST_METHOD_HMC = 2 };
 int best_burn_in(best_ctx* ctx, best_state* st, int32_t method, int32_t n_iter, int64_t n_steps,
                  int64_t n_adapt, int64_t block, uint64_t seed, float* eps_inout, float target_accept,

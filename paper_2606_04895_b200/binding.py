@@ -24,7 +24,7 @@ EXPORTS = [
     "best_step_mh", "best_step_mala", "best_step_hmc", "best_step_aies", "best_set_adaptation",
     "best_adapt_stats", "best_get_whitening", "best_set_whitening", "best_state_get",
     "best_state_get_f64", "best_state_last_log_alpha", "best_state_set", "best_launch_count",
-    "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box", "best_burn_in", "best_step_aies_de", "best_rminus1",
+    "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box", "best_burn_in", "best_step_aies_de", "best_rminus1", "best_probe_l2_read",
 ]
 
 
@@ -80,6 +80,7 @@ def lib():
     L.best_set_step_scale.argtypes = [vp, vp]
     L.best_set_hard_box.argtypes = [vp, i32]
     L.best_rminus1.argtypes = [vp, i64, i64, i32, C.POINTER(C.c_double), vp]
+    L.best_probe_l2_read.argtypes = [i64, i32, C.POINTER(C.c_double), vp]
     L.best_burn_in.argtypes = [vp, vp, i32, i32, i64, i64, i64, u64, C.POINTER(C.c_float), C.c_float, i32,
                                C.c_double, vp, C.POINTER(C.c_double), vp, vp]
     L.best_state_get.argtypes = [vp, vp, vp, vp, C.POINTER(u64), vp, C.POINTER(u64), vp]
@@ -203,6 +204,13 @@ def rminus1(trace, stream=0) -> float:
         raise ValueError("trace must be contiguous")
     out = C.c_double()
     _check(lib().best_rminus1(_ptr(trace), n, nb, d, C.byref(out), stream or None))
+    return out.value
+
+
+def probe_l2_read(n_bytes=32 << 20, passes=20, stream=0) -> float:
+    """best_probe_l2_read: GB/s of all SMs re-reading an L2-resident buffer."""
+    out = C.c_double()
+    _check(lib().best_probe_l2_read(n_bytes, passes, C.byref(out), stream or None))
     return out.value
 
 

@@ -213,7 +213,67 @@ __global__ void k_rminus1_finalize(const double* __restrict__ accS, int nblkS, c
 }  // namespace
 }  // namespace best
 
+namespace best {
+namespace {
+// L2 read-bandwidth probe: every CTA sweeps the WHOLE buffer `passes` times with 16-byte loads, each CTA
+// starting at its own offset so that the CTAs do not walk in lockstep.  After the first touch the buffer is
+// served from L2 (callers keep it well below the 126 MB).  The xor keeps the loads alive.
+__global__ void __launch_bounds__(512) k_l2_read_probe(const uint4* __restrict__ buf, int64_t n16, int passes,
+                                                       unsigned* __restrict__ sink) {
+  unsigned acc = 0;
+  const int64_t start = ((int64_t)blockIdx.x * 7919 * 512) % n16;
+  for (int p = 0; p < passes; ++p) {
+    for (int64_t i0 = 0; i0 < n16; i0 += 512 * 4) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        int64_t i = start + i0 + (int64_t)u * 512 + threadIdx.x;
+        if (i >= n16) i -= n16;
+        if (i < n16) {
+          const uint4 v = __ldcg(buf + i);
+          acc ^= v.x ^ v.y ^ v.z ^ v.w;
+        }
+      }
+    }
+  }
+  if (acc == 0x9E3779B9u) sink[0] = acc;   // practically never; defeats dead-code elimination
+}
+}  // namespace
+}  // namespace best
+
 using namespace best;
+
+extern "C" int best_probe_l2_read(int64_t bytes, int32_t passes, double* gb_per_s_host, void* stream) {
+  if (!gb_per_s_host || bytes < (1 << 20) || bytes > (96ll << 20) || (bytes & 8191) || passes < 1 || passes > 1000) {
+    set_error("best_probe_l2_read: 1 MiB <= bytes <= 96 MiB (multiple of 8 KiB), 1 <= passes <= 1000");
+    return BEST_ERR_ARG;
+  }
+  cudaStream_t s = (cudaStream_t)stream;
+  int dev = 0, n_sm = 0;
+  BEST_CUDA(cudaGetDevice(&dev));
+  BEST_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  unsigned char* buf = nullptr;
+  BEST_TRY(dev_alloc(&buf, (size_t)bytes + 16));
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  auto done = [&](int rc) { cudaFree(buf); if (e0) cudaEventDestroy(e0); if (e1) cudaEventDestroy(e1); return rc; };
+  unsigned* sink = reinterpret_cast<unsigned*>(buf + bytes);
+  float ms = 0.0f;
+  if (cudaMemsetAsync(buf, 1, (size_t)bytes + 16, s) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess ||
+      cudaEventCreate(&e1) != cudaSuccess) { set_error("best_probe_l2_read: CUDA failure"); return done(BEST_ERR_CUDA); }
+  const int64_t n16 = bytes / 16;
+  k_l2_read_probe<<<n_sm, 512, 0, s>>>(reinterpret_cast<const uint4*>(buf), n16, 1, sink);   // first touch
+  cudaEventRecord(e0, s);
+  k_l2_read_probe<<<n_sm, 512, 0, s>>>(reinterpret_cast<const uint4*>(buf), n16, passes, sink);
+  cudaEventRecord(e1, s);
+  count_launch(2);
+  if (cudaGetLastError() != cudaSuccess || cudaEventSynchronize(e1) != cudaSuccess ||
+      cudaEventElapsedTime(&ms, e0, e1) != cudaSuccess) {
+    set_error("best_probe_l2_read: CUDA failure");
+    cudaGetLastError();
+    return done(BEST_ERR_CUDA);
+  }
+  *gb_per_s_host = (double)bytes * (double)passes * (double)n_sm / ((double)ms * 1e-3) / 1e9;
+  return done(BEST_OK);
+}
 
 extern "C" int best_rminus1(const float* trace_dev, int64_t n, int64_t B, int32_t d, double* rminus1_host,
                             void* stream) {

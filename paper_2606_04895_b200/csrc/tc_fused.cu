@@ -45,16 +45,22 @@ constexpr int kRows = 128;           // TMEM lanes == MMA M
 //                CTA (lanes 64..127 hold the upper half of N for the same 64 rows), so a whole
 //                1024-wide layer of accumulators fits TMEM and the operand is rewritten in place.
 template <int ROWS> struct Geo {
-  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32 || ROWS == 264 || ROWS == 265, "tile geometry");
-  static constexpr bool kPair = (ROWS == 264 || ROWS == 265);
+  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32 || ROWS == 264 || ROWS == 265 || ROWS == 233, "tile geometry");
+  static constexpr bool kPair = (ROWS == 264 || ROWS == 265 || ROWS == 233);
   // ROWS = 265: CTA pair for 512-wide layers.  64 chains per CTA need only 64 KB of operand and 256
   // TMEM columns per layer, so BOTH are double-buffered: an op reads operand buffer (op & 1) and its
   // epilogue writes the other one, accumulators alternate between two sets of TMEM columns.  No
   // in-place hazard is left: the next op's MMAs start on the first finished k-chunk while this op's
   // epilogue is still running.
-  static constexpr bool kPingPong = (ROWS == 265);
-  static constexpr bool kInPlace = (ROWS == 128 || ROWS == 264 || ROWS == 265);   // operand stays in SMEM
-  static constexpr int kTileRows = kPair ? 64 : ROWS;
+  // ROWS = 233: geometry 265 with only 32 CHAINS per CTA (rows 32..63 of the CTA's 64 MMA rows are phantom:
+  // never written, their accumulator lanes never read).  The epilogue warps of the phantom row quarter do
+  // nothing at all, so the 8 working warps have two issue slots per scheduler cycle pair to themselves and a
+  // batch too small to fill the chip with 64-chain CTAs (4096 chains = 64 CTAs) spreads over twice the SMs.
+  static constexpr bool kPingPong = (ROWS == 265 || ROWS == 233);
+  static constexpr bool kInPlace = (ROWS == 128 || ROWS == 264 || ROWS == 265 || ROWS == 233);   // operand stays in SMEM
+  static constexpr int kTileRows = kPair ? 64 : ROWS;   // rows of the CTA's operand / act' blocks
+  static constexpr int kChains = (ROWS == 233) ? 32 : kTileRows;   // chains the CTA advances
+  static constexpr int kEpiArrive = (ROWS == 233) ? 256 : 512;      // epilogue threads that run (per CTA)
   static constexpr int kAChunk = kTileRows * 128;      // bytes of one 64-column k-chunk
   static constexpr int kEpiActive = kPair ? 512 : ROWS * 4;   // epilogue threads with MLP epilogue work
   static constexpr int kNBuf = kPair ? 4 : 2;          // accumulator buffers

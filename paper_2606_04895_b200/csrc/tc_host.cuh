@@ -12,7 +12,7 @@ template <int METHOD, int ROWS>
 __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
   const Params& P = *C.P;
   const int d = P.d;
-  const int64_t r_in_launch = (int64_t)blockIdx.x * Geo<ROWS>::kTileRows + C.row;
+  const int64_t r_in_launch = (int64_t)blockIdx.x * Geo<ROWS>::kChains + C.row;
   const bool valid = r_in_launch < R.B;
   const bool lead = valid && C.k == 0;
 
@@ -242,12 +242,12 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     for (int i = 0; i < kMaxKch; ++i) {
       // arrivals per phase: in place = every epilogue thread (pair: the 256 of the lane half that owns the
       // k-chunk); L2-image tiles = warp 3 alone (+ the bulk copy's bytes)
-      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : kEpiThreads);   // pair: 256 of each CTA
+      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : Geo<ROWS>::kEpiArrive);   // pair: half of each CTA's
       ptx::mbar_init(bars.a_free(i), Geo<ROWS>::kPair ? 2 : 1);   // pair kernels: two issuing warps
     }
     for (int i = 0; i < 4; ++i) {
       ptx::mbar_init(bars.d_full(i), 1);
-      ptx::mbar_init(bars.d_free(i), Geo<ROWS>::kPair ? 2 * kEpiThreads : Geo<ROWS>::kEpiActive);   // pair: both CTAs
+      ptx::mbar_init(bars.d_free(i), Geo<ROWS>::kPair ? 2 * Geo<ROWS>::kEpiArrive : Geo<ROWS>::kEpiActive);   // pair: both CTAs
     }
     for (int i = 0; i < 4; ++i) ptx::mbar_init(bars.epi_done(i), Geo<ROWS>::kEpiActive);
     ptx::mbar_init(bars.xin_done(), Geo<ROWS>::kEpiActive);
@@ -341,13 +341,15 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     asm volatile("" : "+r"(C.a_thr0), "+r"(C.a_thr1), "+r"(C.bias_thr), "+r"(C.wouts_thr), "+r"(C.v_thr),
                       "+r"(C.tmem_lane), "+r"(C.sbase), "+l"(C.dact_thr));
 #endif
-    if (Geo<ROWS>::kPair && C.half == 1) {
+    if (C.row >= Geo<ROWS>::kChains) {
+      // phantom rows (geometry 233: the odd row quarters; L2-image tiles: lanes ROWS..127): nothing to do
+    } else if (Geo<ROWS>::kPair && C.half == 1) {
       // upper lane half of a CTA pair: MLP epilogues only, in step with the sampler threads
       const float th0[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
       float gm[8], op_;
       for (int64_t e = 0; e < n_evals; ++e) tc_eval<ROWS>(C, th0, R.want_grad != 0, op_, gm);
-    } else if (C.row < Geo<ROWS>::kTileRows) {
-      sampler_thread<METHOD, ROWS>(C, R);   // lanes kTileRows..127 are phantom rows
+    } else {
+      sampler_thread<METHOD, ROWS>(C, R);
     }
   }
   ptx::tc_fence_before();
@@ -377,6 +379,7 @@ struct TcPlan {
   size_t dact_cap = 0, aimg_cap = 0;
   int n_sm = 0;
   bool no_pair = false;  // BEST_TC_ROWS=64|32 forces the single-CTA L2-image geometries
+  bool no_233 = false;   // BEST_TC_NO233 (environment, read at best_create): A/B measurements of geometry 233
   int force_rows = 0;   // BEST_TC_ROWS=128|64|32 (environment, read at best_create): measurements only
 };
 
@@ -411,9 +414,9 @@ uint16_t f32_to_bf16(float f) {  // round to nearest even
 template <int METHOD, int ROWS>
 int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
   TcPlan* pl = ctx->tc;
-  tc::Params& P = (ROWS == 265 && pl->has_pp) ? pl->Pp : pl->P;
-  constexpr int kTileRows = tc::Geo<ROWS>::kTileRows;
-  int64_t n_tiles = (rows + kTileRows - 1) / kTileRows;
+  tc::Params& P = ((ROWS == 265 || ROWS == 233) && pl->has_pp) ? pl->Pp : pl->P;
+  constexpr int kTileRows = tc::Geo<ROWS>::kTileRows, kChains = tc::Geo<ROWS>::kChains;
+  int64_t n_tiles = (rows + kChains - 1) / kChains;
   if (tc::Geo<ROWS>::kPair) n_tiles = (n_tiles + 1) & ~(int64_t)1;   // whole CTA pairs
   // scratch: act' blocks (forward -> backward) and, for ROWS < 128, the next-operand image
   P.dact_tile_elems = (size_t)(P.n_hidden - 1) * P.H * kTileRows;
@@ -473,8 +476,15 @@ int pick_rows(const TcPlan* pl, int64_t rows, int n_sm) {
     // 512-wide: 128-chain single-CTA tiles or 64-chain CTA pairs (operand + accumulators double-buffered).
     // Measured per evaluation of one tile (HMC, B200): 52 us against 33 us, so the pairs win whenever
     // they do not need more waves of CTAs: the 4096-chain config, the small points of the sweep.
-    const int64_t t128 = (rows + 127) / 128, t64 = ((rows + 63) / 64 + 1) & ~(int64_t)1;
-    const double c128 = (double)((t128 + n_sm - 1) / n_sm) * 52.0, c265 = (double)((t64 + n_sm - 1) / n_sm) * 33.0;
+    // Geometry 233 (32 chains per CTA of a pair, the other 32 MMA rows phantom) has the same tensor work per
+    // CTA as 265 and half the epilogue work: measured 36.1 us against 38.7 us per MALA step of a tile, so it
+    // wins only while twice the CTAs still fit in one wave (4096 chains: 128 CTAs on 148 SMs, +7 %).
+    const int64_t t128 = (rows + 127) / 128, t64 = ((rows + 63) / 64 + 1) & ~(int64_t)1,
+                  t32 = ((rows + 31) / 32 + 1) & ~(int64_t)1;
+    const int64_t pair_slots = n_sm & ~1;   // CTAs of whole pairs resident at once
+    const double c128 = (double)((t128 + n_sm - 1) / n_sm) * 52.0, c265 = (double)((t64 + pair_slots - 1) / pair_slots) * 33.0,
+                 c233 = (double)((t32 + pair_slots - 1) / pair_slots) * 30.8;
+    if (c233 < c265 && c233 < c128 && !pl->no_233) return 233;
     return c265 < c128 ? 265 : 128;
   }
   if (pl->P.H != 1024) return 128;
@@ -494,6 +504,7 @@ int launch_tc(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
     case 128: return launch_tc_geo<METHOD, 128>(ctx, R, rows, s);
     case 264: return launch_tc_geo<METHOD, 264>(ctx, R, rows, s);
     case 265: return launch_tc_geo<METHOD, 265>(ctx, R, rows, s);
+    case 233: return launch_tc_geo<METHOD, 233>(ctx, R, rows, s);
     case 64: return launch_tc_geo<METHOD, 64>(ctx, R, rows, s);
     default: return launch_tc_geo<METHOD, 32>(ctx, R, rows, s);
   }
@@ -539,9 +550,10 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   const int d = cfg->d;
   TcPlan* pl = new TcPlan();
   ctx->tc = pl;
+  pl->no_233 = std::getenv("BEST_TC_NO233") != nullptr;
   if (const char* e = std::getenv("BEST_TC_ROWS")) {
     const int v = std::atoi(e);
-    if ((v == 64 || v == 32 || (v == 128 && !r64) || (v == 264 && r64) || (v == 265 && H == 512))) pl->force_rows = v;
+    if ((v == 64 || v == 32 || (v == 128 && !r64) || (v == 264 && r64) || ((v == 265 || v == 233) && H == 512))) pl->force_rows = v;
   }
   tc::Params& P = pl->P;
   P.bias16 = r64 ? 1 : 0;

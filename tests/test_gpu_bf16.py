@@ -115,12 +115,12 @@ def test_T1_1024_two_hidden_tanh(B, O):
         ctx.close()
 
 
-@pytest.mark.parametrize("rows", [265, 64, 32])
+@pytest.mark.parametrize("rows", [265, 233, 64, 32])
 def test_T1_small_tile_geometries(B, O, rows, monkeypatch):
     """The 64-/32-chain tile geometries (operand through the L2 image) on the 27→512⁴→1 net: same
     parity bar as the 128-chain tiles, plus one MALA and one AIES step against the 128-chain result."""
     base = WL.lcdm(n_chains=8, mlp_scale=1.0)
-    n = 5 * (rows if rows <= 128 else 64) + 19
+    n = 5 * {265: 64, 233: 32}.get(rows, rows) + 19
     pts = WL.probe_points(base, n, seed=29)
     w = WL.mlp_only(base)
     monkeypatch.setenv("BEST_TC_ROWS", str(rows))
