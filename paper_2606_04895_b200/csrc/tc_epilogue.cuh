@@ -249,7 +249,7 @@ __device__ __forceinline__ void publish_a(EpiCtx& C, int jn0, int n) {
 // with the chunk's four 64-row blocks of B in the order 0,2,1,3, so that one round of the epilogue (both
 // halves, same grp) completes two CONSECUTIVE k-chunks of the next operand.
 __device__ __forceinline__ int pair_jn(const OpDesc& op, int c, int half, int grp, int ngrp) {
-  return op.paired ? c * (op.ncols >> 6) + grp * 2 + half : c * (op.ncols >> 6) + half * ngrp + grp;
+  return op.perm ? c * (op.ncols >> 6) + grp * 2 + half : c * (op.ncols >> 6) + half * ngrp + grp;
 }
 
 // Order in which a thread walks the 64-column groups of an N-chunk.  BEST_TC_STAGGER (off): the warps of the
@@ -330,7 +330,7 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
     const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
     const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && (c != op.nch - 1);
     // act' of the first group can be fetched before the accumulator is complete
-    const int jstep = (Geo<ROWS>::kPair && op.paired) ? 2 : 1;
+    const int jstep = (Geo<ROWS>::kPair && op.perm) ? 2 : 1;
     const int jnc = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, 0, ngrp) : c * ngrp;   // group 0 of this chunk
     const int jn0 = jnc + stagger<ROWS>(C, 0, ngrp) * jstep;
     const uint8_t* dp = dact_l + (size_t)jn0 * kDBlk;
@@ -379,7 +379,7 @@ __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool wa
   for (int oi = 0; oi < n_ops; ++oi, ++C.o) {
     const OpDesc op = P.ops[oi];
     int written = 0;
-    C.a_wr = (uint32_t)((oi + 1) & 1) * 65536u;   // (ping-pong) the buffer the NEXT op reads
+    C.a_wr = (uint32_t)((oi + 1) & 1) * (uint32_t)Geo<ROWS>::kPPStride;   // (ping-pong) the buffer the NEXT op reads
     if (op.epi == EPI_FWD_HID) {
       if (P.act == BEST_ACT_SILU) epi_fwd<BEST_ACT_SILU, false, ROWS>(C, op, want_grad, acc2, written);
       else epi_fwd<BEST_ACT_TANH, false, ROWS>(C, op, want_grad, acc2, written);

@@ -61,11 +61,18 @@ template <int ROWS> struct Geo {
   static constexpr int kTileRows = kPair ? 64 : ROWS;   // rows of the CTA's operand / act' blocks
   static constexpr int kChains = (ROWS == 233) ? 32 : kTileRows;   // chains the CTA advances
   static constexpr int kEpiArrive = (ROWS == 233) ? 256 : 512;      // epilogue threads that run (per CTA)
-  static constexpr int kAChunk = kTileRows * 128;      // bytes of one 64-column k-chunk
+  // bytes between consecutive 64-column k-chunks of the operand.  Geometry 233 keeps only its 32 real rows:
+  // the MMA reads the following chunk's rows as its phantom rows 32..63 (finite bf16 of the same chain tile or
+  // weight-ring bytes; their accumulator lanes are never read), which halves the operand buffers (2 x 32 KB)
+  // and leaves room for an 8-stage weight ring: four stages in flight cover only ~450 cycles per stage of
+  // the L2 latency, measured as the issue rate of the N-chunk-outer order.
+  static constexpr int kAChunk = (ROWS == 233) ? 4096 : kTileRows * 128;
+  static constexpr int kPPStride = (ROWS == 233) ? 32768 : 65536;   // ping-pong: bytes between the two operand buffers
+  static constexpr int kStagesOff = (ROWS == 233) ? 65536 : 131072; // weight ring: offset in the carve-up (SmemLayout::STAGES)
   static constexpr int kEpiActive = kPair ? 512 : ROWS * 4;   // epilogue threads with MLP epilogue work
   static constexpr int kNBuf = kPair ? 4 : 2;          // accumulator buffers
   static constexpr int kBufCols = kPair ? 128 : 256;   // TMEM columns per buffer
-  static constexpr int kStagesG = 4;                   // weight ring: stages
+  static constexpr int kStagesG = (ROWS == 233) ? 8 : 4;   // weight ring: stages
   static constexpr int kStageBytesG = 16384;           // ... of this many bytes per CTA (pair: one K = 64 slice)
 };
 constexpr int kAChunkBytes = 16384;  // R64 = false chunk pitch (also the exchange-slot size)
@@ -115,6 +122,7 @@ struct OpDesc {
   int epi;
   int layer;  // FWD: hidden layer index (0-based) whose bias/act is applied; BWD_HID: layer whose act' multiplies
   int paired; // CTA-pair kernel, 1024-wide: N-chunks are issued two at a time, k-chunk outer (see mma_loop_pair)
+  int perm;   // CTA-pair kernels: the four 64-row blocks of a B chunk are packed 0,2,1,3 (see pair_jn)
 };
 
 struct Params {
@@ -176,6 +184,9 @@ struct SmemLayout {
   static constexpr int TOTAL = TMEMPTR + 16;
 };
 static_assert(SmemLayout::TOTAL + 1024 <= 232448, "shared memory budget");
+static_assert(Geo<265>::kStagesOff == SmemLayout::STAGES && Geo<128>::kStagesOff == SmemLayout::STAGES, "weight ring offset");
+static_assert(Geo<233>::kStagesOff + Geo<233>::kStagesG * Geo<233>::kStageBytesG <= SmemLayout::BIAS &&
+              Geo<233>::kPPStride + 8 * Geo<233>::kAChunk <= Geo<233>::kStagesOff, "geometry 233 carve-up");
 
 struct Bars {  // mbarrier addresses are computed, never looked up (keeps them out of local memory)
   uint32_t base;
@@ -331,9 +342,10 @@ __device__ void loader_loop(const Params& P, const Bars& bars, uint32_t a_base, 
 // full barrier, and the peer's epilogue threads arrive on the leader's a_ready / d_free directly
 // (shared::cluster address with the rank bit cleared).
 // ------------------------------------------------------------------------------------------------
+template <int ROWS>
 __device__ void producer_loop_pair(const Params& P, const Bars& bars, uint32_t stage_base, uint32_t rank,
                                    int64_t n_evals, int n_ops) {
-  constexpr uint32_t NS = 4, SB = 16384;
+  constexpr uint32_t NS = Geo<ROWS>::kStagesG, SB = Geo<ROWS>::kStageBytesG;
   uint32_t t = 0;   // stage counter: one stage = one 64-wide k-chunk = two K32 tiles (this CTA's halves)
   for (int64_t e = 0; e < n_evals; ++e) {
     uint32_t src = 0;   // byte offset inside the pack
@@ -394,7 +406,7 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
             const uint32_t d_tmem = tmem_base + bq * Geo<ROWS>::kBufCols;
             for (int j = 0; j < op.kch; ++j) {
               if (c == 0) ptx::mbar_wait(bars.a_ready(j), o & 1u);
-              const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? (oi & 1) * 65536 : 0)) >> 4);
+              const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? (oi & 1) * Geo<ROWS>::kPPStride : 0)) >> 4);
               const uint32_t tt = t + 2u * (uint32_t)j + (uint32_t)wq, s = tt % NS, use_s = tt / NS;
               ptx::mbar_wait(bars.full(s), use_s & 1u);
               ptx::tc_fence_after();
@@ -435,7 +447,7 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
             const uint32_t s = t % NS, use_s = t / NS;
             ptx::mbar_wait(bars.full(s), use_s & 1u);   // both CTAs' halves of both K32 tiles
             ptx::tc_fence_after();
-            const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? (oi & 1) * 65536 : 0)) >> 4);
+            const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? (oi & 1) * Geo<ROWS>::kPPStride : 0)) >> 4);
             const uint64_t bd = bdesc0 + (uint64_t)((s * SB) >> 4);
             if (elect_one()) {
               ptx::mma_bf16_ss_2cta(d_tmem, ad, bd, idesc, j != 0 ? 1u : 0u);

@@ -299,9 +299,9 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     if (Geo<ROWS>::kPair) {
       const uint32_t rank = ptx::cluster_ctarank();
       if (warp == 0) {
-        producer_loop_pair(P, bars, sbase + SmemLayout::STAGES, rank, n_evals, n_ops);
+        producer_loop_pair<ROWS>(P, bars, sbase + Geo<ROWS>::kStagesOff, rank, n_evals, n_ops);
       } else if ((warp == 1 || warp == 3) && rank == 0) {
-        mma_loop_pair<true, ROWS>(P, bars, sbase + SmemLayout::A, sbase + SmemLayout::STAGES, tmem_base, n_evals, n_ops,
+        mma_loop_pair<true, ROWS>(P, bars, sbase + SmemLayout::A, sbase + Geo<ROWS>::kStagesOff, tmem_base, n_evals, n_ops,
                                   warp == 3 ? 1 : 0);
       }
     } else if (warp == 0) {
@@ -372,6 +372,9 @@ struct TcPlan {
   bool has_pp = false;
   uint8_t* wpack = nullptr;
   uint8_t* wpack_p = nullptr;
+  tc::Params Pn{};           // geometry 233: N-chunk outer order with the permuted row blocks, own weight pack
+  uint8_t* wpack_n = nullptr;
+  int order233 = 2;          // 0 = Pp (paired order), 1 = P (N-chunk outer), 2 = Pn
   float* bias = nullptr;
   float* w_out = nullptr;
   uint16_t* dact = nullptr;
@@ -414,7 +417,8 @@ uint16_t f32_to_bf16(float f) {  // round to nearest even
 template <int METHOD, int ROWS>
 int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
   TcPlan* pl = ctx->tc;
-  tc::Params& P = ((ROWS == 265 || ROWS == 233) && pl->has_pp) ? pl->Pp : pl->P;
+  tc::Params& P = (ROWS == 265 && pl->has_pp) ? pl->Pp
+                : (ROWS == 233 && pl->has_pp) ? (pl->order233 == 0 ? pl->Pp : (pl->order233 == 1 ? pl->P : pl->Pn)) : pl->P;
   constexpr int kTileRows = tc::Geo<ROWS>::kTileRows, kChains = tc::Geo<ROWS>::kChains;
   int64_t n_tiles = (rows + kChains - 1) / kChains;
   if (tc::Geo<ROWS>::kPair) n_tiles = (n_tiles + 1) & ~(int64_t)1;   // whole CTA pairs
@@ -564,9 +568,9 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   const int paired = (r64 && pl->force_rows != 64 && pl->force_rows != 32) ? 1 : 0;
   int no = 0;
   for (int l = 0; l < K; ++l)
-    P.ops[no++] = tc::OpDesc{l == 0 ? 1 : kchH, nch, ncols, l == K - 1 ? tc::EPI_FWD_LAST : tc::EPI_FWD_HID, l, paired};
+    P.ops[no++] = tc::OpDesc{l == 0 ? 1 : kchH, nch, ncols, l == K - 1 ? tc::EPI_FWD_LAST : tc::EPI_FWD_HID, l, paired, paired};
   P.n_ops_fwd = no;
-  for (int l = K - 1; l >= 1; --l) P.ops[no++] = tc::OpDesc{kchH, nch, ncols, tc::EPI_BWD_HID, l - 1, paired};
+  for (int l = K - 1; l >= 1; --l) P.ops[no++] = tc::OpDesc{kchH, nch, ncols, tc::EPI_BWD_HID, l - 1, paired, paired};
   P.ops[no++] = tc::OpDesc{kchH, 1, 32, tc::EPI_BWD_FINAL, 0, 0};
   P.n_ops_all = no;
   P.dact_tile_elems = 0;   // set per launch (depends on the tile geometry)
@@ -618,7 +622,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
           for (int kk = 0; kk < 32; ++kk) {
             const size_t off = (size_t)r * 32 + ((((kk >> 3) ^ ((r >> 1) & 3))) << 3) + (kk & 7);
             // paired ops (CTA-pair kernels): B row blocks in the order 0,2,1,3, see pair_jn()
-            const int rl = (op.paired && op.ncols == 256) ? ((((r >> 6) & 1) * 2 + (r >> 7)) << 6) + (r & 63) : r;
+            const int rl = (op.perm && op.ncols == 256) ? ((((r >> 6) & 1) * 2 + (r >> 7)) << 6) + (r & 63) : r;
             const float wv = Bm(c * op.ncols + rl, k32 * 32 + kk);
             pack[base + off] = BEST_TC_ACT_F16 ? f32_to_f16(wv) : f32_to_bf16(wv);
           }
@@ -656,7 +660,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   if (H == 512 && !(std::getenv("BEST_TC_PP_NOUTER"))) {
     // geometry 265 issues the two N-chunks of a layer from two warps (k-chunk outer): same ops, paired order
     pl->Pp = P;
-    for (int oi = 0; oi + 1 < P.n_ops_all; ++oi) pl->Pp.ops[oi].paired = 1;
+    for (int oi = 0; oi + 1 < P.n_ops_all; ++oi) pl->Pp.ops[oi].paired = pl->Pp.ops[oi].perm = 1;
     const std::vector<uint16_t> pack_p = build_pack(pl->Pp);
     if ((rc = dev_alloc(&pl->wpack_p, pack_p.size() * 2))) return rc;
     BEST_CUDA(cudaMemcpy(pl->wpack_p, pack_p.data(), pack_p.size() * 2, cudaMemcpyHostToDevice));
@@ -664,6 +668,18 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
     if ((rc = make_wmap(&pl->Pp.wmap8, pl->wpack_p, pack_p.size() * 2, 32))) return rc;
     if ((rc = make_wmap(&pl->Pp.wmap1, pl->wpack_p, pack_p.size() * 2, 4))) return rc;
     pl->has_pp = true;
+    // geometry 233: N-chunk outer (one issuing warp; the epilogue of the first N-chunk overlaps the MMAs of
+    // the second) with the permuted row blocks, own pack.  BEST_TC_233_ORDER = paired | nouter | nperm (A/B).
+    pl->Pn = P;
+    for (int oi = 0; oi + 1 < P.n_ops_all; ++oi) pl->Pn.ops[oi].perm = 1;
+    const std::vector<uint16_t> pack_n = build_pack(pl->Pn);
+    if ((rc = dev_alloc(&pl->wpack_n, pack_n.size() * 2))) return rc;
+    BEST_CUDA(cudaMemcpy(pl->wpack_n, pack_n.data(), pack_n.size() * 2, cudaMemcpyHostToDevice));
+    pl->Pn.wpack = pl->wpack_n;
+    if ((rc = make_wmap(&pl->Pn.wmap8, pl->wpack_n, pack_n.size() * 2, 32))) return rc;
+    if ((rc = make_wmap(&pl->Pn.wmap1, pl->wpack_n, pack_n.size() * 2, 4))) return rc;
+    if (const char* e = std::getenv("BEST_TC_233_ORDER"))
+      pl->order233 = !std::strcmp(e, "paired") ? 0 : (!std::strcmp(e, "nouter") ? 1 : 2);
   }
   return BEST_OK;
 }
@@ -671,7 +687,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
 void tc_plan_destroy(best_ctx* ctx) {
   TcPlan* pl = ctx->tc;
   if (!pl) return;
-  cudaFree(pl->wpack); cudaFree(pl->wpack_p); cudaFree(pl->bias); cudaFree(pl->w_out); cudaFree(pl->dact); cudaFree(pl->aimg);
+  cudaFree(pl->wpack); cudaFree(pl->wpack_p); cudaFree(pl->wpack_n); cudaFree(pl->bias); cudaFree(pl->w_out); cudaFree(pl->dact); cudaFree(pl->aimg);
   delete pl;
   ctx->tc = nullptr;
 }

@@ -55,3 +55,11 @@ def test_no_cpu_fallback():
         binding.Context(WL.tiny())
     assert e.value.code == binding.BEST_ERR_CUDA
     assert "no CPU fallback" in str(e.value)
+
+
+def test_probe_argument_errors_need_no_gpu():
+    from paper_2606_04895_b200 import binding
+    for bad in ((1 << 19, 10), (200 << 20, 10), (16 << 20, 0)):
+        with pytest.raises(binding.BestError) as e:
+            binding.probe_l2_read(*bad)
+        assert e.value.code == binding.BEST_ERR_ARG

@@ -537,3 +537,14 @@ def test_argument_errors(B):
     lp = np.zeros(0, np.float32)
     ctx.logp_grad(np.zeros((0, w.d), np.float32), 0, lp, None)   # empty batch
     ctx.close()
+
+
+def test_probe_l2_read(B):
+    """best_probe_l2_read: an L2-resident buffer is read faster than HBM can deliver (6.5 TB/s measured copy)
+    and slower than any plausible L2 (50 TB/s); argument errors are reported, not clamped."""
+    gbs = B.probe_l2_read(16 << 20, 10)
+    assert 3.0e3 < gbs < 5.0e4, gbs
+    for bad in ((1 << 19, 10), (200 << 20, 10), ((16 << 20) + 16, 10), (16 << 20, 0)):
+        with pytest.raises(B.BestError) as e:
+            B.probe_l2_read(*bad)
+        assert e.value.code == B.BEST_ERR_ARG
