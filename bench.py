@@ -308,7 +308,7 @@ def main():
             out_logp = np.zeros(w.n_chains, np.float32)
             import ctypes as C
             lib = B.lib()
-            n_e2e = max(5, steps // 2)
+            n_e2e = max(10, steps)
 
             def e2e_once():
                 st.set(host_theta, step=0)                       # H2D of θ (+ logp/grad refresh on device)

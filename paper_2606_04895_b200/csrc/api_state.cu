@@ -121,6 +121,7 @@ int best_state_create(best_ctx* ctx, int64_t n_chains, const float* theta0, void
   A(&st->p_theta, B * d); A(&st->p_grad, B * d); A(&st->p_logp, B);
   A(&st->q, B * d); A(&st->h0, B); A(&st->last_la, B);
   if (!rc) rc = dev_alloc(&st->n_accept, B);
+  if (!rc) rc = dev_alloc(&st->stage, B * d);
   if (rc) { best_state_destroy(st); return rc; }
   cudaMemset(st->n_accept, 0, sizeof(unsigned long long) * B);
   cudaMemset(st->last_la, 0, sizeof(double) * B);
@@ -134,7 +135,7 @@ void best_state_destroy(best_state* st) {
   if (!st) return;
   cudaFree(st->theta); cudaFree(st->grad); cudaFree(st->logp);
   cudaFree(st->p_theta); cudaFree(st->p_grad); cudaFree(st->p_logp);
-  cudaFree(st->q); cudaFree(st->h0); cudaFree(st->last_la); cudaFree(st->n_accept);
+  cudaFree(st->q); cudaFree(st->h0); cudaFree(st->last_la); cudaFree(st->n_accept); cudaFree(st->stage);
   delete st;
 }
 
@@ -143,12 +144,10 @@ int best_state_set(best_state* st, const float* theta, uint64_t step, void* stre
   cudaStream_t s = (cudaStream_t)stream;
   best_ctx* ctx = st->ctx;
   const size_t nb = sizeof(float) * st->B * ctx->d;
-  DevBuf tmp;
   const float* src = theta;
   if (!is_device_ptr(theta)) {
-    BEST_TRY(tmp.alloc(nb));
-    BEST_CUDA(cudaMemcpyAsync(tmp.p, theta, nb, cudaMemcpyHostToDevice, s));
-    src = (const float*)tmp.p;
+    BEST_CUDA(cudaMemcpyAsync(st->stage, theta, nb, cudaMemcpyHostToDevice, s));
+    src = st->stage;
   }
   BEST_TRY(rows_f32_to_soa_f64(src, st->theta, st->B, ctx->d, st->B, s));
   st->step = step;
@@ -168,21 +167,19 @@ int best_state_get(best_state* st, float* theta, float* logp, float* grad, uint6
     BEST_TRY(eval_target_soa(ctx, st->theta, B, B, st->logp, st->grad, s));
     st->grad_valid = true;
   }
-  DevBuf tmp;
-  BEST_TRY(tmp.alloc(sizeof(float) * B * d));
   if (theta) {
-    BEST_TRY(soa_f64_to_rows_f32(st->theta, (float*)tmp.p, B, d, B, s));
-    BEST_CUDA(cudaMemcpyAsync(theta, tmp.p, sizeof(float) * B * d, cudaMemcpyDeviceToHost, s));
+    BEST_TRY(soa_f64_to_rows_f32(st->theta, st->stage, B, d, B, s));
+    BEST_CUDA(cudaMemcpyAsync(theta, st->stage, sizeof(float) * B * d, cudaMemcpyDeviceToHost, s));
     BEST_CUDA(cudaStreamSynchronize(s));
   }
   if (grad) {
-    BEST_TRY(soa_f64_to_rows_f32(st->grad, (float*)tmp.p, B, d, B, s));
-    BEST_CUDA(cudaMemcpyAsync(grad, tmp.p, sizeof(float) * B * d, cudaMemcpyDeviceToHost, s));
+    BEST_TRY(soa_f64_to_rows_f32(st->grad, st->stage, B, d, B, s));
+    BEST_CUDA(cudaMemcpyAsync(grad, st->stage, sizeof(float) * B * d, cudaMemcpyDeviceToHost, s));
     BEST_CUDA(cudaStreamSynchronize(s));
   }
   if (logp) {
-    BEST_TRY(soa_f64_to_rows_f32(st->logp, (float*)tmp.p, B, 1, B, s));
-    BEST_CUDA(cudaMemcpyAsync(logp, tmp.p, sizeof(float) * B, cudaMemcpyDeviceToHost, s));
+    BEST_TRY(soa_f64_to_rows_f32(st->logp, st->stage, B, 1, B, s));
+    BEST_CUDA(cudaMemcpyAsync(logp, st->stage, sizeof(float) * B, cudaMemcpyDeviceToHost, s));
   }
   if (n_accept)
     BEST_CUDA(cudaMemcpyAsync(n_accept, st->n_accept, sizeof(uint64_t) * B, cudaMemcpyDeviceToHost, s));

@@ -116,6 +116,7 @@ struct best_state {
   double *q = nullptr, *h0 = nullptr;
   double* last_la = nullptr;
   unsigned long long* n_accept = nullptr;
+  float* stage = nullptr;  // [B*d] fp32 row-major staging for best_state_set / _get (no allocation per call)
 };
 
 namespace best {

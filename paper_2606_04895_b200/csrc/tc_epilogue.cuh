@@ -10,6 +10,12 @@
 // instruction count: 32-bit shared-space addresses, packed f32x2 math, one MUFU per element,
 // per-thread addresses hoisted into EpiCtx.
 #pragma once
+#ifndef BEST_TC_DBG_NODACT
+#define BEST_TC_DBG_NODACT 0
+#endif
+#ifndef BEST_TC_DBG_NOFENCE
+#define BEST_TC_DBG_NOFENCE 0
+#endif
 
 namespace best {
 namespace tc {
@@ -38,7 +44,16 @@ struct EpiCtx {
 };
 
 // arrive on a barrier the MMA issuer waits on: the CTA's own, or (second CTA of a pair) the leader's
+// BEST_TC_WARP_ARRIVE = 1: ONE arrival per warp (lane 0, after __syncwarp has ordered the other lanes' fences
+// before it) instead of one per thread: a barrier phase then takes 8-32 same-address mbarrier updates (half of
+// them remote in a CTA pair) instead of 256-1024.  Every call site is warp-uniform.  Parity-green but measured
+// 1-2 % SLOWER on every workload on B200 (default line 1.206e8 -> 1.194e8, MH 16k 6.55e8 -> 6.41e8, AIES 1.59e8 ->
+// 1.56e8): the extra warp barrier costs more than the same-address arrivals did, so it is off.
 __device__ __forceinline__ void arrive_mma(const EpiCtx& C, uint32_t bar) {
+#if BEST_TC_WARP_ARRIVE
+  __syncwarp();
+  if ((C.row & 31) != 0) return;
+#endif
   if (C.to_leader) ptx::mbar_arrive_leader(bar);
   else ptx::mbar_arrive(bar);
 }
@@ -226,7 +241,7 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, co
     }
   }
 #endif
-  if (!LAST && want_grad) {
+  if (!LAST && want_grad && !BEST_TC_DBG_NODACT) {
     uint8_t* dptr = dact_l + (size_t)jn * kDBlk;
     ptx::stg_128(dptr, dp[0], dp[1], dp[2], dp[3]);
     ptx::stg_128(dptr + kDPiece, dp[4], dp[5], dp[6], dp[7]);
@@ -237,7 +252,7 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, co
 template <int ROWS>
 __device__ __forceinline__ void publish_a(EpiCtx& C, int jn0, int n) {
   if (Geo<ROWS>::kInPlace) {
-#if !BEST_TC_CONSUMER_FENCE
+#if !BEST_TC_CONSUMER_FENCE && !BEST_TC_DBG_NOFENCE
     ptx::fence_proxy_async();
 #endif
     for (int i = 0; i < n; ++i) arrive_mma(C, C.bars.a_ready(jn0 + i));
@@ -334,7 +349,9 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
     const int jnc = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, 0, ngrp) : c * ngrp;   // group 0 of this chunk
     const int jn0 = jnc + stagger<ROWS>(C, 0, ngrp) * jstep;
     const uint8_t* dp = dact_l + (size_t)jn0 * kDBlk;
-    uint4 a0 = ptx::ldg_128(dp), a1 = ptx::ldg_128(dp + kDPiece);
+    uint4 a0, a1;
+    if (BEST_TC_DBG_NODACT) { a0 = make_uint4(0x3f803f80u, 0x3f803f80u, 0x3f803f80u, 0x3f803f80u); a1 = a0; }
+    else { a0 = ptx::ldg_128(dp); a1 = ptx::ldg_128(dp + kDPiece); }
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
@@ -344,7 +361,7 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
       const uint4 d0 = a0, d1 = a1;
-      if (g0 + 1 < ngrp) {   // prefetch the next group's act'
+      if (g0 + 1 < ngrp && !BEST_TC_DBG_NODACT) {   // prefetch the next group's act'
         const uint8_t* dn = dact_l + (size_t)(jnc + stagger<ROWS>(C, g0 + 1, ngrp) * jstep) * kDBlk;
         a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
       }

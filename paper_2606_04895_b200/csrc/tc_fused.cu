@@ -99,6 +99,17 @@ constexpr int kThreads = (kCtrlWarps + kEpiWarps) * 32;
 #endif
 // Two register-allocation experiments, both measured SLOWER on B200 (HMC 16k chains: 1006 TFLOP/s
 // with neither, 938 with pinned per-thread constants, 881 with setmaxnreg 40/104) and so off:
+// Timing decomposition of the pair kernels (build-time, results are garbage): bit 0 = the producer signals full
+// stages without loading, bit 1 = no MMAs are issued; BEST_TC_DBG_NODACT / _NOFENCE (tc_epilogue.cuh) drop the act'
+// scratch traffic / the proxy fence.  Measured on B200, geometry 233, default line (ms per 100 MALA steps): full
+// 3.39-3.48, no loads 3.42, no MMAs 3.05, neither 2.95, no act' traffic 3.22 (2.67 with neither), no fence 3.44:
+// 85 % of a step is the epilogue/sampler chain alone.  (As a run-time flag the check cost 2.5 % in the issue loop.)
+#ifndef BEST_TC_WARP_ARRIVE
+#define BEST_TC_WARP_ARRIVE 0
+#endif
+#ifndef BEST_TC_DBG_SKIP
+#define BEST_TC_DBG_SKIP 0
+#endif
 #ifndef BEST_TC_SETMAXNREG
 #define BEST_TC_SETMAXNREG 0
 #endif
@@ -359,9 +370,13 @@ __device__ void producer_loop_pair(const Params& P, const Bars& bars, uint32_t s
         ptx::mbar_wait(bars.empty(s), (use & 1u) ^ 1u);
         if (elect_one()) {
           // all four halves' bytes land on the LEADER's full barrier; only the leader arrives on it
-          if (rank == 0) ptx::mbar_arrive_expect_tx(bars.full(s), 2u * bytes);
-          ptx::tma_2sm_load_2d(stage_base + s * SB, tmap, bars.full(s), 0, (int)((src + rank * half) >> 8));
-          ptx::tma_2sm_load_2d(stage_base + s * SB + half, tmap, bars.full(s), 0, (int)((src + bytes + rank * half) >> 8));
+          if (BEST_TC_DBG_SKIP & 1) {
+            if (rank == 0) ptx::mbar_arrive(bars.full(s));
+          } else {
+            if (rank == 0) ptx::mbar_arrive_expect_tx(bars.full(s), 2u * bytes);
+            ptx::tma_2sm_load_2d(stage_base + s * SB, tmap, bars.full(s), 0, (int)((src + rank * half) >> 8));
+            ptx::tma_2sm_load_2d(stage_base + s * SB + half, tmap, bars.full(s), 0, (int)((src + bytes + rank * half) >> 8));
+          }
         }
         __syncwarp();
         src += 2u * bytes;
@@ -450,10 +465,12 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
             const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? (oi & 1) * Geo<ROWS>::kPPStride : 0)) >> 4);
             const uint64_t bd = bdesc0 + (uint64_t)((s * SB) >> 4);
             if (elect_one()) {
-              ptx::mma_bf16_ss_2cta(d_tmem, ad, bd, idesc, j != 0 ? 1u : 0u);
-              ptx::mma_bf16_ss_2cta(d_tmem, ad + 2, bd + 2, idesc, 1u);
-              ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
-              ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
+              if (!(BEST_TC_DBG_SKIP & 2)) {
+                ptx::mma_bf16_ss_2cta(d_tmem, ad, bd, idesc, j != 0 ? 1u : 0u);
+                ptx::mma_bf16_ss_2cta(d_tmem, ad + 2, bd + 2, idesc, 1u);
+                ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
+                ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
+              }
               ptx::mma_commit_2cta(bars.empty(s));
               if (last_c && !Geo<ROWS>::kPingPong) { ptx::mma_commit_2cta(bars.a_free(j)); ptx::mma_commit_2cta(bars.a_free(j)); }
             }

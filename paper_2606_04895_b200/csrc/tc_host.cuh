@@ -235,6 +235,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   float* vecs = reinterpret_cast<float*>(smem + SmemLayout::VECS);
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + SmemLayout::TMEMPTR);
 
+  constexpr int kArr = BEST_TC_WARP_ARRIVE ? 32 : 1;   // threads per arrival on the barriers the MMA issuer waits on
   if (tid == 0) {
     for (int i = 0; i < 8; ++i) {
       ptx::mbar_init(bars.full(i), 1); ptx::mbar_init(bars.empty(i), 1);
@@ -242,12 +243,12 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     for (int i = 0; i < kMaxKch; ++i) {
       // arrivals per phase: in place = every epilogue thread (pair: the 256 of the lane half that owns the
       // k-chunk); L2-image tiles = warp 3 alone (+ the bulk copy's bytes)
-      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : Geo<ROWS>::kEpiArrive);   // pair: half of each CTA's
+      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : Geo<ROWS>::kEpiArrive / kArr);   // pair: half of each CTA's
       ptx::mbar_init(bars.a_free(i), Geo<ROWS>::kPair ? 2 : 1);   // pair kernels: two issuing warps
     }
     for (int i = 0; i < 4; ++i) {
       ptx::mbar_init(bars.d_full(i), 1);
-      ptx::mbar_init(bars.d_free(i), Geo<ROWS>::kPair ? 2 * Geo<ROWS>::kEpiArrive : Geo<ROWS>::kEpiActive);   // pair: both CTAs
+      ptx::mbar_init(bars.d_free(i), (Geo<ROWS>::kPair ? 2 * Geo<ROWS>::kEpiArrive : Geo<ROWS>::kEpiActive) / kArr);   // pair: both CTAs
     }
     for (int i = 0; i < 4; ++i) ptx::mbar_init(bars.epi_done(i), Geo<ROWS>::kEpiActive);
     ptx::mbar_init(bars.xin_done(), Geo<ROWS>::kEpiActive);
