@@ -24,7 +24,7 @@ sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/r1c_ncu_full.md, r1e_ncu_full.md, r1f_ncu_full.md); None where no capture exists.
-NCU_TRAFFIC_BYTES = {("lcdm_mala", 100, "bf16"): 5.281792e6 + 0.275968e6,      # r1f, best_tc_kernel<1,233>
+NCU_TRAFFIC_BYTES = {("lcdm_mala", 100, "bf16"): 5.242112e6 + 0.218112e6,      # r1f, best_tc_kernel<1,233>
                      ("hmc", 1, "bf16"): 10.798848e6 + 9.035520e6,           # r1c, best_tc_kernel<2,128>
                      ("aies", 1, "bf16"): 14.427904e6 + 0.0}                 # r1e, per half-ensemble launch
 
