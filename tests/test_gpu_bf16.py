@@ -395,3 +395,18 @@ def test_T7_nonfinite(B):
     assert rejected.sum() >= 200
     assert np.array_equal(after["theta"][rejected], before["theta"][rejected])
     ctx.close()
+
+
+# ---- BASELINE.json's full sizes, in the launch configuration bench.py times --------------------------
+@pytest.mark.parametrize("name,make,n,method,kw", [
+    ("configs[1]", "lcdm", 4096, "mala", dict(eps=0.3)),
+    ("configs[2]", "lcdm3", 16384, "hmc", dict(eps=0.1, n_leapfrog=16)),
+    ("configs[3]", "sterile", 32768, "aies", dict(a=2.0)),
+])
+def test_T2_full_size_single_step(B, O, name, make, n, method, kw):
+    """One sampler step of every chain at the full batch of BASELINE configs[1..3] (the geometry pick_rows
+    chooses there: 233 / 128 / 264) against the oracle on ALL chains: the oracle needs 1-25 s for these."""
+    w = {"lcdm": lambda: WL.lcdm(n_chains=n), "lcdm3": lambda: WL.lcdm(n_chains=n, mlp_scale=3.0),
+         "sterile": lambda: WL.sterile(n_chains=n)}[make]()
+    info = _single_step_stat(B, O, w, method, seed=77, **kw)
+    assert info["n"] == n
