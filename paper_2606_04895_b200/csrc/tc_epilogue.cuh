@@ -341,17 +341,23 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
   const int ngrp = Geo<ROWS>::kPair ? (op.ncols >> 7) : (op.ncols >> 6);
   constexpr uint32_t kDBlk = Geo<ROWS>::kTileRows * 128, kDPiece = Geo<ROWS>::kTileRows * 16;
   const uint8_t* dact_l = C.dact_thr + (size_t)(op.layer * (C.P->H >> 6)) * kDBlk;
+  const int jstep = (Geo<ROWS>::kPair && op.perm) ? 2 : 1;
+  // act' is fetched one group ahead, ACROSS N-chunk boundaries as well: the first group of an op is requested
+  // before its accumulator is complete, the first group of the next N-chunk while the last group of this one is
+  // processed (requesting it only at the top of the chunk exposed an L2 round trip per chunk: in the N-chunk-outer
+  // order the next chunk's accumulator is usually complete by then).
+  uint4 a0, a1;
+  {
+    const int jnc0 = Geo<ROWS>::kPair ? pair_jn(op, 0, C.half, 0, ngrp) : 0;
+    const uint8_t* dp = dact_l + (size_t)(jnc0 + stagger<ROWS>(C, 0, ngrp) * jstep) * kDBlk;
+    if (BEST_TC_DBG_NODACT) { a0 = make_uint4(0x3f803f80u, 0x3f803f80u, 0x3f803f80u, 0x3f803f80u); a1 = a0; }
+    else { a0 = ptx::ldg_128(dp); a1 = ptx::ldg_128(dp + kDPiece); }
+  }
   for (int c = 0; c < op.nch; ++c, ++C.g) {
     const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
     const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && (c != op.nch - 1);
-    // act' of the first group can be fetched before the accumulator is complete
-    const int jstep = (Geo<ROWS>::kPair && op.perm) ? 2 : 1;
     const int jnc = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, 0, ngrp) : c * ngrp;   // group 0 of this chunk
-    const int jn0 = jnc + stagger<ROWS>(C, 0, ngrp) * jstep;
-    const uint8_t* dp = dact_l + (size_t)jn0 * kDBlk;
-    uint4 a0, a1;
-    if (BEST_TC_DBG_NODACT) { a0 = make_uint4(0x3f803f80u, 0x3f803f80u, 0x3f803f80u, 0x3f803f80u); a1 = a0; }
-    else { a0 = ptx::ldg_128(dp); a1 = ptx::ldg_128(dp + kDPiece); }
+    const int jnc_next = Geo<ROWS>::kPair ? pair_jn(op, c + 1, C.half, 0, ngrp) : (c + 1) * ngrp;
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
@@ -361,8 +367,10 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
       const uint4 d0 = a0, d1 = a1;
-      if (g0 + 1 < ngrp && !BEST_TC_DBG_NODACT) {   // prefetch the next group's act'
-        const uint8_t* dn = dact_l + (size_t)(jnc + stagger<ROWS>(C, g0 + 1, ngrp) * jstep) * kDBlk;
+      if ((g0 + 1 < ngrp || c + 1 < op.nch) && !BEST_TC_DBG_NODACT) {   // prefetch the next group's act'
+        const int jnn = (g0 + 1 < ngrp) ? jnc + stagger<ROWS>(C, g0 + 1, ngrp) * jstep
+                                        : jnc_next + stagger<ROWS>(C, 0, ngrp) * jstep;
+        const uint8_t* dn = dact_l + (size_t)jnn * kDBlk;
         a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
       }
       ptx::tmem_ld_wait();
