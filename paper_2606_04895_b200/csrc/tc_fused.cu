@@ -45,8 +45,12 @@ constexpr int kRows = 128;           // TMEM lanes == MMA M
 //                CTA (lanes 64..127 hold the upper half of N for the same 64 rows), so a whole
 //                1024-wide layer of accumulators fits TMEM and the operand is rewritten in place.
 template <int ROWS> struct Geo {
-  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32 || ROWS == 264 || ROWS == 265 || ROWS == 233, "tile geometry");
-  static constexpr bool kPair = (ROWS == 264 || ROWS == 265 || ROWS == 233);
+  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32 || ROWS == 264 || ROWS == 265 || ROWS == 233 || ROWS == 232, "tile geometry");
+  static constexpr bool kPair = (ROWS == 264 || ROWS == 265 || ROWS == 233 || ROWS == 232);
+  // ROWS = 232: geometry 264 (1024-wide, in place) with 32 chains per CTA, the compact operand (16 chunks at a
+  // 4 KB pitch = 64 KB) and the 8-stage weight ring of geometry 233 -- for batches that leave SMs idle with
+  // 64-chain CTAs (the small points of the configs[4] sweep).
+  static constexpr bool kHalf = (ROWS == 233 || ROWS == 232);   // 32 chains in the CTA's 64 MMA rows
   // ROWS = 265: CTA pair for 512-wide layers.  64 chains per CTA need only 64 KB of operand and 256
   // TMEM columns per layer, so BOTH are double-buffered: an op reads operand buffer (op & 1) and its
   // epilogue writes the other one, accumulators alternate between two sets of TMEM columns.  No
@@ -57,22 +61,22 @@ template <int ROWS> struct Geo {
   // nothing at all, so the 8 working warps have two issue slots per scheduler cycle pair to themselves and a
   // batch too small to fill the chip with 64-chain CTAs (4096 chains = 64 CTAs) spreads over twice the SMs.
   static constexpr bool kPingPong = (ROWS == 265 || ROWS == 233);
-  static constexpr bool kInPlace = (ROWS == 128 || ROWS == 264 || ROWS == 265 || ROWS == 233);   // operand stays in SMEM
+  static constexpr bool kInPlace = (ROWS == 128 || kPair);   // operand stays in SMEM
   static constexpr int kTileRows = kPair ? 64 : ROWS;   // rows of the CTA's operand / act' blocks
-  static constexpr int kChains = (ROWS == 233) ? 32 : kTileRows;   // chains the CTA advances
-  static constexpr int kEpiArrive = (ROWS == 233) ? 256 : 512;      // epilogue threads that run (per CTA)
+  static constexpr int kChains = kHalf ? 32 : kTileRows;   // chains the CTA advances
+  static constexpr int kEpiArrive = kHalf ? 256 : 512;      // epilogue threads that run (per CTA)
   // bytes between consecutive 64-column k-chunks of the operand.  Geometry 233 keeps only its 32 real rows:
   // the MMA reads the following chunk's rows as its phantom rows 32..63 (finite bf16 of the same chain tile or
   // weight-ring bytes; their accumulator lanes are never read), which halves the operand buffers (2 x 32 KB)
   // and leaves room for an 8-stage weight ring: four stages in flight cover only ~450 cycles per stage of
   // the L2 latency, measured as the issue rate of the N-chunk-outer order.
-  static constexpr int kAChunk = (ROWS == 233) ? 4096 : kTileRows * 128;
+  static constexpr int kAChunk = kHalf ? 4096 : kTileRows * 128;
   static constexpr int kPPStride = (ROWS == 233) ? 32768 : 65536;   // ping-pong: bytes between the two operand buffers
-  static constexpr int kStagesOff = (ROWS == 233) ? 65536 : 131072; // weight ring: offset in the carve-up (SmemLayout::STAGES)
+  static constexpr int kStagesOff = kHalf ? 65536 : 131072; // weight ring: offset in the carve-up (SmemLayout::STAGES)
   static constexpr int kEpiActive = kPair ? 512 : ROWS * 4;   // epilogue threads with MLP epilogue work
   static constexpr int kNBuf = kPair ? 4 : 2;          // accumulator buffers
   static constexpr int kBufCols = kPair ? 128 : 256;   // TMEM columns per buffer
-  static constexpr int kStagesG = (ROWS == 233) ? 8 : 4;   // weight ring: stages
+  static constexpr int kStagesG = kHalf ? 8 : 4;   // weight ring: stages
   static constexpr int kStageBytesG = 16384;           // ... of this many bytes per CTA (pair: one K = 64 slice)
 };
 constexpr int kAChunkBytes = 16384;  // R64 = false chunk pitch (also the exchange-slot size)
@@ -198,6 +202,7 @@ static_assert(SmemLayout::TOTAL + 1024 <= 232448, "shared memory budget");
 static_assert(Geo<265>::kStagesOff == SmemLayout::STAGES && Geo<128>::kStagesOff == SmemLayout::STAGES, "weight ring offset");
 static_assert(Geo<233>::kStagesOff + Geo<233>::kStagesG * Geo<233>::kStageBytesG <= SmemLayout::BIAS &&
               Geo<233>::kPPStride + 8 * Geo<233>::kAChunk <= Geo<233>::kStagesOff, "geometry 233 carve-up");
+static_assert(16 * Geo<232>::kAChunk <= Geo<232>::kStagesOff, "geometry 232 carve-up");
 
 struct Bars {  // mbarrier addresses are computed, never looked up (keeps them out of local memory)
   uint32_t base;

@@ -493,7 +493,11 @@ int pick_rows(const TcPlan* pl, int64_t rows, int n_sm) {
     return c265 < c128 ? 265 : 128;
   }
   if (pl->P.H != 1024) return 128;
-  if (!pl->no_pair) return 264;   // CTA pairs (cta_group::2): the 1024-wide operand in place at full MMA rate
+  if (!pl->no_pair) {   // CTA pairs (cta_group::2): the 1024-wide operand in place at full MMA rate
+    // 32 chains per CTA (geometry 232) while twice the CTAs still fit one wave, as 233 for 512-wide layers
+    const int64_t t32 = ((rows + 31) / 32 + 1) & ~(int64_t)1;
+    return (t32 <= (n_sm & ~1) && !pl->no_233) ? 232 : 264;
+  }
   return (rows + 63) / 64 >= n_sm ? 64 : ((rows + 31) / 32 > (rows + 63) / 64 && rows <= 32 * (int64_t)n_sm ? 32 : 64);
 }
 
@@ -510,6 +514,7 @@ int launch_tc(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
     case 264: return launch_tc_geo<METHOD, 264>(ctx, R, rows, s);
     case 265: return launch_tc_geo<METHOD, 265>(ctx, R, rows, s);
     case 233: return launch_tc_geo<METHOD, 233>(ctx, R, rows, s);
+    case 232: return launch_tc_geo<METHOD, 232>(ctx, R, rows, s);
     case 64: return launch_tc_geo<METHOD, 64>(ctx, R, rows, s);
     default: return launch_tc_geo<METHOD, 32>(ctx, R, rows, s);
   }
@@ -558,7 +563,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   pl->no_233 = std::getenv("BEST_TC_NO233") != nullptr;
   if (const char* e = std::getenv("BEST_TC_ROWS")) {
     const int v = std::atoi(e);
-    if ((v == 64 || v == 32 || (v == 128 && !r64) || (v == 264 && r64) || ((v == 265 || v == 233) && H == 512))) pl->force_rows = v;
+    if ((v == 64 || v == 32 || (v == 128 && !r64) || ((v == 264 || v == 232) && r64) || ((v == 265 || v == 233) && H == 512))) pl->force_rows = v;
   }
   tc::Params& P = pl->P;
   P.bias16 = r64 ? 1 : 0;

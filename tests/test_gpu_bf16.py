@@ -76,7 +76,7 @@ def test_T1_other_shapes(B, O, hidden, act):
         ctx.close()
 
 
-@pytest.mark.parametrize("geometry", ["pair", "rows64"])
+@pytest.mark.parametrize("geometry", ["pair", "pair264", "rows64"])
 @pytest.mark.parametrize("variant", ["full", "mlp_only"])
 def test_T1_sterile_1024_logp_grad(B, O, variant, geometry, monkeypatch):
     """BASELINE configs[3]/[4] network 29→1024⁴→1 SiLU on the CTA-pair kernel (cta_group::2, operand in
@@ -84,6 +84,8 @@ def test_T1_sterile_1024_logp_grad(B, O, variant, geometry, monkeypatch):
     points on/off the banana ridge, box faces, outliers; several tiles + ragged tail."""
     if geometry == "rows64":
         monkeypatch.setenv("BEST_TC_ROWS", "64")
+    if geometry == "pair264":      # "pair" takes geometry 232 at this size (32 chains per CTA); force the 64-chain pairs
+        monkeypatch.setenv("BEST_TC_ROWS", "264")
     base = WL.sterile(n_chains=8)
     n = 64 * 5 + 37
     pts = WL.probe_points(base, n, seed=23)
