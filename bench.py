@@ -414,7 +414,7 @@ def main():
             orc["cores"] = cb["cores"]
             sweep["oracle"] = orc
         extra["sweep_adapt500"] = sweep
-        # Small-batch path: every 128-chain tile (one CTA pair) streams the forward and the
+        # Small-batch path: every tile (one CTA pair: 64 chains in geometry 232, 128 in 264) streams the forward and the
         # backward weight pack from L2 once per evaluation: algorithmic bytes = tiles x 2|W| per MALA step,
         # |W| = 2 B x MACs (bf16, unpadded).  Denominator: best_probe_l2_read (148 CTAs re-reading a 32 MiB
         # buffer that stays in the 126 MB L2, 16-byte loads, 20 passes, best of 3).
@@ -422,7 +422,8 @@ def main():
         small = {"l2_resident_read_GB_per_s": l2_gbs, "hbm_copy_GB_per_s": peaks.get("hbm_gbs")}
         for nb in (1, 64, 1024):
             k = sweep[f"mala_{nb}"]
-            tiles = (nb + 127) // 128
+            per_pair = 64 if nb <= 4736 else 128      # geometry 232 (32 chains per CTA) while it fits one wave, else 264
+            tiles = (nb + per_pair - 1) // per_pair
             by = tiles * 2 * 2 * rr["w"].macs
             gbs = by / (k["ms_per_sampler_step"] * 1e-3) / 1e9
             small[f"mala_{nb}"] = {"tiles": tiles, "weight_bytes_per_step": by, "ms_per_sampler_step": k["ms_per_sampler_step"],

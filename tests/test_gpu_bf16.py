@@ -412,3 +412,22 @@ def test_T2_full_size_single_step(B, O, name, make, n, method, kw):
          "sterile": lambda: WL.sterile(n_chains=n)}[make]()
     info = _single_step_stat(B, O, w, method, seed=77, **kw)
     assert info["n"] == n
+
+
+def test_T1_geometry_232_matches_264(B, monkeypatch):
+    """32- and 64-chain CTA pairs on the 29→1024⁴→1 net: the geometry changes no arithmetic, so sampler steps
+    (MALA, HMC, both AIES moves) are bit-identical, ragged tail included."""
+    wf = WL.sterile(n_chains=300)
+    outs = []
+    for r in (232, 264):
+        monkeypatch.setenv("BEST_TC_ROWS", str(r))
+        c2 = B.Context(wf, B.PREC_BF16)
+        st = c2.new_state(wf.theta0)
+        st.step_mala(3, 5, f32(0.01))
+        st.step_hmc(2, 9, f32(0.03), 4)
+        st.step_aies(2, 6, 2.0)
+        st.step_aies_de(1, 8, 0.1)
+        outs.append(st.get(want_grad=True))
+        c2.close()
+    for k in ("theta", "logp", "grad", "n_accept"):
+        assert np.array_equal(outs[0][k], outs[1][k]), k
