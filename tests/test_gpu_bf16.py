@@ -431,3 +431,18 @@ def test_T1_geometry_232_matches_264(B, monkeypatch):
         c2.close()
     for k in ("theta", "logp", "grad", "n_accept"):
         assert np.array_equal(outs[0][k], outs[1][k]), k
+
+
+@pytest.mark.parametrize("make,n", [("lcdm", 4736), ("lcdm", 4737), ("lcdm", 9473), ("sterile", 4736), ("sterile", 4737)])
+def test_T1_geometry_switch_points(B, O, make, n):
+    """Batch sizes on both sides of pick_rows' switch points (32-chain pairs fill one wave of 148 SMs up to
+    4736 chains; 64-chain pairs of the 512-wide net up to 9472): every point against the oracle."""
+    base = WL.lcdm(n_chains=8) if make == "lcdm" else WL.sterile(n_chains=8)
+    pts = WL.probe_points(base, n, seed=41)
+    ctx = B.Context(base, B.PREC_BF16)
+    lp = np.zeros(n, np.float32)
+    g = np.zeros((n, base.d), np.float32)
+    ctx.logp_grad(pts, n, lp, g)
+    lp_ref, g_ref = O.Oracle(base).logp_grad(pts)
+    check_logp_grad(lp, g, lp_ref, g_ref, TOL[1], f"{make}/n={n}")
+    ctx.close()
