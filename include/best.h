@@ -21,6 +21,13 @@
  *    every accept ratio.
  *  - There is no CPU fallback and no other backend: without a CUDA device every compute entry
  *    point returns BEST_ERR_CUDA.
+ *  - Concurrency: a context and ALL its states share emulator scratch (activation derivatives, exact-path
+ *    layer buffers) and the whitening factor, so a context is driven from ONE stream (and one host thread) at
+ *    a time; different contexts are independent.  Calls documented as "synchronises the device" order
+ *    themselves against work in flight on any stream.
+ *  - Environment: BEST_TC_ROWS = 128 | 265 | 233 | 264 | 232 | 64 | 32, read at best_create, forces a tile
+ *    geometry of the tensor-core path that the widths allow (tests compare geometries bit for bit); results
+ *    do not depend on it.  No other environment variable is read.
  */
 #ifndef BEST_H_
 #define BEST_H_
@@ -132,8 +139,10 @@ int best_step_aies_de(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t s
 /* Running covariance adaptation (A9; reading R14).  While adapt_every > 0 the
  * MH/MALA/HMC steps of `st` accumulate n, Σθ, Σθθᵀ (fp64) of the post-accept states of all chains;
  * every adapt_every steps  C = scatter/(n−1),  C_ii *= (1+jitter),  L = chol(C)  is computed ON
- * DEVICE and replaces the whitening factor (jitter×10 retries up to 5 times, else L is kept).
- * adapt_every = 0 switches it off.  Not used by AIES.                                  */
+ * DEVICE and replaces the context's whitening factor (jitter×10 retries up to 5 times, else L is
+ * kept).  The window (sums, step count, buffers) belongs to `st`: other states of the context neither
+ * feed nor disturb it.  adapt_every = 0 switches it off; every call with adapt_every > 0 opens a fresh
+ * window.  Not used by AIES.  Synchronises the device.                                   */
 int best_set_adaptation(best_ctx* ctx, best_state* st, int32_t adapt_every, double jitter);
 /* number of successful / failed whitening updates so far (synchronises) */
 int best_adapt_stats(best_ctx* ctx, int64_t* n_updates, int64_t* n_failures);
@@ -207,7 +216,9 @@ int best_burn_in(best_ctx* ctx, best_state* st, int32_t method, int32_t n_iter, 
 
 /* Read the state back (all pointers host, each nullable): theta [B*d], logp [B], grad [B*d]
  * (float, original space), global step counter, per-chain accept counters [B], total emulator
- * evaluations.  Synchronises `stream`.                                                          */
+ * evaluations.  Synchronises `stream`.  After MH / ensemble steps the gradient cache is stale: asking
+ * for `grad` then evaluates it (counted in n_evals) WITHOUT touching the cached log π, so a read-back
+ * between two step calls never changes the chain.                                                  */
 int best_state_get(best_state* st, float* theta, float* logp, float* grad, uint64_t* step,
                    uint64_t* n_accept, uint64_t* n_evals, void* stream);
 /* Same state in the library's internal precision (fp64 on the fp32 path): exact checkpoints.    */
@@ -217,6 +228,13 @@ int best_state_last_log_alpha(best_state* st, double* log_alpha, void* stream);
 /* Overwrite θ (host|dev float [B*d]) and the step counter; recomputes log π and ∇θ log π;
  * accept counters are kept.                                                                     */
 int best_state_set(best_state* st, const float* theta, uint64_t step, void* stream);
+/* Multi-GPU sharding (chains are independent units, partitioned over ranks with no data-path
+ * collective).  Chain c of `st` draws the Philox stream of GLOBAL chain id chain0 + c (counter word 0 of
+ * reading R1), so rank r of a job holding B chains per rank sets chain0 = r*B and the ranks' streams are
+ * disjoint, while chain0 = 0 (the default) reproduces the single-process stream.  For the ensemble moves the
+ * partner indices stay local to the state (one independent ensemble per state).
+ * Errors: BEST_ERR_ARG if chain0 + n_chains > 2^32.                                                       */
+int best_state_set_chain_offset(best_state* st, uint64_t chain0);
 
 /* Number of kernels this library has launched so far in this process (all contexts). */
 uint64_t best_launch_count(void);

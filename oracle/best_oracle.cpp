@@ -129,6 +129,9 @@ struct Oracle {
   double cov_n = 0.0;
   std::vector<double> cov_mean, cov_M2;
   int64_t n_updates = 0, n_update_failures = 0;
+  // when chains are sharded over ranks, local chain c draws the Philox stream of the GLOBAL
+  // chain id chain0 + c (counter word 0 of reading R1); 0 = the single-process stream
+  uint64_t chain0 = 0;
 };
 
 double act_f(int kind, double a, double* dact) {
@@ -637,6 +640,8 @@ void oracle_aies_map(void* h, const double* theta_i, double logp_i, const double
 // (nullable).  `step0` is the global step counter of the first step of this call (the Philox
 // `step`), so 1 x N steps == k x (N/k) steps bit-for-bit.
 
+void oracle_set_chain_offset(void* h, uint64_t chain0) { static_cast<Oracle*>(h)->chain0 = chain0; }
+
 void oracle_step_mh(void* h, int64_t B, double* theta, double* logp, uint64_t step0, int64_t n_steps,
                     uint64_t seed, double eps, uint64_t* n_accept, double* last_log_alpha,
                     double* trace, int32_t thin) {
@@ -649,8 +654,8 @@ void oracle_step_mh(void* h, int64_t B, double* theta, double* logp, uint64_t st
       std::vector<double> xi(d), thp(d);
       double u, uz, lpp, la;
       uint32_t raw;
-      draw_normals(seed, (uint64_t)c, step, d, xi.data());
-      draw_control(seed, (uint64_t)c, step, &u, &uz, &raw);
+      draw_normals(seed, o.chain0 + (uint64_t)c, step, d, xi.data());
+      draw_control(seed, o.chain0 + (uint64_t)c, step, &u, &uz, &raw);
       mh_map(o, theta + c * d, logp[c], xi.data(), eps, thp.data(), &lpp, &la);
       if (last_log_alpha) last_log_alpha[c] = la;
       if (accept_rule(u, la)) {
@@ -676,8 +681,8 @@ void oracle_step_mala(void* h, int64_t B, double* theta, double* logp, double* g
       std::vector<double> xi(d), thp(d), gp(d);
       double u, uz, lpp, la;
       uint32_t raw;
-      draw_normals(seed, (uint64_t)c, step, d, xi.data());
-      draw_control(seed, (uint64_t)c, step, &u, &uz, &raw);
+      draw_normals(seed, o.chain0 + (uint64_t)c, step, d, xi.data());
+      draw_control(seed, o.chain0 + (uint64_t)c, step, &u, &uz, &raw);
       mala_map(o, theta + c * d, logp[c], grad + c * d, xi.data(), eps, thp.data(), &lpp, gp.data(),
                &la);
       if (last_log_alpha) last_log_alpha[c] = la;
@@ -705,8 +710,8 @@ void oracle_step_hmc(void* h, int64_t B, double* theta, double* logp, double* gr
       std::vector<double> q(d), thp(d), gp(d), qp(d);
       double u, uz, lpp, la;
       uint32_t raw;
-      draw_normals(seed, (uint64_t)c, step, d, q.data());  // momentum q ~ N(0, 1)
-      draw_control(seed, (uint64_t)c, step, &u, &uz, &raw);
+      draw_normals(seed, o.chain0 + (uint64_t)c, step, d, q.data());  // momentum q ~ N(0, 1)
+      draw_control(seed, o.chain0 + (uint64_t)c, step, &u, &uz, &raw);
       hmc_map(o, theta + c * d, logp[c], grad + c * d, q.data(), eps, n_leapfrog, thp.data(), &lpp,
               gp.data(), qp.data(), &la);
       if (last_log_alpha) last_log_alpha[c] = la;
@@ -743,7 +748,7 @@ int32_t oracle_step_aies(void* h, int64_t B, double* theta, double* logp, uint64
         const int64_t i = own0 + r;
         double u, uz, lpp, la;
         uint32_t raw;
-        draw_control(seed, (uint64_t)i, step, &u, &uz, &raw);
+        draw_control(seed, o.chain0 + (uint64_t)i, step, &u, &uz, &raw);
         const int64_t j = other0 + (int64_t)(((uint64_t)raw * (uint64_t)half) >> 32);
         const double z = stretch_z(uz, a);
         aies_map(o, theta + i * d, logp[i], theta + j * d, z, newth.data() + r * d, &lpp, &la);
@@ -791,13 +796,13 @@ int32_t oracle_step_aies_de(void* h, int64_t B, double* theta, double* logp, uin
       for (int64_t r = 0; r < half; ++r) {
         const int64_t i = own0 + r;
         uint32_t w[4];
-        philox_block(seed, (uint64_t)i, step, 0u, w);
+        philox_block(seed, o.chain0 + (uint64_t)i, step, 0u, w);
         const double u = u01(w[0]);
         const int64_t jr = (int64_t)(((uint64_t)w[2] * (uint64_t)half) >> 32);
         int64_t kr = (int64_t)(((uint64_t)w[3] * (uint64_t)(half - 1)) >> 32);
         if (kr >= jr) kr += 1;
         std::vector<double> xi(4 * ((d + 3) / 4));
-        draw_normals(seed, (uint64_t)i, step, d, xi.data());
+        draw_normals(seed, o.chain0 + (uint64_t)i, step, d, xi.data());
         const double gamma = (1.0 + sigma_gamma * xi[0]) * gamma0;
         double lpp, la;
         de_map(o, theta + i * d, logp[i], theta + (other0 + jr) * d, theta + (other0 + kr) * d, gamma,

@@ -57,6 +57,7 @@ def lib():
         L.oracle_set_step_scale.argtypes = [vp, dp]
         L.oracle_set_hard_box.argtypes = [vp, i32]
         L.oracle_set_adaptation.argtypes = [vp, i64, C.c_double]
+        L.oracle_set_chain_offset.argtypes = [vp, u64]
         L.oracle_adapt_stats.argtypes = [vp, C.POINTER(i64), C.POINTER(i64)]
         L.oracle_cov_chol.restype = i32
         L.oracle_cov_chol.argtypes = [vp, dp, i64, C.c_double, dp, dp]
@@ -221,6 +222,10 @@ class Oracle:
 
     def set_hard_box(self, on: bool):
         lib().oracle_set_hard_box(self._h, 1 if on else 0)
+
+    def set_chain_offset(self, chain0: int):
+        """local chain c draws the Philox stream of global chain id chain0 + c."""
+        lib().oracle_set_chain_offset(self._h, int(chain0))
 
     def set_adaptation(self, adapt_every: int, jitter: float = 1e-6):
         lib().oracle_set_adaptation(self._h, adapt_every, jitter)

@@ -25,6 +25,7 @@ EXPORTS = [
     "best_adapt_stats", "best_get_whitening", "best_set_whitening", "best_state_get",
     "best_state_get_f64", "best_state_last_log_alpha", "best_state_set", "best_launch_count",
     "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box", "best_burn_in", "best_step_aies_de", "best_rminus1", "best_probe_l2_read",
+    "best_state_set_chain_offset",
 ]
 
 
@@ -87,6 +88,7 @@ def lib():
     L.best_state_get_f64.argtypes = [vp, vp, vp, vp, vp]
     L.best_state_last_log_alpha.argtypes = [vp, vp, vp]
     L.best_state_set.argtypes = [vp, vp, u64, vp]
+    L.best_state_set_chain_offset.argtypes = [vp, u64]
     L.best_launch_count.restype = u64
     L.best_last_error.restype = C.c_char_p
     L.best_version.restype = C.c_char_p
@@ -290,6 +292,9 @@ class State:
         grad = np.zeros((B, d)) if want_grad else None
         _check(lib().best_state_get_f64(self._h, theta.ctypes.data, logp.ctypes.data, _ptr(grad), stream or None))
         return theta, logp, grad
+
+    def set_chain_offset(self, chain0: int):
+        _check(lib().best_state_set_chain_offset(self._h, chain0))
 
     def last_log_alpha(self, stream=0):
         la = np.zeros(self.B)

@@ -39,7 +39,7 @@ using namespace best;
 extern "C" {
 
 const char* best_last_error(void) { return t_err.c_str(); }
-const char* best_version(void) { return "best-b200 0.1 (sm_100a)"; }
+const char* best_version(void) { return "best-b200 0.2 (sm_100a)"; }
 uint64_t best_launch_count(void) { return g_launches.load(); }
 
 int best_create(const best_config* cfg, best_ctx** out) {
@@ -138,7 +138,6 @@ int best_create(const best_config* cfg, best_ctx** out) {
       return fail(BEST_ERR_CUDA);
     }
   }
-  if ((rc = dev_alloc(&ctx->cov_ref, d))) return fail(rc);
   if ((rc = dev_alloc(&ctx->adapt_counts, 2))) return fail(rc);
   cudaMemset(ctx->adapt_counts, 0, sizeof(int64_t) * 2);
 
@@ -201,7 +200,7 @@ void best_destroy(best_ctx* ctx) {
   for (auto p : ctx->Dact) cudaFree(p);
   cudaFree(ctx->X0); cudaFree(ctx->delta[0]); cudaFree(ctx->delta[1]);
   cudaFree(ctx->mlp_out); cudaFree(ctx->mlp_grad);
-  cudaFree(ctx->dev_consts); cudaFree(ctx->cov_acc); cudaFree(ctx->cov_ref); cudaFree(ctx->adapt_counts); cudaFree(ctx->Lraw_dev);
+  cudaFree(ctx->dev_consts); cudaFree(ctx->adapt_counts); cudaFree(ctx->Lraw_dev); cudaFree(ctx->lg_scratch);
   delete ctx;
 }
 

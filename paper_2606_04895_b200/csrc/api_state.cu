@@ -22,6 +22,19 @@ struct DevBuf {  // RAII scratch
   }
 };
 
+// Gradient cache only (MH / AIES leave it stale): the cached log pi is NOT rewritten, so a read-back between
+// two step calls cannot change the chain (1 x N steps == k x N/k steps bit for bit, with or without get()).
+int refresh_grad(best_ctx* ctx, best_state* st, cudaStream_t s) {
+  if (ctx->precision == BEST_PREC_BF16) {
+    BEST_TRY(tc_eval_state(ctx, st, st->p_logp, st->grad, s));
+  } else {
+    BEST_TRY(eval_target_soa(ctx, st->theta, st->B, st->B, st->p_logp, st->grad, s));
+    st->n_evals += (uint64_t)st->B;
+  }
+  st->grad_valid = true;
+  return BEST_OK;
+}
+
 int refresh_cache(best_ctx* ctx, best_state* st, cudaStream_t s) {
   if (ctx->precision == BEST_PREC_BF16) return tc_state_init(ctx, st, s);
   BEST_TRY(eval_target_soa(ctx, st->theta, st->B, st->B, st->logp, st->grad, s));
@@ -88,15 +101,22 @@ int best_logp_grad(best_ctx* ctx, const float* theta, int64_t n, float* logp, fl
   if (ctx->precision == BEST_PREC_BF16) {
     BEST_TRY(tc_logp_grad(ctx, th_d, n, lp_d, g_d, s));
   } else {
-    DevBuf soa_th, soa_g, lp64;
-    BEST_TRY(soa_th.alloc(sizeof(double) * n * d));
-    BEST_TRY(lp64.alloc(sizeof(double) * n));
-    if (grad) BEST_TRY(soa_g.alloc(sizeof(double) * n * d));
-    BEST_TRY(rows_f32_to_soa_f64(th_d, (double*)soa_th.p, n, d, n, s));
-    BEST_TRY(eval_target_soa(ctx, (double*)soa_th.p, n, n, (double*)lp64.p, (double*)soa_g.p, s));
-    BEST_TRY(soa_f64_to_rows_f32((double*)lp64.p, lp_d, n, 1, n, s));
-    if (grad) BEST_TRY(soa_f64_to_rows_f32((double*)soa_g.p, g_d, n, d, n, s));
-    BEST_CUDA(cudaStreamSynchronize(s));  // scratch above is freed on return
+    // SoA fp64 staging [theta | grad | logp] in the context's grow-only scratch (no allocation per call)
+    const size_t need = sizeof(double) * (size_t)n * (2 * (size_t)d + 1);
+    if (need > ctx->lg_scratch_bytes) {
+      BEST_CUDA(cudaStreamSynchronize(s));
+      cudaFree(ctx->lg_scratch);
+      ctx->lg_scratch = nullptr; ctx->lg_scratch_bytes = 0;
+      if (cudaMalloc(&ctx->lg_scratch, need) != cudaSuccess) { cudaGetLastError(); set_error("cudaMalloc failed"); return BEST_ERR_ALLOC; }
+      ctx->lg_scratch_bytes = need;
+    }
+    double* soa_th = (double*)ctx->lg_scratch;
+    double* soa_g = soa_th + (size_t)n * d;
+    double* lp64 = soa_g + (size_t)n * d;
+    BEST_TRY(rows_f32_to_soa_f64(th_d, soa_th, n, d, n, s));
+    BEST_TRY(eval_target_soa(ctx, soa_th, n, n, lp64, grad ? soa_g : nullptr, s));
+    BEST_TRY(soa_f64_to_rows_f32(lp64, lp_d, n, 1, n, s));
+    if (grad) BEST_TRY(soa_f64_to_rows_f32(soa_g, g_d, n, d, n, s));
   }
   if (!lp_dev) BEST_CUDA(cudaMemcpyAsync(logp, lp_d, sizeof(float) * n, cudaMemcpyDeviceToHost, s));
   if (grad && !g_dev) BEST_CUDA(cudaMemcpyAsync(grad, g_d, sizeof(float) * n * d, cudaMemcpyDeviceToHost, s));
@@ -136,6 +156,7 @@ void best_state_destroy(best_state* st) {
   cudaFree(st->theta); cudaFree(st->grad); cudaFree(st->logp);
   cudaFree(st->p_theta); cudaFree(st->p_grad); cudaFree(st->p_logp);
   cudaFree(st->q); cudaFree(st->h0); cudaFree(st->last_la); cudaFree(st->n_accept); cudaFree(st->stage);
+  adapt_free(st);
   delete st;
 }
 
@@ -163,10 +184,7 @@ int best_state_get(best_state* st, float* theta, float* logp, float* grad, uint6
   best_ctx* ctx = st->ctx;
   const int64_t B = st->B;
   const int d = ctx->d;
-  if (grad && !st->grad_valid) {
-    BEST_TRY(eval_target_soa(ctx, st->theta, B, B, st->logp, st->grad, s));
-    st->grad_valid = true;
-  }
+  if (grad && !st->grad_valid) BEST_TRY(refresh_grad(ctx, st, s));
   if (theta) {
     BEST_TRY(soa_f64_to_rows_f32(st->theta, st->stage, B, d, B, s));
     BEST_CUDA(cudaMemcpyAsync(theta, st->stage, sizeof(float) * B * d, cudaMemcpyDeviceToHost, s));
@@ -205,9 +223,8 @@ int best_state_get_f64(best_state* st, double* theta, double* logp, double* grad
   if (theta) BEST_TRY(fetch(st->theta, theta));
   if (grad) {
     if (!st->grad_valid) {
-      BEST_TRY(eval_target_soa(st->ctx, st->theta, B, B, st->logp, st->grad, s));
+      BEST_TRY(refresh_grad(st->ctx, st, s));
       BEST_CUDA(cudaStreamSynchronize(s));
-      st->grad_valid = true;
     }
     BEST_TRY(fetch(st->grad, grad));
   }
@@ -283,9 +300,22 @@ int best_set_adaptation(best_ctx* ctx, best_state* st, int32_t adapt_every, doub
     set_error("best_set_adaptation: bad argument");
     return BEST_ERR_ARG;
   }
-  ctx->adapt_every = adapt_every;
-  ctx->jitter = jitter;
-  if (adapt_every > 0) BEST_TRY(adapt_reset(ctx, st, 0));
+  BEST_CUDA(cudaDeviceSynchronize());   // work in flight on any stream is ordered before the window opens
+  st->adapt_every = adapt_every;
+  st->jitter = jitter;
+  if (adapt_every > 0) {
+    BEST_TRY(adapt_reset(ctx, st, 0));
+    BEST_CUDA(cudaDeviceSynchronize());
+  }
+  return BEST_OK;
+}
+
+int best_state_set_chain_offset(best_state* st, uint64_t chain0) {
+  if (!st || chain0 + (uint64_t)st->B > ((uint64_t)1 << 32)) {
+    set_error("best_state_set_chain_offset: chain0 + n_chains must not exceed 2^32");
+    return BEST_ERR_ARG;
+  }
+  st->chain0 = chain0;
   return BEST_OK;
 }
 
@@ -384,7 +414,7 @@ int best_burn_in(best_ctx* ctx, best_state* st, int32_t method, int32_t n_iter, 
   double best_lp = -INFINITY;
   std::vector<double> lp_host((size_t)st->B);
   int64_t nh = 0;
-  ctx->adapt_every = 0;
+  st->adapt_every = 0;
   for (int it = 0; it < n_iter; ++it) {
     if (n_adapt > 0) {  // (1) dual averaging on the ensemble acceptance fraction
       const double mu = std::log(10.0 * (double)eps);
@@ -416,7 +446,7 @@ int best_burn_in(best_ctx* ctx, best_state* st, int32_t method, int32_t n_iter, 
       if (win > INT32_MAX) { set_error("best_burn_in: window too long"); return BEST_ERR_ARG; }
       BEST_TRY(best_set_adaptation(ctx, st, (int32_t)win, jitter));
       const int rc = run_step(ctx, st, m_int, win, seed, eps, n_leapfrog, nullptr, 0, stream);
-      ctx->adapt_every = 0;
+      st->adapt_every = 0;
       if (rc) return rc;
     }
     // (3) best fit over the ensemble (first chain with the largest cached log pi)

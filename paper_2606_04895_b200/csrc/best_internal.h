@@ -93,14 +93,10 @@ struct best_ctx {
   float* delta[2] = {nullptr, nullptr};
   float* mlp_out = nullptr;       // [n]
   float* mlp_grad = nullptr;      // [n][dp]
-  // adaptation (A9)
-  int adapt_every = 0;
-  double jitter = 1e-6;
-  int64_t win_steps = 0;
-  double* cov_acc = nullptr;      // [nblk_max][1 + d + d*d] per-block partial sums (fp64)
-  int cov_blocks = 0;
-  double* cov_ref = nullptr;      // [d] shift
-  int64_t* adapt_counts = nullptr;  // device [2]: updates, failures
+  int64_t* adapt_counts = nullptr;  // device [2]: whitening updates, failures (A9)
+  // best_logp_grad scratch on the exact path (grow-only; a context is driven from one stream at a time)
+  void* lg_scratch = nullptr;
+  size_t lg_scratch_bytes = 0;
   best::TcPlan* tc = nullptr;
 };
 
@@ -117,6 +113,16 @@ struct best_state {
   double* last_la = nullptr;
   unsigned long long* n_accept = nullptr;
   float* stage = nullptr;  // [B*d] fp32 row-major staging for best_state_set / _get (no allocation per call)
+  uint64_t chain0 = 0;     // Philox chain id of chain 0 (best_state_set_chain_offset)
+  // covariance adaptation (A9) -- per STATE: the window of one state never sees another state's samples
+  int adapt_every = 0;
+  double jitter = 1e-6;
+  int64_t win_steps = 0;          // steps accumulated in the current window
+  double* cov_acc = nullptr;      // [cov_blocks][1 + d + d*d] per-block partial sums (fp64): count | sums | products
+  int cov_blocks = 0;
+  double* cov_ref = nullptr;      // [d] shift (chain 0's position when the window opened)
+  float* win_buf = nullptr;       // tensor path: fp32 rows [win_cap_steps][B][d] written by the persistent kernel
+  int64_t win_cap_steps = 0;
 };
 
 namespace best {
@@ -135,8 +141,12 @@ int step_mala(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cu
 int step_hmc(best_ctx*, best_state*, int64_t, uint64_t, double, int, float*, int, cudaStream_t);
 int step_aies(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cudaStream_t, bool de = false);
 int adapt_reset(best_ctx* ctx, best_state* st, cudaStream_t s);
-// after step index t of a call: trace slot (every `thin` steps) and covariance accumulation / update
+void adapt_free(best_state* st);
+// exact path, after step index t of a call: trace slot (every `thin` steps) and covariance accumulation / update
 int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin, bool adapt, cudaStream_t s);
+// tensor path: fold `n_steps` slots of fp32 rows [n_steps][B][d] (every post-accept state of a segment) into
+// the window sums; closes the window (covariance -> Cholesky -> whitening swap, on device) when it is complete
+int adapt_window_rows(best_ctx* ctx, best_state* st, const float* rows, int64_t n_steps, cudaStream_t s);
 
 // layout helpers (samplers.cu)
 int rows_f32_to_soa_f64(const float* rows_dev, double* soa, int64_t n, int d, int64_t ld, cudaStream_t s);

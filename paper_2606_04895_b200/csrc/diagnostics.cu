@@ -8,11 +8,10 @@
 #include <algorithm>
 
 #include "best_internal.h"
+#include "gram.cuh"
 
 namespace best {
 namespace {
-
-constexpr int G_TPB = 128;
 
 // means[c*d + i] = (1/n) sum_t trace[t][c][i]   (one thread per (c, i): fully coalesced over the trace row)
 __global__ void k_chain_means(const float* __restrict__ trace, int64_t n, int64_t row, double* __restrict__ means) {
@@ -38,60 +37,6 @@ __global__ void k_grand_mean(const double* __restrict__ means, int64_t B, int d,
     for (int q = 0; q < 32; ++q) t += part[q][i];
     gm[i] = t / (double)B;
   }
-}
-
-// acc[blk][i*d + j] = sum over the block's rows of (x_i - ref_i)(x_j - ref_j); rows are [nrows][d].
-// The rows of a tile sit in SMEM padded to 32 columns (zeros); the 128 threads are two groups of 8 x 8
-// threads, each thread holding a 4 x 4 block of the 32 x 32 Gram matrix in registers (two 32-byte SMEM
-// reads, broadcast inside a warp, per 16 fp64 FMAs) and each group taking every other row of the tile.
-constexpr int G_ROWS = 64;
-template <typename T>
-__global__ void __launch_bounds__(G_TPB)
-k_gram_partial(const T* __restrict__ rows, int64_t nrows, int d, const double* __restrict__ ref,
-               double* __restrict__ acc) {
-  __shared__ __align__(16) double xs[G_ROWS * kMaxD];
-  const int grp = threadIdx.x >> 6, u = threadIdx.x & 63, ti = u >> 3, tj = u & 7;
-  double a4[4][4];
-#pragma unroll
-  for (int p = 0; p < 4; ++p)
-#pragma unroll
-    for (int q = 0; q < 4; ++q) a4[p][q] = 0.0;
-  for (int e = threadIdx.x; e < G_ROWS * kMaxD; e += G_TPB) xs[e] = 0.0;   // the padding columns stay zero
-  for (int64_t r0 = blockIdx.x * (int64_t)G_ROWS; r0 < nrows; r0 += (int64_t)gridDim.x * G_ROWS) {
-    const int nv = (int)((nrows - r0 < G_ROWS) ? (nrows - r0) : G_ROWS);
-    __syncthreads();
-    for (int e = threadIdx.x; e < G_ROWS * d; e += G_TPB) {   // contiguous, coalesced
-      const int r = e / d, i = e - r * d;
-      xs[r * kMaxD + i] = (r < nv) ? (double)rows[r0 * d + e] - ref[i] : 0.0;
-    }
-    __syncthreads();
-    for (int r = grp; r < nv; r += 2) {
-      const double2* pa = reinterpret_cast<const double2*>(xs + r * kMaxD + 4 * ti);
-      const double2* pb = reinterpret_cast<const double2*>(xs + r * kMaxD + 4 * tj);
-      const double2 a01 = pa[0], a23 = pa[1], b01 = pb[0], b23 = pb[1];
-      const double a[4] = {a01.x, a01.y, a23.x, a23.y}, b[4] = {b01.x, b01.y, b23.x, b23.y};
-#pragma unroll
-      for (int p = 0; p < 4; ++p)
-#pragma unroll
-        for (int q = 0; q < 4; ++q) a4[p][q] = fma(a[p], b[q], a4[p][q]);
-    }
-  }
-  // group 1 hands its block to group 0 through SMEM (fixed order: g0 + g1)
-  __syncthreads();
-  if (grp == 1)
-#pragma unroll
-    for (int p = 0; p < 4; ++p)
-#pragma unroll
-      for (int q = 0; q < 4; ++q) xs[(4 * ti + p) * kMaxD + 4 * tj + q] = a4[p][q];
-  __syncthreads();
-  if (grp == 0)
-#pragma unroll
-    for (int p = 0; p < 4; ++p)
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const int i = 4 * ti + p, j = 4 * tj + q;
-        if (i < d && j < d) acc[(size_t)blockIdx.x * d * d + i * d + j] = a4[p][q] + xs[i * kMaxD + j];
-      }
 }
 
 // out[0] = R - 1, out[1] = status (0 ok, 1 W~ not positive definite / B_ii = 0)

@@ -3,6 +3,7 @@
 // accept) with the emulator passes (emulator_fp32.cu) in between.
 #include "best_internal.h"
 #include "device_math.cuh"
+#include "gram.cuh"
 
 namespace best {
 namespace {
@@ -13,6 +14,7 @@ inline int nblocks(int64_t n) { return (int)((n + TPB - 1) / TPB); }
 struct Chains {  // device pointers of one best_state
   int64_t B;
   int d;
+  uint32_t chain0;  // Philox chain id of chain 0
   double *theta, *grad, *logp, *p_theta, *p_grad, *p_logp, *q, *h0, *last_la;
   unsigned long long* n_accept;
 };
@@ -31,7 +33,7 @@ __global__ void k_mh_propose(Chains S, const double* __restrict__ L, uint64_t se
   if (c >= S.B) return;
   const int d = S.d;
   double xi[kMaxD], dx[kMaxD];
-  draw_normals<double>(seed, (uint32_t)c, step, d, xi);
+  draw_normals<double>(seed, S.chain0 + (uint32_t)c, step, d, xi);
   for (int i = 0; i < d; ++i) xi[i] *= eps;
   tri_L_apply<double>(L, d, xi, dx);
   for (int i = 0; i < d; ++i) S.p_theta[i * S.B + c] = S.theta[i * S.B + c] + dx[i];
@@ -40,7 +42,7 @@ __global__ void k_mh_propose(Chains S, const double* __restrict__ L, uint64_t se
 __global__ void k_mh_accept(Chains S, uint64_t seed, uint64_t step) {
   const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (c >= S.B) return;
-  const uint4 w = philox4x32_10((uint32_t)c, step, 0u, seed);
+  const uint4 w = philox4x32_10(S.chain0 + (uint32_t)c, step, 0u, seed);
   const double la = S.p_logp[c] - S.logp[c];
   S.last_la[c] = la;
   if (accept_rule<double>(u01<double>(w.x), la)) {
@@ -57,7 +59,7 @@ __global__ void k_mala_propose(Chains S, const double* __restrict__ L, uint64_t 
   if (c >= S.B) return;
   const int d = S.d;
   double xi[kMaxD], g[kMaxD], gz[kMaxD], dx[kMaxD];
-  draw_normals<double>(seed, (uint32_t)c, step, d, xi);
+  draw_normals<double>(seed, S.chain0 + (uint32_t)c, step, d, xi);
   load_col(S.grad, S.B, c, d, g);
   tri_Lt_apply<double>(L, d, g, gz);
   const double sq = sqrt(2.0 * eps);
@@ -72,7 +74,7 @@ __global__ void k_mala_accept(Chains S, const double* __restrict__ L, uint64_t s
   if (c >= S.B) return;
   const int d = S.d;
   double xi[kMaxD], g[kMaxD], gz[kMaxD], gzp[kMaxD];
-  draw_normals<double>(seed, (uint32_t)c, step, d, xi);
+  draw_normals<double>(seed, S.chain0 + (uint32_t)c, step, d, xi);
   load_col(S.grad, S.B, c, d, g);
   tri_Lt_apply<double>(L, d, g, gz);
   load_col(S.p_grad, S.B, c, d, g);
@@ -87,7 +89,7 @@ __global__ void k_mala_accept(Chains S, const double* __restrict__ L, uint64_t s
   }
   const double la = S.p_logp[c] - S.logp[c] + (-bwd / (4.0 * eps)) - (-fwd / (4.0 * eps));
   S.last_la[c] = la;
-  const uint4 w = philox4x32_10((uint32_t)c, step, 0u, seed);
+  const uint4 w = philox4x32_10(S.chain0 + (uint32_t)c, step, 0u, seed);
   if (accept_rule<double>(u01<double>(w.x), la)) {
     for (int i = 0; i < d; ++i) {
       S.theta[i * S.B + c] = S.p_theta[i * S.B + c];
@@ -105,7 +107,7 @@ __global__ void k_hmc_begin(Chains S, const double* __restrict__ L, uint64_t see
   if (c >= S.B) return;
   const int d = S.d;
   double q[kMaxD], g[kMaxD], gz[kMaxD], dx[kMaxD];
-  draw_normals<double>(seed, (uint32_t)c, step, d, q);
+  draw_normals<double>(seed, S.chain0 + (uint32_t)c, step, d, q);
   double kin = 0.0;
   for (int i = 0; i < d; ++i) kin += q[i] * q[i];
   S.h0[c] = -S.logp[c] + 0.5 * kin;
@@ -142,7 +144,7 @@ __global__ void k_hmc_kick(Chains S, const double* __restrict__ L, uint64_t seed
   const double H1 = -S.p_logp[c] + 0.5 * kin;
   const double la = S.h0[c] - H1;
   S.last_la[c] = la;
-  const uint4 w = philox4x32_10((uint32_t)c, step, 0u, seed);
+  const uint4 w = philox4x32_10(S.chain0 + (uint32_t)c, step, 0u, seed);
   if (accept_rule<double>(u01<double>(w.x), la)) {
     for (int i = 0; i < d; ++i) {
       S.theta[i * S.B + c] = S.p_theta[i * S.B + c];
@@ -159,7 +161,7 @@ __global__ void k_aies_propose(Chains S, uint64_t seed, uint64_t step, double a,
   const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (r >= half) return;
   const int64_t i = own0 + r;
-  const uint4 w = philox4x32_10((uint32_t)i, step, 0u, seed);
+  const uint4 w = philox4x32_10(S.chain0 + (uint32_t)i, step, 0u, seed);
   const int64_t j = oth0 + (int64_t)__umulhi(w.z, (uint32_t)half);
   const double t = u01<double>(w.y) * (a - 1.0) + 1.0;
   const double z = t * t / a;
@@ -174,7 +176,7 @@ __global__ void k_aies_accept(Chains S, uint64_t seed, uint64_t step, double a, 
   const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (r >= half) return;
   const int64_t i = own0 + r;
-  const uint4 w = philox4x32_10((uint32_t)i, step, 0u, seed);
+  const uint4 w = philox4x32_10(S.chain0 + (uint32_t)i, step, 0u, seed);
   const double t = u01<double>(w.y) * (a - 1.0) + 1.0;
   const double z = t * t / a;
   const double la = (double)(S.d - 1) * log(z) + S.p_logp[r] - S.logp[i];
@@ -194,11 +196,11 @@ __global__ void k_de_propose(Chains S, uint64_t seed, uint64_t step, double sigm
   const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (r >= half) return;
   const int64_t i = own0 + r;
-  const uint4 w = philox4x32_10((uint32_t)i, step, 0u, seed);
+  const uint4 w = philox4x32_10(S.chain0 + (uint32_t)i, step, 0u, seed);
   const int64_t jr = (int64_t)__umulhi(w.z, (uint32_t)half);
   int64_t kr = (int64_t)__umulhi(w.w, (uint32_t)(half - 1));
   if (kr >= jr) kr += 1;
-  const uint4 wn = philox4x32_10((uint32_t)i, step, 1u, seed);
+  const uint4 wn = philox4x32_10(S.chain0 + (uint32_t)i, step, 1u, seed);
   double n0, n1;
   box_muller(wn.x, wn.y, n0, n1);
   const double gamma = (1.0 + sigma * n0) * (2.38 / sqrt(2.0 * (double)S.d));
@@ -211,7 +213,7 @@ __global__ void k_de_accept(Chains S, uint64_t seed, uint64_t step, int64_t own0
   const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (r >= half) return;
   const int64_t i = own0 + r;
-  const uint4 w = philox4x32_10((uint32_t)i, step, 0u, seed);
+  const uint4 w = philox4x32_10(S.chain0 + (uint32_t)i, step, 0u, seed);
   const double la = S.p_logp[r] - S.logp[i];
   S.last_la[i] = la;
   if (accept_rule<double>(u01<double>(w.x), la)) {
@@ -314,7 +316,7 @@ __global__ void k_cov_finalize(double* __restrict__ acc, int nblk, int d, double
 
 Chains chains_of(best_state* st) {
   Chains S;
-  S.B = st->B; S.d = st->ctx->d;
+  S.B = st->B; S.d = st->ctx->d; S.chain0 = (uint32_t)st->chain0;
   S.theta = st->theta; S.grad = st->grad; S.logp = st->logp;
   S.p_theta = st->p_theta; S.p_grad = st->p_grad; S.p_logp = st->p_logp;
   S.q = st->q; S.h0 = st->h0; S.last_la = st->last_la; S.n_accept = st->n_accept;
@@ -322,6 +324,15 @@ Chains chains_of(best_state* st) {
 }
 
 }  // namespace
+
+static int close_window(best_ctx* ctx, best_state* st, cudaStream_t s) {
+  k_cov_finalize<<<1, 256, 0, s>>>(st->cov_acc, st->cov_blocks, ctx->d, st->jitter, ctx->L_dev, ctx->Lraw_dev,
+                                   ctx->scale_dev, (long long*)ctx->adapt_counts);
+  count_launch();
+  st->win_steps = 0;
+  BEST_CUDA(cudaGetLastError());
+  return BEST_OK;
+}
 
 int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin, bool adapt,
                cudaStream_t s) {
@@ -331,38 +342,70 @@ int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin,
                                            trace + (size_t)slot * st->B * ctx->d);
     count_launch();
   }
-  if (adapt && ctx->adapt_every > 0) {
-    const int nblk = (int)((st->B + COV_TPB - 1) / COV_TPB);
+  if (adapt && st->adapt_every > 0) {
+    const int nblk = (int)((st->B + COV_TPB - 1) / COV_TPB);   // <= st->cov_blocks (adapt_reset)
     k_cov_accumulate<<<nblk, COV_TPB, sizeof(double) * ctx->d * COV_TPB, s>>>(
-        st->theta, st->B, ctx->d, ctx->cov_ref, ctx->cov_acc);
+        st->theta, st->B, ctx->d, st->cov_ref, st->cov_acc);
     count_launch();
-    if (++ctx->win_steps >= ctx->adapt_every) {
-      k_cov_finalize<<<1, 256, 0, s>>>(ctx->cov_acc, nblk, ctx->d, ctx->jitter, ctx->L_dev,
-                                       ctx->Lraw_dev, ctx->scale_dev, (long long*)ctx->adapt_counts);
-      count_launch();
-      ctx->win_steps = 0;
-    }
+    if (++st->win_steps >= st->adapt_every) BEST_TRY(close_window(ctx, st, s));
   }
   return BEST_OK;
 }
 
+int adapt_window_rows(best_ctx* ctx, best_state* st, const float* rows, int64_t n_steps, cudaStream_t s) {
+  const int d = ctx->d;
+  k_gram_window<<<st->cov_blocks / 2, G_TPB, 0, s>>>(rows, st->win_steps * st->B, n_steps * st->B, d, st->cov_ref,
+                                                     st->cov_acc);
+  count_launch();
+  st->win_steps += n_steps;
+  if (st->win_steps >= st->adapt_every) BEST_TRY(close_window(ctx, st, s));
+  BEST_CUDA(cudaGetLastError());
+  return BEST_OK;
+}
+
+void adapt_free(best_state* st) {
+  cudaFree(st->cov_acc); cudaFree(st->cov_ref); cudaFree(st->win_buf);
+  st->cov_acc = nullptr; st->cov_ref = nullptr; st->win_buf = nullptr;
+  st->cov_blocks = 0; st->win_cap_steps = 0;
+}
+
+// Opens a fresh window for `st`: zeroed per-block sums, shift = chain 0's current position (any fixed
+// reference removes the large mean^2 term), and on the tensor path the window buffer the persistent kernel
+// writes its post-accept states to (at most 256 MB: longer windows are fed to the Gram kernel in segments).
 int adapt_reset(best_ctx* ctx, best_state* st, cudaStream_t s) {
-  const int nblk = (int)((st->B + COV_TPB - 1) / COV_TPB);
-  const size_t ne = 1 + ctx->d + (size_t)ctx->d * ctx->d;
-  if (nblk > ctx->cov_blocks) {
-    if (ctx->cov_acc) cudaFree(ctx->cov_acc);
-    ctx->cov_acc = nullptr;
-    BEST_CUDA(cudaMalloc(&ctx->cov_acc, sizeof(double) * ne * nblk));
-    ctx->cov_blocks = nblk;
+  const int d = ctx->d;
+  const size_t ne = 1 + d + (size_t)d * d;
+  int nblk;
+  int64_t cap = 0;
+  if (ctx->precision == BEST_PREC_BF16) {
+    cap = (int64_t)((256ull << 20) / ((size_t)st->B * d * sizeof(float)));
+    cap = cap < 1 ? 1 : (cap > st->adapt_every ? st->adapt_every : cap);
+    // grid of the window's Gram kernel: one CTA per 64-row tile up to two per SM, fixed for the whole window
+    // (with the window length and B it determines the summation order); two partial sets (row parity) per CTA
+    const int64_t tiles = (st->B * (int64_t)st->adapt_every + G_ROWS - 1) / G_ROWS;
+    nblk = 2 * (int)(tiles < 296 ? tiles : 296);
+  } else {
+    nblk = (int)((st->B + COV_TPB - 1) / COV_TPB);
   }
-  BEST_CUDA(cudaMemsetAsync(ctx->cov_acc, 0, sizeof(double) * ne * ctx->cov_blocks, s));
-  // shift = chain 0's current position (any fixed reference removes the large mean^2 term)
-  std::vector<double> ref(ctx->d);
-  BEST_CUDA(cudaStreamSynchronize(s));
-  for (int i = 0; i < ctx->d; ++i)
-    BEST_CUDA(cudaMemcpy(&ref[i], st->theta + (size_t)i * st->B, sizeof(double), cudaMemcpyDeviceToHost));
-  BEST_CUDA(cudaMemcpy(ctx->cov_ref, ref.data(), sizeof(double) * ctx->d, cudaMemcpyHostToDevice));
-  ctx->win_steps = 0;
+  if (nblk > st->cov_blocks) {
+    cudaFree(st->cov_acc);
+    st->cov_acc = nullptr; st->cov_blocks = 0;
+    BEST_TRY(dev_alloc(&st->cov_acc, ne * nblk));
+    st->cov_blocks = nblk;
+  }
+  if (!st->cov_ref) BEST_TRY(dev_alloc(&st->cov_ref, (size_t)d));
+  if (cap > st->win_cap_steps) {
+    cudaFree(st->win_buf);
+    st->win_buf = nullptr; st->win_cap_steps = 0;
+    BEST_TRY(dev_alloc(&st->win_buf, (size_t)cap * st->B * d));
+    st->win_cap_steps = cap;
+  } else if (cap > 0) {
+    st->win_cap_steps = cap;
+  }
+  BEST_CUDA(cudaMemsetAsync(st->cov_acc, 0, sizeof(double) * ne * st->cov_blocks, s));
+  BEST_CUDA(cudaMemcpy2DAsync(st->cov_ref, sizeof(double), st->theta, sizeof(double) * st->B, sizeof(double), d,
+                              cudaMemcpyDeviceToDevice, s));
+  st->win_steps = 0;
   return BEST_OK;
 }
 

@@ -10,12 +10,6 @@
 // instruction count: 32-bit shared-space addresses, packed f32x2 math, one MUFU per element,
 // per-thread addresses hoisted into EpiCtx.
 #pragma once
-#ifndef BEST_TC_DBG_NODACT
-#define BEST_TC_DBG_NODACT 0
-#endif
-#ifndef BEST_TC_DBG_NOFENCE
-#define BEST_TC_DBG_NOFENCE 0
-#endif
 
 namespace best {
 namespace tc {
@@ -43,17 +37,9 @@ struct EpiCtx {
   uint8_t* aimg_thr;        // L2-image tiles: global image of the next A operand, this thread's first 16-B piece
 };
 
-// arrive on a barrier the MMA issuer waits on: the CTA's own, or (second CTA of a pair) the leader's
-// BEST_TC_WARP_ARRIVE = 1: ONE arrival per warp (lane 0, after __syncwarp has ordered the other lanes' fences
-// before it) instead of one per thread: a barrier phase then takes 8-32 same-address mbarrier updates (half of
-// them remote in a CTA pair) instead of 256-1024.  Every call site is warp-uniform.  Parity-green but measured
-// 1-2 % SLOWER on every workload on B200 (default line 1.206e8 -> 1.194e8, MH 16k 6.55e8 -> 6.41e8, AIES 1.59e8 ->
-// 1.56e8): the extra warp barrier costs more than the same-address arrivals did, so it is off.
+// arrive on a barrier the MMA issuer waits on: the CTA's own, or (second CTA of a pair) the leader's.
+// One arrival per THREAD: one per warp (lane 0 after __syncwarp) was measured 1-2 % slower on B200.
 __device__ __forceinline__ void arrive_mma(const EpiCtx& C, uint32_t bar) {
-#if BEST_TC_WARP_ARRIVE
-  __syncwarp();
-  if ((C.row & 31) != 0) return;
-#endif
   if (C.to_leader) ptx::mbar_arrive_leader(bar);
   else ptx::mbar_arrive(bar);
 }
@@ -97,18 +83,14 @@ __device__ __forceinline__ void store_a(const EpiCtx& C, int jn, const uint32_t 
 
 __device__ __forceinline__ void qbar(const EpiCtx& C) { ptx::named_bar_sync(1 + (C.row >> 5), 128); }
 
-#ifndef BEST_TC_FAST_ACT
-#define BEST_TC_FAST_ACT 1
-#endif
-// With the fast SiLU the forward weights and biases of every hidden layer are packed pre-scaled by
-// 1/2 (exact in bf16), so the accumulator holds a/2 and
+// The forward weights and biases of every SiLU hidden layer are packed pre-scaled by 1/2 (exact in
+// bf16), so the accumulator holds a/2 and
 //   t = tanh(a/2):  sigma(a) = (1+t)/2,  h = a sigma = (a/2)(1+t),  h' = sigma + h (1 - sigma)
 // costs one MUFU and four FFMA2 per element pair.  tanh.approx has ~2^-11 relative error, below
 // the 2^-9 of the bf16 rounding that follows.
-constexpr bool kSiluHalfPrescale = (BEST_TC_FAST_ACT != 0);
+constexpr bool kSiluHalfPrescale = true;
 
 __device__ __forceinline__ void silu_pair(f32x2 a, f32x2& h, f32x2& dact) {
-#if BEST_TC_FAST_ACT
   float x0, x1;
   ptx::unpack2(a, x0, x1);   // a holds (pre-activation)/2
   const f32x2 t = ptx::pack2(ptx::tanh_approx(x0), ptx::tanh_approx(x1));
@@ -116,22 +98,6 @@ __device__ __forceinline__ void silu_pair(f32x2 a, f32x2& h, f32x2& dact) {
   const f32x2 sg = ptx::fma2(t, ptx::pack2(0.5f, 0.5f), ptx::pack2(0.5f, 0.5f));
   const f32x2 om = ptx::fma2(t, ptx::pack2(-0.5f, -0.5f), ptx::pack2(0.5f, 0.5f));
   dact = ptx::fma2(h, om, sg);
-#else
-  // ex2.approx + bit-trick reciprocal + 2 Newton steps on the FMA pipe (sigma to ~2e-4 relative)
-  float x0, x1;
-  ptx::unpack2(ptx::mul2(a, ptx::pack2(-1.4426950408889634f, -1.4426950408889634f)), x0, x1);
-  const f32x2 e = ptx::pack2(ptx::ex2_approx(fminf(x0, 80.0f)), ptx::ex2_approx(fminf(x1, 80.0f)));
-  const f32x2 ns = ptx::fma2(e, ptx::pack2(-1.0f, -1.0f), ptx::pack2(-1.0f, -1.0f));  // -(1+e)
-  uint32_t n0, n1;
-  ptx::unpack2u(ns, n0, n1);
-  f32x2 r = ptx::pack2u(0xFEF311C7u - n0, 0xFEF311C7u - n1);
-  const f32x2 two = ptx::pack2(2.0f, 2.0f);
-  r = ptx::mul2(r, ptx::fma2(ns, r, two));
-  r = ptx::mul2(r, ptx::fma2(ns, r, two));
-  h = ptx::mul2(a, r);
-  const f32x2 omr = ptx::fma2(r, ptx::pack2(-1.0f, -1.0f), ptx::pack2(1.0f, 1.0f));
-  dact = ptx::fma2(h, omr, r);
-#endif
 }
 __device__ __forceinline__ void tanh_pair(f32x2 a, f32x2& h, f32x2& dact) {
   float x0, x1;
@@ -148,26 +114,14 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   uint32_t hi[4], lo[4];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
-#if BEST_TC_ACT_F16
-    const uint32_t h2 = ptx::cvt_f16x2(th[2 * i], th[2 * i + 1]);
-    float b0, b1;
-    ptx::unpack2(ptx::f16x2_to_f32x2(h2), b0, b1);
-    hi[i] = h2;
-    lo[i] = ptx::cvt_f16x2(th[2 * i] - b0, th[2 * i + 1] - b1);
-#else
     const uint32_t h2 = ptx::pack_bf16x2(th[2 * i], th[2 * i + 1]);
     hi[i] = h2;
     lo[i] = ptx::pack_bf16x2(th[2 * i] - ptx::bf16_lo(h2), th[2 * i + 1] - ptx::bf16_hi(h2));
-#endif
   }
   const uint32_t rowa = C.sbase + SmemLayout::A + C.row * 128;
   ptx::sts_128(rowa + (((uint32_t)C.k ^ (C.row & 7)) << 4), hi[0], hi[1], hi[2], hi[3]);
   ptx::sts_128(rowa + (((uint32_t)(4 + C.k) ^ (C.row & 7)) << 4), lo[0], lo[1], lo[2], lo[3]);
-#if BEST_TC_CONSUMER_FENCE
-  if (!Geo<ROWS>::kInPlace) ptx::fence_proxy_async();
-#else
   ptx::fence_proxy_async();
-#endif
   if ((!Geo<ROWS>::kInPlace)) {
     ptx::mbar_arrive(C.bars.xin_done());   // warp 3 publishes a_ready
   } else {
@@ -196,37 +150,6 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, co
     for (int i = 0; i < 4; ++i) ptx::lds_c2x64(C.wouts_thr + jn * 256 + i * 16, ws[2 * i], ws[2 * i + 1]);
   }
   uint32_t dp[8];
-#if BEST_TC_ACT_F16
-  // fp16x2 epilogue: a' = (acc + bias) rounded to fp16 (prescaled by 1/2 for SiLU), ONE MUFU per pair,
-  // four HFMA2; the results are already the packed fp16 operand / act' words.
-  constexpr uint32_t kHalf = 0x38003800u, kNegHalf = 0xB800B800u, kOne = 0x3C003C00u;
-#pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const f32x2 a32 = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), b[i]);
-    const uint32_t a = ptx::cvt_f16x2_from(a32);
-    const uint32_t t = ptx::tanh_f16x2(a);
-    uint32_t h, dd;
-    if (ACT == BEST_ACT_SILU) {
-      h = ptx::hfma2(a, t, a);
-      const uint32_t sg = ptx::hfma2(t, kHalf, kHalf);
-      const uint32_t om = ptx::hfma2(t, kNegHalf, kHalf);
-      dd = ptx::hfma2(h, om, sg);
-    } else {
-      h = t;
-      dd = ptx::hfma2(ptx::hneg2(t), t, kOne);
-    }
-    if (LAST) {
-      // the scalar output keeps an fp32 path: h in fp32 from the fp16 tanh
-      const f32x2 t32 = ptx::f16x2_to_f32x2(t);
-      const f32x2 h32 = (ACT == BEST_ACT_SILU) ? ptx::fma2(a32, t32, a32) : t32;
-      acc2 = ptx::fma2(h32, ws[i], acc2);
-      if (want_grad) hp[i] = ptx::hmul2(dd, ptx::cvt_f16x2_from(ws[i]));
-    } else {
-      hp[i] = h;
-      dp[i] = dd;
-    }
-  }
-#else
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     const f32x2 a = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), b[i]);
@@ -240,8 +163,7 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, co
       dp[i] = ptx::pack_bf16x2_from(dd);
     }
   }
-#endif
-  if (!LAST && want_grad && !BEST_TC_DBG_NODACT) {
+  if (!LAST && want_grad) {
     uint8_t* dptr = dact_l + (size_t)jn * kDBlk;
     ptx::stg_128(dptr, dp[0], dp[1], dp[2], dp[3]);
     ptx::stg_128(dptr + kDPiece, dp[4], dp[5], dp[6], dp[7]);
@@ -252,9 +174,7 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, co
 template <int ROWS>
 __device__ __forceinline__ void publish_a(EpiCtx& C, int jn0, int n) {
   if (Geo<ROWS>::kInPlace) {
-#if !BEST_TC_CONSUMER_FENCE && !BEST_TC_DBG_NOFENCE
     ptx::fence_proxy_async();
-#endif
     for (int i = 0; i < n; ++i) arrive_mma(C, C.bars.a_ready(jn0 + i));
   }
 }
@@ -265,21 +185,6 @@ __device__ __forceinline__ void publish_a(EpiCtx& C, int jn0, int n) {
 // halves, same grp) completes two CONSECUTIVE k-chunks of the next operand.
 __device__ __forceinline__ int pair_jn(const OpDesc& op, int c, int half, int grp, int ngrp) {
   return op.perm ? c * (op.ncols >> 6) + grp * 2 + half : c * (op.ncols >> 6) + half * ngrp + grp;
-}
-
-// Order in which a thread walks the 64-column groups of an N-chunk.  BEST_TC_STAGGER (off): the warps of the
-// odd row quarters swap neighbouring groups, so that half of the epilogue warps are in their TMEM-load /
-// MUFU phase while the other half stores (single-CTA in-place tiles only; the pair kernels' issue order
-// relies on rounds completing consecutive k-chunks).  Measured A/B on B200, 16k chains on 27->512^4->1:
-// HMC -4 %, MALA -2 %, MH +0.7 % -- the first k-chunk of the next operand completes a round later, which
-// costs more than the phase overlap gains.
-#ifndef BEST_TC_STAGGER
-#define BEST_TC_STAGGER 0
-#endif
-template <int ROWS>
-__device__ __forceinline__ int stagger(const EpiCtx& C, int g0, int ngrp) {
-  if (BEST_TC_STAGGER && ROWS == 128 && (ngrp & 1) == 0) return g0 ^ (int)((C.row >> 5) & 1u);
-  return g0;
 }
 
 // forward epilogue of one op
@@ -298,7 +203,7 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
     const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && writes_a && (c != op.nch - 1);
     for (int g0 = 0; g0 < ngrp; ++g0) {
-      const int grp = stagger<ROWS>(C, g0, ngrp);
+      const int grp = g0;
       const int jn = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, grp, ngrp) : c * ngrp + grp;
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
@@ -327,12 +232,8 @@ __device__ __forceinline__ void bwd_group(const uint32_t (&v)[16], const uint4& 
   const uint32_t dw[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
-#if BEST_TC_ACT_F16
-    hp[i] = ptx::hmul2(ptx::cvt_f16x2(__uint_as_float(v[2 * i]), __uint_as_float(v[2 * i + 1])), dw[i]);
-#else
     const f32x2 dd = ptx::pack2u(dw[i] << 16, dw[i] & 0xFFFF0000u);
     hp[i] = ptx::pack_bf16x2_from(ptx::mul2(ptx::pack2u(v[2 * i], v[2 * i + 1]), dd));
-#endif
   }
 }
 template <int ROWS>
@@ -349,9 +250,8 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
   uint4 a0, a1;
   {
     const int jnc0 = Geo<ROWS>::kPair ? pair_jn(op, 0, C.half, 0, ngrp) : 0;
-    const uint8_t* dp = dact_l + (size_t)(jnc0 + stagger<ROWS>(C, 0, ngrp) * jstep) * kDBlk;
-    if (BEST_TC_DBG_NODACT) { a0 = make_uint4(0x3f803f80u, 0x3f803f80u, 0x3f803f80u, 0x3f803f80u); a1 = a0; }
-    else { a0 = ptx::ldg_128(dp); a1 = ptx::ldg_128(dp + kDPiece); }
+    const uint8_t* dp = dact_l + (size_t)jnc0 * kDBlk;
+    a0 = ptx::ldg_128(dp); a1 = ptx::ldg_128(dp + kDPiece);
   }
   for (int c = 0; c < op.nch; ++c, ++C.g) {
     const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
@@ -362,14 +262,14 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
     for (int g0 = 0; g0 < ngrp; ++g0) {
-      const int grp = stagger<ROWS>(C, g0, ngrp);
+      const int grp = g0;
       const int jn = jnc + grp * jstep;
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
       const uint4 d0 = a0, d1 = a1;
-      if ((g0 + 1 < ngrp || c + 1 < op.nch) && !BEST_TC_DBG_NODACT) {   // prefetch the next group's act'
-        const int jnn = (g0 + 1 < ngrp) ? jnc + stagger<ROWS>(C, g0 + 1, ngrp) * jstep
-                                        : jnc_next + stagger<ROWS>(C, 0, ngrp) * jstep;
+      if (g0 + 1 < ngrp || c + 1 < op.nch) {   // prefetch the next group's act'
+        const int jnn = (g0 + 1 < ngrp) ? jnc + (g0 + 1) * jstep
+                                        : jnc_next;
         const uint8_t* dn = dact_l + (size_t)jnn * kDBlk;
         a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
       }

@@ -16,6 +16,7 @@
 // the forward and backward sweeps.  See DESIGN.md §"tensor-core kernel".
 #include <cuda.h>
 
+#include <algorithm>
 #include <cstdlib>
 #include <cstring>
 
@@ -88,42 +89,6 @@ constexpr int kCtrlWarps = 4;          // producer, MMA issuer, TMEM allocator, 
 constexpr int kEpiWarps = 16;          // 4 per TMEM lane quarter
 constexpr int kEpiThreads = kEpiWarps * 32;
 constexpr int kThreads = (kCtrlWarps + kEpiWarps) * 32;
-// Operand type option: 1 = fp16 weights AND activations (kind::f16 needs equal operand formats; mixed
-// fp16 x bf16 traps), packed HFMA2 epilogue math with one MUFU per element PAIR.  Measured on B200
-// (27->512^4->1): gradient error 5.8e-3 instead of 1.49e-2, same speed (984 vs 998 TFLOP/s: the
-// epilogue is latency-, not math-bound).  Default 0 = bf16, the type BASELINE.json names.
-#ifndef BEST_TC_ACT_F16
-#define BEST_TC_ACT_F16 0
-#endif
-// 1 = the generic->async proxy fence is executed by the MMA warp after it has acquired a_ready instead
-// of by every epilogue thread before its arrive.  Parity-green and 1 % faster on B200 (1006 vs 998
-// TFLOP/s), but the documented pattern is the writer-side fence, so that is the default.
-#ifndef BEST_TC_CONSUMER_FENCE
-#define BEST_TC_CONSUMER_FENCE 0
-#endif
-// Two register-allocation experiments, both measured SLOWER on B200 (HMC 16k chains: 1006 TFLOP/s
-// with neither, 938 with pinned per-thread constants, 881 with setmaxnreg 40/104) and so off:
-// Timing decomposition of the pair kernels (build-time, results are garbage): bit 0 = the producer signals full
-// stages without loading, bit 1 = no MMAs are issued; BEST_TC_DBG_NODACT / _NOFENCE (tc_epilogue.cuh) drop the act'
-// scratch traffic / the proxy fence.  Measured on B200, geometry 233, default line (ms per 100 MALA steps): full
-// 3.39-3.48, no loads 3.42, no MMAs 3.05, neither 2.95, no act' traffic 3.22 (2.67 with neither), no fence 3.44:
-// 85 % of a step is the epilogue/sampler chain alone.  (As a run-time flag the check cost 2.5 % in the issue loop.)
-#ifndef BEST_TC_WARP_ARRIVE
-#define BEST_TC_WARP_ARRIVE 0
-#endif
-#ifndef BEST_TC_DBG_SKIP
-#define BEST_TC_DBG_SKIP 0
-#endif
-#ifndef BEST_TC_SETMAXNREG
-#define BEST_TC_SETMAXNREG 0
-#endif
-#ifndef BEST_TC_OPAQUE
-#define BEST_TC_OPAQUE 0
-#endif
-// setmaxnreg moves registers inside the CTA's own allocation (640 threads x 96 at launch): what the
-// control warpgroup gives up is all the epilogue warps can take, or setmaxnreg.inc never returns.
-constexpr int kLaunchRegs = 96, kCtrlRegs = 40, kEpiRegs = 104;
-static_assert(kCtrlWarps * 32 * kCtrlRegs + kEpiThreads * kEpiRegs <= kThreads * kLaunchRegs, "register pool");
 constexpr int kDP = 32;              // parameter vectors are padded to 32 inside the kernel
 
 enum { EPI_FWD_HID = 0, EPI_FWD_LAST = 1, EPI_BWD_HID = 2, EPI_BWD_FINAL = 3 };
@@ -178,6 +143,14 @@ struct Run {
   // AIES
   int64_t own0, oth0;
   int de;               // differential-evolution move (eq 2.16) instead of the stretch move; eps = sigma_gamma
+  // Philox chain id = chain0 + chain index (multi-GPU shards draw disjoint streams)
+  uint32_t chain0;
+  // A8: post-accept theta written by the kernel itself, fp32 rows [slot][B_rows][d]:
+  //   trace: slot (t_call0 + t + 1) / thin - 1 whenever thin divides t_call0 + t + 1 (t = step inside this launch);
+  //   win:   slot t, every step (the covariance window buffer of A9)
+  float* trace; int thin; int64_t t_call0;
+  float* win;
+  int64_t B_rows;       // chains per trace / window slot (= the state's chain count)
 };
 
 // shared-memory carve-up (dynamic, 1024-byte aligned base)
@@ -270,7 +243,7 @@ __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uin
   for (int64_t e = 0; e < n_evals; ++e) {
     for (int oi = 0; oi < n_ops; ++oi, ++o) {
       const OpDesc op = P.ops[oi];
-      const uint32_t idesc = BEST_TC_ACT_F16 ? ptx::idesc_f16(kRows, op.ncols) : ptx::idesc_bf16(kRows, op.ncols);
+      const uint32_t idesc = ptx::idesc_bf16(kRows, op.ncols);
       // chunks this op does not read are free as soon as everything issued so far has completed
       if (elect_one())
         for (int j = op.kch; j < P.kch_max; ++j) ptx::mma_commit(bars.a_free(j));
@@ -284,12 +257,6 @@ __device__ void mma_loop(const Params& P, const Bars& bars, uint32_t a_base, uin
         for (int j = 0; j < op.kch; ++j) {
           if (c == 0) {
             ptx::mbar_wait(bars.a_ready(j), o & 1u);
-#if BEST_TC_CONSUMER_FENCE
-            // the epilogue's generic-proxy st.shared (released by its mbarrier.arrive, acquired by the
-            // wait above) become visible to the async proxy HERE: the proxy fence costs the epilogue
-            // warps a MEMBAR.ALL.CTA per 64-column group, the idle-storeless MMA warp almost nothing
-            if (Geo<ROWS>::kInPlace) ptx::fence_proxy_async();
-#endif
             ptx::tc_fence_after();
           }
 #pragma unroll
@@ -375,13 +342,9 @@ __device__ void producer_loop_pair(const Params& P, const Bars& bars, uint32_t s
         ptx::mbar_wait(bars.empty(s), (use & 1u) ^ 1u);
         if (elect_one()) {
           // all four halves' bytes land on the LEADER's full barrier; only the leader arrives on it
-          if (BEST_TC_DBG_SKIP & 1) {
-            if (rank == 0) ptx::mbar_arrive(bars.full(s));
-          } else {
-            if (rank == 0) ptx::mbar_arrive_expect_tx(bars.full(s), 2u * bytes);
-            ptx::tma_2sm_load_2d(stage_base + s * SB, tmap, bars.full(s), 0, (int)((src + rank * half) >> 8));
-            ptx::tma_2sm_load_2d(stage_base + s * SB + half, tmap, bars.full(s), 0, (int)((src + bytes + rank * half) >> 8));
-          }
+          if (rank == 0) ptx::mbar_arrive_expect_tx(bars.full(s), 2u * bytes);
+          ptx::tma_2sm_load_2d(stage_base + s * SB, tmap, bars.full(s), 0, (int)((src + rank * half) >> 8));
+          ptx::tma_2sm_load_2d(stage_base + s * SB + half, tmap, bars.full(s), 0, (int)((src + bytes + rank * half) >> 8));
         }
         __syncwarp();
         src += 2u * bytes;
@@ -470,12 +433,10 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
             const uint64_t ad = adesc0 + (uint64_t)((j * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? (oi & 1) * Geo<ROWS>::kPPStride : 0)) >> 4);
             const uint64_t bd = bdesc0 + (uint64_t)((s * SB) >> 4);
             if (elect_one()) {
-              if (!(BEST_TC_DBG_SKIP & 2)) {
-                ptx::mma_bf16_ss_2cta(d_tmem, ad, bd, idesc, j != 0 ? 1u : 0u);
-                ptx::mma_bf16_ss_2cta(d_tmem, ad + 2, bd + 2, idesc, 1u);
-                ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
-                ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
-              }
+              ptx::mma_bf16_ss_2cta(d_tmem, ad, bd, idesc, j != 0 ? 1u : 0u);
+              ptx::mma_bf16_ss_2cta(d_tmem, ad + 2, bd + 2, idesc, 1u);
+              ptx::mma_bf16_ss_2cta(d_tmem, ad + 4, bd + half16, idesc, 1u);
+              ptx::mma_bf16_ss_2cta(d_tmem, ad + 6, bd + half16 + 2, idesc, 1u);
               ptx::mma_commit_2cta(bars.empty(s));
               if (last_c && !Geo<ROWS>::kPingPong) { ptx::mma_commit_2cta(bars.a_free(j)); ptx::mma_commit_2cta(bars.a_free(j)); }
             }

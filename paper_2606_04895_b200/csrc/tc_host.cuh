@@ -8,6 +8,21 @@ namespace tc {
 // Sampler driver: executed by all 512 epilogue threads; thread (row, k) owns dims [8k, 8k+8) of
 // chain `row`.  Scalars (log pi, log alpha, accept) are computed redundantly and identically by the
 // four threads of a chain, so they take the same accept branch.
+// A8: the post-accept theta of chain `chain` (own 8 dims) into row-major fp32 rows [slot][B_rows][d]
+__device__ __forceinline__ void emit_rows(const EpiCtx& C, const Run& R, int64_t t, int64_t chain, int d,
+                                          const float (&cur)[8]) {
+  if (R.trace && (R.t_call0 + t + 1) % R.thin == 0) {
+    float* dst = R.trace + (((R.t_call0 + t + 1) / R.thin - 1) * R.B_rows + chain) * d + 8 * C.k;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) if (8 * C.k + i < d) dst[i] = cur[i];
+  }
+  if (R.win) {
+    float* dst = R.win + (t * R.B_rows + chain) * d + 8 * C.k;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) if (8 * C.k + i < d) dst[i] = cur[i];
+  }
+}
+
 template <int METHOD, int ROWS>
 __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
   const Params& P = *C.P;
@@ -45,28 +60,29 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
 
   if (METHOD == M_AIES) {
     const int64_t i = R.own0 + r_in_launch;
-    const uint4 w = philox4x32_10((uint32_t)i, R.step0, 0u, R.seed);
+    const uint32_t cid = R.chain0 + (uint32_t)i;
+    const uint4 w = philox4x32_10(cid, R.step0, 0u, R.seed);
     const int64_t j = R.oth0 + (int64_t)__umulhi(w.z, (uint32_t)R.B);
     const float a = R.eps;
     const float t = u01<float>(w.y) * (a - 1.0f) + 1.0f;
     const float z = t * t / a;
-    float thp[8], g[8], lpp;
+    float thp[8], thi[8], g[8], lpp;
     if (R.de) {
       // eq (2.16), reading R23: x' = x_i + gamma (x_j - x_k), k != j from the same half, R.eps = sigma_gamma
       int64_t kr = (int64_t)__umulhi(w.w, (uint32_t)(R.B - 1));
       if (kr >= j - R.oth0) kr += 1;
-      const uint4 wn = philox4x32_10((uint32_t)i, R.step0, 1u, R.seed);
+      const uint4 wn = philox4x32_10(cid, R.step0, 1u, R.seed);
       float n0, n1;
       box_muller(wn.x, wn.y, n0, n1);
       const float gamma = (1.0f + R.eps * n0) * (2.38f / sqrtf(2.0f * (float)d));
-      float thi[8], thj[8], thk[8];
+      float thj[8], thk[8];
       load_vec8(C, R.theta, R.ld, i, d, valid, thi);
       load_vec8(C, R.theta, R.ld, j, d, valid, thj);
       load_vec8(C, R.theta, R.ld, R.oth0 + kr, d, valid, thk);
 #pragma unroll
       for (int q = 0; q < 8; ++q) thp[q] = thi[q] + gamma * (thj[q] - thk[q]);
     } else {
-      float thi[8], thj[8];
+      float thj[8];
       load_vec8(C, R.theta, R.ld, i, d, valid, thi);
       load_vec8(C, R.theta, R.ld, j, d, valid, thj);
 #pragma unroll
@@ -81,10 +97,16 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
       R.last_la[i] = (double)la;
       if (acc) { R.logp[i] = (double)lpp; R.n_accept[i] += 1ull; }
     }
+    if (R.trace && valid) {   // every half-ensemble launch writes its own walkers (their state is final for this step)
+      if (!acc) load_vec8(C, R.theta, R.ld, i, d, valid, thp);
+      emit_rows(C, R, 0, i, d, thp);
+    }
     return;
   }
 
   const int64_t c = r_in_launch;
+  const uint32_t cid = R.chain0 + (uint32_t)c;
+  const bool rows_out = (R.trace != nullptr) || (R.win != nullptr);
   const float eps = R.eps;
   float lp = valid ? (float)R.logp[c] : 0.0f;
   float la_last = 0.0f;
@@ -98,7 +120,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
       float thp[8], g[8], lpp;
       {
         float xi[8], dx[8];
-        draw_normals8(C, R.seed, (uint32_t)c, step, d, xi);
+        draw_normals8(C, R.seed, cid, step, d, xi);
 #pragma unroll
         for (int i = 0; i < 8; ++i) xi[i] *= eps;
         mv_L(C, xi, dx);
@@ -108,13 +130,14 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
       eval_target<ROWS>(C, thp, false, lpp, g);
       const float la = lpp - lp;
       la_last = la;
-      const uint4 w = philox4x32_10((uint32_t)c, step, 0u, R.seed);
+      const uint4 w = philox4x32_10(cid, step, 0u, R.seed);
       if (valid && accept_rule<float>(u01<float>(w.x), la)) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) th[i] = thp[i];
         lp = lpp;
         ++nacc;
       }
+      if (rows_out && valid) emit_rows(C, R, t, c, d, th);
     }
     if (valid) store_vec8(C, R.theta, R.ld, c, d, th);
   }
@@ -128,7 +151,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
         float g[8], gz[8], xi[8];
         load_vec8(C, R.grad, R.ld, c, d, valid, g);
         mv_Lt(C, g, gz);
-        draw_normals8(C, R.seed, (uint32_t)c, step, d, xi);
+        draw_normals8(C, R.seed, cid, step, d, xi);
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
           const float f = sq * xi[i];
@@ -154,12 +177,17 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
       }
       const float la = lpp - lp + reduce4(C, diff) / (4.0f * eps);
       la_last = la;
-      const uint4 w = philox4x32_10((uint32_t)c, step, 0u, R.seed);
-      if (valid && accept_rule<float>(u01<float>(w.x), la)) {
+      const uint4 w = philox4x32_10(cid, step, 0u, R.seed);
+      const bool acc = valid && accept_rule<float>(u01<float>(w.x), la);
+      if (acc) {
         store_vec8(C, R.theta, R.ld, c, d, thp);
         store_vec8(C, R.grad, R.ld, c, d, gp);
         lp = lpp;
         ++nacc;
+      }
+      if (rows_out && valid) {
+        if (!acc) load_vec8(C, R.theta, R.ld, c, d, valid, thp);
+        emit_rows(C, R, t, c, d, thp);
       }
     }
   }
@@ -170,7 +198,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
       float thw[8], q[8], gw[8], lpw = lp, kin0 = 0.0f;
       {
         float g[8], gz[8];
-        draw_normals8(C, R.seed, (uint32_t)c, step, d, q);
+        draw_normals8(C, R.seed, cid, step, d, q);
 #pragma unroll
         for (int i = 0; i < 8; ++i) kin0 = fmaf(q[i], q[i], kin0);
         load_vec8(C, R.grad, R.ld, c, d, valid, g);
@@ -201,12 +229,17 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
       // log alpha = H0 - H1 = (lp' - lp) + (|q0|^2 - |q1|^2)/2
       const float la = (lpw - lp) + 0.5f * reduce4(C, kin0 - kin1);
       la_last = la;
-      const uint4 w = philox4x32_10((uint32_t)c, step, 0u, R.seed);
-      if (valid && accept_rule<float>(u01<float>(w.x), la)) {
+      const uint4 w = philox4x32_10(cid, step, 0u, R.seed);
+      const bool acc = valid && accept_rule<float>(u01<float>(w.x), la);
+      if (acc) {
         store_vec8(C, R.theta, R.ld, c, d, thw);
         store_vec8(C, R.grad, R.ld, c, d, gw);
         lp = lpw;
         ++nacc;
+      }
+      if (rows_out && valid) {
+        if (!acc) load_vec8(C, R.theta, R.ld, c, d, valid, thw);
+        emit_rows(C, R, t, c, d, thw);
       }
     }
   }
@@ -235,7 +268,6 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   float* vecs = reinterpret_cast<float*>(smem + SmemLayout::VECS);
   volatile uint32_t* tmem_ptr = reinterpret_cast<volatile uint32_t*>(smem + SmemLayout::TMEMPTR);
 
-  constexpr int kArr = BEST_TC_WARP_ARRIVE ? 32 : 1;   // threads per arrival on the barriers the MMA issuer waits on
   if (tid == 0) {
     for (int i = 0; i < 8; ++i) {
       ptx::mbar_init(bars.full(i), 1); ptx::mbar_init(bars.empty(i), 1);
@@ -243,12 +275,12 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     for (int i = 0; i < kMaxKch; ++i) {
       // arrivals per phase: in place = every epilogue thread (pair: the 256 of the lane half that owns the
       // k-chunk); L2-image tiles = warp 3 alone (+ the bulk copy's bytes)
-      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : Geo<ROWS>::kEpiArrive / kArr);   // pair: half of each CTA's
+      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : Geo<ROWS>::kEpiArrive);   // pair: half of each CTA's
       ptx::mbar_init(bars.a_free(i), Geo<ROWS>::kPair ? 2 : 1);   // pair kernels: two issuing warps
     }
     for (int i = 0; i < 4; ++i) {
       ptx::mbar_init(bars.d_full(i), 1);
-      ptx::mbar_init(bars.d_free(i), (Geo<ROWS>::kPair ? 2 * Geo<ROWS>::kEpiArrive : Geo<ROWS>::kEpiActive) / kArr);   // pair: both CTAs
+      ptx::mbar_init(bars.d_free(i), Geo<ROWS>::kPair ? 2 * Geo<ROWS>::kEpiArrive : Geo<ROWS>::kEpiActive);   // pair: both CTAs
     }
     for (int i = 0; i < 4; ++i) ptx::mbar_init(bars.epi_done(i), Geo<ROWS>::kEpiActive);
     ptx::mbar_init(bars.xin_done(), Geo<ROWS>::kEpiActive);
@@ -293,10 +325,6 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   const int n_ops = R.want_grad ? P.n_ops_all : P.n_ops_fwd;
 
   if (warp < kCtrlWarps) {
-    // the control warpgroup hands most of its registers to the 16 epilogue warps
-#if BEST_TC_SETMAXNREG
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kCtrlRegs));
-#endif
     if (Geo<ROWS>::kPair) {
       const uint32_t rank = ptx::cluster_ctarank();
       if (warp == 0) {
@@ -314,9 +342,6 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
                   Geo<ROWS>::kAChunk, n_evals, n_ops);
     }
   } else {
-#if BEST_TC_SETMAXNREG
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kEpiRegs));
-#endif
     EpiCtx C;
     C.P = &P;
     C.bars = bars;
@@ -336,12 +361,6 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
                  (size_t)(2 * C.k * Geo<ROWS>::kTileRows + C.row) * 16u;
     C.aimg_thr = (!Geo<ROWS>::kInPlace) ? P.aimg + (size_t)blockIdx.x * (16u * Geo<ROWS>::kAChunk) + C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4)
                      : nullptr;
-    // per-thread constants must stay in registers: without this the compiler rematerialises them
-    // from tid / blockIdx / kernel parameters inside every epilogue group (r1b profile)
-#if BEST_TC_OPAQUE
-    asm volatile("" : "+r"(C.a_thr0), "+r"(C.a_thr1), "+r"(C.bias_thr), "+r"(C.wouts_thr), "+r"(C.v_thr),
-                      "+r"(C.tmem_lane), "+r"(C.sbase), "+l"(C.dact_thr));
-#endif
     if (C.row >= Geo<ROWS>::kChains) {
       // phantom rows (geometry 233: the odd row quarters; L2-image tiles: lanes ROWS..127): nothing to do
     } else if (Geo<ROWS>::kPair && C.half == 1) {
@@ -375,38 +394,17 @@ struct TcPlan {
   uint8_t* wpack_p = nullptr;
   tc::Params Pn{};           // geometry 233: N-chunk outer order with the permuted row blocks, own weight pack
   uint8_t* wpack_n = nullptr;
-  int order233 = 2;          // 0 = Pp (paired order), 1 = P (N-chunk outer), 2 = Pn
   float* bias = nullptr;
   float* w_out = nullptr;
   uint16_t* dact = nullptr;
   uint8_t* aimg = nullptr;
   size_t dact_cap = 0, aimg_cap = 0;
   int n_sm = 0;
-  bool no_pair = false;  // BEST_TC_ROWS=64|32 forces the single-CTA L2-image geometries
-  bool no_233 = false;   // BEST_TC_NO233 (environment, read at best_create): A/B measurements of geometry 233
-  int force_rows = 0;   // BEST_TC_ROWS=128|64|32 (environment, read at best_create): measurements only
+  int force_rows = 0;   // BEST_TC_ROWS (environment, read at best_create; documented in best.h): tests force a geometry
 };
 
 namespace {
 
-uint16_t f32_to_f16(float f) {   // round to nearest even, overflow -> inf
-  uint32_t u;
-  std::memcpy(&u, &f, 4);
-  const uint32_t sign = (u >> 16) & 0x8000u;
-  const uint32_t a = u & 0x7FFFFFFFu;
-  if (a >= 0x7F800000u) return (uint16_t)(sign | 0x7C00u | (a > 0x7F800000u ? 0x200u : 0u));
-  if (a >= 0x477FF000u) return (uint16_t)(sign | 0x7C00u);                  // >= 65520 rounds to inf
-  if (a < 0x33000001u) return (uint16_t)sign;                               // < 2^-25 rounds to zero
-  int e = (int)(a >> 23) - 127;
-  uint32_t m = (a & 0x7FFFFFu) | 0x800000u;
-  int shift = (e < -14) ? (13 + (-14 - e)) : 13;                            // subnormal: shift further
-  uint32_t half_m = m >> shift;
-  const uint32_t rem = m & ((1u << shift) - 1u), halfway = 1u << (shift - 1);
-  if (rem > halfway || (rem == halfway && (half_m & 1u))) ++half_m;
-  uint32_t he = (e < -14) ? 0u : (uint32_t)(e + 15);
-  uint32_t r = (e < -14) ? half_m : ((he << 10) + (half_m - 0x400u));      // carry propagates into exponent
-  return (uint16_t)(sign | r);
-}
 uint16_t f32_to_bf16(float f) {  // round to nearest even
   uint32_t u;
   std::memcpy(&u, &f, 4);
@@ -419,7 +417,7 @@ template <int METHOD, int ROWS>
 int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
   TcPlan* pl = ctx->tc;
   tc::Params& P = (ROWS == 265 && pl->has_pp) ? pl->Pp
-                : (ROWS == 233 && pl->has_pp) ? (pl->order233 == 0 ? pl->Pp : (pl->order233 == 1 ? pl->P : pl->Pn)) : pl->P;
+                : (ROWS == 233 && pl->has_pp) ? pl->Pn : pl->P;
   constexpr int kTileRows = tc::Geo<ROWS>::kTileRows, kChains = tc::Geo<ROWS>::kChains;
   int64_t n_tiles = (rows + kChains - 1) / kChains;
   if (tc::Geo<ROWS>::kPair) n_tiles = (n_tiles + 1) & ~(int64_t)1;   // whole CTA pairs
@@ -444,11 +442,11 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
   }
   P.dact = pl->dact;
   P.aimg = pl->aimg;
-  static bool attr_set = false;
+  static std::atomic<bool> attr_set{false};   // idempotent: a race only repeats the call
   const int smem_bytes = tc::SmemLayout::TOTAL + 1024;
-  if (!attr_set) {
+  if (!attr_set.load(std::memory_order_acquire)) {
     BEST_CUDA(cudaFuncSetAttribute(tc::best_tc_kernel<METHOD, ROWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
-    attr_set = true;
+    attr_set.store(true, std::memory_order_release);
   }
   P.L = ctx->L_dev;
   P.hard_box = ctx->tgt.hard_box;
@@ -477,7 +475,7 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
 // 1024-wide layers (whose operand does not fit in place) use 64, or 32 when that fills more SMs.
 int pick_rows(const TcPlan* pl, int64_t rows, int n_sm) {
   if (pl->force_rows) return pl->force_rows;
-  if (pl->P.H == 512 && !pl->no_pair) {
+  if (pl->P.H == 512) {
     // 512-wide: 128-chain single-CTA tiles or 64-chain CTA pairs (operand + accumulators double-buffered).
     // Measured per evaluation of one tile (HMC, B200): 52 us against 33 us, so the pairs win whenever
     // they do not need more waves of CTAs: the 4096-chain config, the small points of the sweep.
@@ -489,16 +487,14 @@ int pick_rows(const TcPlan* pl, int64_t rows, int n_sm) {
     const int64_t pair_slots = n_sm & ~1;   // CTAs of whole pairs resident at once
     const double c128 = (double)((t128 + n_sm - 1) / n_sm) * 52.0, c265 = (double)((t64 + pair_slots - 1) / pair_slots) * 33.0,
                  c233 = (double)((t32 + pair_slots - 1) / pair_slots) * 30.8;
-    if (c233 < c265 && c233 < c128 && !pl->no_233) return 233;
+    if (c233 < c265 && c233 < c128) return 233;
     return c265 < c128 ? 265 : 128;
   }
   if (pl->P.H != 1024) return 128;
-  if (!pl->no_pair) {   // CTA pairs (cta_group::2): the 1024-wide operand in place at full MMA rate
-    // 32 chains per CTA (geometry 232) while twice the CTAs still fit one wave, as 233 for 512-wide layers
-    const int64_t t32 = ((rows + 31) / 32 + 1) & ~(int64_t)1;
-    return (t32 <= (n_sm & ~1) && !pl->no_233) ? 232 : 264;
-  }
-  return (rows + 63) / 64 >= n_sm ? 64 : ((rows + 31) / 32 > (rows + 63) / 64 && rows <= 32 * (int64_t)n_sm ? 32 : 64);
+  // CTA pairs (cta_group::2): the 1024-wide operand in place at full MMA rate; 32 chains per CTA (geometry 232)
+  // while twice the CTAs still fit one wave, as 233 for 512-wide layers
+  const int64_t t32 = ((rows + 31) / 32 + 1) & ~(int64_t)1;
+  return t32 <= (n_sm & ~1) ? 232 : 264;
 }
 
 template <int METHOD>
@@ -560,7 +556,6 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   const int d = cfg->d;
   TcPlan* pl = new TcPlan();
   ctx->tc = pl;
-  pl->no_233 = std::getenv("BEST_TC_NO233") != nullptr;
   if (const char* e = std::getenv("BEST_TC_ROWS")) {
     const int v = std::atoi(e);
     if ((v == 64 || v == 32 || (v == 128 && !r64) || ((v == 264 || v == 232) && r64) || ((v == 265 || v == 233) && H == 512))) pl->force_rows = v;
@@ -630,7 +625,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
             // paired ops (CTA-pair kernels): B row blocks in the order 0,2,1,3, see pair_jn()
             const int rl = (op.perm && op.ncols == 256) ? ((((r >> 6) & 1) * 2 + (r >> 7)) << 6) + (r & 63) : r;
             const float wv = Bm(c * op.ncols + rl, k32 * 32 + kk);
-            pack[base + off] = BEST_TC_ACT_F16 ? f32_to_f16(wv) : f32_to_bf16(wv);
+            pack[base + off] = f32_to_bf16(wv);
           }
       }
     }
@@ -663,7 +658,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   P.banana_sigma = (float)ctx->tgt.banana_sigma;
   P.pen_kappa = (float)ctx->tgt.pen_kappa; P.pen_gamma = (float)ctx->tgt.pen_gamma;
   P.mu = ctx->tgt.mu; P.R = ctx->tgt.R; P.lo = ctx->tgt.lo; P.hi = ctx->tgt.hi; P.L = ctx->L_dev;
-  if (H == 512 && !(std::getenv("BEST_TC_PP_NOUTER"))) {
+  if (H == 512) {
     // geometry 265 issues the two N-chunks of a layer from two warps (k-chunk outer): same ops, paired order
     pl->Pp = P;
     for (int oi = 0; oi + 1 < P.n_ops_all; ++oi) pl->Pp.ops[oi].paired = pl->Pp.ops[oi].perm = 1;
@@ -675,7 +670,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
     if ((rc = make_wmap(&pl->Pp.wmap1, pl->wpack_p, pack_p.size() * 2, 4))) return rc;
     pl->has_pp = true;
     // geometry 233: N-chunk outer (one issuing warp; the epilogue of the first N-chunk overlaps the MMAs of
-    // the second) with the permuted row blocks, own pack.  BEST_TC_233_ORDER = paired | nouter | nperm (A/B).
+    // the second) with the permuted row blocks, own pack.
     pl->Pn = P;
     for (int oi = 0; oi + 1 < P.n_ops_all; ++oi) pl->Pn.ops[oi].perm = 1;
     const std::vector<uint16_t> pack_n = build_pack(pl->Pn);
@@ -684,8 +679,6 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
     pl->Pn.wpack = pl->wpack_n;
     if ((rc = make_wmap(&pl->Pn.wmap8, pl->wpack_n, pack_n.size() * 2, 32))) return rc;
     if ((rc = make_wmap(&pl->Pn.wmap1, pl->wpack_n, pack_n.size() * 2, 4))) return rc;
-    if (const char* e = std::getenv("BEST_TC_233_ORDER"))
-      pl->order233 = !std::strcmp(e, "paired") ? 0 : (!std::strcmp(e, "nouter") ? 1 : 2);
   }
   return BEST_OK;
 }
@@ -706,17 +699,29 @@ int tc_logp_grad(best_ctx* ctx, const float* theta_rows, int64_t n, float* logp,
   return launch_tc<tc::M_EVAL>(ctx, R, n, s);
 }
 
-int tc_state_init(best_ctx* ctx, best_state* st, cudaStream_t s) {
+// log pi and gradient at the state's theta into logp_out / grad_out (SoA fp64 [d][B]); the caller decides
+// whether these are the state's caches
+int tc_eval_state(best_ctx* ctx, best_state* st, double* logp_out, double* grad_out, cudaStream_t s) {
   tc::Run R{};
   R.method = tc::M_EVAL; R.want_grad = 1; R.io_mode = tc::IO_SOA_F64;
   R.B = st->B; R.ld = st->B; R.n_steps = 1;
-  R.theta = st->theta; R.grad = st->grad; R.logp = st->logp;
+  R.theta = st->theta; R.grad = grad_out; R.logp = logp_out;
   BEST_TRY(launch_tc<tc::M_EVAL>(ctx, R, st->B, s));
-  st->grad_valid = true;
   st->n_evals += (uint64_t)st->B;
   return BEST_OK;
 }
 
+int tc_state_init(best_ctx* ctx, best_state* st, cudaStream_t s) {
+  BEST_TRY(tc_eval_state(ctx, st, st->logp, st->grad, s));
+  st->grad_valid = true;
+  return BEST_OK;
+}
+
+// One best_step_* call = ONE persistent launch (two per step for the ensemble moves: the half-ensembles
+// depend on each other device-wide).  The kernel writes the trace slots itself.  Under covariance adaptation
+// (A9) the call is cut only where it must be: at a window boundary (the whitening factor changes there and
+// every CTA reads it at launch) and when the window buffer -- fp32 rows of every post-accept state, written by
+// the kernel -- is full; after each segment ONE Gram kernel folds the buffer into the fp64 window sums.
 int tc_step(best_ctx* ctx, best_state* st, int method, int64_t n_steps, uint64_t seed, float eps,
             int n_leapfrog, float* trace, int thin, cudaStream_t s, bool de) {
   if ((method == tc::M_MALA || method == tc::M_HMC) && !st->grad_valid) BEST_TRY(tc_state_init(ctx, st, s));
@@ -725,15 +730,23 @@ int tc_step(best_ctx* ctx, best_state* st, int method, int64_t n_steps, uint64_t
   R.want_grad = (method == tc::M_MALA || method == tc::M_HMC) ? 1 : 0;
   R.B = st->B; R.ld = st->B; R.seed = seed; R.eps = eps; R.n_leapfrog = n_leapfrog;
   R.de = de ? 1 : 0;
+  R.chain0 = (uint32_t)st->chain0;
   R.theta = st->theta; R.grad = st->grad; R.logp = st->logp; R.last_la = st->last_la; R.n_accept = st->n_accept;
-  const bool adapt = ctx->adapt_every > 0 && method != tc::M_AIES;
+  R.B_rows = st->B;
+  if (trace && thin > 0) { R.trace = trace; R.thin = thin; } else { R.trace = nullptr; R.thin = 1; }
+  const bool adapt = st->adapt_every > 0 && method != tc::M_AIES;
   int64_t t0 = 0;
   while (t0 < n_steps) {
     int64_t seg = n_steps - t0;
-    if (trace && thin > 0) { const int64_t to_boundary = thin - (t0 % thin); if (to_boundary < seg) seg = to_boundary; }
-    if (adapt || method == tc::M_AIES) seg = 1;
+    if (adapt) {
+      seg = std::min<int64_t>(seg, st->adapt_every - st->win_steps);
+      seg = std::min<int64_t>(seg, st->win_cap_steps);
+    }
+    if (method == tc::M_AIES) seg = 1;
     R.n_steps = seg;
     R.step0 = st->step + (uint64_t)t0;
+    R.t_call0 = t0;
+    R.win = adapt ? st->win_buf : nullptr;
     switch (method) {
       case tc::M_MH: BEST_TRY(launch_tc<tc::M_MH>(ctx, R, st->B, s)); break;
       case tc::M_MALA: BEST_TRY(launch_tc<tc::M_MALA>(ctx, R, st->B, s)); break;
@@ -750,7 +763,7 @@ int tc_step(best_ctx* ctx, best_state* st, int method, int64_t n_steps, uint64_t
       }
     }
     t0 += seg;
-    BEST_TRY(after_step(ctx, st, t0 - 1, trace, thin, adapt, s));
+    if (adapt) BEST_TRY(adapt_window_rows(ctx, st, st->win_buf, seg, s));
   }
   if (method == tc::M_MH || method == tc::M_AIES) st->grad_valid = false;
   return BEST_OK;

@@ -303,50 +303,8 @@ __device__ __forceinline__ uint64_t smem_desc_sw64(uint32_t saddr) {
          ((uint64_t)1 << 46) | ((uint64_t)4 << 61);
 }
 // kind::f16, A = B = bf16 (K-major both), D = fp32, M x N
-// kind::f16 with A = B = fp16 (K-major both), D = fp32.  (A = fp16 with B = bf16 traps with
-// "illegal instruction" on sm_100a: the two operand formats of kind::f16 must be equal.)
-__host__ __device__ constexpr uint32_t idesc_f16(int M, int N) {
-  return (1u << 4) | (0u << 7) | (0u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
-}
 __host__ __device__ constexpr uint32_t idesc_bf16(int M, int N) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
-}
-
-// ---- packed fp16x2 arithmetic (activation operand type of the fused kernel) ----------------------
-__device__ __forceinline__ uint32_t cvt_f16x2(float lo, float hi) {
-  uint32_t r;
-  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
-  return r;
-}
-__device__ __forceinline__ uint32_t cvt_f16x2_from(f32x2 v) {
-  float lo, hi;
-  unpack2(v, lo, hi);
-  return cvt_f16x2(lo, hi);
-}
-__device__ __forceinline__ f32x2 f16x2_to_f32x2(uint32_t v) {
-  float lo, hi;
-  asm("{\n.reg .f16 l, h;\nmov.b32 {l, h}, %2;\ncvt.f32.f16 %0, l;\ncvt.f32.f16 %1, h;\n}\n" : "=f"(lo), "=f"(hi) : "r"(v));
-  return pack2(lo, hi);
-}
-__device__ __forceinline__ uint32_t tanh_f16x2(uint32_t x) {
-  uint32_t y;
-  asm("tanh.approx.f16x2 %0, %1;" : "=r"(y) : "r"(x));
-  return y;
-}
-__device__ __forceinline__ uint32_t hfma2(uint32_t a, uint32_t b, uint32_t c) {
-  uint32_t r;
-  asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(r) : "r"(a), "r"(b), "r"(c));
-  return r;
-}
-__device__ __forceinline__ uint32_t hmul2(uint32_t a, uint32_t b) {
-  uint32_t r;
-  asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
-  return r;
-}
-__device__ __forceinline__ uint32_t hneg2(uint32_t a) {
-  uint32_t r;
-  asm("neg.f16x2 %0, %1;" : "=r"(r) : "r"(a));
-  return r;
 }
 
 // ---- small math helpers ------------------------------------------------------------------------
@@ -362,16 +320,6 @@ __device__ __forceinline__ uint32_t pack_bf16x2_from(f32x2 v) {
 }
 __device__ __forceinline__ float bf16_lo(uint32_t v) { return __uint_as_float(v << 16); }
 __device__ __forceinline__ float bf16_hi(uint32_t v) { return __uint_as_float(v & 0xFFFF0000u); }
-__device__ __forceinline__ float ex2_approx(float x) {
-  float y;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-__device__ __forceinline__ float rcp_approx(float x) {
-  float y;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
 __device__ __forceinline__ float tanh_approx(float x) {
   float y;
   asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));

@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 from paper_2606_04895_b200 import workloads as WL
-from parity_util import TOL, accept_margins, check_logp_grad
+from parity_util import TOL, accept_margins, check_logp_grad, expected_mismatches, log_alpha_bound
 
 pytestmark = pytest.mark.gpu
 
@@ -60,9 +60,11 @@ def test_T1_lcdm_logp_grad(B, O, variant, scale):
                                         ((128, 128, 128), WL.ACT_SILU), ((256, 256), WL.ACT_TANH),
                                         ((512,), WL.ACT_SILU)])
 def test_T1_other_shapes(B, O, hidden, act):
-    """Other supported tile shapes (N-chunk = 64/128/256, 1..3 hidden layers).  north_star's 2e-2 is
-    stated for the BASELINE networks (tested above); narrow random nets average the bf16 rounding of
-    fewer terms, so these shape-coverage cases use 3e-2."""
+    """Other supported tile shapes (N-chunk = 64/128/256, 1..3 hidden layers).  north_star's 2e-2 is stated for
+    the BASELINE networks (tested above at 2e-2); SURVEY R17's emulation puts those at 1.2e-2 already, and the
+    bf16 rounding of the activations averages over the layer width, so narrow random nets sit higher: measured
+    on B200 2.0e-2 (64 x 64 SiLU) and 2.8e-2 (128^3 SiLU) on the MLP-only gradient, everything else below
+    2e-2.  These shape-coverage cases therefore run at 3e-2 and print what they measure."""
     base = WL.tiny(activation=act, hidden=hidden, mlp_scale=1.0)
     n = 300
     pts = _posterior_like(base, n, seed=3)
@@ -72,7 +74,8 @@ def test_T1_other_shapes(B, O, hidden, act):
         g = np.zeros((n, w.d), np.float32)
         ctx.logp_grad(pts, n, lp, g)
         lp_ref, g_ref = O.Oracle(w).logp_grad(pts)
-        check_logp_grad(lp, g, lp_ref, g_ref, 3e-2, f"{hidden}/{act}/{w.name}")
+        e = check_logp_grad(lp, g, lp_ref, g_ref, 3e-2, f"{hidden}/{act}/{w.name}")
+        print(f"[T1-bf16] {hidden}/{act}/{w.name}: logp err/S {e[0]:.2e}, grad ratio {e[1]:.2e}")
         ctx.close()
 
 
@@ -113,7 +116,8 @@ def test_T1_1024_two_hidden_tanh(B, O):
         g = np.zeros((n, w.d), np.float32)
         ctx.logp_grad(pts, n, lp, g)
         lp_ref, g_ref = O.Oracle(w).logp_grad(pts)
-        check_logp_grad(lp, g, lp_ref, g_ref, 3e-2, f"1024x2/tanh/{w.name}")
+        e = check_logp_grad(lp, g, lp_ref, g_ref, TOL[1], f"1024x2/tanh/{w.name}")
+        print(f"[T1-bf16] 1024x2/tanh/{w.name}: logp err/S {e[0]:.2e}, grad ratio {e[1]:.2e}")
         ctx.close()
 
 
@@ -156,37 +160,84 @@ def test_unsupported_shapes(B):
         assert e.value.code == B.BEST_ERR_UNSUPPORTED
 
 
-def _single_step_stat(B, O, w, method, seed, setup=None, **kw):
+def _single_step_stat(B, O, w, method, seed, setup=None, chain0=0, oracle_rows=None, step_scale=None, **kw):
+    """One sampler step from identical state and Philox streams on the tensor-core path and in the oracle.
+    Checked (reading R8 on the bf16 path; bounds derived in parity_util.log_alpha_bound / DESIGN.md §2):
+      * max |Δ log α| over ALL chains ≤ the bound that north_star's 2e-2 implies for this method;
+      * the number of differing accept decisions ≤ what those |Δ log α| imply (exact expectation + 5 σ);
+      * every differing decision lies inside its own chain's |Δ log α|;
+      * MH / stretch / DE: the PROPOSAL's log π (reconstructed from log α and the cached log π) on every chain,
+        accepted or not;
+      * post-step θ, log π and -- MALA / HMC -- the gradient cache on the chains that took the same decision.
+    `oracle_rows` (slice) restricts the oracle to a block of chains of a larger GPU batch (independent-chain moves)."""
     kw = {k: (f32(v) if isinstance(v, float) else v) for k, v in kw.items()}
     ctx = B.Context(w, B.PREC_BF16)
-    orc = O.Oracle(w)
+    rows = slice(0, w.n_chains) if oracle_rows is None else oracle_rows
+    import copy
+    wo = w
+    if oracle_rows is not None:
+        assert method in ("mh", "mala", "hmc")
+        wo = copy.copy(w)
+        wo.theta0 = w.theta0[rows]
+        wo.n_chains = wo.theta0.shape[0]
+    orc = O.Oracle(wo)
+    orc.set_chain_offset(chain0 + rows.start)
     if setup is not None:
         setup(ctx, orc)
     st = ctx.new_state(w.theta0)
-    ost = orc.new_state(w.theta0)
-    th0 = ost.theta.copy()
+    st.set_chain_offset(chain0)
+    ost = orc.new_state(wo.theta0)
+    th0, lp0_ref, g0_ref = ost.theta.copy(), ost.logp.copy(), ost.grad.copy()
+    before = st.get(want_grad=False)
     getattr(st, "step_" + method)(1, seed, **kw)
     getattr(ost, "step_" + method)(1, seed, **kw)
-    la = st.last_log_alpha()
+    la = st.last_log_alpha()[rows]
     out = st.get(want_grad=(method in ("mala", "hmc")))
+    out = {k: (v[rows] if isinstance(v, np.ndarray) else v) for k, v in out.items()}
+    lp0_gpu = before["logp"][rows].astype(np.float64)
+    la_ref = ost.last_log_alpha
     acc, acc_ref = out["n_accept"].astype(np.int64), ost.n_accept.astype(np.int64)
-    m = accept_margins(O, seed, 0, w.n_chains, ost.last_log_alpha)
-    with np.errstate(invalid="ignore"):      # hard box: (-inf) - (-inf), masked by the where
-        dla = np.abs(np.where(la == ost.last_log_alpha, 0.0, la - ost.last_log_alpha))
+    m = accept_margins(O, seed, 0, wo.n_chains, la_ref, chains=range(chain0 + rows.start, chain0 + rows.stop))
+    with np.errstate(invalid="ignore"):      # hard box / divergent trajectories: ±inf and NaN are handled below
+        dla = np.abs(np.where(la == la_ref, 0.0, la - la_ref))
+        # Decisions can only differ where exp(log α) is not 0 or 1 to ~20 digits: the bound derived from north_star's
+        # tolerance is checked on that CORE (|log α_ref| ≤ 50).  Outside it (proposals far off the banana ridge or
+        # outside the hard box, divergent HMC trajectories: log α down to −1e59, −inf, NaN) both sides must be
+        # surely rejecting / surely accepting; the fp32 state turns |log π| ~ 1e5 into absolute errors ~ 1 there.
+        core = np.isfinite(la_ref) & (np.abs(la_ref) <= 50.0)
+        sure_rej, sure_acc = ~(la_ref > -50.0), la_ref > 50.0
+        assert (~(la[sure_rej] > -45.0)).all() and (la[sure_acc] > 45.0).all()
+    assert np.isfinite(dla[core]).all()
     mism = acc != acc_ref
-    info = dict(n=w.n_chains, mismatch_rate=float(mism.mean()), max_dla=float(dla.max()),
-                median_dla=float(np.median(dla)), accept_rate=float(acc_ref.mean()))
+    bound, parts = log_alpha_bound(O, orc, wo, method if method != "aies_de" else "aies", th0, g0_ref, seed, 0, kw,
+                                   chain0=chain0 + rows.start, step_scale=step_scale)
+    n_exp = expected_mismatches(la, la_ref)
+    info = dict(n=wo.n_chains, mismatches=int(mism.sum()), expected_mismatches=round(n_exp, 2),
+                max_dla=float(dla[core].max()), bound_dla=float(bound), median_dla=float(np.median(dla[core])),
+                core=int(core.sum()), accept_rate=float(acc_ref.mean()))
     print(f"[T2-bf16] {w.name}/{method}: {info}")
-    # every mismatch lies inside the measured |Δ log α| of its own chain (+ fp32 slack)
-    assert (m[mism] <= dla[mism] + 1e-5).all(), info
-    assert mism.mean() < 0.02 and np.median(dla) < 2e-2, info
+    assert dla[core].max() <= bound, (info, parts)
+    assert np.median(dla[core]) <= 2.0 * parts["e_lp"] + parts["slack"], (info, parts)   # the typical chain: two evaluations' worth
+    assert mism.sum() <= n_exp + 5.0 * np.sqrt(n_exp) + 2, info
+    assert (m[mism] <= dla[mism] + 1e-5).all(), info          # a differing decision needs log u between the two log α's
+    S = np.abs(ost.logp).max()
+    if method in ("mh", "aies", "aies_de"):
+        # proposal log π on EVERY core chain, accepted or not: log π(θ′) = log α + cached log π(θ) − exact terms
+        # (which cancel in the difference)
+        d_lpp = np.abs((la + lp0_gpu) - (la_ref + lp0_ref))[core]
+        assert d_lpp.max() <= TOL[1] * S, (info, float(d_lpp.max()))
     same = ~mism
     scale = np.abs(ost.theta).max(axis=0)
     assert (np.abs(out["theta"][same] - ost.theta[same]) <= 2e-3 * scale + 1e-6).all()
     rej = same & (acc_ref == 0)
     assert np.array_equal(out["theta"][rej], th0[rej].astype(np.float32))
-    S = np.abs(ost.logp).max()
     assert np.abs(out["logp"][same] - ost.logp[same]).max() <= TOL[1] * S
+    if method in ("mala", "hmc"):
+        num = np.linalg.norm(out["grad"][same].astype(np.float64) - ost.grad[same], axis=1)
+        den = np.linalg.norm(ost.grad[same], axis=1)
+        info["grad_cache_ratio"] = float((num / den).max())
+        print(f"[T2-bf16] {w.name}/{method}: post-step gradient cache ratio {info['grad_cache_ratio']:.2e}")
+        assert (num <= TOL[1] * den).all(), info
     ctx.close()
     return info
 
@@ -212,7 +263,8 @@ def test_N1_step_scale_single_step(B, O, net, method, kw):
     w = WL.lcdm(n_chains=1024 + 40, mlp_scale=3.0 if method == "hmc" else 1.0) if net == "lcdm" else WL.sterile(n_chains=600)
     s = np.exp(np.random.default_rng(3).uniform(np.log(0.3), np.log(3.0), w.d))
     s[-2:] = 10.0 if net == "lcdm" else 3.0
-    info = _single_step_stat(B, O, w, method, seed=91, setup=lambda c, o: (c.set_step_scale(s), o.set_step_scale(s)), **kw)
+    info = _single_step_stat(B, O, w, method, seed=91, setup=lambda c, o: (c.set_step_scale(s), o.set_step_scale(s)),
+                             step_scale=s, **kw)
     assert 0.02 < info["accept_rate"] < 0.999, info
 
 
@@ -345,23 +397,30 @@ def test_T5_gaussian_closed_form_moments(B, method, d):
     ctx.close()
 
 
-def test_T5_lcdm_moments_vs_fp32_path(B):
-    """ΛCDM-like short MALA run: bf16-path moments vs the exact path's (independent seeds, 4 SE)."""
+def test_T5_lcdm_moments_vs_oracle(B, O):
+    """ΛCDM-like short MALA run (no closed form: SURVEY T5 asks for GPU vs oracle): per-dimension means of the
+    tensor-core path against the ORACLE's own run of the same target (independent seeds), within 4 standard
+    errors (SE from the across-chain variance of per-chain time averages), and the acceptance rate."""
     import torch
-    w = WL.lcdm(n_chains=512)
-    res = []
-    for prec, seed in ((B.PREC_BF16, 5), (B.PREC_FP32, 6)):
-        ctx = B.Context(w, prec)
-        st = ctx.new_state(w.theta0)
-        st.step_mala(50, seed, 0.3)
-        tr = torch.zeros(100, 512, w.d, device="cuda")
-        st.step_mala(200, seed, 0.3, trace=tr, thin=2)
-        torch.cuda.synchronize()
-        res.append((tr.cpu().numpy().astype(np.float64).mean(axis=0), st.get(want_grad=False)["n_accept"].mean() / 250))
-        ctx.close()
-    (a, ra), (b, rb) = res
-    se = np.sqrt(a.var(axis=0, ddof=1) / 512 + b.var(axis=0, ddof=1) / 512)
-    assert np.all(np.abs(a.mean(axis=0) - b.mean(axis=0)) < 4 * se)
+    n_ch, burn, n, thin = 256, 50, 200, 2
+    w = WL.lcdm(n_chains=n_ch)
+    ctx = B.Context(w, B.PREC_BF16)
+    st = ctx.new_state(w.theta0)
+    st.step_mala(burn, 5, f32(0.3))
+    tr = torch.zeros(n // thin, n_ch, w.d, device="cuda")
+    st.step_mala(n, 5, f32(0.3), trace=tr, thin=thin)
+    torch.cuda.synchronize()
+    a = tr.cpu().numpy().astype(np.float64).mean(axis=0)
+    ra = st.get(want_grad=False)["n_accept"].mean() / (burn + n)
+    ctx.close()
+    ost = O.Oracle(w).new_state(w.theta0)
+    ost.step_mala(burn, 6, f32(0.3))
+    b = ost.step_mala(n, 6, f32(0.3), thin=thin).mean(axis=0)
+    rb = ost.n_accept.mean() / (burn + n)
+    se = np.sqrt(a.var(axis=0, ddof=1) / n_ch + b.var(axis=0, ddof=1) / n_ch)
+    z = np.abs(a.mean(axis=0) - b.mean(axis=0)) / se
+    print(f"[T5-bf16] lcdm MALA vs oracle: max |z| {z.max():.2f}, acceptance {ra:.3f} vs {rb:.3f}")
+    assert np.all(z < 4.0)
     assert abs(ra - rb) < 0.02
 
 
@@ -446,3 +505,161 @@ def test_T1_geometry_switch_points(B, O, make, n):
     lp_ref, g_ref = O.Oracle(base).logp_grad(pts)
     check_logp_grad(lp, g, lp_ref, g_ref, TOL[1], f"{make}/n={n}")
     ctx.close()
+
+
+# ---- the end points of the configs[4] sweep, in the launch configuration bench.py times ------------------
+@pytest.mark.parametrize("method,kw", [("mh", dict(eps=0.3)), ("mala", dict(eps=0.01)), ("hmc", dict(eps=0.03, n_leapfrog=8))])
+@pytest.mark.parametrize("n", [1, 64])
+def test_T2_sweep_small_points(B, O, n, method, kw):
+    """1 and 64 chains on 29→1024⁴→1 (one CTA pair / one cluster): every chain against the oracle."""
+    _single_step_stat(B, O, WL.sterile(n_chains=n), method, seed=13, **kw)
+
+
+@pytest.mark.parametrize("method,kw", [("mh", dict(eps=0.3)), ("mala", dict(eps=0.01)), ("hmc", dict(eps=0.03, n_leapfrog=8))])
+def test_T2_sweep_65536_chains(B, O, method, kw):
+    """65 536 chains on 29→1024⁴→1: the oracle on three blocks of 192 chains (first tiles, a block straddling
+    tile and wave boundaries in the middle, the very last chains), drawing the same Philox streams through
+    its chain offset."""
+    w = WL.sterile(n_chains=65536)
+    for r0 in (0, 32768 - 96, 65536 - 192):
+        info = _single_step_stat(B, O, w, method, seed=19, oracle_rows=slice(r0, r0 + 192), **kw)
+        assert info["n"] == 192
+
+
+def test_T4_get_between_steps_changes_nothing(B):
+    """a read-back (which refreshes the stale gradient cache after MH / stretch moves) must not touch
+    the cached log π: 5 steps + get() + 7 steps == 12 steps bit for bit, and the same across a MALA call."""
+    w = WL.lcdm(n_chains=300)
+    ctx = B.Context(w, B.PREC_BF16)
+    for meth, kw in (("mh", dict(eps=f32(0.3))), ("aies", dict(a=2.0))):
+        a, b = ctx.new_state(w.theta0), ctx.new_state(w.theta0)
+        getattr(a, "step_" + meth)(12, 3, **kw)
+        getattr(b, "step_" + meth)(5, 3, **kw)
+        mid = b.get(want_grad=True)                  # evaluates the gradient, must leave log π alone
+        assert np.isfinite(mid["grad"]).all()
+        getattr(b, "step_" + meth)(7, 3, **kw)
+        ga, gb = a.get(want_grad=False), b.get(want_grad=False)
+        for k in ("theta", "logp", "n_accept"):
+            assert np.array_equal(ga[k], gb[k]), (meth, k)
+        assert gb["n_evals"] == ga["n_evals"] + 300   # the read-back's gradient evaluation is counted
+        # ... and a gradient-based call afterwards starts from the same caches either way
+        a.step_mala(3, 4, f32(0.3)); b.step_mala(3, 4, f32(0.3))
+        ga, gb = a.get(), b.get()
+        for k in ("theta", "logp", "grad", "n_accept"):
+            assert np.array_equal(ga[k], gb[k]), (meth, k)
+    ctx.close()
+
+
+def test_T4_trace_written_by_the_kernel(B):
+    """The persistent kernel writes the trace slots itself (A8): slot k of one 12-step call with thin = 3 is the
+    state after 3(k+1) steps of a run made of 3-step calls, bit for bit; stretch moves included (each
+    half-ensemble launch writes its own walkers)."""
+    import torch
+    for make, n in ((WL.lcdm, 300), (WL.sterile, 130)):
+        w = make(n_chains=n)
+        ctx = B.Context(w, B.PREC_BF16)
+        eps = dict(mh=0.3, mala=0.3 if make is WL.lcdm else 0.01, hmc=0.1 if make is WL.lcdm else 0.03)
+        for meth, kw in (("mh", dict(eps=f32(eps["mh"]))), ("mala", dict(eps=f32(eps["mala"]))),
+                         ("hmc", dict(eps=f32(eps["hmc"]), n_leapfrog=3)), ("aies", dict(a=2.0)), ("aies_de", dict(sigma_gamma=0.1))):
+            a, b = ctx.new_state(w.theta0), ctx.new_state(w.theta0)
+            tr = torch.full((4, n, w.d), float("nan"), device="cuda")
+            getattr(a, "step_" + meth)(12, 3, trace=tr, thin=3, **kw)
+            torch.cuda.synchronize()
+            tr = tr.cpu().numpy()
+            for k in range(4):
+                getattr(b, "step_" + meth)(3, 3, **kw)
+                assert np.array_equal(tr[k], b.get(want_grad=False)["theta"]), (meth, k)
+        ctx.close()
+
+
+def test_T6_adaptation_persistent_segments(B, O):
+    """A9 with the persistent kernel: the window is fed from the kernel-written window buffer in segments; the
+    result must not depend on how the call is cut (one 90-step call == 9 calls of 10 steps, bit for bit, two
+    windows of 45), must agree with the oracle's factor from the GPU's own trace, and two states of one context
+    keep separate windows."""
+    import torch
+    w = WL.lcdm(n_chains=700, hidden=64, n_hidden=2)
+    w.L = np.diag(np.sqrt(np.diag(w.Sigma)))
+    res = []
+    for calls in (1, 9):
+        ctx = B.Context(w, B.PREC_BF16)
+        st, other = ctx.new_state(w.theta0), ctx.new_state(w.theta0[:130])
+        st.set_adaptation(45, 1e-6)
+        tr = torch.zeros(90, 700, w.d, device="cuda")
+        per = 90 // calls
+        for k in range(calls):
+            st.step_mala(per, 21, f32(0.05), trace=tr[k * per:(k + 1) * per], thin=1)
+            other.step_mh(2, 5, f32(0.05))          # a second state of the same context: no window of its own
+        torch.cuda.synchronize()
+        res.append((ctx.get_whitening(), st.get(), tr.cpu().numpy().astype(np.float64), ctx.adapt_stats()))
+        ctx.close()
+    (L1, s1, t1, a1), (L9, s9, t9, a9) = res
+    assert a1 == a9 == (2, 0)
+    assert np.array_equal(L1, L9) and np.array_equal(t1, t9)
+    for k in ("theta", "logp", "grad", "n_accept"):
+        assert np.array_equal(s1[k], s9[k]), k
+    rc, _, Lo = O.Oracle(w).cov_chol(t1[45:].reshape(-1, w.d), 1e-6)     # the second window
+    assert rc == 0
+    assert np.abs(L1 - Lo).max() / np.abs(Lo).max() < 1e-6
+
+
+def test_T6_single_chain_windows(B, O):
+    """configs[4] at B = 1 ('C may be near-singular -- O6's jitter-retry / keep-old-L rule is
+    exercised here on purpose').  (a) a 500-step window of ONE chain on the banana target: the device factor
+    equals the oracle's from the GPU's own trace, or both keep the old factor; (b) a window in which no proposal
+    is accepted (C = 0 exactly): every retry fails on both sides, the factor is kept and counted as a failure."""
+    import torch
+    w = WL.sterile(n_chains=1)
+    ctx = B.Context(w, B.PREC_BF16)
+    st = ctx.new_state(w.theta0)
+    L0 = ctx.get_whitening()
+    st.set_adaptation(500, 1e-6)
+    tr = torch.zeros(500, 1, w.d, device="cuda")
+    st.step_mh(500, 3, f32(0.3), trace=tr, thin=1)
+    torch.cuda.synchronize()
+    t = tr.cpu().numpy().astype(np.float64).reshape(-1, w.d)
+    n_distinct = len(np.unique(t, axis=0))
+    rc, _, Lo = O.Oracle(w).cov_chol(t, 1e-6)
+    Lg = ctx.get_whitening()
+    print(f"[T6-bf16] B=1 window: {n_distinct} distinct points, oracle rc {rc}, stats {ctx.adapt_stats()}")
+    if rc == 0:
+        assert ctx.adapt_stats() == (1, 0)
+        assert np.abs(Lg - Lo).max() / np.abs(Lo).max() < 1e-6
+    else:
+        assert ctx.adapt_stats() == (0, 1) and np.array_equal(Lg, L0)
+    # (b) nothing moves: eps so large that every proposal leaves the box by far
+    st.set_adaptation(7, 1e-6)
+    tr = torch.zeros(7, 1, w.d, device="cuda")
+    st.step_mh(7, 4, f32(500.0), trace=tr, thin=1)
+    torch.cuda.synchronize()
+    t = tr.cpu().numpy().astype(np.float64).reshape(-1, w.d)
+    assert len(np.unique(t, axis=0)) == 1
+    rc2, _, _ = O.Oracle(w).cov_chol(t, 1e-6)
+    assert rc2 != 0
+    assert ctx.adapt_stats()[1] == (1 if rc != 0 else 0) + 1 and np.array_equal(ctx.get_whitening(), Lg)
+    ctx.close()
+
+
+@pytest.mark.parametrize("prec", ["bf16", "fp32"])
+def test_E_chain_offset_streams(B, O, prec):
+    """rank r of a sharded job sets chain0 = r·B.  A state with offset c0 must reproduce chains
+    [c0, c0 + n) of one big state bit for bit (independent-chain moves), differ from the offset-0 stream, and
+    match the oracle driven with the same offset."""
+    P = B.PREC_BF16 if prec == "bf16" else B.PREC_FP32
+    w = WL.lcdm(n_chains=512, hidden=64, n_hidden=2) if prec == "bf16" else WL.tiny(n_chains=512)
+    ctx = B.Context(w, P)
+    big = ctx.new_state(w.theta0)
+    lo, hi = ctx.new_state(w.theta0[:256]), ctx.new_state(w.theta0[256:])
+    hi.set_chain_offset(256)
+    same0 = ctx.new_state(w.theta0[256:])           # same chains WITHOUT the offset: must differ
+    for st in (big, lo, hi, same0):
+        st.step_mh(3, 9, f32(0.3)); st.step_mala(3, 9, f32(0.2)); st.step_hmc(2, 9, f32(0.1), 3)
+    g, gl, gh, g0 = big.get(), lo.get(), hi.get(), same0.get()
+    for k in ("theta", "logp", "grad", "n_accept"):
+        assert np.array_equal(g[k][:256], gl[k]) and np.array_equal(g[k][256:], gh[k]), k
+    assert not np.array_equal(gh["theta"], g0["theta"])
+    with pytest.raises(B.BestError):
+        hi.set_chain_offset((1 << 32) - 100)
+    ctx.close()
+    if prec == "bf16":
+        _single_step_stat(B, O, WL.lcdm(n_chains=300), "mala", seed=5, chain0=4096, eps=0.3)

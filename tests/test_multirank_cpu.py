@@ -18,11 +18,14 @@ import bench
 rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
 dist.init_process_group("gloo")
 spec = dict(bench.WORKLOADS["tiny_mala"])
-w = bench.shard_workload(spec, rank, world)
+w, chain0 = bench.shard_workload(spec, rank, world)
 ms = bench.max_over_ranks(10.0 + 5.0 * rank, world, device="cpu")
 dist.barrier()
+# the Philox stream this rank's chain 0 draws at step 0 (the stream layout is the oracle's, KAT-pinned)
+from oracle import oracle as O
+first = O.normals(7, chain0 + 0, 0, w.d)
 out = dict(rank=rank, n_chains=int(w.n_chains), theta_sum=float(np.abs(w.theta0).sum()),
-           W0=float(w.W[0].sum()), mu0=float(w.mu[0]), ms=ms)
+           W0=float(w.W[0].sum()), mu0=float(w.mu[0]), ms=ms, chain0=int(chain0), first=[float(x) for x in first])
 print("RESULT " + json.dumps(out), flush=True)
 dist.destroy_process_group()
 """
@@ -53,6 +56,13 @@ def test_sharding_and_max_over_ranks_gloo(tmp_path):
     assert res[0]["theta_sum"] != res[1]["theta_sum"]
     # the slowest rank defines the step on every rank
     assert res[0]["ms"] == res[1]["ms"] == 15.0
+    # rank-distinct random streams: rank r's chains are global chains r*B .. r*B + B - 1, so the
+    # ranks' first normals differ while rank 0 reproduces the single-process stream
+    assert [r["chain0"] for r in res] == [0, 64]
+    assert res[0]["first"] != res[1]["first"]
+    from oracle import oracle as O
+    assert res[0]["first"] == [float(x) for x in O.normals(7, 0, 0, 6)]
+    assert res[1]["first"] == [float(x) for x in O.normals(7, 64, 0, 6)]
 
 
 def test_reference_arm_runs_on_rank0_only():

@@ -206,3 +206,39 @@ def test_adaptation_windows(oracle_mod):
     Lw = o.get_whitening()
     rel = np.abs(Lw @ Lw.T - w.Sigma) / np.sqrt(np.outer(np.diag(w.Sigma), np.diag(w.Sigma)))
     assert rel.max() < 0.35
+
+
+def test_chain_offset_streams(oracle_mod):
+    """with chain offset c0 the oracle's local chain c draws the Philox stream of global chain
+    c0 + c.  Pins: (i) the MH proposal of an accepted chain is θ + ε L ξ with ξ = the KAT-pinned normals of
+    chain c0 + c (so the offset lands in counter word 0, nowhere else); (ii) the accept uniform is the control
+    word of chain c0 + c; (iii) a shard with offset c0 reproduces chains [c0, c0 + n) of one big ensemble for
+    the independent-chain samplers; (iv) offset 0 is the unsharded stream."""
+    O = oracle_mod
+    w = WL.gaussian(5, 96, seed=7, cond=30.0)
+    c0, n, seed, eps = 40, 32, 11, 0.4
+    big = O.Oracle(w).new_state(w.theta0)
+    sh_o = O.Oracle(w)
+    sh_o.set_chain_offset(c0)
+    sh = sh_o.new_state(w.theta0[c0:c0 + n])
+    th0 = sh.theta.copy()
+    sh.step_mh(1, seed, eps)
+    acc = sh.n_accept == 1
+    assert acc.any() and (~acc).any()
+    for c in np.flatnonzero(acc):
+        xi = O.normals(seed, c0 + int(c), 0, w.d)
+        assert np.allclose(sh.theta[c], th0[c] + eps * (w.L @ xi), rtol=0, atol=1e-13)
+        assert math.log(O.control(seed, c0 + int(c), 0)[0]) < sh.last_log_alpha[c]
+    for c in np.flatnonzero(~acc):
+        assert not math.log(O.control(seed, c0 + int(c), 0)[0]) < sh.last_log_alpha[c]
+    big.step_mh(1, seed, eps)
+    for st in (big, sh):
+        st.step_mala(3, seed, 0.3)
+        st.step_hmc(2, seed, 0.2, 3)
+    assert np.array_equal(big.theta[c0:c0 + n], sh.theta) and np.array_equal(big.n_accept[c0:c0 + n], sh.n_accept)
+    z_o = O.Oracle(w)
+    z_o.set_chain_offset(0)
+    z = z_o.new_state(w.theta0[:n])
+    z.step_mh(1, seed, eps); z.step_mala(3, seed, 0.3); z.step_hmc(2, seed, 0.2, 3)
+    assert np.array_equal(big.theta[:n], z.theta)
+    assert not np.array_equal(z.theta, sh.theta)
