@@ -121,8 +121,14 @@ struct best_state {
   double* cov_acc = nullptr;      // [cov_blocks][1 + d + d*d] per-block partial sums (fp64): count | sums | products
   int cov_blocks = 0;
   double* cov_ref = nullptr;      // [d] shift (chain 0's position when the window opened)
-  float* win_buf = nullptr;       // tensor path: fp32 rows [win_cap_steps][B][d] written by the persistent kernel
-  int64_t win_cap_steps = 0;
+  // tensor path: two fp32 row buffers [win_cap_steps][B][d] that the persistent kernel writes in turn; the Gram
+  // kernel of a segment runs on `side`, concurrently with the next segment's persistent launch
+  float* win_buf[2] = {nullptr, nullptr};
+  int64_t win_cap_steps = 0;      // steps per segment of the current window
+  int64_t win_cap_alloc = 0;      // steps the buffers were allocated for
+  int win_flip = 0;
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_seg[2] = {nullptr, nullptr}, ev_gram[2] = {nullptr, nullptr};
 };
 
 namespace best {
@@ -146,7 +152,9 @@ void adapt_free(best_state* st);
 int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin, bool adapt, cudaStream_t s);
 // tensor path: fold `n_steps` slots of fp32 rows [n_steps][B][d] (every post-accept state of a segment) into
 // the window sums; closes the window (covariance -> Cholesky -> whitening swap, on device) when it is complete
-int adapt_window_rows(best_ctx* ctx, best_state* st, const float* rows, int64_t n_steps, cudaStream_t s);
+int adapt_window_rows(best_ctx* ctx, best_state* st, int buf, int64_t n_steps, cudaStream_t s);
+// the window buffer the next segment may write (waits, on `s`, until its previous contents have been folded)
+int adapt_acquire_buffer(best_state* st, cudaStream_t s, int* buf);
 
 // layout helpers (samplers.cu)
 int rows_f32_to_soa_f64(const float* rows_dev, double* soa, int64_t n, int d, int64_t ld, cudaStream_t s);

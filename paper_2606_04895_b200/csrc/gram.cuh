@@ -8,6 +8,10 @@ namespace best {
 
 constexpr int G_TPB = 128;
 constexpr int G_ROWS = 64;
+// Position of column i inside a 32-double row of the SMEM tile: the first 16 slots hold the pairs (4t, 4t+1),
+// t = 0..7, the last 16 the pairs (4t+2, 4t+3), so that the eight threads of a quarter-warp (t = 0..7) read one
+// contiguous 128-byte run per 16-byte load (in natural order the 32-byte stride made these loads 2-way conflicted)
+__host__ __device__ constexpr int gram_pos(int i) { return ((i & 2) << 3) | ((i >> 2) << 1) | (i & 1); }
 
 // out[blk][i*d + j] = sum over the block's rows of (x_i - ref_i)(x_j - ref_j); rows are [nrows][d].
 // The rows of a tile sit in SMEM padded to 32 columns (zeros); the 128 threads are two groups of 8 x 8
@@ -28,15 +32,19 @@ k_gram_partial(const T* __restrict__ rows, int64_t nrows, int d, const double* _
   for (int64_t r0 = blockIdx.x * (int64_t)G_ROWS; r0 < nrows; r0 += (int64_t)gridDim.x * G_ROWS) {
     const int nv = (int)((nrows - r0 < G_ROWS) ? (nrows - r0) : G_ROWS);
     __syncthreads();
-    for (int e = threadIdx.x; e < G_ROWS * d; e += G_TPB) {   // contiguous, coalesced
-      const int r = e / d, i = e - r * d;
-      xs[r * kMaxD + i] = (r < nv) ? (double)rows[r0 * d + e] - ref[i] : 0.0;
+    {   // lane = column, warp = row (mod 4): 4 d-byte runs per instruction, no index division
+      const int i = threadIdx.x & 31;
+      if (i < d) {
+        const double ri = ref[i];
+        for (int r = threadIdx.x >> 5; r < G_ROWS; r += G_TPB / 32)
+          xs[r * kMaxD + gram_pos(i)] = (r < nv) ? (double)rows[(r0 + r) * d + i] - ri : 0.0;
+      }
     }
     __syncthreads();
     for (int r = grp; r < nv; r += 2) {
-      const double2* pa = reinterpret_cast<const double2*>(xs + r * kMaxD + 4 * ti);
-      const double2* pb = reinterpret_cast<const double2*>(xs + r * kMaxD + 4 * tj);
-      const double2 a01 = pa[0], a23 = pa[1], b01 = pb[0], b23 = pb[1];
+      const double2* pa = reinterpret_cast<const double2*>(xs + r * kMaxD) + ti;
+      const double2* pb = reinterpret_cast<const double2*>(xs + r * kMaxD) + tj;
+      const double2 a01 = pa[0], a23 = pa[8], b01 = pb[0], b23 = pb[8];
       const double a[4] = {a01.x, a01.y, a23.x, a23.y}, b[4] = {b01.x, b01.y, b23.x, b23.y};
 #pragma unroll
       for (int p = 0; p < 4; ++p)
@@ -96,15 +104,19 @@ k_gram_window(const float* __restrict__ rows, int64_t row0, int64_t nrows, int d
     const int64_t g0 = T * G_ROWS;
     const int lo = (int)(g0 < row0 ? row0 - g0 : 0), hi = (int)(g0 + G_ROWS > rend ? rend - g0 : G_ROWS);   // rows [lo, hi) of the tile
     __syncthreads();
-    for (int e = threadIdx.x + lo * d; e < hi * d; e += G_TPB) {
-      const int r = e / d, i = e - r * d;
-      xs[r * kMaxD + i] = (double)rows[(g0 - row0) * d + e] - ref[i];
+    {   // lane = column, warp = row (mod 4): 4 d-byte runs per instruction, no index division
+      const int i = threadIdx.x & 31;
+      if (i < d) {
+        const double ri = ref[i];
+        for (int r = lo + (threadIdx.x >> 5); r < hi; r += G_TPB / 32)
+          xs[r * kMaxD + gram_pos(i)] = (double)rows[(g0 - row0 + r) * d + i] - ri;
+      }
     }
     __syncthreads();
     for (int r = lo + ((lo ^ grp) & 1); r < hi; r += 2) {   // this group's parity
-      const double2* pa = reinterpret_cast<const double2*>(xs + r * kMaxD + 4 * ti);
-      const double2* pb = reinterpret_cast<const double2*>(xs + r * kMaxD + 4 * tj);
-      const double2 a01 = pa[0], a23 = pa[1], b01 = pb[0], b23 = pb[1];
+      const double2* pa = reinterpret_cast<const double2*>(xs + r * kMaxD) + ti;
+      const double2* pb = reinterpret_cast<const double2*>(xs + r * kMaxD) + tj;
+      const double2 a01 = pa[0], a23 = pa[8], b01 = pb[0], b23 = pb[8];
       const double a[4] = {a01.x, a01.y, a23.x, a23.y}, b[4] = {b01.x, b01.y, b23.x, b23.y};
 #pragma unroll
       for (int p = 0; p < 4; ++p)

@@ -267,10 +267,19 @@ __global__ void k_cov_finalize(double* __restrict__ acc, int nblk, int d, double
   __shared__ double S[1 + kMaxD + kMaxD * kMaxD];
   __shared__ double Cm[kMaxD * kMaxD], Lt[kMaxD * kMaxD];
   const int ne = 1 + d + d * d;
-  for (int e = threadIdx.x; e < ne; e += blockDim.x) {
+  for (int e = threadIdx.x; e < ne; e += blockDim.x) {   // partials are added in block order (fixed), loads 8 at a time
     double s = 0.0;
-    for (int b = 0; b < nblk; ++b) { s += acc[(size_t)b * ne + e]; acc[(size_t)b * ne + e] = 0.0; }
+    int b = 0;
+    for (; b + 8 <= nblk; b += 8) {
+      double v[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) v[u] = acc[(size_t)(b + u) * ne + e];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) s += v[u];
+    }
+    for (; b < nblk; ++b) s += acc[(size_t)b * ne + e];
     S[e] = s;
+    for (b = 0; b < nblk; ++b) acc[(size_t)b * ne + e] = 0.0;   // the next window starts from zero
   }
   __syncthreads();
   if (threadIdx.x != 0) return;
@@ -326,7 +335,7 @@ Chains chains_of(best_state* st) {
 }  // namespace
 
 static int close_window(best_ctx* ctx, best_state* st, cudaStream_t s) {
-  k_cov_finalize<<<1, 256, 0, s>>>(st->cov_acc, st->cov_blocks, ctx->d, st->jitter, ctx->L_dev, ctx->Lraw_dev,
+  k_cov_finalize<<<1, 1024, 0, s>>>(st->cov_acc, st->cov_blocks, ctx->d, st->jitter, ctx->L_dev, ctx->Lraw_dev,
                                    ctx->scale_dev, (long long*)ctx->adapt_counts);
   count_launch();
   st->win_steps = 0;
@@ -352,20 +361,46 @@ int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin,
   return BEST_OK;
 }
 
-int adapt_window_rows(best_ctx* ctx, best_state* st, const float* rows, int64_t n_steps, cudaStream_t s) {
+int adapt_acquire_buffer(best_state* st, cudaStream_t s, int* buf) {
+  const int b = st->win_flip;
+  st->win_flip ^= 1;
+  BEST_CUDA(cudaStreamWaitEvent(s, st->ev_gram[b], 0));   // (never recorded: no-op)
+  *buf = b;
+  return BEST_OK;
+}
+
+// Called right after the persistent launch of a segment on `s`.  The Gram kernel runs on the state's side stream
+// behind that launch, so it overlaps the NEXT segment's persistent kernel (it fits on the SMs that kernel leaves
+// idle: 20 of 148 at 16 384 chains, the tail of the last wave otherwise); Gram launches are ordered among
+// themselves by the side stream, the window close waits for the last one on `s`.
+int adapt_window_rows(best_ctx* ctx, best_state* st, int buf, int64_t n_steps, cudaStream_t s) {
   const int d = ctx->d;
-  k_gram_window<<<st->cov_blocks / 2, G_TPB, 0, s>>>(rows, st->win_steps * st->B, n_steps * st->B, d, st->cov_ref,
-                                                     st->cov_acc);
+  BEST_CUDA(cudaEventRecord(st->ev_seg[buf], s));
+  BEST_CUDA(cudaStreamWaitEvent(st->side, st->ev_seg[buf], 0));
+  k_gram_window<<<st->cov_blocks / 2, G_TPB, 0, st->side>>>(st->win_buf[buf], st->win_steps * st->B, n_steps * st->B, d,
+                                                            st->cov_ref, st->cov_acc);
   count_launch();
-  st->win_steps += n_steps;
-  if (st->win_steps >= st->adapt_every) BEST_TRY(close_window(ctx, st, s));
   BEST_CUDA(cudaGetLastError());
+  BEST_CUDA(cudaEventRecord(st->ev_gram[buf], st->side));
+  st->win_steps += n_steps;
+  if (st->win_steps >= st->adapt_every) {
+    BEST_CUDA(cudaStreamWaitEvent(s, st->ev_gram[buf], 0));
+    BEST_TRY(close_window(ctx, st, s));
+  }
   return BEST_OK;
 }
 
 void adapt_free(best_state* st) {
-  cudaFree(st->cov_acc); cudaFree(st->cov_ref); cudaFree(st->win_buf);
-  st->cov_acc = nullptr; st->cov_ref = nullptr; st->win_buf = nullptr;
+  if (st->side) cudaStreamSynchronize(st->side);
+  cudaFree(st->cov_acc); cudaFree(st->cov_ref); cudaFree(st->win_buf[0]); cudaFree(st->win_buf[1]);
+  for (int i = 0; i < 2; ++i) {
+    if (st->ev_seg[i]) cudaEventDestroy(st->ev_seg[i]);
+    if (st->ev_gram[i]) cudaEventDestroy(st->ev_gram[i]);
+    st->ev_seg[i] = st->ev_gram[i] = nullptr;
+  }
+  if (st->side) cudaStreamDestroy(st->side);
+  st->side = nullptr;
+  st->cov_acc = nullptr; st->cov_ref = nullptr; st->win_buf[0] = st->win_buf[1] = nullptr;
   st->cov_blocks = 0; st->win_cap_steps = 0;
 }
 
@@ -378,12 +413,13 @@ int adapt_reset(best_ctx* ctx, best_state* st, cudaStream_t s) {
   int nblk;
   int64_t cap = 0;
   if (ctx->precision == BEST_PREC_BF16) {
-    cap = (int64_t)((256ull << 20) / ((size_t)st->B * d * sizeof(float)));
+    cap = (int64_t)((128ull << 20) / ((size_t)st->B * d * sizeof(float)));   // two buffers of at most 128 MB
     cap = cap < 1 ? 1 : (cap > st->adapt_every ? st->adapt_every : cap);
-    // grid of the window's Gram kernel: one CTA per 64-row tile up to two per SM, fixed for the whole window
+    // grid of the window's Gram kernel: one CTA per 64-row tile up to four per SM, fixed for the whole window
     // (with the window length and B it determines the summation order); two partial sets (row parity) per CTA
     const int64_t tiles = (st->B * (int64_t)st->adapt_every + G_ROWS - 1) / G_ROWS;
-    nblk = 2 * (int)(tiles < 296 ? tiles : 296);
+    const int64_t want = (tiles + 15) / 16;   // >= 16 tiles per CTA before the grid grows: few partial sets for small batches
+    nblk = 2 * (int)(want < 1 ? 1 : (want < 592 ? want : 592));
   } else {
     nblk = (int)((st->B + COV_TPB - 1) / COV_TPB);
   }
@@ -394,12 +430,24 @@ int adapt_reset(best_ctx* ctx, best_state* st, cudaStream_t s) {
     st->cov_blocks = nblk;
   }
   if (!st->cov_ref) BEST_TRY(dev_alloc(&st->cov_ref, (size_t)d));
-  if (cap > st->win_cap_steps) {
-    cudaFree(st->win_buf);
-    st->win_buf = nullptr; st->win_cap_steps = 0;
-    BEST_TRY(dev_alloc(&st->win_buf, (size_t)cap * st->B * d));
-    st->win_cap_steps = cap;
-  } else if (cap > 0) {
+  if (cap > 0) {
+    if (!st->side) {
+      BEST_CUDA(cudaStreamCreateWithFlags(&st->side, cudaStreamNonBlocking));
+      for (int i = 0; i < 2; ++i) {
+        BEST_CUDA(cudaEventCreateWithFlags(&st->ev_seg[i], cudaEventDisableTiming));
+        BEST_CUDA(cudaEventCreateWithFlags(&st->ev_gram[i], cudaEventDisableTiming));
+      }
+    }
+    BEST_CUDA(cudaStreamSynchronize(st->side));
+    if (cap > st->win_cap_alloc) {
+      for (int i = 0; i < 2; ++i) {
+        cudaFree(st->win_buf[i]);
+        st->win_buf[i] = nullptr;
+      }
+      st->win_cap_alloc = 0;
+      for (int i = 0; i < 2; ++i) BEST_TRY(dev_alloc(&st->win_buf[i], (size_t)cap * st->B * d));
+      st->win_cap_alloc = cap;
+    }
     st->win_cap_steps = cap;
   }
   BEST_CUDA(cudaMemsetAsync(st->cov_acc, 0, sizeof(double) * ne * st->cov_blocks, s));

@@ -28,6 +28,7 @@ struct EpiCtx {
   int half;             // CTA pair: 0 = lanes 0..63 (lower N half, runs the sampler), 1 = lanes 64..127
   uint32_t o, g;        // op / n-chunk counters (mirror the MMA issuer)
   uint32_t vslot, pslot;  // rotating scratch slots
+  uint32_t emit_pending;  // this thread has committed a bulk copy out of the row staging area (emit_tile)
   // per-thread constants
   uint32_t a_thr0, a_thr1;  // shared addresses of this thread's two 16-B pieces in A k-chunk 0 (SW128)
   uint32_t bias_thr;        // shared address of bias[0][16k]
@@ -110,6 +111,10 @@ __device__ __forceinline__ void tanh_pair(f32x2 a, f32x2& h, f32x2& dact) {
 template <int ROWS>
 __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   if (Geo<ROWS>::kPair && C.half != 0) return;   // the upper lane half only takes part in the MLP epilogues
+  if (C.emit_pending) {   // the row staging area (operand bytes 48-64 KB) is about to become operand again
+    ptx::bulk_wait_read0();
+    C.emit_pending = 0;
+  }
   if (!Geo<ROWS>::kPingPong) ptx::mbar_wait(C.bars.a_free(0), (C.o & 1u) ^ 1u);
   uint32_t hi[4], lo[4];
 #pragma unroll

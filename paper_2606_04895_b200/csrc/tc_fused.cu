@@ -87,7 +87,6 @@ constexpr int kStages = 4;
 constexpr int kMaxOps = 12;
 constexpr int kCtrlWarps = 4;          // producer, MMA issuer, TMEM allocator, spare
 constexpr int kEpiWarps = 16;          // 4 per TMEM lane quarter
-constexpr int kEpiThreads = kEpiWarps * 32;
 constexpr int kThreads = (kCtrlWarps + kEpiWarps) * 32;
 constexpr int kDP = 32;              // parameter vectors are padded to 32 inside the kernel
 

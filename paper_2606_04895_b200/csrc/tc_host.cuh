@@ -8,18 +8,50 @@ namespace tc {
 // Sampler driver: executed by all 512 epilogue threads; thread (row, k) owns dims [8k, 8k+8) of
 // chain `row`.  Scalars (log pi, log alpha, accept) are computed redundantly and identically by the
 // four threads of a chain, so they take the same accept branch.
-// A8: the post-accept theta of chain `chain` (own 8 dims) into row-major fp32 rows [slot][B_rows][d]
-__device__ __forceinline__ void emit_rows(const EpiCtx& C, const Run& R, int64_t t, int64_t chain, int d,
-                                          const float (&cur)[8]) {
-  if (R.trace && (R.t_call0 + t + 1) % R.thin == 0) {
-    float* dst = R.trace + (((R.t_call0 + t + 1) / R.thin - 1) * R.B_rows + chain) * d + 8 * C.k;
+// A8: the post-accept theta of the CTA's chains into row-major fp32 rows [slot][B_rows][d] -- the trace slot of
+// this step (every `thin` steps) and / or the covariance window slot (every step).  The rows of a tile are
+// contiguous in both, so the sampler threads stage them in shared memory (operand bytes 48-64 KB, dead between
+// two evaluations) and ONE thread sends the block with a bulk async copy: direct stores (8 x 4 B per thread at a
+// 4d-byte stride across lanes, 32 sectors per instruction) cost ~3.5 k cycles of LSU time per step and SM, measured
+// as 2-5 % of a step.  Called by every sampler thread of the CTA (a CTA-wide named barrier inside); `valid` masks
+// the ragged tail, `first` is the global index of the tile's first chain inside a slot.  Unaligned blocks (a
+// chain count that is not a multiple of 4, an unaligned trace pointer) fall back to direct stores.
+template <int ROWS>
+__device__ __forceinline__ void emit_tile(EpiCtx& C, const Run& R, int64_t t, int64_t first, int d,
+                                          const float (&cur)[8], bool valid) {
+  const bool tr_now = R.trace != nullptr && (R.t_call0 + t + 1) % R.thin == 0;
+  if (!tr_now && R.win == nullptr) return;   // (uniform over the CTA)
+  const int64_t in_launch = (int64_t)blockIdx.x * Geo<ROWS>::kChains;
+  int nvalid = (int)((R.B - in_launch < Geo<ROWS>::kChains) ? (R.B - in_launch) : Geo<ROWS>::kChains);
+  if (nvalid < 0) nvalid = 0;   // (a pair's padding CTA)
+  const uint32_t bytes = (uint32_t)(nvalid * d) * 4u;
+  float* dst_tr = tr_now ? R.trace + (((R.t_call0 + t + 1) / R.thin - 1) * R.B_rows + first) * d : nullptr;
+  float* dst_win = R.win ? R.win + (t * R.B_rows + first) * d : nullptr;
+  const bool bulk = ((bytes | (uint32_t)reinterpret_cast<uintptr_t>(dst_tr) | (uint32_t)reinterpret_cast<uintptr_t>(dst_win)) & 15u) == 0u;
+  if (bulk) {
+    const uint32_t stage = C.sbase + SmemLayout::A + 49152u;
+    if (valid) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) if (8 * C.k + i < d) dst[i] = cur[i];
-  }
-  if (R.win) {
-    float* dst = R.win + (t * R.B_rows + chain) * d + 8 * C.k;
+      for (int i = 0; i < 8; ++i)
+        if (8 * C.k + i < d) ptx::sts_32(stage + (uint32_t)(C.row * d + 8 * C.k + i) * 4u, cur[i]);
+    }
+    ptx::named_bar_sync(9, Geo<ROWS>::kChains * 4);
+    if (C.row == 0 && C.k == 0 && nvalid > 0) {
+      ptx::fence_proxy_async();
+      if (dst_tr) ptx::bulk_s2g(dst_tr, stage, bytes);
+      if (dst_win) ptx::bulk_s2g(dst_win, stage, bytes);
+      ptx::bulk_commit();
+      C.emit_pending = 1;
+    }
+  } else if (valid) {
+    const int64_t off = (int64_t)C.row * d + 8 * C.k;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) if (8 * C.k + i < d) dst[i] = cur[i];
+    for (int i = 0; i < 8; ++i) {
+      if (8 * C.k + i < d) {
+        if (dst_tr) dst_tr[off + i] = cur[i];
+        if (dst_win) dst_win[off + i] = cur[i];
+      }
+    }
   }
 }
 
@@ -97,9 +129,10 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
       R.last_la[i] = (double)la;
       if (acc) { R.logp[i] = (double)lpp; R.n_accept[i] += 1ull; }
     }
-    if (R.trace && valid) {   // every half-ensemble launch writes its own walkers (their state is final for this step)
-      if (!acc) load_vec8(C, R.theta, R.ld, i, d, valid, thp);
-      emit_rows(C, R, 0, i, d, thp);
+    if (R.trace) {   // every half-ensemble launch writes its own walkers (their state is final for this step)
+      if (valid && !acc) load_vec8(C, R.theta, R.ld, i, d, valid, thp);
+      emit_tile<ROWS>(C, R, 0, R.own0 + (int64_t)blockIdx.x * Geo<ROWS>::kChains, d, thp, valid);
+      if (C.emit_pending) ptx::bulk_wait0();
     }
     return;
   }
@@ -107,6 +140,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
   const int64_t c = r_in_launch;
   const uint32_t cid = R.chain0 + (uint32_t)c;
   const bool rows_out = (R.trace != nullptr) || (R.win != nullptr);
+  const int64_t tile0 = (int64_t)blockIdx.x * Geo<ROWS>::kChains;   // first chain of this CTA's tile
   const float eps = R.eps;
   float lp = valid ? (float)R.logp[c] : 0.0f;
   float la_last = 0.0f;
@@ -137,7 +171,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
         lp = lpp;
         ++nacc;
       }
-      if (rows_out && valid) emit_rows(C, R, t, c, d, th);
+      if (rows_out) emit_tile<ROWS>(C, R, t, tile0, d, th, valid);
     }
     if (valid) store_vec8(C, R.theta, R.ld, c, d, th);
   }
@@ -185,9 +219,9 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
         lp = lpp;
         ++nacc;
       }
-      if (rows_out && valid) {
-        if (!acc) load_vec8(C, R.theta, R.ld, c, d, valid, thp);
-        emit_rows(C, R, t, c, d, thp);
+      if (rows_out) {
+        if (valid && !acc) load_vec8(C, R.theta, R.ld, c, d, valid, thp);
+        emit_tile<ROWS>(C, R, t, tile0, d, thp, valid);
       }
     }
   }
@@ -237,9 +271,9 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
         lp = lpw;
         ++nacc;
       }
-      if (rows_out && valid) {
-        if (!acc) load_vec8(C, R.theta, R.ld, c, d, valid, thw);
-        emit_rows(C, R, t, c, d, thw);
+      if (rows_out) {
+        if (valid && !acc) load_vec8(C, R.theta, R.ld, c, d, valid, thw);
+        emit_tile<ROWS>(C, R, t, tile0, d, thw, valid);
       }
     }
   }
@@ -249,6 +283,7 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
     R.last_la[c] = (double)la_last;
     R.n_accept[c] += nacc;
   }
+  if (C.emit_pending) ptx::bulk_wait0();   // the staging area must outlive the copy
 }
 
 template <int METHOD, int ROWS>
@@ -351,7 +386,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     C.to_leader = (Geo<ROWS>::kPair && ptx::cluster_ctarank() != 0) ? 1 : 0;
     C.k = (warp - kCtrlWarps) >> 2;
     C.tmem_lane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
-    C.o = 0; C.g = 0; C.vslot = 0; C.pslot = 0;
+    C.o = 0; C.g = 0; C.vslot = 0; C.pslot = 0; C.emit_pending = 0;
     C.a_thr0 = sbase + SmemLayout::A + C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4);
     C.a_thr1 = sbase + SmemLayout::A + C.row * 128 + (((2 * C.k + 1) ^ (C.row & 7)) << 4);
     C.bias_thr = sbase + SmemLayout::BIAS + C.k * (P.bias16 ? 32 : 64);
@@ -746,7 +781,9 @@ int tc_step(best_ctx* ctx, best_state* st, int method, int64_t n_steps, uint64_t
     R.n_steps = seg;
     R.step0 = st->step + (uint64_t)t0;
     R.t_call0 = t0;
-    R.win = adapt ? st->win_buf : nullptr;
+    int wb = 0;
+    if (adapt) BEST_TRY(adapt_acquire_buffer(st, s, &wb));
+    R.win = adapt ? st->win_buf[wb] : nullptr;
     switch (method) {
       case tc::M_MH: BEST_TRY(launch_tc<tc::M_MH>(ctx, R, st->B, s)); break;
       case tc::M_MALA: BEST_TRY(launch_tc<tc::M_MALA>(ctx, R, st->B, s)); break;
@@ -763,7 +800,7 @@ int tc_step(best_ctx* ctx, best_state* st, int method, int64_t n_steps, uint64_t
       }
     }
     t0 += seg;
-    if (adapt) BEST_TRY(adapt_window_rows(ctx, st, st->win_buf, seg, s));
+    if (adapt) BEST_TRY(adapt_window_rows(ctx, st, wb, seg, s));
   }
   if (method == tc::M_MH || method == tc::M_AIES) st->grad_valid = false;
   return BEST_OK;

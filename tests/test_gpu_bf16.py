@@ -224,7 +224,8 @@ def _single_step_stat(B, O, w, method, seed, setup=None, chain0=0, oracle_rows=N
     if method in ("mh", "aies", "aies_de"):
         # proposal log π on EVERY core chain, accepted or not: log π(θ′) = log α + cached log π(θ) − exact terms
         # (which cancel in the difference)
-        d_lpp = np.abs((la + lp0_gpu) - (la_ref + lp0_ref))[core]
+        with np.errstate(invalid="ignore"):
+            d_lpp = np.abs((la + lp0_gpu) - (la_ref + lp0_ref))[core]
         assert d_lpp.max() <= TOL[1] * S, (info, float(d_lpp.max()))
     same = ~mism
     scale = np.abs(ost.theta).max(axis=0)
