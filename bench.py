@@ -237,7 +237,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
-    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp32"])
+    ap.add_argument("--precision", default="bf16", choices=["bf16", "fp32", "fp32tc"])
     ap.add_argument("--inner", type=int, default=0, help="sampler steps per bench step (0 = workload default)")
     ap.add_argument("--chains", type=int, default=0, help="override the number of chains per GPU")
     ap.add_argument("--trace", action="store_true", help="write the trace (thin = 1) inside the timed region")
@@ -267,7 +267,7 @@ def main():
         dist.barrier()
     from paper_2606_04895_b200 import binding as B
     B.lib()
-    prec = B.PREC_BF16 if args.precision == "bf16" else B.PREC_FP32
+    prec = {"bf16": B.PREC_BF16, "fp32": B.PREC_FP32, "fp32tc": B.PREC_FP32_TC}[args.precision]
 
     def barrier():
         if world > 1:
@@ -403,14 +403,21 @@ def main():
         extra = {}
         n_x = max(5, args.steps // 4)
         # the other configs, each with its own fraction of the measured peak
-        for name in ("lcdm_mala", "lcdm_mala_16k", "lcdm_mh_16k", "aies", "sterile_mala_16k", "sterile_hmc_65k", "hmc_fp32"):
-            sp = dict(WORKLOADS[name.replace("_fp32", "")])
+        for name in ("lcdm_mala", "lcdm_mala_16k", "lcdm_mh_16k", "aies", "sterile_mala_16k", "sterile_hmc_65k", "hmc_fp32",
+                     "hmc_fp32tc"):
+            sp = dict(WORKLOADS[name.replace("_fp32tc", "").replace("_fp32", "")])
             if name.endswith("_fp32"):      # exact path: one trajectory per bench step
                 sp["inner"] = 1
                 rr = measure(sp, n_x, 3, prec=B.PREC_FP32)
                 extra[name] = summarize(sp, rr, n_x)
                 extra[name]["frac_of_peak"] = extra[name]["tflops"] / fp32_peak_tf
                 extra[name]["peak"] = "FP32 FFMA 74.5 TFLOP/s (derived)"
+            elif name.endswith("_fp32tc"):  # exact path with split-operand tensor-core GEMMs (3 fp16 MMAs per product)
+                sp["inner"] = 1
+                rr = measure(sp, n_x, 3, prec=B.PREC_FP32_TC)
+                extra[name] = summarize(sp, rr, n_x)
+                extra[name]["frac_of_peak"] = extra[name]["tflops"] / (peak_tf / 3.0)
+                extra[name]["peak"] = "measured bf16 peak / 3 (three fp16 MMAs per product; fp16 and bf16 share the pipe rate)"
             else:
                 rr = measure(sp, n_x, 3)
                 extra[name] = summarize(sp, rr, n_x)

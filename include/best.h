@@ -52,7 +52,12 @@ enum {
 enum { BEST_ACT_TANH = 0, BEST_ACT_SILU = 1 };
 enum {
   BEST_PREC_FP32 = 0, /* FFMA emulator, fp64 chain state and Gaussian/whitening algebra          */
-  BEST_PREC_BF16 = 1  /* tcgen05 tensor-core emulator: bf16 operands, fp32 accumulate            */
+  BEST_PREC_BF16 = 1, /* tcgen05 tensor-core emulator: bf16 operands, fp32 accumulate            */
+  BEST_PREC_FP32_TC = 2 /* the exact path's structure (fp64 chain state and algebra, one GEMM per layer) with every
+                         GEMM on the tensor cores at fp32 accuracy: operands split into fp16 pairs, three MMAs per
+                         product, four fp32 accumulators (north_star "bf16/fp32 variants").  log pi / gradient within
+                         rel 1e-5 of the oracle like BEST_PREC_FP32; accept decisions identical to the oracle's
+                         outside |log u - log alpha| < 1e-5 (FP32: 1e-6).  Hidden widths >= 64.               */
 };
 
 /* Target  log π(θ) = −½(θ−μ)ᵀΣ⁻¹(θ−μ) + s·MLP(θ) − (θ_j − θ_i²)²/(2σ²) − pen(θ)

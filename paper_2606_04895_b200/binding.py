@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libbest.so")
 
 BEST_OK, BEST_ERR_ARG, BEST_ERR_CUDA, BEST_ERR_NOT_SPD, BEST_ERR_UNSUPPORTED, BEST_ERR_ALLOC = 0, -1, -2, -3, -4, -5
 ACT_TANH, ACT_SILU = 0, 1
-PREC_FP32, PREC_BF16 = 0, 1
+PREC_FP32, PREC_BF16, PREC_FP32_TC = 0, 1, 2
 METHOD_MH, METHOD_MALA, METHOD_HMC = 0, 1, 2
 
 EXPORTS = [

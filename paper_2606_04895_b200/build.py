@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OUT = os.path.join(HERE, "libbest.so")
 SOURCES = ["api.cu", "api_state.cu", "emulator_fp32.cu", "samplers.cu", "steps.cu", "tc_fused.cu",
-           "diagnostics.cu"]
+           "diagnostics.cu", "emulator_tc32.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

@@ -61,7 +61,7 @@ int best_create(const best_config* cfg, best_ctx** out) {
     set_error("best_create: unknown activation");
     return BEST_ERR_ARG;
   }
-  if (cfg->precision != BEST_PREC_FP32 && cfg->precision != BEST_PREC_BF16) {
+  if (cfg->precision != BEST_PREC_FP32 && cfg->precision != BEST_PREC_BF16 && cfg->precision != BEST_PREC_FP32_TC) {
     set_error("best_create: unknown precision");
     return BEST_ERR_ARG;
   }
@@ -185,6 +185,9 @@ int best_create(const best_config* cfg, best_ctx** out) {
   if (cfg->precision == BEST_PREC_BF16) {
     rc = tc_plan_create(ctx, cfg);
     if (rc) return fail(rc);
+  } else if (cfg->precision == BEST_PREC_FP32_TC) {
+    rc = tc32_plan_create(ctx, cfg);
+    if (rc) return fail(rc);
   }
   if (cudaDeviceSynchronize() != cudaSuccess) { set_error("best_create: device error"); return fail(BEST_ERR_CUDA); }
   *out = ctx;
@@ -194,6 +197,7 @@ int best_create(const best_config* cfg, best_ctx** out) {
 void best_destroy(best_ctx* ctx) {
   if (!ctx) return;
   if (ctx->tc) tc_plan_destroy(ctx);
+  if (ctx->tc32) tc32_plan_destroy(ctx);
   for (auto p : ctx->W) cudaFree(p);
   for (auto p : ctx->b) cudaFree(p);
   for (auto p : ctx->H) cudaFree(p);

@@ -70,6 +70,9 @@ struct TargetDev {
 };
 
 struct TcPlan;  // bf16 tensor-core path (tc_fused.cu)
+}  // namespace best
+namespace best {
+struct Tc32Plan;  // fp32-accurate split-operand tensor-core GEMMs of the exact path (emulator_tc32.cu)
 
 }  // namespace best
 
@@ -98,6 +101,7 @@ struct best_ctx {
   void* lg_scratch = nullptr;
   size_t lg_scratch_bytes = 0;
   best::TcPlan* tc = nullptr;
+  best::Tc32Plan* tc32 = nullptr;
 };
 
 struct best_state {
@@ -137,6 +141,11 @@ namespace best {
 // X0 = ctx->X0 must already hold the inputs [n][dp]; results in ctx->mlp_out / ctx->mlp_grad.
 int mlp_fp32_reserve(best_ctx* ctx, int64_t n);
 int mlp_fp32_run(best_ctx* ctx, int64_t n, bool want_grad, cudaStream_t s);
+// emulator_tc32.cu: the same GEMMs on the tensor cores with fp16-pair split operands (fp32-accurate)
+int tc32_plan_create(best_ctx* ctx, const best_config* cfg);
+void tc32_plan_destroy(best_ctx* ctx);
+int tc32_gemm(best_ctx* ctx, bool forward, int layer, const float* A, int lda, float* C, int ldc, int M,
+              const float* bias, float* aux, int ldaux, int epi, cudaStream_t s);
 
 // Full target for SoA fp64 inputs (samplers.cu): theta [d][ld] (first n columns used).
 int eval_target_soa(best_ctx* ctx, const double* theta, int64_t ld, int64_t n, double* logp,
