@@ -159,7 +159,10 @@ class Context:
 
     def close(self):
         if getattr(self, "_h", None):
-            lib().best_destroy(self._h)
+            try:
+                lib().best_destroy(self._h)
+            except TypeError:      # interpreter shutdown: the module globals are already gone
+                pass
             self._h = None
 
     def __del__(self):
@@ -234,7 +237,10 @@ class State:
 
     def close(self):
         if getattr(self, "_h", None):
-            lib().best_state_destroy(self._h)
+            try:
+                lib().best_state_destroy(self._h)
+            except TypeError:      # interpreter shutdown: the module globals are already gone
+                pass
             self._h = None
 
     def __del__(self):

@@ -234,10 +234,16 @@ extern "C" int best_rminus1(const float* trace_dev, int64_t n, int64_t B, int32_
   const int nblkM = (int)std::min<int64_t>((B + G_ROWS - 1) / G_ROWS, 148);
   double* buf = nullptr;
   const size_t n_means = (size_t)row, n_tot = n_means + (size_t)d + (size_t)(nblkS + nblkM) * dd + 2;
-  BEST_TRY(dev_alloc(&buf, n_tot));
+  // stream-ordered allocation: cudaMalloc / cudaFree per call synchronise the device (measured: 2.7 ms calls with
+  // 50-100 ms outliers)
+  if (cudaMallocAsync((void**)&buf, sizeof(double) * n_tot, s) != cudaSuccess) {
+    cudaGetLastError();
+    set_error("best_rminus1: allocation failed");
+    return BEST_ERR_ALLOC;
+  }
   double *means = buf, *gm = means + n_means, *accS = gm + d, *accM = accS + (size_t)nblkS * dd,
          *out = accM + (size_t)nblkM * dd;
-  auto done = [&](int rc) { cudaFree(buf); return rc; };
+  auto done = [&](int rc) { cudaFreeAsync(buf, s); return rc; };
   k_chain_means<<<(unsigned)((row + 255) / 256), 256, 0, s>>>(trace_dev, n, row, means);
   k_grand_mean<<<1, 1024, 0, s>>>(means, B, d, gm);
   k_gram_partial<float><<<nblkS, G_TPB, 0, s>>>(trace_dev, n * B, d, gm, accS);
