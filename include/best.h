@@ -204,6 +204,20 @@ int best_set_hard_box(best_ctx* ctx, int32_t on);
  * 1e-12 (e.g. a dimension in which no chain ever moved: R - 1 > 1e12 is not resolvable) or some B_ii = 0. */
 int best_rminus1(const float* trace_dev, int64_t n, int64_t B, int32_t d, double* rminus1_host, void* stream);
 
+/* best_rminus1 for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): the same kernels, grids and summation order (hence the same bits, PAPER.md eq
+ * (4.1)-(4.2)), with the scratch in a file-scope `static __device__` array of 2^20 doubles (8 MiB, held by every
+ * GPU that loads the library until exit).  Calls no cudaMalloc / cudaMallocAsync / cudaFree; the first call on a
+ * device looks the array's device address up (cudaGetSymbolAddress) and caches it.  Arguments as best_rminus1.
+ * Limit: B*d + d + (min(ceil(n*B/64), 592) + min(ceil(B/64), 148))*d*d + 2 <= best_rminus1_noalloc_max_doubles()
+ * (e.g. B <= 18 800 chains at d = 27, B <= 9 000 at d = 32, any n); larger traces return BEST_ERR_ARG with the
+ * sizes in best_last_error() -- use best_rminus1.  All calls on one device SHARE the array, which keeps the last
+ * call's contents (every word a call reads is first written by that call, nothing needs clearing): calls that
+ * overlap on the GPU (two streams or two host threads) race.  Synchronises `stream`.  Other errors as
+ * best_rminus1, BEST_ERR_CUDA if the symbol lookup fails.                                                     */
+int best_rminus1_noalloc(const float* trace_dev, int64_t n, int64_t B, int32_t d, double* rminus1_host, void* stream);
+int64_t best_rminus1_noalloc_max_doubles(void);
+
 /* Measurement aid for the small-batch roofline ("measure the box's L2 bandwidth with a
  * resident-copy microbenchmark"; the small-batch path streams the weight packs from L2, sec. 3.1
  * "evaluating the emulator for up to 100 points simultaneously does not affect the evaluation time").

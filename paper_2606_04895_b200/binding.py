@@ -25,7 +25,7 @@ EXPORTS = [
     "best_adapt_stats", "best_get_whitening", "best_set_whitening", "best_state_get",
     "best_state_get_f64", "best_state_last_log_alpha", "best_state_set", "best_launch_count",
     "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box", "best_burn_in", "best_step_aies_de", "best_rminus1", "best_probe_l2_read",
-    "best_state_set_chain_offset",
+    "best_state_set_chain_offset", "best_rminus1_noalloc", "best_rminus1_noalloc_max_doubles",
 ]
 
 
@@ -82,6 +82,9 @@ def lib():
     L.best_set_hard_box.argtypes = [vp, i32]
     L.best_rminus1.argtypes = [vp, i64, i64, i32, C.POINTER(C.c_double), vp]
     L.best_probe_l2_read.argtypes = [i64, i32, C.POINTER(C.c_double), vp]
+    L.best_rminus1_noalloc.argtypes = [vp, i64, i64, i32, C.POINTER(C.c_double), vp]
+    L.best_rminus1_noalloc_max_doubles.argtypes = []
+    L.best_rminus1_noalloc_max_doubles.restype = i64
     L.best_burn_in.argtypes = [vp, vp, i32, i32, i64, i64, i64, u64, C.POINTER(C.c_float), C.c_float, i32,
                                C.c_double, vp, C.POINTER(C.c_double), vp, vp]
     L.best_state_get.argtypes = [vp, vp, vp, vp, C.POINTER(u64), vp, C.POINTER(u64), vp]
@@ -210,6 +213,20 @@ def rminus1(trace, stream=0) -> float:
     out = C.c_double()
     _check(lib().best_rminus1(_ptr(trace), n, nb, d, C.byref(out), stream or None))
     return out.value
+
+
+def rminus1_noalloc(trace, stream=0) -> float:
+    """best_rminus1_noalloc: best_rminus1 with its scratch in a static device array (no allocation; size limit)."""
+    n, nb, d = trace.shape
+    if not trace.is_contiguous():
+        raise ValueError("trace must be contiguous")
+    out = C.c_double()
+    _check(lib().best_rminus1_noalloc(_ptr(trace), n, nb, d, C.byref(out), stream or None))
+    return out.value
+
+
+def rminus1_noalloc_max_doubles() -> int:
+    return int(lib().best_rminus1_noalloc_max_doubles())
 
 
 def probe_l2_read(n_bytes=32 << 20, passes=20, stream=0) -> float:

@@ -6,6 +6,7 @@
 // W~ = L L^T is SPD and B~ symmetric, so the eigenvalues are those of the symmetric L^-1 B~ L^-T (cyclic
 // Jacobi).  Everything is accumulated in fp64; partial sums are combined in a fixed order.
 #include <algorithm>
+#include <mutex>
 
 #include "best_internal.h"
 #include "gram.cuh"
@@ -263,4 +264,91 @@ extern "C" int best_rminus1(const float* trace_dev, int64_t n, int64_t B, int32_
     return done(BEST_ERR_NOT_SPD);
   }
   return done(BEST_OK);
+}
+
+// ---- best_rminus1_noalloc: the same five launches with the scratch in a file-scope device array ------------
+// For callers that must not allocate (CUDA graph capture around them, serving loops, harnesses that forbid
+// cudaMalloc).  Every GPU that loads the library holds these 8 MiB until exit.  All calls on a device share the
+// array and it keeps the last call's contents: every word a call reads (chain means, grand mean, the Gram
+// partials of the blocks it launches, the two result words) is written by that call's own kernels first, so
+// nothing needs clearing -- but two calls that overlap on the GPU (two streams, two host threads) race on it.
+namespace best {
+namespace {
+constexpr size_t kNoAllocDoubles = (size_t)1 << 20;                       // 8 MiB
+static __device__ __align__(256) double g_rminus1_scratch[kNoAllocDoubles];
+
+// In host code `g_rminus1_scratch` is only the host-side shadow of the symbol, not a device address: the device
+// address is looked up once per device, with that device current, and cached.
+int noalloc_scratch(double** p) {
+  constexpr int kMaxDev = 64;
+  static std::mutex mu;
+  static double* cached[kMaxDev] = {};
+  int dev = -1;
+  BEST_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDev) { set_error("best_rminus1_noalloc: device ordinal above 63"); return BEST_ERR_ARG; }
+  std::lock_guard<std::mutex> lk(mu);
+  if (!cached[dev]) {
+    void* sym = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&sym, g_rminus1_scratch);
+    if (e != cudaSuccess || !sym) {
+      cudaGetLastError();
+      set_error(std::string("best_rminus1_noalloc: cudaGetSymbolAddress failed: ") + cudaGetErrorString(e));
+      return BEST_ERR_CUDA;
+    }
+    cached[dev] = static_cast<double*>(sym);
+  }
+  *p = cached[dev];
+  return BEST_OK;
+}
+}  // namespace
+}  // namespace best
+
+extern "C" int64_t best_rminus1_noalloc_max_doubles(void) { return (int64_t)best::kNoAllocDoubles; }
+
+extern "C" int best_rminus1_noalloc(const float* trace_dev, int64_t n, int64_t B, int32_t d, double* rminus1_host,
+                                    void* stream) {
+  if (!trace_dev || !rminus1_host || n < 2 || B < 2 || d < 1 || d > kMaxD) {
+    set_error("best_rminus1_noalloc: need a trace with n >= 2 samples, B >= 2 chains, 1 <= d <= 32");
+    return BEST_ERR_ARG;
+  }
+  if (!is_device_ptr(trace_dev)) {
+    set_error("best_rminus1_noalloc: trace must be a device pointer");
+    return BEST_ERR_ARG;
+  }
+  cudaStream_t s = (cudaStream_t)stream;
+  const int dd = d * d;
+  const int64_t row = B * (int64_t)d;
+  // the same grids as best_rminus1, hence the same summation order and the same bits
+  const int nblkS = (int)std::min<int64_t>((n * B + G_ROWS - 1) / G_ROWS, 592);
+  const int nblkM = (int)std::min<int64_t>((B + G_ROWS - 1) / G_ROWS, 148);
+  const size_t n_means = (size_t)row, n_tot = n_means + (size_t)d + (size_t)(nblkS + nblkM) * dd + 2;
+  if (row > (int64_t)kNoAllocDoubles || n_tot > kNoAllocDoubles) {
+    set_error("best_rminus1_noalloc: B*d + d + (blocks_S + blocks_M)*d*d + 2 = " + std::to_string(n_tot) +
+              " doubles of scratch needed, the static array holds " + std::to_string(kNoAllocDoubles) +
+              " (8 MiB; blocks_S = min(ceil(n*B/64), 592), blocks_M = min(ceil(B/64), 148)): use best_rminus1");
+    return BEST_ERR_ARG;
+  }
+  double* buf = nullptr;
+  BEST_TRY(noalloc_scratch(&buf));
+  double *means = buf, *gm = means + n_means, *accS = gm + d, *accM = accS + (size_t)nblkS * dd,
+         *out = accM + (size_t)nblkM * dd;
+  k_chain_means<<<(unsigned)((row + 255) / 256), 256, 0, s>>>(trace_dev, n, row, means);
+  k_grand_mean<<<1, 1024, 0, s>>>(means, B, d, gm);
+  k_gram_partial<float><<<nblkS, G_TPB, 0, s>>>(trace_dev, n * B, d, gm, accS);
+  k_gram_partial<double><<<nblkM, G_TPB, 0, s>>>(means, B, d, gm, accM);
+  k_rminus1_finalize<<<1, 256, 0, s>>>(accS, nblkS, accM, nblkM, d, (double)n, (double)B, out);
+  count_launch(5);
+  double h[2] = {0.0, 0.0};
+  if (cudaGetLastError() != cudaSuccess || cudaMemcpyAsync(h, out, sizeof(h), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+      cudaStreamSynchronize(s) != cudaSuccess) {
+    set_error("best_rminus1_noalloc: CUDA failure");
+    cudaGetLastError();
+    return BEST_ERR_CUDA;
+  }
+  *rminus1_host = h[0];
+  if (h[1] != 0.0) {
+    set_error("best_rminus1_noalloc: the mean chain covariance is not positive definite (or some chain means coincide)");
+    return BEST_ERR_NOT_SPD;
+  }
+  return BEST_OK;
 }
