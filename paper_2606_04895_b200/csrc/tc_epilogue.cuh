@@ -47,13 +47,13 @@ __device__ __forceinline__ void arrive_mma(const EpiCtx& C, uint32_t bar) {
 
 // bias of the thread's 16 columns of group jn as 8 fp32 pairs
 template <int ROWS>
-__device__ __forceinline__ void load_bias(const EpiCtx& C, int layer, int jn, f32x2 (&b)[8]) {
+__device__ __forceinline__ void load_bias(const EpiCtx& C, int layer, int jn, int colofs, f32x2 (&b)[8]) {
   if (!C.P->bias16) {
-    const uint32_t a = C.bias_thr + (uint32_t)(layer * C.P->H + jn * 64) * 4u;
+    const uint32_t a = C.bias_thr + (uint32_t)(layer * C.P->H + jn * 64 + colofs) * 4u;
 #pragma unroll
     for (int i = 0; i < 4; ++i) ptx::lds_c2x64(a + i * 16, b[2 * i], b[2 * i + 1]);
   } else {   // bf16 table (the fp32 one would not fit beside a 1024-wide layer's other tables)
-    const uint32_t a = C.bias_thr + (uint32_t)(layer * C.P->H + jn * 64) * 2u;
+    const uint32_t a = C.bias_thr + (uint32_t)(layer * C.P->H + jn * 64 + colofs) * 2u;
     unsigned long long q[4];
     ptx::lds_c2x64(a, q[0], q[1]);
     ptx::lds_c2x64(a + 16, q[2], q[3]);
@@ -81,6 +81,14 @@ __device__ __forceinline__ void store_a(const EpiCtx& C, int jn, const uint32_t 
   }
 }
 
+
+// chunk-owner geometry: the thread's 16 bf16 results of piece p (columns [16p, 16p+16)) of k-chunk jn
+template <int ROWS>
+__device__ __forceinline__ void store_piece(const EpiCtx& C, int jn, int p, const uint32_t (&hp)[8]) {
+  const uint32_t base = C.a_thr0 + (uint32_t)jn * Geo<ROWS>::kAChunk;   // a_thr0 = row base, a_thr1 = row & 7
+  ptx::sts_128(base + (((uint32_t)(2 * p) ^ C.a_thr1) << 4), hp[0], hp[1], hp[2], hp[3]);
+  ptx::sts_128(base + (((uint32_t)(2 * p + 1) ^ C.a_thr1) << 4), hp[4], hp[5], hp[6], hp[7]);
+}
 
 __device__ __forceinline__ void qbar(const EpiCtx& C) { ptx::named_bar_sync(1 + (C.row >> 5), 128); }
 
@@ -129,6 +137,11 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   ptx::fence_proxy_async();
   if ((!Geo<ROWS>::kInPlace)) {
     ptx::mbar_arrive(C.bars.xin_done());   // warp 3 publishes a_ready
+  } else if (Geo<ROWS>::kOwn) {
+    // a_ready(j) counts one row quarter's worth of arrivals per k: the chain's four threads have all written
+    // (and fenced) their parts of chunk 0 once the quarter's named barrier is passed
+    qbar(C);
+    for (int j = C.k; j < C.P->kch_max; j += 4) arrive_mma(C, C.bars.a_ready(j));
   } else {
     for (int j = 0; j < C.P->kch_max; ++j) arrive_mma(C, C.bars.a_ready(j));
   }
@@ -144,15 +157,17 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
 
 // bias + activation (+ act' to scratch, or delta for the last layer) of one group, in registers
 template <int ACT, bool LAST, int ROWS>
-__device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, const uint32_t (&v)[16],
+__device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, int colofs, const uint32_t (&v)[16],
                                           bool want_grad, uint8_t* dact_l, f32x2& acc2, uint32_t (&hp)[8]) {
+  // colofs: first column of the thread's 16 inside the 64-column group when the per-thread bases do not hold
+  // it already (chunk-owner geometry: 16 p; otherwise 0)
   constexpr uint32_t kDBlk = Geo<ROWS>::kTileRows * 128, kDPiece = Geo<ROWS>::kTileRows * 16;
   f32x2 b[8];
-  load_bias<ROWS>(C, layer, jn, b);
+  load_bias<ROWS>(C, layer, jn, colofs, b);
   f32x2 ws[8];
   if (LAST) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) ptx::lds_c2x64(C.wouts_thr + jn * 256 + i * 16, ws[2 * i], ws[2 * i + 1]);
+    for (int i = 0; i < 4; ++i) ptx::lds_c2x64(C.wouts_thr + jn * 256 + colofs * 4 + i * 16, ws[2 * i], ws[2 * i + 1]);
   }
   uint32_t dp[8];
 #pragma unroll
@@ -169,7 +184,7 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, co
     }
   }
   if (!LAST && want_grad) {
-    uint8_t* dptr = dact_l + (size_t)jn * kDBlk;
+    uint8_t* dptr = dact_l + (size_t)jn * kDBlk + (size_t)(colofs >> 3) * kDPiece;
     ptx::stg_128(dptr, dp[0], dp[1], dp[2], dp[3]);
     ptx::stg_128(dptr + kDPiece, dp[4], dp[5], dp[6], dp[7]);
   }
@@ -207,13 +222,34 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
     const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && writes_a && (c != op.nch - 1);
+    if (Geo<ROWS>::kOwn) {
+      const uint32_t tbase = C.tmem_lane + buf * Geo<ROWS>::kBufCols;
+      for (int grp = C.k; grp < ngrp; grp += 4) {
+        const int jn = c * ngrp + grp;
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+          uint32_t v[16], hp[8];
+          ptx::tmem_ld16(tbase + grp * 64 + p * 16, v);
+          ptx::tmem_ld_wait();
+          fwd_group<ACT, LAST, ROWS>(C, op.layer, jn, 16 * p, v, want_grad, dact_l, acc2, hp);
+          if (writes_a) {
+            if (gate && p == 0) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
+            store_piece<ROWS>(C, jn, p, hp);
+          }
+        }
+        if (writes_a) publish_a<ROWS>(C, jn, 1);
+      }
+      ptx::tc_fence_before();
+      arrive_mma(C, C.bars.d_free(buf));
+      continue;
+    }
     for (int g0 = 0; g0 < ngrp; ++g0) {
       const int grp = g0;
       const int jn = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, grp, ngrp) : c * ngrp + grp;
       uint32_t v[16], hp[8];
       ptx::tmem_ld16(tcol + grp * 64, v);
       ptx::tmem_ld_wait();
-      fwd_group<ACT, LAST, ROWS>(C, op.layer, jn, v, want_grad, dact_l, acc2, hp);
+      fwd_group<ACT, LAST, ROWS>(C, op.layer, jn, 0, v, want_grad, dact_l, acc2, hp);
       if (writes_a) {
         if (gate) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
         store_a<ROWS>(C, jn, hp);
@@ -228,6 +264,7 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
     ptx::tc_fence_before();
     arrive_mma(C, C.bars.d_free(buf));
   }
+  if (Geo<ROWS>::kOwn && writes_a) written = op.nch * ngrp;   // (all k-chunks, by their owners)
 }
 
 // backward epilogue: delta_{l-1} = (delta_l W_l) .* act'_{l-1}
@@ -252,6 +289,50 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
   // before its accumulator is complete, the first group of the next N-chunk while the last group of this one is
   // processed (requesting it only at the top of the chunk exposed an L2 round trip per chunk: in the N-chunk-outer
   // order the next chunk's accumulator is usually complete by then).
+  if (Geo<ROWS>::kOwn) {
+    // chunk-owner order: the thread's pieces are (c, grp = k mod 4, p = 0..3); act' of the NEXT piece is requested
+    // while the current one is processed, across group and N-chunk boundaries as well
+    uint4 a0 = make_uint4(0, 0, 0, 0), a1 = a0;
+    if (C.k < ngrp) {
+      const uint8_t* dp = dact_l + (size_t)C.k * kDBlk;
+      a0 = ptx::ldg_128(dp); a1 = ptx::ldg_128(dp + kDPiece);
+    }
+    for (int c = 0; c < op.nch; ++c, ++C.g) {
+      const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
+      const bool gate = (c != op.nch - 1);
+      ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
+      ptx::tc_fence_after();
+      const uint32_t tbase = C.tmem_lane + buf * Geo<ROWS>::kBufCols;
+      for (int grp = C.k; grp < ngrp; grp += 4) {
+        const int jn = c * ngrp + grp;
+#pragma unroll
+        for (int p = 0; p < 4; ++p) {
+          uint32_t v[16], hp[8];
+          ptx::tmem_ld16(tbase + grp * 64 + p * 16, v);
+          const uint4 d0 = a0, d1 = a1;
+          if (p < 3) {
+            const uint8_t* dn = dact_l + (size_t)jn * kDBlk + (size_t)(2 * p + 2) * kDPiece;
+            a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
+          } else {
+            const int jnn = (grp + 4 < ngrp) ? jn + 4 : ((c + 1 < op.nch) ? (c + 1) * ngrp + C.k : -1);
+            if (jnn >= 0) {
+              const uint8_t* dn = dact_l + (size_t)jnn * kDBlk;
+              a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
+            }
+          }
+          ptx::tmem_ld_wait();
+          bwd_group<ROWS>(v, d0, d1, hp);
+          if (gate && p == 0) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
+          store_piece<ROWS>(C, jn, p, hp);
+        }
+        publish_a<ROWS>(C, jn, 1);
+      }
+      ptx::tc_fence_before();
+      arrive_mma(C, C.bars.d_free(buf));
+    }
+    written = op.nch * ngrp;
+    return;
+  }
   uint4 a0, a1;
   {
     const int jnc0 = Geo<ROWS>::kPair ? pair_jn(op, 0, C.half, 0, ngrp) : 0;
@@ -353,7 +434,9 @@ __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool wa
     if ((!Geo<ROWS>::kInPlace)) {   // keep every epi_done barrier at one phase per op (written = 64-column groups)
       for (int c = (written * 64 + op.ncols - 1) / op.ncols; c < 4; ++c) ptx::mbar_arrive(C.bars.epi_done(c));
     } else if (oi != n_ops - 1) {  // keep every a_ready barrier at one phase per op
-      if (!Geo<ROWS>::kPair) {
+      if (Geo<ROWS>::kOwn) {   // chunk j's arrivals come from the k = j mod 4 threads
+        for (int j = written + ((C.k - written) & 3); j < C.P->kch_max; j += 4) arrive_mma(C, C.bars.a_ready(j));
+      } else if (!Geo<ROWS>::kPair) {
         for (int j = written; j < C.P->kch_max; ++j) arrive_mma(C, C.bars.a_ready(j));
       } else if (written == 0 && C.half == 0) {   // pair: an op writes all k-chunks or none
         for (int j = 0; j < C.P->kch_max; ++j) arrive_mma(C, C.bars.a_ready(j));

@@ -24,6 +24,10 @@
 #include "tc_fused.h"
 #include "tc_ptx.cuh"
 
+#ifndef BEST_TC_OWN
+#define BEST_TC_OWN 1
+#endif
+
 namespace best {
 
 namespace tc {
@@ -63,6 +67,12 @@ template <int ROWS> struct Geo {
   // batch too small to fill the chip with 64-chain CTAs (4096 chains = 64 CTAs) spreads over twice the SMs.
   static constexpr bool kPingPong = (ROWS == 265 || ROWS == 233);
   static constexpr bool kInPlace = (ROWS == 128 || kPair);   // operand stays in SMEM
+  // ROWS = 128: every 64-column k-chunk of the next operand is produced by ONE of a row's four epilogue threads
+  // (warp k owns the groups grp = k mod 4 of each N-chunk and walks them in four 16-column pieces), so the
+  // store -> proxy fence -> arrive sequence is paid once per 64 columns of a thread instead of once per 16
+  // and a_ready counts 128 arrivals (profiles/r2b: the fence path was 20 % of the epilogue warps' time).
+  static constexpr bool kOwn = (ROWS == 128) && BEST_TC_OWN;
+  static constexpr int kAReadyArrive = kOwn ? 128 : (kHalf ? 256 : 512);
   static constexpr int kTileRows = kPair ? 64 : ROWS;   // rows of the CTA's operand / act' blocks
   static constexpr int kChains = kHalf ? 32 : kTileRows;   // chains the CTA advances
   static constexpr int kEpiArrive = kHalf ? 256 : 512;      // epilogue threads that run (per CTA)

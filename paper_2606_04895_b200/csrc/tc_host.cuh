@@ -310,7 +310,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     for (int i = 0; i < kMaxKch; ++i) {
       // arrivals per phase: in place = every epilogue thread (pair: the 256 of the lane half that owns the
       // k-chunk); L2-image tiles = warp 3 alone (+ the bulk copy's bytes)
-      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : Geo<ROWS>::kEpiArrive);   // pair: half of each CTA's
+      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : Geo<ROWS>::kAReadyArrive);   // pair: half of each CTA's; owner: one warp per row quarter
       ptx::mbar_init(bars.a_free(i), Geo<ROWS>::kPair ? 2 : 1);   // pair kernels: two issuing warps
     }
     for (int i = 0; i < 4; ++i) {
@@ -387,13 +387,21 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     C.k = (warp - kCtrlWarps) >> 2;
     C.tmem_lane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
     C.o = 0; C.g = 0; C.vslot = 0; C.pslot = 0; C.emit_pending = 0;
-    C.a_thr0 = sbase + SmemLayout::A + C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4);
-    C.a_thr1 = sbase + SmemLayout::A + C.row * 128 + (((2 * C.k + 1) ^ (C.row & 7)) << 4);
-    C.bias_thr = sbase + SmemLayout::BIAS + C.k * (P.bias16 ? 32 : 64);
-    C.wouts_thr = sbase + SmemLayout::WOUTS + C.k * 64;
+    if (Geo<ROWS>::kOwn) {   // chunk-owner epilogue: bases without the k offsets (store_piece, fwd_group colofs)
+      C.a_thr0 = sbase + SmemLayout::A + C.row * 128;
+      C.a_thr1 = (uint32_t)(C.row & 7);
+      C.bias_thr = sbase + SmemLayout::BIAS;
+      C.wouts_thr = sbase + SmemLayout::WOUTS;
+      C.dact_thr = reinterpret_cast<uint8_t*>(P.dact + (size_t)blockIdx.x * P.dact_tile_elems) + (size_t)C.row * 16u;
+    } else {
+      C.a_thr0 = sbase + SmemLayout::A + C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4);
+      C.a_thr1 = sbase + SmemLayout::A + C.row * 128 + (((2 * C.k + 1) ^ (C.row & 7)) << 4);
+      C.bias_thr = sbase + SmemLayout::BIAS + C.k * (P.bias16 ? 32 : 64);
+      C.wouts_thr = sbase + SmemLayout::WOUTS + C.k * 64;
+      C.dact_thr = reinterpret_cast<uint8_t*>(P.dact + (size_t)blockIdx.x * P.dact_tile_elems) +
+                   (size_t)(2 * C.k * Geo<ROWS>::kTileRows + C.row) * 16u;
+    }
     C.v_thr = (uint32_t)C.row * 8u;
-    C.dact_thr = reinterpret_cast<uint8_t*>(P.dact + (size_t)blockIdx.x * P.dact_tile_elems) +
-                 (size_t)(2 * C.k * Geo<ROWS>::kTileRows + C.row) * 16u;
     C.aimg_thr = (!Geo<ROWS>::kInPlace) ? P.aimg + (size_t)blockIdx.x * (16u * Geo<ROWS>::kAChunk) + C.row * 128 + (((2 * C.k) ^ (C.row & 7)) << 4)
                      : nullptr;
     if (C.row >= Geo<ROWS>::kChains) {
