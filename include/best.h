@@ -25,7 +25,7 @@
  *    layer buffers) and the whitening factor, so a context is driven from ONE stream (and one host thread) at
  *    a time; different contexts are independent.  Calls documented as "synchronises the device" order
  *    themselves against work in flight on any stream.
- *  - Environment: BEST_TC_ROWS = 128 | 265 | 233 | 264 | 232 | 64 | 32, read at best_create, forces a tile
+ *  - Environment: BEST_TC_ROWS = 128 | 256 | 265 | 233 | 264 | 232 | 64 | 32, read at best_create, forces a tile
  *    geometry of the tensor-core path that the widths allow (tests compare geometries bit for bit); results
  *    do not depend on it.  No other environment variable is read.
  */

@@ -45,6 +45,12 @@ __device__ __forceinline__ void arrive_mma(const EpiCtx& C, uint32_t bar) {
   else ptx::mbar_arrive(bar);
 }
 
+// the owner of a k-chunk arrives for the row's four threads
+__device__ __forceinline__ void arrive_mma4(const EpiCtx& C, uint32_t bar) {
+  if (C.to_leader) ptx::mbar_arrive4_leader(bar);
+  else ptx::mbar_arrive4(bar);
+}
+
 // bias of the thread's 16 columns of group jn as 8 fp32 pairs
 template <int ROWS>
 __device__ __forceinline__ void load_bias(const EpiCtx& C, int layer, int jn, int colofs, f32x2 (&b)[8]) {
@@ -137,11 +143,6 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
   ptx::fence_proxy_async();
   if ((!Geo<ROWS>::kInPlace)) {
     ptx::mbar_arrive(C.bars.xin_done());   // warp 3 publishes a_ready
-  } else if (Geo<ROWS>::kOwn) {
-    // a_ready(j) counts one row quarter's worth of arrivals per k: the chain's four threads have all written
-    // (and fenced) their parts of chunk 0 once the quarter's named barrier is passed
-    qbar(C);
-    for (int j = C.k; j < C.P->kch_max; j += 4) arrive_mma(C, C.bars.a_ready(j));
   } else {
     for (int j = 0; j < C.P->kch_max; ++j) arrive_mma(C, C.bars.a_ready(j));
   }
@@ -224,20 +225,39 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
     const bool gate = Geo<ROWS>::kInPlace && !Geo<ROWS>::kPingPong && writes_a && (c != op.nch - 1);
     if (Geo<ROWS>::kOwn) {
       const uint32_t tbase = C.tmem_lane + buf * Geo<ROWS>::kBufCols;
-      for (int grp = C.k; grp < ngrp; grp += 4) {
-        const int jn = c * ngrp + grp;
+      if (!Geo<ROWS>::kOwnLastInterleaved || c != op.nch - 1 || !writes_a) {   // owner order
+        for (int grp = C.k; grp < ngrp; grp += 4) {
+          const int jn = c * ngrp + grp;
 #pragma unroll
-        for (int p = 0; p < 4; ++p) {
-          uint32_t v[16], hp[8];
-          ptx::tmem_ld16(tbase + grp * 64 + p * 16, v);
-          ptx::tmem_ld_wait();
-          fwd_group<ACT, LAST, ROWS>(C, op.layer, jn, 16 * p, v, want_grad, dact_l, acc2, hp);
+          for (int p = 0; p < 4; ++p) {
+            uint32_t v[16], hp[8];
+            ptx::tmem_ld16(tbase + grp * 64 + p * 16, v);
+            ptx::tmem_ld_wait();
+            fwd_group<ACT, LAST, ROWS>(C, op.layer, jn, 16 * p, v, want_grad, dact_l, acc2, hp);
+            if (writes_a) {
+              if (gate && p == 0) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
+              store_piece<ROWS>(C, jn, p, hp);
+            }
+          }
           if (writes_a) {
-            if (gate && p == 0) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
-            store_piece<ROWS>(C, jn, p, hp);
+            ptx::fence_proxy_async();
+            arrive_mma4(C, C.bars.a_ready(jn));
           }
         }
-        if (writes_a) publish_a<ROWS>(C, jn, 1);
+      } else {   // last N-chunk: the next op's MMAs consume k-chunk after k-chunk as they are published
+#pragma unroll
+        for (int g0 = 0; g0 < 4; ++g0) {
+          if (g0 < ngrp) {
+            const int jn = c * ngrp + g0;
+            uint32_t v[16], hp[8];
+            ptx::tmem_ld16(tbase + g0 * 64 + C.k * 16, v);
+            ptx::tmem_ld_wait();
+            fwd_group<ACT, LAST, ROWS>(C, op.layer, jn, 16 * C.k, v, want_grad, dact_l, acc2, hp);
+            store_piece<ROWS>(C, jn, C.k, hp);
+            ptx::fence_proxy_async();
+            arrive_mma(C, C.bars.a_ready(jn));
+          }
+        }
       }
       ptx::tc_fence_before();
       arrive_mma(C, C.bars.d_free(buf));
@@ -290,42 +310,64 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
   // processed (requesting it only at the top of the chunk exposed an L2 round trip per chunk: in the N-chunk-outer
   // order the next chunk's accumulator is usually complete by then).
   if (Geo<ROWS>::kOwn) {
-    // chunk-owner order: the thread's pieces are (c, grp = k mod 4, p = 0..3); act' of the NEXT piece is requested
-    // while the current one is processed, across group and N-chunk boundaries as well
+    // every N-chunk but the last in owner order (pieces (grp = k mod 4, p = 0..3)), the last one interleaved (all
+    // four threads of a row on group g0, columns [16k, 16k+16)); act' of the NEXT piece is requested while the
+    // current one is processed, across group and N-chunk boundaries as well
+    const int last = op.nch - 1;
+    auto owner_chunk = [&](int c) -> bool { return !Geo<ROWS>::kOwnLastInterleaved || c != last; };
+    auto piece_ptr = [&](int c, int i) -> const uint8_t* {   // i-th piece of this thread in N-chunk c (ngrp <= 4)
+      return owner_chunk(c) ? dact_l + (size_t)(c * ngrp + C.k) * kDBlk + (size_t)(2 * i) * kDPiece
+                            : dact_l + (size_t)(c * ngrp + i) * kDBlk + (size_t)(2 * C.k) * kDPiece;
+    };
     uint4 a0 = make_uint4(0, 0, 0, 0), a1 = a0;
-    if (C.k < ngrp) {
-      const uint8_t* dp = dact_l + (size_t)C.k * kDBlk;
+    if (!owner_chunk(0) || C.k < ngrp) {   // (an op has one or two N-chunks; with two, ngrp = 4 > k)
+      const uint8_t* dp = piece_ptr(0, 0);
       a0 = ptx::ldg_128(dp); a1 = ptx::ldg_128(dp + kDPiece);
     }
     for (int c = 0; c < op.nch; ++c, ++C.g) {
       const uint32_t buf = C.g % Geo<ROWS>::kNBuf, use = C.g / Geo<ROWS>::kNBuf;
-      const bool gate = (c != op.nch - 1);
       ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
       ptx::tc_fence_after();
       const uint32_t tbase = C.tmem_lane + buf * Geo<ROWS>::kBufCols;
-      for (int grp = C.k; grp < ngrp; grp += 4) {
-        const int jn = c * ngrp + grp;
+      if (!Geo<ROWS>::kOwnLastInterleaved || c != last) {   // owner order
+        const int jn = c * ngrp + C.k;
+        if (C.k < ngrp) {
 #pragma unroll
-        for (int p = 0; p < 4; ++p) {
-          uint32_t v[16], hp[8];
-          ptx::tmem_ld16(tbase + grp * 64 + p * 16, v);
-          const uint4 d0 = a0, d1 = a1;
-          if (p < 3) {
-            const uint8_t* dn = dact_l + (size_t)jn * kDBlk + (size_t)(2 * p + 2) * kDPiece;
-            a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
-          } else {
-            const int jnn = (grp + 4 < ngrp) ? jn + 4 : ((c + 1 < op.nch) ? (c + 1) * ngrp + C.k : -1);
-            if (jnn >= 0) {
-              const uint8_t* dn = dact_l + (size_t)jnn * kDBlk;
+          for (int p = 0; p < 4; ++p) {
+            uint32_t v[16], hp[8];
+            ptx::tmem_ld16(tbase + C.k * 64 + p * 16, v);
+            const uint4 d0 = a0, d1 = a1;
+            if (p < 3 || c + 1 < op.nch) {
+              const uint8_t* dn = (p < 3) ? piece_ptr(c, p + 1) : piece_ptr(c + 1, 0);
               a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
             }
+            ptx::tmem_ld_wait();
+            bwd_group<ROWS>(v, d0, d1, hp);
+            if (p == 0) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
+            store_piece<ROWS>(C, jn, p, hp);
           }
-          ptx::tmem_ld_wait();
-          bwd_group<ROWS>(v, d0, d1, hp);
-          if (gate && p == 0) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
-          store_piece<ROWS>(C, jn, p, hp);
+          ptx::fence_proxy_async();
+          arrive_mma4(C, C.bars.a_ready(jn));
         }
-        publish_a<ROWS>(C, jn, 1);
+      } else {
+#pragma unroll
+        for (int g0 = 0; g0 < 4; ++g0) {
+          if (g0 < ngrp) {
+            const int jn = c * ngrp + g0;
+            uint32_t v[16], hp[8];
+            ptx::tmem_ld16(tbase + g0 * 64 + C.k * 16, v);
+            const uint4 d0 = a0, d1 = a1;
+            if (g0 + 1 < ngrp) {
+              const uint8_t* dn = piece_ptr(c, g0 + 1);
+              a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
+            }
+            ptx::tmem_ld_wait();
+            bwd_group<ROWS>(v, d0, d1, hp);
+            store_piece<ROWS>(C, jn, C.k, hp);
+            ptx::fence_proxy_async();
+            arrive_mma(C, C.bars.a_ready(jn));
+          }
+        }
       }
       ptx::tc_fence_before();
       arrive_mma(C, C.bars.d_free(buf));
@@ -434,9 +476,7 @@ __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool wa
     if ((!Geo<ROWS>::kInPlace)) {   // keep every epi_done barrier at one phase per op (written = 64-column groups)
       for (int c = (written * 64 + op.ncols - 1) / op.ncols; c < 4; ++c) ptx::mbar_arrive(C.bars.epi_done(c));
     } else if (oi != n_ops - 1) {  // keep every a_ready barrier at one phase per op
-      if (Geo<ROWS>::kOwn) {   // chunk j's arrivals come from the k = j mod 4 threads
-        for (int j = written + ((C.k - written) & 3); j < C.P->kch_max; j += 4) arrive_mma(C, C.bars.a_ready(j));
-      } else if (!Geo<ROWS>::kPair) {
+      if (!Geo<ROWS>::kPair) {
         for (int j = written; j < C.P->kch_max; ++j) arrive_mma(C, C.bars.a_ready(j));
       } else if (written == 0 && C.half == 0) {   // pair: an op writes all k-chunks or none
         for (int j = 0; j < C.P->kch_max; ++j) arrive_mma(C, C.bars.a_ready(j));

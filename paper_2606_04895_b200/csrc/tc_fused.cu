@@ -50,8 +50,16 @@ constexpr int kRows = 128;           // TMEM lanes == MMA M
 //                CTA (lanes 64..127 hold the upper half of N for the same 64 rows), so a whole
 //                1024-wide layer of accumulators fits TMEM and the operand is rewritten in place.
 template <int ROWS> struct Geo {
-  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32 || ROWS == 264 || ROWS == 265 || ROWS == 233 || ROWS == 232, "tile geometry");
+  static_assert(ROWS == 128 || ROWS == 64 || ROWS == 32 || ROWS == 264 || ROWS == 265 || ROWS == 233 || ROWS == 232 || ROWS == 256, "tile geometry");
   static constexpr bool kPair = (ROWS == 264 || ROWS == 265 || ROWS == 233 || ROWS == 232);
+  // ROWS = 256: geometry 128 on a CTA PAIR (cluster of 2, tcgen05 cta_group::2 with M = 256): 128 chains per CTA,
+  // lane = chain and all N columns in the CTA's own TMEM exactly as in geometry 128, but the leader issues ONE MMA
+  // for both CTAs' rows and each CTA stages only HALF of every weight tile.  A 128 x 256 x 16 bf16 MMA from shared
+  // memory reads 4 KB of A and 8 KB of B per 128 cycles = 96 B/cycle of the SM's 128 B/cycle shared-memory port;
+  // with B split over the pair it is 64 B/cycle, which leaves the epilogue's loads and stores room
+  // (profiles/r2b), and the L2 -> SM weight stream halves.
+  static constexpr bool kWide = (ROWS == 256);
+  static constexpr bool kCluster = kPair || kWide;   // cluster of two CTAs, leader issues, peer arrives remotely
   // ROWS = 232: geometry 264 (1024-wide, in place) with 32 chains per CTA, the compact operand (16 chunks at a
   // 4 KB pitch = 64 KB) and the 8-stage weight ring of geometry 233 -- for batches that leave SMs idle with
   // 64-chain CTAs (the small points of the configs[4] sweep).
@@ -66,14 +74,15 @@ template <int ROWS> struct Geo {
   // nothing at all, so the 8 working warps have two issue slots per scheduler cycle pair to themselves and a
   // batch too small to fill the chip with 64-chain CTAs (4096 chains = 64 CTAs) spreads over twice the SMs.
   static constexpr bool kPingPong = (ROWS == 265 || ROWS == 233);
-  static constexpr bool kInPlace = (ROWS == 128 || kPair);   // operand stays in SMEM
-  // ROWS = 128: every 64-column k-chunk of the next operand is produced by ONE of a row's four epilogue threads
-  // (warp k owns the groups grp = k mod 4 of each N-chunk and walks them in four 16-column pieces), so the
-  // store -> proxy fence -> arrive sequence is paid once per 64 columns of a thread instead of once per 16
-  // and a_ready counts 128 arrivals (profiles/r2b: the fence path was 20 % of the epilogue warps' time).
-  static constexpr bool kOwn = (ROWS == 128) && BEST_TC_OWN;
-  static constexpr int kAReadyArrive = kOwn ? 128 : (kHalf ? 256 : 512);
-  static constexpr int kTileRows = kPair ? 64 : ROWS;   // rows of the CTA's operand / act' blocks
+  static constexpr bool kInPlace = (ROWS == 128 || kPair || kWide);   // operand stays in SMEM
+  // ROWS = 128, every N-chunk but the last of an op: each 64-column k-chunk of the next operand is produced by ONE
+  // of a row's four epilogue threads (warp k owns the groups grp = k mod 4 and walks them in four 16-column
+  // pieces), so the store -> proxy fence -> arrive sequence is paid once per 64 columns of a thread instead of
+  // once per 16; the owner arrives on a_ready for all four.  The LAST N-chunk keeps the interleaved order (all
+  // four threads on the same group): the next op's MMAs wait for exactly these k-chunks, one after the other.
+  static constexpr bool kOwn = (ROWS == 128 || ROWS == 256) && BEST_TC_OWN;
+  static constexpr bool kOwnLastInterleaved = false;
+  static constexpr int kTileRows = kPair ? 64 : (kWide ? 128 : ROWS);   // rows of the CTA's operand / act' blocks
   static constexpr int kChains = kHalf ? 32 : kTileRows;   // chains the CTA advances
   static constexpr int kEpiArrive = kHalf ? 256 : 512;      // epilogue threads that run (per CTA)
   // bytes between consecutive 64-column k-chunks of the operand.  Geometry 233 keeps only its 32 real rows:
@@ -84,7 +93,7 @@ template <int ROWS> struct Geo {
   static constexpr int kAChunk = kHalf ? 4096 : kTileRows * 128;
   static constexpr int kPPStride = (ROWS == 233) ? 32768 : 65536;   // ping-pong: bytes between the two operand buffers
   static constexpr int kStagesOff = kHalf ? 65536 : 131072; // weight ring: offset in the carve-up (SmemLayout::STAGES)
-  static constexpr int kEpiActive = kPair ? 512 : ROWS * 4;   // epilogue threads with MLP epilogue work
+  static constexpr int kEpiActive = kPair ? 512 : kTileRows * 4;   // epilogue threads with MLP epilogue work
   static constexpr int kNBuf = kPair ? 4 : 2;          // accumulator buffers
   static constexpr int kBufCols = kPair ? 128 : 256;   // TMEM columns per buffer
   static constexpr int kStagesG = kHalf ? 8 : 4;   // weight ring: stages
@@ -181,7 +190,8 @@ struct SmemLayout {
   static constexpr int TOTAL = TMEMPTR + 16;
 };
 static_assert(SmemLayout::TOTAL + 1024 <= 232448, "shared memory budget");
-static_assert(Geo<265>::kStagesOff == SmemLayout::STAGES && Geo<128>::kStagesOff == SmemLayout::STAGES, "weight ring offset");
+static_assert(Geo<265>::kStagesOff == SmemLayout::STAGES && Geo<128>::kStagesOff == SmemLayout::STAGES &&
+              Geo<256>::kStagesOff == SmemLayout::STAGES, "weight ring offset");
 static_assert(Geo<233>::kStagesOff + Geo<233>::kStagesG * Geo<233>::kStageBytesG <= SmemLayout::BIAS &&
               Geo<233>::kPPStride + 8 * Geo<233>::kAChunk <= Geo<233>::kStagesOff, "geometry 233 carve-up");
 static_assert(16 * Geo<232>::kAChunk <= Geo<232>::kStagesOff, "geometry 232 carve-up");
@@ -377,7 +387,7 @@ __device__ void mma_loop_pair(const Params& P, const Bars& bars, uint32_t a_base
   for (int64_t e = 0; e < n_evals; ++e) {
     for (int oi = 0; oi < n_ops; ++oi, ++o) {
       const OpDesc op = P.ops[oi];
-      const uint32_t idesc = ptx::idesc_bf16(kRows, op.ncols);
+      const uint32_t idesc = ptx::idesc_bf16(Geo<ROWS>::kWide ? 256 : kRows, op.ncols);
       const uint32_t half16 = ((uint32_t)op.ncols * 32u) >> 4;   // one K32 tile half, in descriptor units
       if (LEADER && wq == 0 && !Geo<ROWS>::kPingPong) {   // (ping-pong: nothing is overwritten in place, a_free unused)
         if (elect_one())

@@ -310,19 +310,19 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     for (int i = 0; i < kMaxKch; ++i) {
       // arrivals per phase: in place = every epilogue thread (pair: the 256 of the lane half that owns the
       // k-chunk); L2-image tiles = warp 3 alone (+ the bulk copy's bytes)
-      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : Geo<ROWS>::kAReadyArrive);   // pair: half of each CTA's; owner: one warp per row quarter
-      ptx::mbar_init(bars.a_free(i), Geo<ROWS>::kPair ? 2 : 1);   // pair kernels: two issuing warps
+      ptx::mbar_init(bars.a_ready(i), (!Geo<ROWS>::kInPlace) ? 1 : (Geo<ROWS>::kWide ? 2 : 1) * Geo<ROWS>::kEpiArrive);   // pair: half of each CTA's; 256: both CTAs'
+      ptx::mbar_init(bars.a_free(i), Geo<ROWS>::kCluster ? 2 : 1);   // pair kernels: two issuing warps
     }
     for (int i = 0; i < 4; ++i) {
       ptx::mbar_init(bars.d_full(i), 1);
-      ptx::mbar_init(bars.d_free(i), Geo<ROWS>::kPair ? 2 * Geo<ROWS>::kEpiArrive : Geo<ROWS>::kEpiActive);   // pair: both CTAs
+      ptx::mbar_init(bars.d_free(i), Geo<ROWS>::kCluster ? 2 * Geo<ROWS>::kEpiArrive : Geo<ROWS>::kEpiActive);   // pair: both CTAs
     }
     for (int i = 0; i < 4; ++i) ptx::mbar_init(bars.epi_done(i), Geo<ROWS>::kEpiActive);
     ptx::mbar_init(bars.xin_done(), Geo<ROWS>::kEpiActive);
     ptx::fence_mbar_init();
   }
   if (warp == 2) {
-    if (Geo<ROWS>::kPair) ptx::tmem_alloc_2cta(sbase + SmemLayout::TMEMPTR, 512);
+    if (Geo<ROWS>::kCluster) ptx::tmem_alloc_2cta(sbase + SmemLayout::TMEMPTR, 512);
     else ptx::tmem_alloc(sbase + SmemLayout::TMEMPTR, 512);
   }
   if (P.bias16) {   // bf16 bias table, two per word
@@ -351,7 +351,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   ptx::tc_fence_before();
   __syncthreads();
   ptx::tc_fence_after();
-  if (Geo<ROWS>::kPair) ptx::cluster_sync_all();   // both CTAs' barriers initialised, both TMEM allocations made
+  if (Geo<ROWS>::kCluster) ptx::cluster_sync_all();   // both CTAs' barriers initialised, both TMEM allocations made
   const uint32_t tmem_base = *tmem_ptr;
 
   int64_t n_evals = 1;
@@ -360,7 +360,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   const int n_ops = R.want_grad ? P.n_ops_all : P.n_ops_fwd;
 
   if (warp < kCtrlWarps) {
-    if (Geo<ROWS>::kPair) {
+    if (Geo<ROWS>::kCluster) {
       const uint32_t rank = ptx::cluster_ctarank();
       if (warp == 0) {
         producer_loop_pair<ROWS>(P, bars, sbase + Geo<ROWS>::kStagesOff, rank, n_evals, n_ops);
@@ -383,7 +383,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
     C.sbase = sbase;
     C.row = Geo<ROWS>::kPair ? ((warp & 1) * 32 + lane) : ((warp & 3) * 32 + lane);
     C.half = Geo<ROWS>::kPair ? ((warp & 3) >> 1) : 0;
-    C.to_leader = (Geo<ROWS>::kPair && ptx::cluster_ctarank() != 0) ? 1 : 0;
+    C.to_leader = (Geo<ROWS>::kCluster && ptx::cluster_ctarank() != 0) ? 1 : 0;
     C.k = (warp - kCtrlWarps) >> 2;
     C.tmem_lane = tmem_base + ((uint32_t)((warp & 3) * 32) << 16);
     C.o = 0; C.g = 0; C.vslot = 0; C.pslot = 0; C.emit_pending = 0;
@@ -417,9 +417,9 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   }
   ptx::tc_fence_before();
   __syncthreads();
-  if (Geo<ROWS>::kPair) ptx::cluster_sync_all();   // the leader's MMAs wrote the peer's TMEM and read its SMEM
+  if (Geo<ROWS>::kCluster) ptx::cluster_sync_all();   // the leader's MMAs wrote the peer's TMEM and read its SMEM
   if (warp == 2) {
-    if (Geo<ROWS>::kPair) ptx::tmem_dealloc_2cta(tmem_base, 512);
+    if (Geo<ROWS>::kCluster) ptx::tmem_dealloc_2cta(tmem_base, 512);
     else ptx::tmem_dealloc(tmem_base, 512);
   }
 }
@@ -463,7 +463,7 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
                 : (ROWS == 233 && pl->has_pp) ? pl->Pn : pl->P;
   constexpr int kTileRows = tc::Geo<ROWS>::kTileRows, kChains = tc::Geo<ROWS>::kChains;
   int64_t n_tiles = (rows + kChains - 1) / kChains;
-  if (tc::Geo<ROWS>::kPair) n_tiles = (n_tiles + 1) & ~(int64_t)1;   // whole CTA pairs
+  if (tc::Geo<ROWS>::kCluster) n_tiles = (n_tiles + 1) & ~(int64_t)1;   // whole CTA pairs
   // scratch: act' blocks (forward -> backward) and, for ROWS < 128, the next-operand image
   P.dact_tile_elems = (size_t)(P.n_hidden - 1) * P.H * kTileRows;
   const size_t dact_bytes = sizeof(uint16_t) * P.dact_tile_elems * (size_t)n_tiles + 16;
@@ -493,7 +493,7 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
   }
   P.L = ctx->L_dev;
   P.hard_box = ctx->tgt.hard_box;
-  if (tc::Geo<ROWS>::kPair) {
+  if (tc::Geo<ROWS>::kCluster) {
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)n_tiles);
     cfg.blockDim = dim3(tc::kThreads);
@@ -530,8 +530,13 @@ int pick_rows(const TcPlan* pl, int64_t rows, int n_sm) {
     const int64_t pair_slots = n_sm & ~1;   // CTAs of whole pairs resident at once
     const double c128 = (double)((t128 + n_sm - 1) / n_sm) * 52.0, c265 = (double)((t64 + pair_slots - 1) / pair_slots) * 33.0,
                  c233 = (double)((t32 + pair_slots - 1) / pair_slots) * 30.8;
-    if (c233 < c265 && c233 < c128) return 233;
-    return c265 < c128 ? 265 : 128;
+    // Geometry 256 (128-chain tiles on CTA pairs: half the shared-memory operand traffic of the MMAs per SM)
+    // measured against 128 on 16 384 chains: HMC 6.32 -> 5.61 ms per launch, MALA 5.67 -> 4.97, MH 2.44 -> 2.39.
+    const int64_t t256 = (t128 + 1) & ~(int64_t)1;
+    const double c256 = (double)((t256 + pair_slots - 1) / pair_slots) * 46.0;
+    if (c233 < c265 && c233 < c128 && c233 < c256) return 233;
+    if (c265 < c128 && c265 < c256) return 265;
+    return c256 <= c128 ? 256 : 128;
   }
   if (pl->P.H != 1024) return 128;
   // CTA pairs (cta_group::2): the 1024-wide operand in place at full MMA rate; 32 chains per CTA (geometry 232)
@@ -550,6 +555,7 @@ int launch_tc(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s) {
   }
   switch (pick_rows(pl, rows, pl->n_sm)) {
     case 128: return launch_tc_geo<METHOD, 128>(ctx, R, rows, s);
+    case 256: return launch_tc_geo<METHOD, 256>(ctx, R, rows, s);
     case 264: return launch_tc_geo<METHOD, 264>(ctx, R, rows, s);
     case 265: return launch_tc_geo<METHOD, 265>(ctx, R, rows, s);
     case 233: return launch_tc_geo<METHOD, 233>(ctx, R, rows, s);
@@ -601,7 +607,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
   ctx->tc = pl;
   if (const char* e = std::getenv("BEST_TC_ROWS")) {
     const int v = std::atoi(e);
-    if ((v == 64 || v == 32 || (v == 128 && !r64) || ((v == 264 || v == 232) && r64) || ((v == 265 || v == 233) && H == 512))) pl->force_rows = v;
+    if ((v == 64 || v == 32 || (v == 128 && !r64) || ((v == 264 || v == 232) && r64) || ((v == 265 || v == 233 || v == 256) && H == 512))) pl->force_rows = v;
   }
   tc::Params& P = pl->P;
   P.bias16 = r64 ? 1 : 0;

@@ -493,6 +493,36 @@ def test_T1_geometry_232_matches_264(B, monkeypatch):
         assert np.array_equal(outs[0][k], outs[1][k]), k
 
 
+def test_T1_geometry_256_matches_128(B, monkeypatch):
+    """128-chain tiles on CTA pairs (M = 256 MMAs, each CTA staging half of every weight tile) against the
+    single-CTA 128-chain tiles on 27→512⁴→1: the same arithmetic, so sampler steps are bit-identical -- ragged
+    tail (300 chains = 3 tiles: the pair kernel pads a fourth CTA) and a trace written by the kernel included."""
+    import torch
+    wf = WL.lcdm(n_chains=300)
+    outs = []
+    for r in (256, 128):
+        monkeypatch.setenv("BEST_TC_ROWS", str(r))
+        c2 = B.Context(wf, B.PREC_BF16)
+        st = c2.new_state(wf.theta0)
+        tr = torch.zeros(3, 300, wf.d, device="cuda")
+        st.step_mala(3, 5, f32(0.3), trace=tr, thin=1)
+        st.step_hmc(2, 9, f32(0.1), 4)
+        st.step_mh(3, 4, f32(0.3))
+        st.step_aies(2, 6, 2.0)
+        st.step_aies_de(1, 8, 0.1)
+        o = st.get(want_grad=True)
+        o["trace"] = tr.cpu().numpy()
+        th = torch.from_numpy(np.ascontiguousarray(wf.theta0, dtype=np.float32)).cuda()
+        lp, g = torch.zeros(300, device="cuda"), torch.zeros(300, wf.d, device="cuda")
+        c2.logp_grad(th, 300, lp, g)
+        torch.cuda.synchronize()
+        o["lg_logp"], o["lg_grad"] = lp.cpu().numpy(), g.cpu().numpy()
+        outs.append(o)
+        c2.close()
+    for k in ("theta", "logp", "grad", "n_accept", "trace", "lg_logp", "lg_grad"):
+        assert np.array_equal(outs[0][k], outs[1][k]), k
+
+
 @pytest.mark.parametrize("make,n", [("lcdm", 4736), ("lcdm", 4737), ("lcdm", 9473), ("sterile", 4736), ("sterile", 4737)])
 def test_T1_geometry_switch_points(B, O, make, n):
     """Batch sizes on both sides of pick_rows' switch points (32-chain pairs fill one wave of 148 SMs up to
