@@ -81,7 +81,7 @@ template <int ROWS> struct Geo {
   // once per 16; the owner arrives on a_ready for all four.  The LAST N-chunk keeps the interleaved order (all
   // four threads on the same group): the next op's MMAs wait for exactly these k-chunks, one after the other.
   static constexpr bool kOwn = (ROWS == 128 || ROWS == 256) && BEST_TC_OWN;
-  static constexpr bool kOwnLastInterleaved = false;
+  static constexpr bool kOwnLastInterleaved = true;
   static constexpr int kTileRows = kPair ? 64 : (kWide ? 128 : ROWS);   // rows of the CTA's operand / act' blocks
   static constexpr int kChains = kHalf ? 32 : kTileRows;   // chains the CTA advances
   static constexpr int kEpiArrive = kHalf ? 256 : 512;      // epilogue threads that run (per CTA)
