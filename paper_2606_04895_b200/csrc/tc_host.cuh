@@ -291,7 +291,10 @@ __global__ void __launch_bounds__(kThreads, 1)
 best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int tid = threadIdx.x, lane = tid & 31;
+  // the warp index through a shuffle: the compiler then knows the role branches are warp-uniform and keeps the MMA
+  // issuer's descriptors, counters and barrier addresses in uniform registers
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
   const uint32_t sbase = ptx::smem_u32(smem);
   const Bars bars = make_bars(sbase + SmemLayout::BARS);
   float* bias_s = reinterpret_cast<float*>(smem + SmemLayout::BIAS);
