@@ -99,26 +99,27 @@ __device__ __forceinline__ void store_piece(const EpiCtx& C, int jn, int p, cons
 __device__ __forceinline__ void qbar(const EpiCtx& C) { ptx::named_bar_sync(1 + (C.row >> 5), 128); }
 
 // The forward weights and biases of every SiLU hidden layer are packed pre-scaled by 1/2 (exact in
-// bf16), so the accumulator holds a/2 and
-//   t = tanh(a/2):  sigma(a) = (1+t)/2,  h = a sigma = (a/2)(1+t),  h' = sigma + h (1 - sigma)
-// costs one MUFU and four FFMA2 per element pair.  tanh.approx has ~2^-11 relative error, below
-// the 2^-9 of the bf16 rounding that follows.
+// bf16), so the accumulator holds a/2 and, with t = tanh(a/2),
+//   sigma(a) = (1+t)/2,  h = a sigma = (a/2)(1+t),  h' = sigma + h (1 - sigma)  =>  e := 2 h' - 1 = t + h (1 - t)
+// costs one MUFU and three FFMA2 per element pair.  The scratch holds e (bf16), not h': the backward weights are
+// packed pre-scaled by 1/2 as well (exact), so the backward accumulator is v = (delta W)/2 and
+// delta_prev = (delta W) h' = v (e + 1) = fma(v, e, v) -- one instruction, as the plain product was.
+// tanh.approx has ~2^-11 relative error, below the 2^-9 of the bf16 rounding that follows.
 constexpr bool kSiluHalfPrescale = true;
 
-__device__ __forceinline__ void silu_pair(f32x2 a, f32x2& h, f32x2& dact) {
+__device__ __forceinline__ void silu_pair(f32x2 a, f32x2& h, f32x2& e) {
   float x0, x1;
   ptx::unpack2(a, x0, x1);   // a holds (pre-activation)/2
   const f32x2 t = ptx::pack2(ptx::tanh_approx(x0), ptx::tanh_approx(x1));
   h = ptx::fma2(a, t, a);
-  const f32x2 sg = ptx::fma2(t, ptx::pack2(0.5f, 0.5f), ptx::pack2(0.5f, 0.5f));
-  const f32x2 om = ptx::fma2(t, ptx::pack2(-0.5f, -0.5f), ptx::pack2(0.5f, 0.5f));
-  dact = ptx::fma2(h, om, sg);
+  const f32x2 om = ptx::fma2(t, ptx::pack2(-1.0f, -1.0f), ptx::pack2(1.0f, 1.0f));
+  e = ptx::fma2(h, om, t);
 }
-__device__ __forceinline__ void tanh_pair(f32x2 a, f32x2& h, f32x2& dact) {
+__device__ __forceinline__ void tanh_pair(f32x2 a, f32x2& h, f32x2& e) {   // h' = 1 - h^2, e = 2 h' - 1 = 1 - 2 h^2
   float x0, x1;
   ptx::unpack2(a, x0, x1);
   h = ptx::pack2(ptx::tanh_approx(x0), ptx::tanh_approx(x1));
-  dact = ptx::fma2(ptx::mul2(h, h), ptx::pack2(-1.0f, -1.0f), ptx::pack2(1.0f, 1.0f));
+  e = ptx::fma2(ptx::mul2(h, h), ptx::pack2(-2.0f, -2.0f), ptx::pack2(1.0f, 1.0f));
 }
 
 // ---- first A operand: theta split into bf16 hi | lo (own 8 dims -> pieces k and 4+k) ------------
@@ -176,9 +177,9 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, in
     const f32x2 a = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), b[i]);
     f32x2 h, dd;
     if (ACT == BEST_ACT_SILU) silu_pair(a, h, dd); else tanh_pair(a, h, dd);
-    if (LAST) {
+    if (LAST) {   // ws = (s w_out)/2: the output dot product is doubled once at the end, delta = h' s w_out = (e + 1) ws
       acc2 = ptx::fma2(h, ws[i], acc2);
-      if (want_grad) hp[i] = ptx::pack_bf16x2_from(ptx::mul2(dd, ws[i]));
+      if (want_grad) hp[i] = ptx::pack_bf16x2_from(ptx::fma2(dd, ws[i], ws[i]));
     } else {
       hp[i] = ptx::pack_bf16x2_from(h);
       dp[i] = ptx::pack_bf16x2_from(dd);
@@ -295,7 +296,8 @@ __device__ __forceinline__ void bwd_group(const uint32_t (&v)[16], const uint4& 
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
     const f32x2 dd = ptx::pack2u(dw[i] << 16, dw[i] & 0xFFFF0000u);
-    hp[i] = ptx::pack_bf16x2_from(ptx::mul2(ptx::pack2u(v[2 * i], v[2 * i + 1]), dd));
+    const f32x2 vv = ptx::pack2u(v[2 * i], v[2 * i + 1]);   // (delta W)/2; dd holds e = 2 act' - 1
+    hp[i] = ptx::pack_bf16x2_from(ptx::fma2(vv, dd, vv));
   }
 }
 template <int ROWS>
@@ -485,7 +487,7 @@ __device__ __forceinline__ void tc_eval(EpiCtx& C, const float (&th)[8], bool wa
   }
   float a0, a1;
   ptx::unpack2(acc2, a0, a1);
-  out_part = a0 + a1;
+  out_part = 2.0f * (a0 + a1);   // (the table holds (s w_out)/2)
   if (Geo<ROWS>::kPair) {   // the output dot product is split over both lane halves
     const uint32_t PX = C.sbase + SmemLayout::PART + 1024u + (uint32_t)C.row * 16u + (uint32_t)C.k * 4u;
     if (C.half == 1) ptx::sts_32(PX, out_part);

@@ -334,7 +334,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   } else {
     for (int i = tid; i < P.n_hidden * P.H; i += kThreads) bias_s[i] = P.bias[i];
   }
-  for (int i = tid; i < P.H; i += kThreads) wouts_s[i] = P.mlp_scale * P.w_out[i];
+  for (int i = tid; i < P.H; i += kThreads) wouts_s[i] = 0.5f * (P.mlp_scale * P.w_out[i]);   // see fwd_group (LAST)
   for (int i = tid; i < kDP * kDP; i += kThreads) {
     const int r = i / kDP, c = i % kDP;
     const float l = (r < P.d && c <= r) ? (float)P.L[r * P.d + c] : 0.0f;
@@ -652,7 +652,7 @@ int tc_plan_create(best_ctx* ctx, const best_config* cfg) {
         if (op.layer == 0) { const int kk = k & 31; return kk < d ? fs * W[0][(size_t)n * d + kk] : 0.0f; }
         return fs * W[op.layer][(size_t)n * H + k];
       }
-      if (op.epi == tc::EPI_BWD_HID) return W[op.layer + 1][(size_t)k * H + n];  // (W_l)^T, l = layer+1
+      if (op.epi == tc::EPI_BWD_HID) return 0.5f * W[op.layer + 1][(size_t)k * H + n];  // (W_l)^T / 2, l = layer+1 (silu_pair)
       return n < d ? W[0][(size_t)k * d + n] : 0.0f;                             // (W_0)^T
     };
     // consumption order of the K32 tiles: N-chunk outer, or (paired ops) two N-chunks at a time with the
