@@ -29,10 +29,12 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures of THIS round's code (profiles/r2_ncu_full.md); None where no capture exists.
-NCU_TRAFFIC_BYTES = {("hmc", "bf16"): 10.993152e6 + 125.417216e6,          # best_tc_kernel<2,128>, 8 trajectories per launch
-                     ("lcdm_mala", "bf16"): 5.245440e6 + 0.445696e6}         # best_tc_kernel<1,233>, 100 steps per launch
-NCU_TRAFFIC_SOURCE = "profiles/r2_ncu_full.md"
+# `ncu --set full` captures of THIS round's code (profiles/r2b_ncu_full.md); None where no capture exists.
+NCU_TRAFFIC_BYTES = {("hmc", "bf16"): 10.766080e6 + 89.711872e6,           # best_tc_kernel<2,256>, 8 trajectories per launch
+                     ("lcdm_mala_16k", "bf16"): 11.711232e6 + 829.322496e6,  # best_tc_kernel<1,256>, 100 steps per launch
+                     ("lcdm_mh_16k", "bf16"): 5.559552e6 + 0.0,              # best_tc_kernel<0,256>, 100 steps per launch
+                     ("lcdm_mala", "bf16"): 5.240832e6 + 0.181760e6}         # best_tc_kernel<1,233>, 100 steps per launch
+NCU_TRAFFIC_SOURCE = "profiles/r2b_ncu_full.md"
 
 # PAPER.md Table 1 (L211-219), best published figure per sampler: sampler steps/s at 20 (1000) chains on a Tesla
 # V100 with XLA JIT -- another machine, an emulator of unstated size: context, not a target
