@@ -157,6 +157,25 @@ __device__ __forceinline__ void write_xin(EpiCtx& C, const float (&th)[8]) {
 // measured 10 % SLOWER); the a_free wait is skipped in the last N-chunk (its d_full commit is
 // ordered after every a_free commit of the op).
 
+// the register arithmetic of 16 columns: hp = next operand (bf16 pairs), dp = e = 2 act' - 1 (hidden layers)
+template <int ACT, bool LAST>
+__device__ __forceinline__ void fwd_math(const uint32_t (&v)[16], const f32x2 (&b)[8], const f32x2 (&ws)[8], bool want_grad,
+                                         f32x2& acc2, uint32_t (&hp)[8], uint32_t (&dp)[8]) {
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const f32x2 a = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), b[i]);
+    f32x2 h, dd;
+    if (ACT == BEST_ACT_SILU) silu_pair(a, h, dd); else tanh_pair(a, h, dd);
+    if (LAST) {   // ws = (s w_out)/2: the output dot product is doubled once at the end, delta = h' s w_out = (e + 1) ws
+      acc2 = ptx::fma2(h, ws[i], acc2);
+      if (want_grad) hp[i] = ptx::pack_bf16x2_from(ptx::fma2(dd, ws[i], ws[i]));
+    } else {
+      hp[i] = ptx::pack_bf16x2_from(h);
+      dp[i] = ptx::pack_bf16x2_from(dd);
+    }
+  }
+}
+
 // bias + activation (+ act' to scratch, or delta for the last layer) of one group, in registers
 template <int ACT, bool LAST, int ROWS>
 __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, int colofs, const uint32_t (&v)[16],
@@ -172,19 +191,7 @@ __device__ __forceinline__ void fwd_group(const EpiCtx& C, int layer, int jn, in
     for (int i = 0; i < 4; ++i) ptx::lds_c2x64(C.wouts_thr + jn * 256 + colofs * 4 + i * 16, ws[2 * i], ws[2 * i + 1]);
   }
   uint32_t dp[8];
-#pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const f32x2 a = ptx::add2(ptx::pack2u(v[2 * i], v[2 * i + 1]), b[i]);
-    f32x2 h, dd;
-    if (ACT == BEST_ACT_SILU) silu_pair(a, h, dd); else tanh_pair(a, h, dd);
-    if (LAST) {   // ws = (s w_out)/2: the output dot product is doubled once at the end, delta = h' s w_out = (e + 1) ws
-      acc2 = ptx::fma2(h, ws[i], acc2);
-      if (want_grad) hp[i] = ptx::pack_bf16x2_from(ptx::fma2(dd, ws[i], ws[i]));
-    } else {
-      hp[i] = ptx::pack_bf16x2_from(h);
-      dp[i] = ptx::pack_bf16x2_from(dd);
-    }
-  }
+  fwd_math<ACT, LAST>(v, b, ws, want_grad, acc2, hp, dp);
   if (!LAST && want_grad) {
     uint8_t* dptr = dact_l + (size_t)jn * kDBlk + (size_t)(colofs >> 3) * kDPiece;
     ptx::stg_128(dptr, dp[0], dp[1], dp[2], dp[3]);
@@ -229,15 +236,33 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
       if (!Geo<ROWS>::kOwnLastInterleaved || c != op.nch - 1 || !writes_a) {   // owner order
         for (int grp = C.k; grp < ngrp; grp += 4) {
           const int jn = c * ngrp + grp;
+          // per-group bases once, the four pieces address with immediates (the owner geometries keep the fp32 bias table)
+          constexpr uint32_t kDBlk = Geo<ROWS>::kTileRows * 128, kDPiece = Geo<ROWS>::kTileRows * 16;
+          const uint32_t bias_a = C.bias_thr + (uint32_t)(op.layer * C.P->H + jn * 64) * 4u;
+          const uint32_t ws_a = C.wouts_thr + (uint32_t)jn * 256u;
+          const uint32_t sts_a = C.a_thr0 + (uint32_t)jn * Geo<ROWS>::kAChunk, x7 = C.a_thr1 << 4;
+          uint8_t* dact_a = dact_l + (size_t)jn * kDBlk;
 #pragma unroll
           for (int p = 0; p < 4; ++p) {
-            uint32_t v[16], hp[8];
+            uint32_t v[16], hp[8], dp[8];
             ptx::tmem_ld16(tbase + grp * 64 + p * 16, v);
+            f32x2 b[8], ws[8];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) ptx::lds_c2x64(bias_a + p * 64 + i * 16, b[2 * i], b[2 * i + 1]);
+            if (LAST) {
+#pragma unroll
+              for (int i = 0; i < 4; ++i) ptx::lds_c2x64(ws_a + p * 64 + i * 16, ws[2 * i], ws[2 * i + 1]);
+            }
             ptx::tmem_ld_wait();
-            fwd_group<ACT, LAST, ROWS>(C, op.layer, jn, 16 * p, v, want_grad, dact_l, acc2, hp);
+            fwd_math<ACT, LAST>(v, b, ws, want_grad, acc2, hp, dp);
+            if (!LAST && want_grad) {
+              ptx::stg_128(dact_a + (2 * p) * kDPiece, dp[0], dp[1], dp[2], dp[3]);
+              ptx::stg_128(dact_a + (2 * p + 1) * kDPiece, dp[4], dp[5], dp[6], dp[7]);
+            }
             if (writes_a) {
               if (gate && p == 0) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
-              store_piece<ROWS>(C, jn, p, hp);
+              ptx::sts_128(sts_a + ((uint32_t)(32 * p) ^ x7), hp[0], hp[1], hp[2], hp[3]);
+              ptx::sts_128(sts_a + ((uint32_t)(32 * p + 16) ^ x7), hp[4], hp[5], hp[6], hp[7]);
             }
           }
           if (writes_a) {
