@@ -271,17 +271,37 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
           }
         }
       } else {   // last N-chunk: the next op's MMAs consume k-chunk after k-chunk as they are published
+        // (per-chunk bases once, immediates per group; requesting the NEXT group's accumulator columns before this
+        // group's arithmetic needs a second 16-register array: 4.7 KB of spills, not kept)
+        constexpr uint32_t kDBlk = Geo<ROWS>::kTileRows * 128, kDPiece = Geo<ROWS>::kTileRows * 16;
+        const int jn0 = c * ngrp;
+        const uint32_t bias_a = C.bias_thr + (uint32_t)(op.layer * C.P->H + jn0 * 64 + 16 * C.k) * 4u;
+        const uint32_t ws_a = C.wouts_thr + (uint32_t)jn0 * 256u + (uint32_t)C.k * 64u;
+        const uint32_t x7 = C.a_thr1 << 4, a0 = C.a_thr0 + (uint32_t)jn0 * Geo<ROWS>::kAChunk;
+        const uint32_t sts0 = a0 + ((uint32_t)(32 * C.k) ^ x7), sts1 = a0 + ((uint32_t)(32 * C.k + 16) ^ x7);
+        uint8_t* dact_a = dact_l + (size_t)jn0 * kDBlk + (size_t)(2 * C.k) * kDPiece;
 #pragma unroll
         for (int g0 = 0; g0 < 4; ++g0) {
           if (g0 < ngrp) {
-            const int jn = c * ngrp + g0;
-            uint32_t v[16], hp[8];
+            uint32_t v[16], hp[8], dp[8];
+            f32x2 b[8], ws[8];
             ptx::tmem_ld16(tbase + g0 * 64 + C.k * 16, v);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) ptx::lds_c2x64(bias_a + g0 * 256 + i * 16, b[2 * i], b[2 * i + 1]);
+            if (LAST) {
+#pragma unroll
+              for (int i = 0; i < 4; ++i) ptx::lds_c2x64(ws_a + g0 * 256 + i * 16, ws[2 * i], ws[2 * i + 1]);
+            }
             ptx::tmem_ld_wait();
-            fwd_group<ACT, LAST, ROWS>(C, op.layer, jn, 16 * C.k, v, want_grad, dact_l, acc2, hp);
-            store_piece<ROWS>(C, jn, C.k, hp);
+            fwd_math<ACT, LAST>(v, b, ws, want_grad, acc2, hp, dp);
+            if (!LAST && want_grad) {
+              ptx::stg_128(dact_a + (size_t)g0 * kDBlk, dp[0], dp[1], dp[2], dp[3]);
+              ptx::stg_128(dact_a + (size_t)g0 * kDBlk + kDPiece, dp[4], dp[5], dp[6], dp[7]);
+            }
+            ptx::sts_128(sts0 + g0 * Geo<ROWS>::kAChunk, hp[0], hp[1], hp[2], hp[3]);
+            ptx::sts_128(sts1 + g0 * Geo<ROWS>::kAChunk, hp[4], hp[5], hp[6], hp[7]);
             ptx::fence_proxy_async();
-            arrive_mma(C, C.bars.a_ready(jn));
+            arrive_mma(C, C.bars.a_ready(jn0 + g0));
           }
         }
       }
