@@ -510,7 +510,11 @@ def test_T1_geometry_256_matches_128(B, monkeypatch):
         st.step_mh(3, 4, f32(0.3))
         st.step_aies(2, 6, 2.0)
         st.step_aies_de(1, 8, 0.1)
+        st.set_adaptation(20, 1e-6)                      # A9 window rows written by the pair kernel: two windows
+        st.step_mala(40, 11, f32(0.2))
+        st.set_adaptation(0, 1e-6)
         o = st.get(want_grad=True)
+        o["L"] = c2.get_whitening()
         o["trace"] = tr.cpu().numpy()
         th = torch.from_numpy(np.ascontiguousarray(wf.theta0, dtype=np.float32)).cuda()
         lp, g = torch.zeros(300, device="cuda"), torch.zeros(300, wf.d, device="cuda")
@@ -519,8 +523,9 @@ def test_T1_geometry_256_matches_128(B, monkeypatch):
         o["lg_logp"], o["lg_grad"] = lp.cpu().numpy(), g.cpu().numpy()
         outs.append(o)
         c2.close()
-    for k in ("theta", "logp", "grad", "n_accept", "trace", "lg_logp", "lg_grad"):
+    for k in ("theta", "logp", "grad", "n_accept", "trace", "lg_logp", "lg_grad", "L"):
         assert np.array_equal(outs[0][k], outs[1][k]), k
+    assert not np.array_equal(outs[0]["L"], np.asarray(wf.L))     # (the windows did replace the factor)
 
 
 @pytest.mark.parametrize("make,n", [("lcdm", 4736), ("lcdm", 4737), ("lcdm", 9473), ("sterile", 4736), ("sterile", 4737)])
