@@ -30,7 +30,7 @@ sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures of THIS round's code (profiles/r2b_ncu_full.md); None where no capture exists.
-NCU_TRAFFIC_BYTES = {("hmc", "bf16"): 10.766080e6 + 89.711872e6,           # best_tc_kernel<2,256>, 8 trajectories per launch
+NCU_TRAFFIC_BYTES = {("hmc", "bf16"): 10.995712e6 + 121.568768e6,          # best_tc_kernel<2,256>, 8 trajectories per launch
                      ("lcdm_mala_16k", "bf16"): 11.711232e6 + 829.322496e6,  # best_tc_kernel<1,256>, 100 steps per launch
                      ("lcdm_mh_16k", "bf16"): 5.559552e6 + 0.0,              # best_tc_kernel<0,256>, 100 steps per launch
                      ("lcdm_mala", "bf16"): 5.240832e6 + 0.181760e6}         # best_tc_kernel<1,233>, 100 steps per launch
