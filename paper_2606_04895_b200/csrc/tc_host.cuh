@@ -178,13 +178,21 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
 
   if (METHOD == M_MALA) {
     const float sq = sqrtf(2.0f * eps);
+    // The whitened gradient L^T g of the current state stays in registers across the steps: the proposal's
+    // L^T g' is needed for the Hastings ratio anyway and becomes it on acceptance (the same fp32 values the
+    // matvec would reproduce from the stored gradient, so a call split into several gives the same bits).
+    float gz[8];
+    {
+      float g[8];
+      load_vec8(C, R.grad, R.ld, c, d, valid, g);
+      mv_Lt(C, g, gz);
+    }
     for (int64_t t = 0; t < R.n_steps; ++t) {
       const uint64_t step = R.step0 + (uint64_t)t;
-      float thp[8], dz[8], gp[8], lpp, fwd = 0.0f;
+      float thp[8], dz[8], gp[8], gzp[8], lpp, fwd = 0.0f;
       {
-        float g[8], gz[8], xi[8];
-        load_vec8(C, R.grad, R.ld, c, d, valid, g);
-        mv_Lt(C, g, gz);
+        float g[8], xi[8], th[8];
+        load_vec8(C, R.theta, R.ld, c, d, valid, th);   // (requested before the normals are drawn)
         draw_normals8(C, R.seed, cid, step, d, xi);
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
@@ -193,21 +201,16 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
           dz[i] = fmaf(eps, gz[i], f);
         }
         mv_L(C, dz, g);  // g <- L dz
-        float th[8];
-        load_vec8(C, R.theta, R.ld, c, d, valid, th);
 #pragma unroll
         for (int i = 0; i < 8; ++i) thp[i] = th[i] + g[i];
       }
       eval_target<ROWS>(C, thp, true, lpp, gp);
       float diff = fwd;
-      {
-        float gzp[8];
-        mv_Lt(C, gp, gzp);
+      mv_Lt(C, gp, gzp);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-          const float r = fmaf(eps, gzp[i], dz[i]);
-          diff = fmaf(-r, r, diff);
-        }
+      for (int i = 0; i < 8; ++i) {
+        const float r = fmaf(eps, gzp[i], dz[i]);
+        diff = fmaf(-r, r, diff);
       }
       const float la = lpp - lp + reduce4(C, diff) / (4.0f * eps);
       la_last = la;
@@ -218,6 +221,8 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
         store_vec8(C, R.grad, R.ld, c, d, gp);
         lp = lpp;
         ++nacc;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) gz[i] = gzp[i];
       }
       if (rows_out) {
         if (valid && !acc) load_vec8(C, R.theta, R.ld, c, d, valid, thp);
