@@ -5,6 +5,8 @@
 //   * sampler algebra: the thread owns parameter dimensions [8k, 8k+8) of its chain; the four
 //     threads of a chain (same lane, four different warps of one TMEM lane quarter) exchange
 //     matvec inputs and partial sums through SMEM with a 128-thread named barrier.
+//   * geometries 128 / 256 (Geo::kOwn): in every N-chunk but the last of an op warp k instead OWNS the
+//     64-column groups grp = k (mod 4) and walks them in four 16-column pieces (one publish per 64 columns).
 // The r1a profile (profiles/r1a_hmc_ncu_full.md) showed these warps to be ISSUE-bound (62.6 k
 // issue cycles per evaluation against 50.7 k MMA cycles), so everything here is written for
 // instruction count: 32-bit shared-space addresses, packed f32x2 math, one MUFU per element,

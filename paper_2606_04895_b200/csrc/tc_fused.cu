@@ -11,6 +11,8 @@
 //                    tcgen05.ld epilogues (bias + activation + act' / delta) on 16 of every 64
 //                    columns each, and cooperatively Philox, whitened proposal, Gaussian / banana /
 //                    box terms and the accept decision on 8 parameter dimensions each.
+// ROWS = 256 (the default for 512-wide layers at >= 9.5 k chains) runs the same tile on a CTA PAIR: cta_group::2
+// MMAs with M = 256, each CTA staging half of every weight tile (Geo<256>).
 // The MLP forward and its input-gradient backprop (A1b, A1c) are a chain of GEMMs whose
 // activations never leave the SM; only act' (bf16) is parked in an L2-resident scratch between
 // the forward and backward sweeps.  See DESIGN.md §"tensor-core kernel".
@@ -23,10 +25,6 @@
 #include "device_math.cuh"
 #include "tc_fused.h"
 #include "tc_ptx.cuh"
-
-#ifndef BEST_TC_OWN
-#define BEST_TC_OWN 1
-#endif
 
 namespace best {
 
@@ -75,12 +73,12 @@ template <int ROWS> struct Geo {
   // batch too small to fill the chip with 64-chain CTAs (4096 chains = 64 CTAs) spreads over twice the SMs.
   static constexpr bool kPingPong = (ROWS == 265 || ROWS == 233);
   static constexpr bool kInPlace = (ROWS == 128 || kPair || kWide);   // operand stays in SMEM
-  // ROWS = 128, every N-chunk but the last of an op: each 64-column k-chunk of the next operand is produced by ONE
+  // ROWS = 128 / 256, every N-chunk but the last of an op: each 64-column k-chunk of the next operand is produced by ONE
   // of a row's four epilogue threads (warp k owns the groups grp = k mod 4 and walks them in four 16-column
   // pieces), so the store -> proxy fence -> arrive sequence is paid once per 64 columns of a thread instead of
   // once per 16; the owner arrives on a_ready for all four.  The LAST N-chunk keeps the interleaved order (all
   // four threads on the same group): the next op's MMAs wait for exactly these k-chunks, one after the other.
-  static constexpr bool kOwn = (ROWS == 128 || ROWS == 256) && BEST_TC_OWN;
+  static constexpr bool kOwn = (ROWS == 128 || ROWS == 256);
   static constexpr bool kOwnLastInterleaved = true;
   static constexpr int kTileRows = kPair ? 64 : (kWide ? 128 : ROWS);   // rows of the CTA's operand / act' blocks
   static constexpr int kChains = kHalf ? 32 : kTileRows;   // chains the CTA advances
