@@ -378,43 +378,53 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
       ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
       ptx::tc_fence_after();
       const uint32_t tbase = C.tmem_lane + buf * Geo<ROWS>::kBufCols;
+      const uint32_t x7 = C.a_thr1 << 4;
       if (!Geo<ROWS>::kOwnLastInterleaved || c != last) {   // owner order
         const int jn = c * ngrp + C.k;
         if (C.k < ngrp) {
+          // bases once per group, immediates per piece (as in epi_fwd)
+          const uint8_t* dact_a = dact_l + (size_t)jn * kDBlk;
+          const uint8_t* dact_n = (c + 1 < op.nch) ? piece_ptr(c + 1, 0) : dact_a;   // first piece of the next N-chunk
+          const uint32_t sts_a = C.a_thr0 + (uint32_t)jn * Geo<ROWS>::kAChunk;
 #pragma unroll
           for (int p = 0; p < 4; ++p) {
             uint32_t v[16], hp[8];
             ptx::tmem_ld16(tbase + C.k * 64 + p * 16, v);
             const uint4 d0 = a0, d1 = a1;
-            if (p < 3 || c + 1 < op.nch) {
-              const uint8_t* dn = (p < 3) ? piece_ptr(c, p + 1) : piece_ptr(c + 1, 0);
-              a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
+            if (p < 3) {
+              a0 = ptx::ldg_128(dact_a + (2 * p + 2) * kDPiece); a1 = ptx::ldg_128(dact_a + (2 * p + 3) * kDPiece);
+            } else if (c + 1 < op.nch) {
+              a0 = ptx::ldg_128(dact_n); a1 = ptx::ldg_128(dact_n + kDPiece);
             }
             ptx::tmem_ld_wait();
             bwd_group<ROWS>(v, d0, d1, hp);
             if (p == 0) ptx::mbar_wait(C.bars.a_free(jn), C.o & 1u);
-            store_piece<ROWS>(C, jn, p, hp);
+            ptx::sts_128(sts_a + ((uint32_t)(32 * p) ^ x7), hp[0], hp[1], hp[2], hp[3]);
+            ptx::sts_128(sts_a + ((uint32_t)(32 * p + 16) ^ x7), hp[4], hp[5], hp[6], hp[7]);
           }
           ptx::fence_proxy_async();
           arrive_mma4(C, C.bars.a_ready(jn));
         }
       } else {
+        const int jn0 = c * ngrp;
+        const uint8_t* dact_a = dact_l + (size_t)jn0 * kDBlk + (size_t)(2 * C.k) * kDPiece;   // + g0 * kDBlk
+        const uint32_t a0s = C.a_thr0 + (uint32_t)jn0 * Geo<ROWS>::kAChunk;
+        const uint32_t sts0 = a0s + ((uint32_t)(32 * C.k) ^ x7), sts1 = a0s + ((uint32_t)(32 * C.k + 16) ^ x7);
 #pragma unroll
         for (int g0 = 0; g0 < 4; ++g0) {
           if (g0 < ngrp) {
-            const int jn = c * ngrp + g0;
             uint32_t v[16], hp[8];
             ptx::tmem_ld16(tbase + g0 * 64 + C.k * 16, v);
             const uint4 d0 = a0, d1 = a1;
             if (g0 + 1 < ngrp) {
-              const uint8_t* dn = piece_ptr(c, g0 + 1);
-              a0 = ptx::ldg_128(dn); a1 = ptx::ldg_128(dn + kDPiece);
+              a0 = ptx::ldg_128(dact_a + (size_t)(g0 + 1) * kDBlk); a1 = ptx::ldg_128(dact_a + (size_t)(g0 + 1) * kDBlk + kDPiece);
             }
             ptx::tmem_ld_wait();
             bwd_group<ROWS>(v, d0, d1, hp);
-            store_piece<ROWS>(C, jn, C.k, hp);
+            ptx::sts_128(sts0 + g0 * Geo<ROWS>::kAChunk, hp[0], hp[1], hp[2], hp[3]);
+            ptx::sts_128(sts1 + g0 * Geo<ROWS>::kAChunk, hp[4], hp[5], hp[6], hp[7]);
             ptx::fence_proxy_async();
-            arrive_mma(C, C.bars.a_ready(jn));
+            arrive_mma(C, C.bars.a_ready(jn0 + g0));
           }
         }
       }
