@@ -167,6 +167,9 @@ struct Run {
   float* trace; int thin; int64_t t_call0;
   float* win;
   int64_t B_rows;       // chains per trace / window slot (= the state's chain count)
+  // EVAL only: tiles of the whole call.  The grid holds at most one wave of CTAs (pairs); CTA b evaluates tiles
+  // b, b + gridDim.x, ... in one launch, so prologue, TMEM allocation and launch are paid once per CTA, not per tile
+  int64_t n_tiles;
 };
 
 // shared-memory carve-up (dynamic, 1024-byte aligned base)

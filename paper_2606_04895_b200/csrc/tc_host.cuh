@@ -59,11 +59,11 @@ template <int METHOD, int ROWS>
 __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
   const Params& P = *C.P;
   const int d = P.d;
-  const int64_t r_in_launch = (int64_t)blockIdx.x * Geo<ROWS>::kChains + C.row;
-  const bool valid = r_in_launch < R.B;
-  const bool lead = valid && C.k == 0;
-
   if (METHOD == M_EVAL) {
+    // tile loop (Run::n_tiles): both CTAs of a pair make the same number of passes (n_tiles and gridDim.x are even)
+    for (int64_t tile = blockIdx.x; tile < R.n_tiles; tile += gridDim.x) {
+    const int64_t r_in_launch = tile * Geo<ROWS>::kChains + C.row;
+    const bool valid = r_in_launch < R.B;
     float th[8], g[8], lp;
     if (R.io_mode == IO_ROWS_F32) {
 #pragma unroll
@@ -87,8 +87,13 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
         if (R.want_grad) store_vec8(C, R.grad, R.ld, r_in_launch, d, g);
       }
     }
+    }
     return;
   }
+
+  const int64_t r_in_launch = (int64_t)blockIdx.x * Geo<ROWS>::kChains + C.row;
+  const bool valid = r_in_launch < R.B;
+  const bool lead = valid && C.k == 0;
 
   if (METHOD == M_AIES) {
     const int64_t i = R.own0 + r_in_launch;
@@ -363,6 +368,7 @@ best_tc_kernel(const __grid_constant__ Params P, const __grid_constant__ Run R) 
   const uint32_t tmem_base = *tmem_ptr;
 
   int64_t n_evals = 1;
+  if (METHOD == M_EVAL) n_evals = (R.n_tiles - (int64_t)blockIdx.x + (int64_t)gridDim.x - 1) / (int64_t)gridDim.x;
   if (METHOD == M_MH || METHOD == M_MALA) n_evals = R.n_steps;
   if (METHOD == M_HMC) n_evals = R.n_steps * R.n_leapfrog;
   const int n_ops = R.want_grad ? P.n_ops_all : P.n_ops_fwd;
@@ -501,9 +507,38 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
   }
   P.L = ctx->L_dev;
   P.hard_box = ctx->tgt.hard_box;
+  tc::Run Rl = R;
+  int64_t grid = n_tiles;
+  if (METHOD == tc::M_EVAL) {
+    // best_logp_grad / cache refresh: one wave of CTAs walks all tiles (Run::n_tiles).  The wave is what the device
+    // holds at once: CTA pairs cannot straddle GPCs, so ask the occupancy calculator instead of assuming n_sm / 2.
+    static std::atomic<int> wave{0};
+    int w = wave.load(std::memory_order_acquire);
+    if (w == 0) {
+      if (tc::Geo<ROWS>::kCluster) {
+        cudaLaunchConfig_t q{};
+        q.gridDim = dim3(2 * (unsigned)pl->n_sm); q.blockDim = dim3(tc::kThreads); q.dynamicSmemBytes = (size_t)smem_bytes;
+        cudaLaunchAttribute qa[1];
+        qa[0].id = cudaLaunchAttributeClusterDimension;
+        qa[0].val.clusterDim.x = 2; qa[0].val.clusterDim.y = 1; qa[0].val.clusterDim.z = 1;
+        q.attrs = qa; q.numAttrs = 1;
+        int nc = 0;
+        BEST_CUDA(cudaOccupancyMaxActiveClusters(&nc, tc::best_tc_kernel<METHOD, ROWS>, &q));
+        w = 2 * nc;
+      } else {
+        int nb = 0;
+        BEST_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, tc::best_tc_kernel<METHOD, ROWS>, tc::kThreads, (size_t)smem_bytes));
+        w = nb * pl->n_sm;
+      }
+      if (w < 2) w = 2;
+      wave.store(w, std::memory_order_release);
+    }
+    Rl.n_tiles = n_tiles;
+    if (grid > w) grid = w;
+  }
   if (tc::Geo<ROWS>::kCluster) {
     cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)n_tiles);
+    cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3(tc::kThreads);
     cfg.dynamicSmemBytes = (size_t)smem_bytes;
     cfg.stream = s;
@@ -511,9 +546,9 @@ int launch_tc_geo(best_ctx* ctx, const tc::Run& R, int64_t rows, cudaStream_t s)
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    BEST_CUDA(cudaLaunchKernelEx(&cfg, tc::best_tc_kernel<METHOD, ROWS>, P, R));
+    BEST_CUDA(cudaLaunchKernelEx(&cfg, tc::best_tc_kernel<METHOD, ROWS>, P, Rl));
   } else {
-    tc::best_tc_kernel<METHOD, ROWS><<<(unsigned)n_tiles, tc::kThreads, smem_bytes, s>>>(P, R);
+    tc::best_tc_kernel<METHOD, ROWS><<<(unsigned)grid, tc::kThreads, smem_bytes, s>>>(P, Rl);
   }
   count_launch();
   BEST_CUDA(cudaGetLastError());
