@@ -29,12 +29,13 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` captures of THIS round's code (profiles/r2b_ncu_full.md); None where no capture exists.
-NCU_TRAFFIC_BYTES = {("hmc", "bf16"): 10.995712e6 + 121.568768e6,          # best_tc_kernel<2,256>, 8 trajectories per launch
+# `ncu --set full` captures of THIS round's code (default line: profiles/r2c_ncu_full.md; the other three:
+# profiles/r2b_ncu_full.md); None where no capture exists.
+NCU_TRAFFIC_BYTES = {("hmc", "bf16"): 11.073280e6 + 126.469120e6,          # best_tc_kernel<2,256>, 8 trajectories per launch
                      ("lcdm_mala_16k", "bf16"): 11.711232e6 + 829.322496e6,  # best_tc_kernel<1,256>, 100 steps per launch
                      ("lcdm_mh_16k", "bf16"): 5.559552e6 + 0.0,              # best_tc_kernel<0,256>, 100 steps per launch
                      ("lcdm_mala", "bf16"): 5.240832e6 + 0.181760e6}         # best_tc_kernel<1,233>, 100 steps per launch
-NCU_TRAFFIC_SOURCE = "profiles/r2b_ncu_full.md"
+NCU_TRAFFIC_SOURCE = "profiles/r2c_ncu_full.md"
 
 # PAPER.md Table 1 (L211-219), best published figure per sampler: sampler steps/s at 20 (1000) chains on a Tesla
 # V100 with XLA JIT -- another machine, an emulator of unstated size: context, not a target
@@ -390,7 +391,7 @@ def main():
         "roofline": {"bound": "tensor" if args.precision == "bf16" else "alu", "achieved": achieved_tf,
                      "peak": this_peak, "unit": "TFLOP/s", "frac": achieved_tf / this_peak,
                      "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.precision)) if is_default_size else None,
-                     "traffic_unit": f"bytes per launch (ncu dram read+write, {NCU_TRAFFIC_SOURCE})",
+                     "traffic_unit": "bytes per launch (ncu dram read+write, %s)" % (NCU_TRAFFIC_SOURCE if args.workload == DEFAULT_WORKLOAD else "profiles/r2b_ncu_full.md"),
                      "peak_source": this_src,
                      "frac_of_sustained": (achieved_tf / peaks["bf16_tflops_sustained"]) if peaks and args.precision == "bf16" else None,
                      "kernel": "best_tc_kernel<%s>" % spec["method"], "flops_per_launch": flops_per_launch,
@@ -438,7 +439,7 @@ def main():
         # best_logp_grad timed directly (BASELINE metric "emulator logp+grad evals/s"): device buffers in and out
         lg = {}
         for make, net in (("lcdm", "27x512^4x1"), ("sterile", "29x1024^4x1")):
-            for npts in (16384, 65536):
+            for npts in (16384, 65536, 262144):   # one wave of CTAs walks all tiles (Run::n_tiles): 1 / 3.5 / 14 passes
                 sp = dict(make=make, mlp_scale=1.0, n_chains=npts)
                 ww = make_workload(sp)
                 ctx = B.Context(ww, B.PREC_BF16)

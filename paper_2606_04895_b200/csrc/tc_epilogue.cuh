@@ -74,6 +74,25 @@ __device__ __forceinline__ void load_bias(const EpiCtx& C, int layer, int jn, in
     }
   }
 }
+// the same from a formed shared address (pair fast path: per-chunk base, the groups address with immediates)
+template <bool B16>
+__device__ __forceinline__ void load_bias_at(uint32_t a, f32x2 (&b)[8]) {
+  if (!B16) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) ptx::lds_c2x64(a + i * 16, b[2 * i], b[2 * i + 1]);
+  } else {
+    unsigned long long q[4];
+    ptx::lds_c2x64(a, q[0], q[1]);
+    ptx::lds_c2x64(a + 16, q[2], q[3]);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      uint32_t w0, w1;
+      ptx::unpack2u(q[i], w0, w1);
+      b[2 * i] = ptx::pack2u(w0 << 16, w0 & 0xFFFF0000u);
+      b[2 * i + 1] = ptx::pack2u(w1 << 16, w1 & 0xFFFF0000u);
+    }
+  }
+}
 // store the thread's 16 bf16 results of group jn as the next A operand (no fence / signal here)
 template <int ROWS>
 __device__ __forceinline__ void store_a(const EpiCtx& C, int jn, const uint32_t (&hp)[8]) {
@@ -311,6 +330,45 @@ __device__ __forceinline__ void epi_fwd(EpiCtx& C, const OpDesc& op, bool want_g
       arrive_mma(C, C.bars.d_free(buf));
       continue;
     }
+    if (Geo<ROWS>::kPair && op.perm && ngrp == 2) {
+      // CTA pairs, permuted row blocks, N = 256: this lane half's two groups are the k-chunks jn0 and jn0 + 2 of the
+      // next operand.  Per-chunk bases once, the groups address with immediates; bias (and output row) requested
+      // under the TMEM load (as in the owner geometries; same arithmetic as the general loop below, same bits)
+      constexpr uint32_t kDPiece = Geo<ROWS>::kTileRows * 16;
+      const int jn0 = c * 4 + C.half;
+      const bool b16 = C.P->bias16 != 0;
+      const uint32_t bias_a = C.bias_thr + (uint32_t)(op.layer * C.P->H + jn0 * 64) * (b16 ? 2u : 4u);
+      const uint32_t ws_a = C.wouts_thr + (uint32_t)jn0 * 256u;
+      const uint32_t aoff = (uint32_t)jn0 * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? C.a_wr : 0u);
+      const uint32_t sts0 = C.a_thr0 + aoff, sts1 = C.a_thr1 + aoff;
+      uint8_t* dact_a = dact_l + (size_t)jn0 * kDBlk;
+      const uint32_t bar_r = C.bars.a_ready(jn0), bar_f = C.bars.a_free(jn0);
+#pragma unroll
+      for (int g0 = 0; g0 < 2; ++g0) {
+        uint32_t v[16], hp[8], dp[8];
+        f32x2 b[8], ws[8];
+        ptx::tmem_ld16(tcol + g0 * 64, v);
+        if (b16) load_bias_at<true>(bias_a + g0 * 256, b); else load_bias_at<false>(bias_a + g0 * 512, b);
+        if (LAST) {
+#pragma unroll
+          for (int i = 0; i < 4; ++i) ptx::lds_c2x64(ws_a + g0 * 512 + i * 16, ws[2 * i], ws[2 * i + 1]);
+        }
+        ptx::tmem_ld_wait();
+        fwd_math<ACT, LAST>(v, b, ws, want_grad, acc2, hp, dp);
+        if (!LAST && want_grad) {
+          ptx::stg_128(dact_a + (size_t)(2 * g0) * kDBlk, dp[0], dp[1], dp[2], dp[3]);
+          ptx::stg_128(dact_a + (size_t)(2 * g0) * kDBlk + kDPiece, dp[4], dp[5], dp[6], dp[7]);
+        }
+        if (writes_a) {
+          if (gate) ptx::mbar_wait(bar_f + g0 * 16, C.o & 1u);
+          ptx::sts_128(sts0 + g0 * 2 * Geo<ROWS>::kAChunk, hp[0], hp[1], hp[2], hp[3]);
+          ptx::sts_128(sts1 + g0 * 2 * Geo<ROWS>::kAChunk, hp[4], hp[5], hp[6], hp[7]);
+          ptx::fence_proxy_async();
+          arrive_mma(C, bar_r + g0 * 16);
+        }
+      }
+      if (writes_a) written = max(written, jn0 + 3);
+    } else
     for (int g0 = 0; g0 < ngrp; ++g0) {
       const int grp = g0;
       const int jn = Geo<ROWS>::kPair ? pair_jn(op, c, C.half, grp, ngrp) : c * ngrp + grp;
@@ -448,6 +506,32 @@ __device__ __forceinline__ void epi_bwd(EpiCtx& C, const OpDesc& op, int& writte
     ptx::mbar_wait(C.bars.d_full(buf), use & 1u);
     ptx::tc_fence_after();
     const uint32_t tcol = C.tmem_lane + buf * Geo<ROWS>::kBufCols + C.k * 16;
+    if (Geo<ROWS>::kPair && op.perm && ngrp == 2) {
+      // (see epi_fwd) k-chunks jnc and jnc + 2; act' of the next group / of the next N-chunk's first group (jnc + 4)
+      // is requested under the TMEM load
+      const uint8_t* dact_a = dact_l + (size_t)jnc * kDBlk;
+      const uint32_t aoff = (uint32_t)jnc * Geo<ROWS>::kAChunk + (Geo<ROWS>::kPingPong ? C.a_wr : 0u);
+      const uint32_t sts0 = C.a_thr0 + aoff, sts1 = C.a_thr1 + aoff;
+      const uint32_t bar_r = C.bars.a_ready(jnc), bar_f = C.bars.a_free(jnc);
+      const bool more = c + 1 < op.nch;
+#pragma unroll
+      for (int g0 = 0; g0 < 2; ++g0) {
+        uint32_t v[16], hp[8];
+        ptx::tmem_ld16(tcol + g0 * 64, v);
+        const uint4 d0 = a0, d1 = a1;
+        if (g0 == 0 || more) {
+          a0 = ptx::ldg_128(dact_a + (size_t)(2 * g0 + 2) * kDBlk); a1 = ptx::ldg_128(dact_a + (size_t)(2 * g0 + 2) * kDBlk + kDPiece);
+        }
+        ptx::tmem_ld_wait();
+        bwd_group<ROWS>(v, d0, d1, hp);
+        if (gate) ptx::mbar_wait(bar_f + g0 * 16, C.o & 1u);
+        ptx::sts_128(sts0 + g0 * 2 * Geo<ROWS>::kAChunk, hp[0], hp[1], hp[2], hp[3]);
+        ptx::sts_128(sts1 + g0 * 2 * Geo<ROWS>::kAChunk, hp[4], hp[5], hp[6], hp[7]);
+        ptx::fence_proxy_async();
+        arrive_mma(C, bar_r + g0 * 16);
+      }
+      written = max(written, jnc + 3);
+    } else
     for (int g0 = 0; g0 < ngrp; ++g0) {
       const int grp = g0;
       const int jn = jnc + grp * jstep;
