@@ -149,6 +149,22 @@ int best_step_aies_de(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t s
  * feed nor disturb it.  adapt_every = 0 switches it off; every call with adapt_every > 0 opens a fresh
  * window.  Not used by AIES.  Synchronises the device.                                   */
 int best_set_adaptation(best_ctx* ctx, best_state* st, int32_t adapt_every, double jitter);
+/* Multi-GPU adaptation (chains are sharded over ranks with no per-step traffic; "covariance
+ * adaptation = one all-reduce of d^2+d+1 fp64 values per window"; the covariance is that of the
+ * whole ensemble of chains).  With an exchange function set, every window of `st` closes as
+ *   own sums -> packet [ n | ref (d) | sum(theta-ref) (d) | sum (theta-ref)(theta-ref)^T (d*d) ]   (np = 1+2d+d*d
+ *   doubles; each rank's sums are about its own reference point `ref`)
+ *   -> fn(send_dev, recv_dev, np, stream, user): an ALL-GATHER over the job's ranks, rank r's packet to
+ *      recv_dev[r*np .. r*np+np), enqueued on `stream` (e.g. ncclAllGather, or torch.distributed
+ *      all_gather_into_tensor under that stream); both pointers are device memory owned by the library;
+ *      return 0, anything else makes the step call fail with BEST_ERR_CUDA
+ *   -> the library moves every packet to rank 0's reference point, adds them in rank order (identical bits
+ *      on all ranks) and computes C, L = chol(C) as in best_set_adaptation from the sums of ALL ranks.
+ * Every rank must close its windows at the same steps (same adapt_every, same step calls).  world_size >= 1;
+ * fn = NULL switches the exchange off.  Allocates (1 + world_size) * np doubles, once.  The callback is called
+ * on the host thread inside best_step_* / best_burn_in.  Errors: BEST_ERR_ARG, BEST_ERR_ALLOC.               */
+typedef int (*best_exchange_fn)(const double* send_dev, double* recv_dev, int64_t count, void* stream, void* user);
+int best_set_adaptation_exchange(best_state* st, best_exchange_fn fn, void* user, int32_t world_size);
 /* number of successful / failed whitening updates so far (synchronises) */
 int best_adapt_stats(best_ctx* ctx, int64_t* n_updates, int64_t* n_failures);
 

@@ -26,7 +26,11 @@ EXPORTS = [
     "best_state_get_f64", "best_state_last_log_alpha", "best_state_set", "best_launch_count",
     "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box", "best_burn_in", "best_step_aies_de", "best_rminus1", "best_probe_l2_read",
     "best_state_set_chain_offset", "best_rminus1_noalloc", "best_rminus1_noalloc_max_doubles",
+    "best_set_adaptation_exchange",
 ]
+
+# int fn(const double* send_dev, double* recv_dev, int64_t count, void* stream, void* user)
+EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p)
 
 
 class BestError(RuntimeError):
@@ -92,6 +96,7 @@ def lib():
     L.best_state_last_log_alpha.argtypes = [vp, vp, vp]
     L.best_state_set.argtypes = [vp, vp, u64, vp]
     L.best_state_set_chain_offset.argtypes = [vp, u64]
+    L.best_set_adaptation_exchange.argtypes = [vp, EXCHANGE_FN, vp, i32]
     L.best_launch_count.restype = u64
     L.best_last_error.restype = C.c_char_p
     L.best_version.restype = C.c_char_p
@@ -282,6 +287,25 @@ class State:
 
     def set_adaptation(self, adapt_every, jitter=1e-6):
         _check(lib().best_set_adaptation(self.ctx._h, self._h, adapt_every, jitter))
+
+    def set_adaptation_exchange(self, fn, world_size):
+        """best_set_adaptation_exchange: fn(send_ptr, recv_ptr, count, stream) -> None / 0 enqueues an all-gather of
+        `count` doubles per rank on `stream` (see distributed.allgather_exchange); fn = None switches it off."""
+        if fn is None:
+            self._xchg = None
+            _check(lib().best_set_adaptation_exchange(self._h, C.cast(None, EXCHANGE_FN), None, world_size))
+            return
+
+        def tramp(send, recv, count, stream, _user):
+            try:
+                rc = fn(send or 0, recv or 0, count, stream or 0)
+                return int(rc or 0)
+            except Exception:          # an exception must not unwind through the C frames
+                import traceback
+                traceback.print_exc()
+                return 1
+        self._xchg = EXCHANGE_FN(tramp)          # keep the trampoline alive as long as the state uses it
+        _check(lib().best_set_adaptation_exchange(self._h, self._xchg, None, world_size))
 
     def burn_in(self, method, n_iter, n_steps, n_adapt, block, seed, eps0, target_accept, n_leapfrog=1,
                 jitter=1e-6, stream=0):

@@ -310,6 +310,24 @@ int best_set_adaptation(best_ctx* ctx, best_state* st, int32_t adapt_every, doub
   return BEST_OK;
 }
 
+int best_set_adaptation_exchange(best_state* st, best_exchange_fn fn, void* user, int32_t world_size) {
+  if (!st || world_size < 1 || world_size > 4096) {
+    set_error("best_set_adaptation_exchange: bad argument");
+    return BEST_ERR_ARG;
+  }
+  BEST_CUDA(cudaDeviceSynchronize());
+  st->xchg_fn = nullptr;
+  cudaFree(st->xchg_buf);
+  st->xchg_buf = nullptr;
+  if (fn) {
+    const int d = st->ctx->d;
+    const size_t np = 1 + 2 * (size_t)d + (size_t)d * d;
+    BEST_TRY(dev_alloc(&st->xchg_buf, np * (size_t)(1 + world_size)));
+    st->xchg_fn = fn; st->xchg_user = user; st->xchg_world = world_size;
+  }
+  return BEST_OK;
+}
+
 int best_state_set_chain_offset(best_state* st, uint64_t chain0) {
   if (!st || chain0 + (uint64_t)st->B > ((uint64_t)1 << 32)) {
     set_error("best_state_set_chain_offset: chain0 + n_chains must not exceed 2^32");

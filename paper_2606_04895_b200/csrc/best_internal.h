@@ -133,6 +133,11 @@ struct best_state {
   int win_flip = 0;
   cudaStream_t side = nullptr;
   cudaEvent_t ev_seg[2] = {nullptr, nullptr}, ev_gram[2] = {nullptr, nullptr};
+  // multi-GPU: the window's sums of ALL ranks feed the covariance (best_set_adaptation_exchange)
+  best_exchange_fn xchg_fn = nullptr;
+  void* xchg_user = nullptr;
+  int xchg_world = 1;
+  double* xchg_buf = nullptr;     // [1 + world] packets of 1 + 2d + d*d doubles: own packet, then the gathered ones
 };
 
 namespace best {

@@ -323,6 +323,47 @@ __global__ void k_cov_finalize(double* __restrict__ acc, int nblk, int d, double
   }
 }
 
+// ---- A9 across ranks ("covariance adaptation = one all-reduce of d^2+d+1 fp64 values per window") ----
+// Every rank's window sums are taken about its OWN reference point, so a rank's packet carries that point as well:
+// packet = [ n | ref (d) | S1 = sum(theta - ref) (d) | S2 = sum (theta - ref)(theta - ref)^T (d*d) ].
+// k_cov_pack adds the per-block partials in block order (as k_cov_finalize does) and clears them.
+__global__ void k_cov_pack(double* __restrict__ acc, int nblk, int d, const double* __restrict__ ref,
+                           double* __restrict__ packet) {
+  const int ne = 1 + d + d * d;
+  for (int e = threadIdx.x; e < ne; e += blockDim.x) {
+    double s = 0.0;
+    for (int b = 0; b < nblk; ++b) { s += acc[(size_t)b * ne + e]; acc[(size_t)b * ne + e] = 0.0; }
+    packet[e == 0 ? 0 : e + d] = s;
+  }
+  for (int i = threadIdx.x; i < d; i += blockDim.x) packet[1 + i] = ref[i];
+}
+// The gathered packets, rank 0 first, moved to rank 0's reference point and added in rank order (every rank gets
+// the same bits): with delta = ref_k - ref_0, theta - ref_0 = (theta - ref_k) + delta, hence
+//   S1' = S1 + n delta,   S2'_ij = S2_ij + S1_i delta_j + delta_i S1_j + n delta_i delta_j.
+// The total goes to partial block 0 (the others are zero after k_cov_pack): k_cov_finalize then runs unchanged.
+__global__ void k_cov_combine(const double* __restrict__ gathered, int world, int d, double* __restrict__ acc) {
+  const int ne = 1 + d + d * d, np = 1 + 2 * d + d * d;
+  for (int e = threadIdx.x; e < ne; e += blockDim.x) {
+    double tot = 0.0;
+    for (int k = 0; k < world; ++k) {
+      const double* pk = gathered + (size_t)k * np;
+      const double n = pk[0];
+      const double *rk = pk + 1, *r0 = gathered + 1, *s1 = pk + 1 + d, *s2 = pk + 1 + 2 * d;
+      if (e == 0) {
+        tot += n;
+      } else if (e <= d) {
+        const int i = e - 1;
+        tot += s1[i] + n * (rk[i] - r0[i]);
+      } else {
+        const int i = (e - 1 - d) / d, j = (e - 1 - d) % d;
+        const double di = rk[i] - r0[i], dj = rk[j] - r0[j];
+        tot += s2[i * d + j] + s1[i] * dj + di * s1[j] + n * di * dj;
+      }
+    }
+    acc[e] = tot;
+  }
+}
+
 Chains chains_of(best_state* st) {
   Chains S;
   S.B = st->B; S.d = st->ctx->d; S.chain0 = (uint32_t)st->chain0;
@@ -335,6 +376,19 @@ Chains chains_of(best_state* st) {
 }  // namespace
 
 static int close_window(best_ctx* ctx, best_state* st, cudaStream_t s) {
+  if (st->xchg_fn) {
+    // own sums -> packet -> the caller's all-gather (enqueued on `s`) -> all ranks' sums about rank 0's reference
+    const int d = ctx->d;
+    const int64_t np = 1 + 2 * (int64_t)d + (int64_t)d * d;
+    k_cov_pack<<<1, 1024, 0, s>>>(st->cov_acc, st->cov_blocks, d, st->cov_ref, st->xchg_buf);
+    count_launch();
+    BEST_CUDA(cudaGetLastError());
+    const int rc = st->xchg_fn(st->xchg_buf, st->xchg_buf + np, np, (void*)s, st->xchg_user);
+    if (rc != 0) { set_error("best_set_adaptation_exchange: the exchange callback returned an error"); return BEST_ERR_CUDA; }
+    k_cov_combine<<<1, 1024, 0, s>>>(st->xchg_buf + np, st->xchg_world, d, st->cov_acc);
+    count_launch();
+    BEST_CUDA(cudaGetLastError());
+  }
   k_cov_finalize<<<1, 1024, 0, s>>>(st->cov_acc, st->cov_blocks, ctx->d, st->jitter, ctx->L_dev, ctx->Lraw_dev,
                                    ctx->scale_dev, (long long*)ctx->adapt_counts);
   count_launch();
@@ -393,6 +447,7 @@ int adapt_window_rows(best_ctx* ctx, best_state* st, int buf, int64_t n_steps, c
 void adapt_free(best_state* st) {
   if (st->side) cudaStreamSynchronize(st->side);
   cudaFree(st->cov_acc); cudaFree(st->cov_ref); cudaFree(st->win_buf[0]); cudaFree(st->win_buf[1]);
+  cudaFree(st->xchg_buf); st->xchg_buf = nullptr; st->xchg_fn = nullptr;
   for (int i = 0; i < 2; ++i) {
     if (st->ev_seg[i]) cudaEventDestroy(st->ev_seg[i]);
     if (st->ev_gram[i]) cudaEventDestroy(st->ev_gram[i]);

@@ -24,7 +24,13 @@ dist.barrier()
 # the Philox stream this rank's chain 0 draws at step 0 (the stream layout is the oracle's, KAT-pinned)
 from oracle import oracle as O
 first = O.normals(7, chain0 + 0, 0, w.d)
-out = dict(rank=rank, n_chains=int(w.n_chains), theta_sum=float(np.abs(w.theta0).sum()),
+# the one exchange step of the sharded path (SURVEY 8(e), best_set_adaptation_exchange): every rank's packet of
+# window sums, rank order -- here on CPU tensors over gloo, on the GPU box the same call over NCCL
+from paper_2606_04895_b200 import distributed as D
+send = torch.arange(5, dtype=torch.float64) + 100.0 * rank
+recv = torch.zeros(5 * world, dtype=torch.float64)
+D.allgather_packets(send, recv)
+out = dict(gathered=recv.tolist(), rank=rank, n_chains=int(w.n_chains), theta_sum=float(np.abs(w.theta0).sum()),
            W0=float(w.W[0].sum()), mu0=float(w.mu[0]), ms=ms, chain0=int(chain0), first=[float(x) for x in first])
 print("RESULT " + json.dumps(out), flush=True)
 dist.destroy_process_group()
@@ -60,6 +66,8 @@ def test_sharding_and_max_over_ranks_gloo(tmp_path):
     # ranks' first normals differ while rank 0 reproduces the single-process stream
     assert [r["chain0"] for r in res] == [0, 64]
     assert res[0]["first"] != res[1]["first"]
+    # the covariance-window exchange: both ranks hold rank 0's packet, then rank 1's
+    assert res[0]["gathered"] == res[1]["gathered"] == [0.0, 1.0, 2.0, 3.0, 4.0, 100.0, 101.0, 102.0, 103.0, 104.0]
     from oracle import oracle as O
     assert res[0]["first"] == [float(x) for x in O.normals(7, 0, 0, 6)]
     assert res[1]["first"] == [float(x) for x in O.normals(7, 64, 0, 6)]
