@@ -165,6 +165,18 @@ int best_set_adaptation(best_ctx* ctx, best_state* st, int32_t adapt_every, doub
  * on the host thread inside best_step_* / best_burn_in.  Errors: BEST_ERR_ARG, BEST_ERR_ALLOC.               */
 typedef int (*best_exchange_fn)(const double* send_dev, double* recv_dev, int64_t count, void* stream, void* user);
 int best_set_adaptation_exchange(best_state* st, best_exchange_fn fn, void* user, int32_t world_size);
+/* Ensemble moves sharded over ranks ("AIES = one all-gather of the complementary half's positions per
+ * half-step").  Every rank holds the WHOLE ensemble in `st` (same theta0, chain offset 0 on all ranks: walker i
+ * draws the Philox stream of walker i whichever rank moves it).  With an exchange function set, best_step_aies
+ * and best_step_aies_de move only walkers [rank*cnt, rank*cnt + cnt) of each half-ensemble, cnt = B/2/world_size,
+ * with partners drawn from the whole other half, and after every half-step call
+ *   fn(send_dev, recv_dev, (d+1)*cnt, stream, user)
+ * -- an all-gather as in best_set_adaptation_exchange -- of the slice just moved ([d+1][cnt] doubles: theta rows, then
+ * log pi), which the library writes into every rank's copy of that half.  After a step all ranks hold the same
+ * theta and log pi, bit for bit those of the unsharded run; acceptance counters cover a rank's own walkers only.
+ * Two all-gathers per step.  A trace pointer is refused (BEST_ERR_ARG) while the exchange is set.
+ * Errors: BEST_ERR_ARG (B/2 not a multiple of world_size, rank outside 0..world_size-1), BEST_ERR_ALLOC.       */
+int best_set_aies_exchange(best_state* st, best_exchange_fn fn, void* user, int32_t rank, int32_t world_size);
 /* number of successful / failed whitening updates so far (synchronises) */
 int best_adapt_stats(best_ctx* ctx, int64_t* n_updates, int64_t* n_failures);
 

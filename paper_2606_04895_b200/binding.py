@@ -26,7 +26,7 @@ EXPORTS = [
     "best_state_get_f64", "best_state_last_log_alpha", "best_state_set", "best_launch_count",
     "best_last_error", "best_version", "best_set_step_scale", "best_set_hard_box", "best_burn_in", "best_step_aies_de", "best_rminus1", "best_probe_l2_read",
     "best_state_set_chain_offset", "best_rminus1_noalloc", "best_rminus1_noalloc_max_doubles",
-    "best_set_adaptation_exchange",
+    "best_set_adaptation_exchange", "best_set_aies_exchange",
 ]
 
 # int fn(const double* send_dev, double* recv_dev, int64_t count, void* stream, void* user)
@@ -97,6 +97,7 @@ def lib():
     L.best_state_set.argtypes = [vp, vp, u64, vp]
     L.best_state_set_chain_offset.argtypes = [vp, u64]
     L.best_set_adaptation_exchange.argtypes = [vp, EXCHANGE_FN, vp, i32]
+    L.best_set_aies_exchange.argtypes = [vp, EXCHANGE_FN, vp, i32, i32]
     L.best_launch_count.restype = u64
     L.best_last_error.restype = C.c_char_p
     L.best_version.restype = C.c_char_p
@@ -306,6 +307,24 @@ class State:
                 return 1
         self._xchg = EXCHANGE_FN(tramp)          # keep the trampoline alive as long as the state uses it
         _check(lib().best_set_adaptation_exchange(self._h, self._xchg, None, world_size))
+
+    def set_aies_exchange(self, fn, rank, world_size):
+        """best_set_aies_exchange: the ensemble moves of this state update the rank's slice of each half-ensemble and
+        all-gather it through fn (same signature as in set_adaptation_exchange); fn = None switches it off."""
+        if fn is None:
+            self._aies_xchg = None
+            _check(lib().best_set_aies_exchange(self._h, C.cast(None, EXCHANGE_FN), None, rank, world_size))
+            return
+
+        def tramp(send, recv, count, stream, _user):
+            try:
+                return int(fn(send or 0, recv or 0, count, stream or 0) or 0)
+            except Exception:
+                import traceback
+                traceback.print_exc()
+                return 1
+        self._aies_xchg = EXCHANGE_FN(tramp)
+        _check(lib().best_set_aies_exchange(self._h, self._aies_xchg, None, rank, world_size))
 
     def burn_in(self, method, n_iter, n_steps, n_adapt, block, seed, eps0, target_accept, n_leapfrog=1,
                 jitter=1e-6, stream=0):

@@ -252,6 +252,10 @@ static int run_step(best_ctx* ctx, best_state* st, int method, int64_t n, uint64
     if (!(eps > 1.f)) { set_error("aies: a must be > 1"); return BEST_ERR_ARG; }
     if (st->B < 2 || (st->B & 1)) { set_error("aies: walker count must be even and >= 2"); return BEST_ERR_ARG; }
   }
+  if (method == M_AIES && st->aies_fn && trace) {
+    set_error("ensemble move sharded over ranks (best_set_aies_exchange): no trace, read the state instead");
+    return BEST_ERR_ARG;
+  }
   if (n == 0) return BEST_OK;
   int rc;
   if (ctx->precision == BEST_PREC_BF16) {
@@ -324,6 +328,24 @@ int best_set_adaptation_exchange(best_state* st, best_exchange_fn fn, void* user
     const size_t np = 1 + 2 * (size_t)d + (size_t)d * d;
     BEST_TRY(dev_alloc(&st->xchg_buf, np * (size_t)(1 + world_size)));
     st->xchg_fn = fn; st->xchg_user = user; st->xchg_world = world_size;
+  }
+  return BEST_OK;
+}
+
+int best_set_aies_exchange(best_state* st, best_exchange_fn fn, void* user, int32_t rank, int32_t world_size) {
+  if (!st || world_size < 1 || rank < 0 || rank >= world_size || (st->B & 1) ||
+      (fn && ((st->B / 2) % world_size != 0 || st->B / 2 / world_size < 1))) {
+    set_error("best_set_aies_exchange: bad argument (the half-ensemble must divide evenly over the ranks)");
+    return BEST_ERR_ARG;
+  }
+  BEST_CUDA(cudaDeviceSynchronize());
+  st->aies_fn = nullptr;
+  cudaFree(st->aies_buf);
+  st->aies_buf = nullptr;
+  if (fn) {
+    const size_t n = (size_t)(st->ctx->d + 1) * (size_t)(st->B / 2 / world_size);
+    BEST_TRY(dev_alloc(&st->aies_buf, n * (size_t)(1 + world_size)));
+    st->aies_fn = fn; st->aies_user = user; st->aies_rank = rank; st->aies_world = world_size;
   }
   return BEST_OK;
 }

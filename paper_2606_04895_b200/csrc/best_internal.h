@@ -138,6 +138,12 @@ struct best_state {
   void* xchg_user = nullptr;
   int xchg_world = 1;
   double* xchg_buf = nullptr;     // [1 + world] packets of 1 + 2d + d*d doubles: own packet, then the gathered ones
+  // sharded ensemble moves (best_set_aies_exchange): every rank holds the whole ensemble, updates walkers
+  // [rank * cnt, +cnt) of each half (cnt = B / 2 / world) and all-gathers them after every half-step
+  best_exchange_fn aies_fn = nullptr;
+  void* aies_user = nullptr;
+  int aies_rank = 0, aies_world = 1;
+  double* aies_buf = nullptr;     // [(1 + world)][d + 1][cnt]: own slice (theta rows, then log pi), then the gathered ones
 };
 
 namespace best {
@@ -161,6 +167,8 @@ int step_mala(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cu
 int step_hmc(best_ctx*, best_state*, int64_t, uint64_t, double, int, float*, int, cudaStream_t);
 int step_aies(best_ctx*, best_state*, int64_t, uint64_t, double, float*, int, cudaStream_t, bool de = false);
 int adapt_reset(best_ctx* ctx, best_state* st, cudaStream_t s);
+// sharded ensemble moves: all-gather the walkers [half0 + rank * cnt, +cnt) that this rank has just updated
+int aies_exchange(best_ctx* ctx, best_state* st, int64_t half0, cudaStream_t s);
 void adapt_free(best_state* st);
 // exact path, after step index t of a call: trace slot (every `thin` steps) and covariance accumulation / update
 int after_step(best_ctx* ctx, best_state* st, int64_t t, float* trace, int thin, bool adapt, cudaStream_t s);

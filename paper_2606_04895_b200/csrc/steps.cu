@@ -156,13 +156,15 @@ __global__ void k_hmc_kick(Chains S, const double* __restrict__ L, uint64_t seed
 }
 
 // ---- AIES stretch move, one half-ensemble (eq 2.13-2.15) ---------------------------------------
+// (`half` walkers are updated by this launch; partners come from the `n_oth` walkers of the other half: the
+// same number unless the ensemble is sharded over ranks, best_set_aies_exchange)
 __global__ void k_aies_propose(Chains S, uint64_t seed, uint64_t step, double a, int64_t own0,
-                               int64_t oth0, int64_t half) {
+                               int64_t oth0, int64_t half, int64_t n_oth) {
   const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (r >= half) return;
   const int64_t i = own0 + r;
   const uint4 w = philox4x32_10(S.chain0 + (uint32_t)i, step, 0u, seed);
-  const int64_t j = oth0 + (int64_t)__umulhi(w.z, (uint32_t)half);
+  const int64_t j = oth0 + (int64_t)__umulhi(w.z, (uint32_t)n_oth);
   const double t = u01<double>(w.y) * (a - 1.0) + 1.0;
   const double z = t * t / a;
   for (int k = 0; k < S.d; ++k) {
@@ -192,13 +194,13 @@ __global__ void k_aies_accept(Chains S, uint64_t seed, uint64_t step, double a, 
 // j != k from the other half (control words 2 and 3), gamma = (1 + sigma * n0) 2.38 / sqrt(2 d) with n0
 // the first normal of slot 1; symmetric proposal, log alpha = log pi(x') - log pi(x_i).
 __global__ void k_de_propose(Chains S, uint64_t seed, uint64_t step, double sigma, int64_t own0,
-                             int64_t oth0, int64_t half) {
+                             int64_t oth0, int64_t half, int64_t n_oth) {
   const int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (r >= half) return;
   const int64_t i = own0 + r;
   const uint4 w = philox4x32_10(S.chain0 + (uint32_t)i, step, 0u, seed);
-  const int64_t jr = (int64_t)__umulhi(w.z, (uint32_t)half);
-  int64_t kr = (int64_t)__umulhi(w.w, (uint32_t)(half - 1));
+  const int64_t jr = (int64_t)__umulhi(w.z, (uint32_t)n_oth);
+  int64_t kr = (int64_t)__umulhi(w.w, (uint32_t)(n_oth - 1));
   if (kr >= jr) kr += 1;
   const uint4 wn = philox4x32_10(S.chain0 + (uint32_t)i, step, 1u, seed);
   double n0, n1;
@@ -448,6 +450,7 @@ void adapt_free(best_state* st) {
   if (st->side) cudaStreamSynchronize(st->side);
   cudaFree(st->cov_acc); cudaFree(st->cov_ref); cudaFree(st->win_buf[0]); cudaFree(st->win_buf[1]);
   cudaFree(st->xchg_buf); st->xchg_buf = nullptr; st->xchg_fn = nullptr;
+  cudaFree(st->aies_buf); st->aies_buf = nullptr; st->aies_fn = nullptr;
   for (int i = 0; i < 2; ++i) {
     if (st->ev_seg[i]) cudaEventDestroy(st->ev_seg[i]);
     if (st->ev_gram[i]) cudaEventDestroy(st->ev_gram[i]);
@@ -565,22 +568,60 @@ int step_hmc(best_ctx* ctx, best_state* st, int64_t n_traj, uint64_t seed, doubl
   return BEST_OK;
 }
 
+// ---- sharded ensemble moves ("AIES = one all-gather of the complementary half's positions per
+// half-step"): the slice this rank has just updated, theta rows then log pi, [d + 1][cnt] ----------------------
+__global__ void k_aies_pack(const double* __restrict__ theta, const double* __restrict__ logp, int64_t B, int d,
+                            int64_t first, int64_t cnt, double* __restrict__ send) {
+  const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (c >= cnt) return;
+  for (int k = 0; k < d; ++k) send[(int64_t)k * cnt + c] = theta[(int64_t)k * B + first + c];
+  send[(int64_t)d * cnt + c] = logp[first + c];
+}
+__global__ void k_aies_unpack(const double* __restrict__ recv, int world, int d, int64_t cnt, int64_t half0,
+                              double* __restrict__ theta, double* __restrict__ logp, int64_t B) {
+  const int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;   // walker of the half: rank c / cnt, slot c % cnt
+  if (c >= cnt * world) return;
+  const double* src = recv + (c / cnt) * (int64_t)(d + 1) * cnt + (c % cnt);
+  for (int k = 0; k < d; ++k) theta[(int64_t)k * B + half0 + c] = src[(int64_t)k * cnt];
+  logp[half0 + c] = src[(int64_t)d * cnt];
+}
+
+int aies_exchange(best_ctx* ctx, best_state* st, int64_t half0, cudaStream_t s) {
+  const int d = ctx->d;
+  const int64_t cnt = st->B / 2 / st->aies_world, n = (int64_t)(d + 1) * cnt;
+  k_aies_pack<<<nblocks(cnt), TPB, 0, s>>>(st->theta, st->logp, st->B, d, half0 + st->aies_rank * cnt, cnt, st->aies_buf);
+  count_launch();
+  BEST_CUDA(cudaGetLastError());
+  if (st->aies_fn(st->aies_buf, st->aies_buf + n, n, (void*)s, st->aies_user) != 0) {
+    set_error("best_set_aies_exchange: the exchange callback returned an error");
+    return BEST_ERR_CUDA;
+  }
+  k_aies_unpack<<<nblocks(cnt * st->aies_world), TPB, 0, s>>>(st->aies_buf + n, st->aies_world, d, cnt, half0, st->theta,
+                                                           st->logp, st->B);
+  count_launch();
+  BEST_CUDA(cudaGetLastError());
+  return BEST_OK;
+}
+
 int step_aies(best_ctx* ctx, best_state* st, int64_t n_steps, uint64_t seed, double a, float* trace,
               int thin, cudaStream_t s, bool de) {
   Chains S = chains_of(st);
   const int64_t half = st->B / 2;
-  const int nb = nblocks(half);
+  // sharded: this rank moves `cnt` walkers of each half, partners are drawn from the whole other half
+  const int64_t cnt = st->aies_fn ? half / st->aies_world : half, off = st->aies_fn ? st->aies_rank * cnt : 0;
+  const int nb = nblocks(cnt);
   for (int64_t t = 0; t < n_steps; ++t) {
     const uint64_t step = st->step + (uint64_t)t;
     for (int hh = 0; hh < 2; ++hh) {
-      const int64_t own0 = hh == 0 ? 0 : half, oth0 = hh == 0 ? half : 0;
-      if (de) k_de_propose<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, oth0, half);   // a = sigma_gamma
-      else k_aies_propose<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, oth0, half);
+      const int64_t half0 = hh == 0 ? 0 : half, own0 = half0 + off, oth0 = hh == 0 ? half : 0;
+      if (de) k_de_propose<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, oth0, cnt, half);   // a = sigma_gamma
+      else k_aies_propose<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, oth0, cnt, half);
       count_launch();
-      BEST_TRY(eval_target_soa(ctx, st->p_theta, st->B, half, st->p_logp, nullptr, s));
-      if (de) k_de_accept<<<nb, TPB, 0, s>>>(S, seed, step, own0, half);
-      else k_aies_accept<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, half);
+      BEST_TRY(eval_target_soa(ctx, st->p_theta, st->B, cnt, st->p_logp, nullptr, s));
+      if (de) k_de_accept<<<nb, TPB, 0, s>>>(S, seed, step, own0, cnt);
+      else k_aies_accept<<<nb, TPB, 0, s>>>(S, seed, step, a, own0, cnt);
       count_launch();
+      if (st->aies_fn) BEST_TRY(aies_exchange(ctx, st, half0, s));
     }
     BEST_TRY(after_step(ctx, st, t, trace, thin, false, s));
   }

@@ -158,6 +158,7 @@ struct Run {
   const float* in_rows; float* out_logp; float* out_grad;
   // AIES
   int64_t own0, oth0;
+  int64_t n_oth;        // walkers of the other half (partner range); = B unless the ensemble is sharded over ranks
   int de;               // differential-evolution move (eq 2.16) instead of the stretch move; eps = sigma_gamma
   // Philox chain id = chain0 + chain index (multi-GPU shards draw disjoint streams)
   uint32_t chain0;

@@ -99,14 +99,14 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
     const int64_t i = R.own0 + r_in_launch;
     const uint32_t cid = R.chain0 + (uint32_t)i;
     const uint4 w = philox4x32_10(cid, R.step0, 0u, R.seed);
-    const int64_t j = R.oth0 + (int64_t)__umulhi(w.z, (uint32_t)R.B);
+    const int64_t j = R.oth0 + (int64_t)__umulhi(w.z, (uint32_t)R.n_oth);
     const float a = R.eps;
     const float t = u01<float>(w.y) * (a - 1.0f) + 1.0f;
     const float z = t * t / a;
     float thp[8], thi[8], g[8], lpp;
     if (R.de) {
       // eq (2.16), reading R23: x' = x_i + gamma (x_j - x_k), k != j from the same half, R.eps = sigma_gamma
-      int64_t kr = (int64_t)__umulhi(w.w, (uint32_t)(R.B - 1));
+      int64_t kr = (int64_t)__umulhi(w.w, (uint32_t)(R.n_oth - 1));
       if (kr >= j - R.oth0) kr += 1;
       const uint4 wn = philox4x32_10(cid, R.step0, 1u, R.seed);
       float n0, n1;
@@ -894,12 +894,18 @@ int tc_step(best_ctx* ctx, best_state* st, int method, int64_t n_steps, uint64_t
       case tc::M_HMC: BEST_TRY(launch_tc<tc::M_HMC>(ctx, R, st->B, s)); break;
       default: {
         const int64_t half = st->B / 2;
+        // sharded (best_set_aies_exchange): this rank moves `cnt` walkers of each half, partners come from the whole
+        // other half, the moved slice is all-gathered after every half-step
+        const int64_t cnt = st->aies_fn ? half / st->aies_world : half, off = st->aies_fn ? st->aies_rank * cnt : 0;
         tc::Run Rh = R;
-        Rh.B = half;
+        Rh.B = cnt;
+        Rh.n_oth = half;
         for (int hh = 0; hh < 2; ++hh) {
-          Rh.own0 = hh == 0 ? 0 : half;
+          const int64_t half0 = hh == 0 ? 0 : half;
+          Rh.own0 = half0 + off;
           Rh.oth0 = hh == 0 ? half : 0;
-          BEST_TRY(launch_tc<tc::M_AIES>(ctx, Rh, half, s));
+          BEST_TRY(launch_tc<tc::M_AIES>(ctx, Rh, cnt, s));
+          if (st->aies_fn) BEST_TRY(aies_exchange(ctx, st, half0, s));
         }
       }
     }

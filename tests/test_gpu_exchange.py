@@ -156,3 +156,94 @@ def test_E_exchange_errors(B):
     st.set_adaptation(10, 1e-6)
     st.step_mh(10, 1, 0.3)
     ctx.close()
+
+
+@pytest.mark.parametrize("de", [False, True])
+@pytest.mark.parametrize("prec", ["fp32", "bf16"])
+def test_E_aies_sharded_two_ranks(B, prec, de):
+    """best_set_aies_exchange: two 'ranks' (two contexts driven by two host threads, the all-gather a rendezvous
+    between their callbacks) each move their slice of every half-ensemble; after 6 steps both hold the state of the
+    unsharded run bit for bit (that run is itself checked against the oracle by the T2 / N3 tests)."""
+    import threading
+    import torch
+    P = B.PREC_BF16 if prec == "bf16" else B.PREC_FP32
+    w = WL.sterile(n_chains=600, hidden=64, n_hidden=2)        # halves of 300, slices of 150: ragged against every tile
+    world, n_steps = 2, 6
+
+    def advance(st):
+        if de:
+            st.step_aies_de(n_steps, 13, 0.1)
+        else:
+            st.step_aies(n_steps, 13, 2.0)
+
+    ctx = B.Context(w, P)
+    st = ctx.new_state(w.theta0)
+    advance(st)
+    ref = st.get(want_grad=False)
+    ctx.close()
+    assert 0.05 < ref["n_accept"].sum() / (600 * n_steps) < 0.95
+
+    bar = threading.Barrier(world)
+    slots, results, errors, calls = [None] * world, [None] * world, [], [0] * world
+
+    def make_fn(rank):
+        def fn(send, recv, count, stream):
+            s, r = _views(send, recv, count, world)
+            slots[rank] = s.clone()
+            torch.cuda.synchronize()
+            bar.wait(timeout=120)
+            for k in range(world):
+                r[k * count:(k + 1) * count].copy_(slots[k])
+            torch.cuda.synchronize()
+            bar.wait(timeout=120)                               # every rank has read before a slot is replaced
+            calls[rank] += 1
+            return 0
+        return fn
+
+    def worker(rank):
+        try:
+            c = B.Context(w, P)
+            s = c.new_state(w.theta0)
+            s.set_aies_exchange(make_fn(rank), rank, world)
+            advance(s)
+            results[rank] = s.get(want_grad=False)
+            c.close()
+        except Exception as e:                                  # noqa: BLE001
+            errors.append(e)
+            bar.abort()
+
+    th = [threading.Thread(target=worker, args=(r,)) for r in range(world)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join(timeout=300)
+    assert not errors, errors
+    assert calls == [2 * n_steps] * world                       # one all-gather per half-step
+    own = np.zeros((world, 600), bool)
+    for r in range(world):
+        own[r, 150 * r:150 * r + 150] = True                    # first half
+        own[r, 300 + 150 * r:300 + 150 * r + 150] = True        # second half
+    for r in range(world):
+        assert np.array_equal(results[r]["theta"], ref["theta"]), r
+        assert np.array_equal(results[r]["logp"], ref["logp"]), r
+        assert np.array_equal(results[r]["n_accept"][own[r]], ref["n_accept"][own[r]])
+        assert (results[r]["n_accept"][~own[r]] == 0).all()
+
+
+def test_E_aies_exchange_errors(B):
+    import torch
+    w = WL.sterile(n_chains=100, hidden=64, n_hidden=2)
+    ctx = B.Context(w, B.PREC_FP32)
+    st = ctx.new_state(w.theta0)
+    for rank, world in ((0, 3), (2, 2), (0, 0)):               # 50 walkers per half do not divide by 3; rank outside
+        with pytest.raises(B.BestError) as e:
+            st.set_aies_exchange(lambda *a: 0, rank, world)
+        assert e.value.code == B.BEST_ERR_ARG
+    st.set_aies_exchange(lambda *a: 0, 0, 2)
+    tr = torch.zeros(1, 100, w.d, device="cuda")
+    with pytest.raises(B.BestError) as e:
+        st.step_aies(1, 1, 2.0, trace=tr, thin=1)
+    assert e.value.code == B.BEST_ERR_ARG
+    st.set_aies_exchange(None, 0, 1)
+    st.step_aies(1, 1, 2.0, trace=tr, thin=1)
+    ctx.close()
