@@ -247,3 +247,45 @@ def test_E_aies_exchange_errors(B):
     st.set_aies_exchange(None, 0, 1)
     st.step_aies(1, 1, 2.0, trace=tr, thin=1)
     ctx.close()
+
+
+def test_E_exchanges_over_nccl_world1(B):
+    """The callbacks of distributed.py over a real NCCL process group (one rank: the only size one GPU allows): the
+    all-gather runs on the library's stream through torch.distributed on zero-copy views of the library's buffers,
+    and both exchanges reproduce the runs without them bit for bit."""
+    import socket
+    import torch
+    import torch.distributed as dist
+    from paper_2606_04895_b200 import distributed as D
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1,
+                            device_id=torch.device("cuda:0"))
+    try:
+        fn = D.allgather_exchange()
+        w = WL.lcdm(n_chains=300, hidden=64, n_hidden=2)
+        w.L = np.diag(np.sqrt(np.diag(w.Sigma)))
+        side = torch.cuda.Stream()                                # a non-default stream: the callback must follow it
+        res = []
+        for use in (False, True):
+            ctx = B.Context(w, B.PREC_BF16)
+            st = ctx.new_state(w.theta0)
+            st.set_adaptation(20, 1e-6)
+            if use:
+                st.set_adaptation_exchange(fn, 1)
+            st.step_mala(60, 3, f32(0.05), stream=side.cuda_stream)
+            st.set_adaptation(0)
+            if use:
+                st.set_aies_exchange(fn, 0, 1)
+            st.step_aies(4, 8, 2.0, stream=side.cuda_stream)
+            side.synchronize()
+            res.append((ctx.get_whitening(), st.get(want_grad=False), ctx.adapt_stats()))
+            ctx.close()
+        (La, sa, aa), (Lb, sb, ab) = res
+        assert aa == ab == (3, 0)
+        assert np.array_equal(La, Lb)
+        for k in ("theta", "logp", "n_accept"):
+            assert np.array_equal(sa[k], sb[k]), k
+    finally:
+        dist.destroy_process_group()
