@@ -152,15 +152,16 @@ def test_T1_small_tile_geometries(B, O, rows, monkeypatch):
     assert np.array_equal(outs[0]["n_accept"], outs[1]["n_accept"])
 
 
-@pytest.mark.parametrize("net,rows", [("lcdm", 0), ("lcdm", 128), ("lcdm", 233), ("lcdm", 265),
-                                      ("sterile", 0), ("sterile", 232), ("sterile", 64)])
-def test_T1_eval_tile_loop(B, O, net, rows, monkeypatch):
+@pytest.mark.parametrize("net,rows,n", [("lcdm", 0, 20011), ("lcdm", 128, 20011), ("lcdm", 233, 20011),
+                                        ("lcdm", 265, 20011), ("sterile", 0, 20011), ("sterile", 232, 20011),
+                                        ("sterile", 64, 20011),
+                                        ("lcdm", 0, 262144), ("sterile", 0, 262144)])   # the sizes bench.py times
+def test_T1_eval_tile_loop(B, O, net, rows, n, monkeypatch):
     """best_logp_grad launches at most one wave of CTAs and CTA b walks tiles b, b + grid, ... (Run::n_tiles):
     20 011 points are 157 tiles of 128 (158 for the pairs), 313 of 64, 626 of 32 -- more than the 148 SMs hold, so
     some CTAs make 2..5 passes and the last tile is ragged.  Parity against the oracle on points of the first
     pass, of every later pass and of the ragged tail; the forward-only launch agrees to fp32 rounding."""
     base = WL.lcdm(n_chains=8, mlp_scale=1.0) if net == "lcdm" else WL.sterile(n_chains=8)
-    n = 20011
     pts = WL.probe_points(base, n, seed=41)
     if rows:
         monkeypatch.setenv("BEST_TC_ROWS", str(rows))
@@ -175,7 +176,8 @@ def test_T1_eval_tile_loop(B, O, net, rows, monkeypatch):
     # (the owner geometries add the output dot product in another column order without the gradient: last ulp)
     assert np.allclose(lp, lp2, rtol=2e-6, atol=0.0)
     idx = np.unique(np.concatenate([np.arange(0, 200), np.arange(4700, 4800), np.arange(9400, 9560),
-                                    np.arange(14200, 14300), np.arange(18900, 19100), np.arange(n - 150, n)]))
+                                    np.arange(14200, 14300), np.arange(18900, 19100), np.arange(n - 150, n)]
+                                   + ([np.arange(k * 18944 + 60, k * 18944 + 90) for k in range(1, 14)] if n > 30000 else [])))
     lp_ref, g_ref = O.Oracle(base).logp_grad(pts[idx])
     check_logp_grad(lp[idx], g[idx], lp_ref, g_ref, TOL[1], f"{net}/rows={rows}/tile loop")
 
