@@ -62,31 +62,31 @@ __device__ __forceinline__ void sampler_thread(EpiCtx& C, const Run& R) {
   if (METHOD == M_EVAL) {
     // tile loop (Run::n_tiles): both CTAs of a pair make the same number of passes (n_tiles and gridDim.x are even)
     for (int64_t tile = blockIdx.x; tile < R.n_tiles; tile += gridDim.x) {
-    const int64_t r_in_launch = tile * Geo<ROWS>::kChains + C.row;
-    const bool valid = r_in_launch < R.B;
-    float th[8], g[8], lp;
-    if (R.io_mode == IO_ROWS_F32) {
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const int gi = 8 * C.k + i;
-        th[i] = (valid && gi < d) ? R.in_rows[r_in_launch * d + gi] : 0.0f;
-      }
-    } else {
-      load_vec8(C, R.theta, R.ld, r_in_launch, d, valid, th);
-    }
-    eval_target<ROWS>(C, th, R.want_grad != 0, lp, g);
-    if (valid) {
+      const int64_t r_in_launch = tile * Geo<ROWS>::kChains + C.row;
+      const bool valid = r_in_launch < R.B;
+      float th[8], g[8], lp;
       if (R.io_mode == IO_ROWS_F32) {
-        if (C.k == 0) R.out_logp[r_in_launch] = lp;
-        if (R.want_grad) {
 #pragma unroll
-          for (int i = 0; i < 8; ++i) if (8 * C.k + i < d) R.out_grad[r_in_launch * d + 8 * C.k + i] = g[i];
+        for (int i = 0; i < 8; ++i) {
+          const int gi = 8 * C.k + i;
+          th[i] = (valid && gi < d) ? R.in_rows[r_in_launch * d + gi] : 0.0f;
         }
       } else {
-        if (C.k == 0) R.logp[r_in_launch] = (double)lp;
-        if (R.want_grad) store_vec8(C, R.grad, R.ld, r_in_launch, d, g);
+        load_vec8(C, R.theta, R.ld, r_in_launch, d, valid, th);
       }
-    }
+      eval_target<ROWS>(C, th, R.want_grad != 0, lp, g);
+      if (valid) {
+        if (R.io_mode == IO_ROWS_F32) {
+          if (C.k == 0) R.out_logp[r_in_launch] = lp;
+          if (R.want_grad) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) if (8 * C.k + i < d) R.out_grad[r_in_launch * d + 8 * C.k + i] = g[i];
+          }
+        } else {
+          if (C.k == 0) R.logp[r_in_launch] = (double)lp;
+          if (R.want_grad) store_vec8(C, R.grad, R.ld, r_in_launch, d, g);
+        }
+      }
     }
     return;
   }
