@@ -30,11 +30,11 @@ sys.path.insert(0, ROOT)
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures of THIS round's code (default line: profiles/r2c_ncu_full.md; the other three:
-# profiles/r2b_ncu_full.md); None where no capture exists.
+# profiles/r2d_ncu_full.md); None where no capture exists.
 NCU_TRAFFIC_BYTES = {("hmc", "bf16"): 11.073280e6 + 126.469120e6,          # best_tc_kernel<2,256>, 8 trajectories per launch
-                     ("lcdm_mala_16k", "bf16"): 11.711232e6 + 829.322496e6,  # best_tc_kernel<1,256>, 100 steps per launch
-                     ("lcdm_mh_16k", "bf16"): 5.559552e6 + 0.0,              # best_tc_kernel<0,256>, 100 steps per launch
-                     ("lcdm_mala", "bf16"): 5.240832e6 + 0.181760e6}         # best_tc_kernel<1,233>, 100 steps per launch
+                     ("lcdm_mala_16k", "bf16"): 17.137920e6 + 1362.267e6,    # best_tc_kernel<1,256>, 100 steps per launch
+                     ("lcdm_mh_16k", "bf16"): 5.554176e6 + 0.0,              # best_tc_kernel<0,256>, 100 steps per launch
+                     ("lcdm_mala", "bf16"): 5.254912e6 + 0.310272e6}         # best_tc_kernel<1,233>, 100 steps per launch
 NCU_TRAFFIC_SOURCE = "profiles/r2c_ncu_full.md"
 
 # PAPER.md Table 1 (L211-219), best published figure per sampler: sampler steps/s at 20 (1000) chains on a Tesla
@@ -391,7 +391,7 @@ def main():
         "roofline": {"bound": "tensor" if args.precision == "bf16" else "alu", "achieved": achieved_tf,
                      "peak": this_peak, "unit": "TFLOP/s", "frac": achieved_tf / this_peak,
                      "traffic": NCU_TRAFFIC_BYTES.get((args.workload, args.precision)) if is_default_size else None,
-                     "traffic_unit": "bytes per launch (ncu dram read+write, %s)" % (NCU_TRAFFIC_SOURCE if args.workload == DEFAULT_WORKLOAD else "profiles/r2b_ncu_full.md"),
+                     "traffic_unit": "bytes per launch (ncu dram read+write, %s)" % (NCU_TRAFFIC_SOURCE if args.workload == DEFAULT_WORKLOAD else "profiles/r2d_ncu_full.md"),
                      "peak_source": this_src,
                      "frac_of_sustained": (achieved_tf / peaks["bf16_tflops_sustained"]) if peaks and args.precision == "bf16" else None,
                      "kernel": "best_tc_kernel<%s>" % spec["method"], "flops_per_launch": flops_per_launch,
