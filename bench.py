@@ -280,7 +280,7 @@ def main():
 
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
-    def measure(spec, steps, warmup, with_e2e=False, prec=prec, adapt_every=0, trace=False, clocks=False):
+    def measure(spec, steps, warmup, with_e2e=False, prec=prec, adapt_every=0, trace=False, clocks=False, exchange=None):
         """Times `steps` bench steps (CUDA events on the launching stream, L2 flushed before each, max over ranks).
         Returns dict(ms_total, ms_list (this rank), launches, clocks, accept_rate, e2e...)."""
         w, chain0 = shard_workload(spec, rank, world)
@@ -289,6 +289,11 @@ def main():
         st.set_chain_offset(chain0)
         if adapt_every:
             st.set_adaptation(adapt_every, 1e-6)
+        if exchange:                                   # (kind, all-gather callback): SURVEY 8(e) exchange at world size 1
+            if exchange[0] == "adapt":
+                st.set_adaptation_exchange(exchange[1], 1)
+            else:
+                st.set_aies_exchange(exchange[1], 0, 1)
         stream = torch.cuda.current_stream().cuda_stream
         inner = spec["inner"]
         tr = torch.empty(inner, w.n_chains, w.d, device="cuda") if trace else None
@@ -514,6 +519,37 @@ def main():
                                    "ms_per_sampler_step": k["ms_per_sampler_step_no_adapt"],
                                    "achieved_l2_GB_per_s": gbs, "frac_of_l2_read": gbs / l2_gbs}
         extra["small_batch"] = small
+        # SURVEY 8(e) exchanges (best_set_adaptation_exchange, best_set_aies_exchange) with the all-gather of
+        # distributed.py over a real NCCL group of ONE rank (all one GPU allows): what pack + NCCL call + combine /
+        # unpack add to a covariance window and to an ensemble half-step -- latency, there is nothing to transfer
+        try:
+            import socket
+            import torch.distributed as dist
+            from paper_2606_04895_b200 import distributed as D
+            with socket.socket() as sk:
+                sk.bind(("127.0.0.1", 0))
+                port = sk.getsockname()[1]
+            dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1,
+                                    device_id=torch.device("cuda", local_rank))
+            try:
+                fn = D.allgather_exchange()
+                xo = {}
+                sp = dict(cfg=4, make="sterile", n_chains=16384, mlp_scale=1.0, method="mh", inner=500, eps=0.3)
+                a = float(np.median(measure(sp, 3, 1, adapt_every=500)["ms_list"]))
+                b = float(np.median(measure(sp, 3, 1, adapt_every=500, exchange=("adapt", fn))["ms_list"]))
+                xo["adapt_window_mh_16k"] = {"ms_per_500_step_window": a, "ms_with_exchange": b,
+                                             "added_us_per_window": 1e3 * (b - a)}
+                sp = dict(WORKLOADS["aies"])
+                a = float(np.median(measure(sp, n_x, 3)["ms_list"])) / sp["inner"]
+                b = float(np.median(measure(sp, n_x, 3, exchange=("aies", fn))["ms_list"])) / sp["inner"]
+                xo["aies_32k"] = {"ms_per_sampler_step": a, "ms_with_exchange": b,
+                                  "added_us_per_half_step": 1e3 * (b - a) / 2,
+                                  "bytes_gathered_per_half_step": 8 * (make_workload(sp, 8).d + 1) * sp["n_chains"] // 2}
+                extra["exchange_world1"] = xo
+            finally:
+                dist.destroy_process_group()
+        except Exception as e:                          # noqa: BLE001  (NCCL not usable on this box: say so, go on)
+            extra["exchange_world1"] = {"error": str(e)[:200]}
         # DE move on the AIES config, the burn-in loop on configs[1], R - 1 of a trace
         sp = dict(WORKLOADS["aies"], method="aies_de", sigma_gamma=0.1)
         extra["aies_de"] = summarize(sp, measure(sp, n_x, 3), n_x)
